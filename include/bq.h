@@ -1,0 +1,183 @@
+/* bq.h — C-ABI boundary of the B200-native even-odd Wilson(-clover) Dirac operator and its
+ * mixed-precision BiCGStab (hot path of arXiv 2111.04457, "Bridge++ 2.0").
+ *
+ * Citations: PAPER.md:N = /root/reference/PAPER.md line N; SURVEY §x = /root/repo/SURVEY.md.
+ *
+ * The paper states the problem as a 4-D lattice x_mu = 1..L_mu with SU(3) link variables
+ * U_mu(x) and a fermion vector of 3 colour x 4 spinor complex components per site, on which the fermion
+ * matrix of Eq. 1 acts:
+ *
+ *   D_{x,y} = [1 + F(x)] d_{x,y} - kappa sum_mu [ (1 - g_mu) U_mu(x) d_{x+mu,y} + (1 + g_mu) U_mu^dag(x-mu) d_{x-mu,y} ]
+ *
+ * with a boundary condition "imposed in each direction", and the linear equation D x = b
+ * solved by a mixed-precision solver (Fig. 1: set_config(U), set_mode("D"),
+ * invert(x, b, nconv, diff)).  Everything below runs on ONE GPU in hand-written CUDA kernels; there is
+ * no CPU fallback: every entry point returns BQ_ECUDA when no device is usable.
+ *
+ * ---------------------------------------------------------------------------------------------
+ * Canonical (caller-side) layouts — all fp64, complex = (re, im) interleaved, C-contiguous:
+ *   site    s = x + Lx*(y + Ly*(z + Lz*t)), 0-based (the paper counts from 1); mu = 0..3 = x,y,z,t
+ *   spinor  psi[s][spin 0..3][colour 0..2][re,im]                     24 doubles per site
+ *   gauge   U[s][mu][row 0..2][col 0..2][re,im]                        72 doubles per site; U_mu(x) as in Eq. 1,
+ *                                                                      row = colour index of the result
+ * Gamma matrices: Euclidean Dirac representation: g_k = [[0,-i s_k],[+i s_k,0]],
+ * g_4 = diag(1,1,-1,-1).
+ *
+ * Internal (device-side) field layout, produced by bq_field_import and consumed by the apply calls:
+ * even-odd (checkerboard) structure-of-arrays.  parity p = (x+y+z+t)&1, half index
+ * h = (x>>1) + (Lx/2)*(y + Ly*(z + Lz*t)), Vh = V/2.  A one-parity spinor is a sequence of 16-byte
+ * "planes", plane k holding for every h the reals [k*W, (k+1)*W) of the site's 24 (W = 16/sizeof(real)):
+ *   BQ_FP64: 12 planes of double2   (Vh*192 bytes)
+ *   BQ_FP32:  6 planes of float4    (Vh* 96 bytes)
+ *   BQ_HALF:  3 planes of 8 x fp16 mantissas v_i/n, then one plane of fp32 n = max_i|v_i| (Vh*52 bytes)
+ * so a warp reads 32 consecutive sites x 128 bits per load.  A BQ_FULL buffer is the even block
+ * followed by the odd block.  bq_field_bytes gives the sizes.  Buffers must be 16-byte aligned.
+ *
+ * Ownership: the caller (PyTorch in this repo) allocates and frees every field buffer and passes raw
+ * DEVICE pointers; the library never keeps them after the call returns.  The handle owns its gauge
+ * copies, clover blocks and solver workspace.  Calls on one handle must not run concurrently.
+ * Unless a `stream` argument says otherwise, work is enqueued on the CUDA legacy default stream and
+ * the call returns without synchronising (bq_solve and bq_gauge_load synchronise before returning).
+ * ---------------------------------------------------------------------------------------------
+ */
+#ifndef BQ_H
+#define BQ_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bq_lattice bq_lattice; /* opaque: geometry, boundary phases, gauge copies, clover, workspaces */
+
+typedef enum {
+    BQ_OK = 0,
+    BQ_EINVAL = 1,           /* NULL pointer, bad enum, |phase| != 1, non-positive tolerance ...            */
+    BQ_EODD_EXTENT = 2,      /* an extent is odd or < 2 (checkerboard needs even L_mu)                    */
+    BQ_ENOGAUGE = 3,         /* apply / solve before bq_gauge_load                                        */
+    BQ_ENOCLOVER = 4,        /* reserved                                                                  */
+    BQ_ESINGULAR_CLOVER = 5, /* a 6x6 clover block is not positive definite (Cholesky failed)             */
+    BQ_ECUDA = 6,            /* CUDA runtime error or no device; text in bq_last_error                    */
+    BQ_ENOMEM = 7,           /* device allocation failed                                                  */
+    BQ_ENOTCONVERGED = 8,    /* solver hit max_inner / max_outer; x holds the best iterate                */
+    BQ_EBREAKDOWN = 9        /* BiCGStab breakdown (rho, <rhat,v> or <t,t> = 0) that a restart did not cure */
+} bq_status;
+
+typedef enum { BQ_FP64 = 0, BQ_FP32 = 1, BQ_HALF = 2 } bq_prec;
+/* BQ_EVEN: out_e = -kappa H_eo in_o;  BQ_ODD: out_o = -kappa H_oe in_e;  BQ_FULL: out = D in (Eq. 1, F = 0). */
+typedef enum { BQ_EVEN = 0, BQ_ODD = 1, BQ_FULL = 2 } bq_parity;
+/* 18 reals per link, or rows 0,1 only (12 reals) with row 2 = conj(row0 x row1) rebuilt in registers. */
+typedef enum { BQ_RECON18 = 0, BQ_RECON12 = 1 } bq_recon;
+
+/* Lattice handle.  bc_phase = 4 x (re, im): psi(x + L_mu mu^) = phi_mu psi(x), |phi_mu| = 1
+ * ("a boundary condition ... is imposed in each direction"; reading S3: the phase multiplies the
+ * forward hop that wraps, its conjugate the backward hop that wraps; it is never folded into the links).
+ * NULL means periodic in x,y,z and antiperiodic in t.  Extents must be even and >= 2, V < 2^31. */
+bq_status bq_lattice_create(int Lx, int Ly, int Lz, int Lt, const double* bc_phase, bq_lattice** out);
+bq_status bq_lattice_destroy(bq_lattice* lat);
+
+/* Static text for a status, and the handle's last error message (valid until the next call on it). */
+const char* bq_status_string(bq_status s);
+const char* bq_last_error(const bq_lattice* lat);
+
+/* set_config: hand the link field to the operator.  U: canonical fp64 layout, 72*V doubles,
+ * HOST or DEVICE pointer (detected).  Copies: the caller may free U afterwards.  Builds the fp64 even-odd
+ * SoA gauge store; fp32 / half and 12-real copies are made on first use.  Invalidates any cached clover term.
+ * U is assumed to be SU(3); it is not checked (BQ_RECON12 silently relies on it).  Synchronises. */
+bq_status bq_gauge_load(bq_lattice* lat, const double* U);
+
+/* Bytes of an internal-layout field of one parity (BQ_EVEN / BQ_ODD) or of the full lattice (BQ_FULL). */
+bq_status bq_field_bytes(const bq_lattice* lat, bq_prec prec, bq_parity parity, size_t* bytes);
+
+/* Layout conversion at the interface (source and solution stay in the caller's layout
+ * and are rearranged "to respect coalesced access" on entry).  canonical: DEVICE pointer, 24*V doubles (the whole
+ * lattice, whatever `parity` says); internal: DEVICE buffer of bq_field_bytes(prec, parity).
+ * import: picks the sites of `parity` (or both), converts fp64 -> prec with round-to-nearest-even; for BQ_HALF
+ *         n = max|v_i| per site, mantissas fp16(v_i/n), an all-zero site stores n = 0 and zero mantissas.
+ * export: writes the sites of `parity` into `canonical` and leaves the other parity's entries untouched. */
+bq_status bq_field_import(bq_lattice* lat, void* internal, const double* canonical, bq_parity parity, bq_prec prec,
+                          void* stream);
+bq_status bq_field_export(bq_lattice* lat, double* canonical, const void* internal, bq_parity parity, bq_prec prec,
+                          void* stream);
+
+/* Hopping term of Eq. 1 on internal-layout fields; F = 0 (the "Wilson matrix"):
+ *   BQ_EVEN: out (even sites) = -kappa sum_mu [(1-g_mu) U_mu(x) in(x+mu) + (1+g_mu) U_mu^dag(x-mu) in(x-mu)], in = odd field
+ *   BQ_ODD : the same with the parities exchanged
+ *   BQ_FULL: out = D in = in - kappa H in, both parities (in, out: [even | odd] buffers)
+ * in and out must not overlap.  One kernel launch per parity on `stream` (a cudaStream_t, NULL = legacy default
+ * stream); no host synchronisation.  Errors: BQ_ENOGAUGE, BQ_EINVAL, BQ_ECUDA (launch error). */
+bq_status bq_wilson_apply(bq_lattice* lat, void* out, const void* in, double kappa, bq_parity parity, bq_prec prec,
+                          bq_recon recon, void* stream);
+
+/* Clover term 1 + F(x) of Eq. 1 — "a 12x12 Hermitian matrix made of the link variables"; formula from
+ * BASELINE.json config 4 / SURVEY O2:  A(x) = 1 - csw*kappa sum_{mu<nu} sigma_mu_nu (x) F_mu_nu(x),
+ * F_mu_nu = (Q - Q^dag)/(8i), Q = the four plaquette leaves at x (trace part NOT removed, S5).
+ * Stored per site as two Hermitian 6x6 chirality blocks (72 reals).
+ * The first call for a given (csw, kappa) after bq_gauge_load builds the blocks and their inverses (Cholesky in
+ * fp64) and caches them; out == NULL && in == NULL means "build only".
+ *   out(x) = A(x) in(x)   (inverse = 0)   or   A(x)^-1 in(x)   (inverse = 1),   x of `parity` (BQ_FULL: all sites).
+ * in/out: internal-layout DEVICE buffers of precision `prec`; out may equal in.  Legacy default stream.
+ * Errors: BQ_ENOGAUGE, BQ_ESINGULAR_CLOVER (build), BQ_EINVAL, BQ_ECUDA. */
+bq_status bq_clover_apply(bq_lattice* lat, double csw, double kappa, void* out, const void* in, bq_parity parity,
+                          int inverse, bq_prec prec);
+
+/* Full Wilson-clover matrix of Eq. 1 on the whole lattice, internal layout ([even | odd] buffers):
+ *   out = D in = A in - kappa H in;   csw = 0 gives the Wilson matrix. */
+bq_status bq_dirac_apply(bq_lattice* lat, void* out, const void* in, double kappa, double csw, bq_prec prec,
+                         bq_recon recon, void* stream);
+
+/* Even-odd preconditioned (Schur complement) operator on even-site fields:
+ *   out_e = A_ee in_e - kappa^2 H_eo A_oo^-1 H_oe in_e      (A = 1 when csw = 0).
+ * tmp: caller-provided scratch field of one parity (same precision).  in, out, tmp must not overlap. */
+bq_status bq_schur_apply(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw,
+                         bq_prec prec, bq_recon recon, void* stream);
+
+typedef struct {
+    int inner_prec;    /* bq_prec: BQ_FP64 = plain fp64 BiCGStab, no outer loop; BQ_FP32 / BQ_HALF = defect correction */
+    int recon;         /* bq_recon used by the inner operator (the fp64 outer operator always uses 18 reals)          */
+    double csw;        /* 0 = Wilson; otherwise the clover term is built for (csw, kappa)                              */
+    double inner_tol;  /* relative residual reduction asked of one inner solve; <= 0 = default (1e-5 fp32, 5e-2 half)    */
+    int max_inner;     /* cap on inner iterations per outer cycle; <= 0 = default (1000 fp32/fp64, 100 half)          */
+    int max_outer;     /* cap on outer cycles; <= 0 = default (50)                                                    */
+    int check_every;   /* inner iterations between host polls of the device-side convergence flag; <= 0 = default (8) */
+    void* stream;      /* reserved, must be NULL (legacy default stream)                                               */
+} bq_solve_opts;
+
+typedef struct {
+    int status;               /* bq_status of the solve                                                         */
+    int outer_cycles;         /* defect-correction cycles (0 for a pure fp64 solve)                             */
+    int inner_iters;          /* total BiCGStab iterations  (= the paper's nconv; reading S9)    */
+    int restarts;             /* BiCGStab restarts after a breakdown or a stalled inner solve                    */
+    double true_rel_residual; /* |b - D x| / |b| recomputed in fp64 with the fp64 operator (= the paper's diff) */
+    double seconds;           /* device time of the whole call (CUDA events), copies of b and x included       */
+} bq_solve_info;
+
+/* invert: solve D x = b on the whole lattice, D = Eq. 1 with the clover term for opts->csw != 0.
+ * b, x: canonical fp64 layout, 24*V doubles each, HOST or DEVICE pointers (detected independently).  x is in/out:
+ * initial guess on entry (zero it if none), solution on return.
+ * Method (readings O3, O4, S10): even-odd Schur system M^ x_e = b^_e solved by BiCGStab; for inner_prec != FP64 by
+ * defect correction — fp64 true residual, low-precision inner BiCGStab on the normalised residual, fp64 update —
+ * then x_o = A_oo^-1 (b_o + kappa H_oe x_e).  Stops when |b^_e - M^ x_e| <= tol*|b| (fp64), then reports the true
+ * full-lattice residual.  opts == NULL: fp32 inner, 18-real, Wilson.  info may be NULL.  Synchronises.
+ * Errors: BQ_ENOGAUGE, BQ_EINVAL (tol <= 0, NULLs), BQ_ENOTCONVERGED, BQ_EBREAKDOWN, BQ_ESINGULAR_CLOVER, BQ_ECUDA. */
+bq_status bq_solve(bq_lattice* lat, const double* b, double* x, double kappa, double tol, const bq_solve_opts* opts,
+                   bq_solve_info* info);
+
+/* Fused BLAS-1 on one-parity internal-layout fields, exposed for tests and benchmarks.
+ * All complex scalars are (re, im) pairs of doubles on the HOST; results are written to HOST doubles after a
+ * stream synchronise.  <a,b> = sum conj(a_i) b_i.  Reductions are accumulated in fp64 for BQ_FP64 and in fp32
+ * per thread, fp64 across threads, for BQ_FP32 / BQ_HALF; the summation order is fixed (bitwise reproducible). */
+bq_status bq_blas_norm2(bq_lattice* lat, const void* a, bq_prec prec, double* result);
+bq_status bq_blas_cdot(bq_lattice* lat, const void* a, const void* b, bq_prec prec, double* result /*[2]*/);
+/* y <- y + alpha x */
+bq_status bq_blas_caxpy(bq_lattice* lat, const double* alpha /*[2]*/, const void* x, void* y, bq_prec prec);
+/* BiCGStab update (iv): x += alpha p + omega s;  r = s - omega t;  returns |r|^2 and <rhat, r>. */
+bq_status bq_blas_bicg_update(bq_lattice* lat, const double* alpha, const double* omega, const void* p, const void* s,
+                              const void* t, const void* rhat, void* x, void* r, bq_prec prec,
+                              double* r_norm2, double* rhat_r /*[2]*/);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BQ_H */

@@ -1,0 +1,246 @@
+"""Thin ctypes binding of libbq.so (include/bq.h) — argument marshalling only.
+
+Every function has the name and argument order of its C counterpart; every step of the path runs in the
+library's CUDA kernels.  torch is used only to own device memory (tensors -> raw pointers) and streams.
+There is no CPU fallback: importing works without a GPU (so that symbol checks can run), but every compute
+call raises BqError (BQ_ECUDA) when no device is present, and loading fails loudly if libbq.so is missing.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libbq.so")
+
+# enums (include/bq.h)
+BQ_OK, BQ_EINVAL, BQ_EODD_EXTENT, BQ_ENOGAUGE, BQ_ENOCLOVER, BQ_ESINGULAR_CLOVER, BQ_ECUDA, BQ_ENOMEM, \
+    BQ_ENOTCONVERGED, BQ_EBREAKDOWN = range(10)
+BQ_FP64, BQ_FP32, BQ_HALF = 0, 1, 2
+BQ_EVEN, BQ_ODD, BQ_FULL = 0, 1, 2
+BQ_RECON18, BQ_RECON12 = 0, 1
+
+EXPORTS = [
+    "bq_lattice_create", "bq_lattice_destroy", "bq_status_string", "bq_last_error", "bq_gauge_load",
+    "bq_field_bytes", "bq_field_import", "bq_field_export", "bq_wilson_apply", "bq_clover_apply",
+    "bq_dirac_apply", "bq_schur_apply", "bq_solve", "bq_blas_norm2", "bq_blas_cdot", "bq_blas_caxpy",
+    "bq_blas_bicg_update",
+]
+
+
+class bq_solve_opts(ctypes.Structure):
+    _fields_ = [("inner_prec", ctypes.c_int), ("recon", ctypes.c_int), ("csw", ctypes.c_double),
+                ("inner_tol", ctypes.c_double), ("max_inner", ctypes.c_int), ("max_outer", ctypes.c_int),
+                ("check_every", ctypes.c_int), ("stream", ctypes.c_void_p)]
+
+
+class bq_solve_info(ctypes.Structure):
+    _fields_ = [("status", ctypes.c_int), ("outer_cycles", ctypes.c_int), ("inner_iters", ctypes.c_int),
+                ("restarts", ctypes.c_int), ("true_rel_residual", ctypes.c_double), ("seconds", ctypes.c_double)]
+
+
+class BqError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"bq status {status}: {msg}")
+        self.status = status
+
+
+_lib = None
+_vp, _dp, _i, _d = ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.c_int, ctypes.c_double
+
+
+def lib():
+    """Load libbq.so (build it first with `python -m paper_2111_04457_b200.build`)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} not found: run `python -m paper_2111_04457_b200.build` "
+                              "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        L.bq_lattice_create.argtypes = [_i, _i, _i, _i, _dp, ctypes.POINTER(_vp)]
+        L.bq_lattice_destroy.argtypes = [_vp]
+        L.bq_status_string.argtypes = [_i]
+        L.bq_status_string.restype = ctypes.c_char_p
+        L.bq_last_error.argtypes = [_vp]
+        L.bq_last_error.restype = ctypes.c_char_p
+        L.bq_gauge_load.argtypes = [_vp, _vp]
+        L.bq_field_bytes.argtypes = [_vp, _i, _i, ctypes.POINTER(ctypes.c_size_t)]
+        L.bq_field_import.argtypes = [_vp, _vp, _vp, _i, _i, _vp]
+        L.bq_field_export.argtypes = [_vp, _vp, _vp, _i, _i, _vp]
+        L.bq_wilson_apply.argtypes = [_vp, _vp, _vp, _d, _i, _i, _i, _vp]
+        L.bq_clover_apply.argtypes = [_vp, _d, _d, _vp, _vp, _i, _i, _i]
+        L.bq_dirac_apply.argtypes = [_vp, _vp, _vp, _d, _d, _i, _i, _vp]
+        L.bq_schur_apply.argtypes = [_vp, _vp, _vp, _vp, _d, _d, _i, _i, _vp]
+        L.bq_solve.argtypes = [_vp, _vp, _vp, _d, _d, ctypes.POINTER(bq_solve_opts), ctypes.POINTER(bq_solve_info)]
+        L.bq_blas_norm2.argtypes = [_vp, _vp, _i, _dp]
+        L.bq_blas_cdot.argtypes = [_vp, _vp, _vp, _i, _dp]
+        L.bq_blas_caxpy.argtypes = [_vp, _dp, _vp, _vp, _i]
+        L.bq_blas_bicg_update.argtypes = [_vp, _dp, _dp, _vp, _vp, _vp, _vp, _vp, _vp, _i, _dp, _dp]
+        for name in EXPORTS:
+            if name not in ("bq_status_string", "bq_last_error"):
+                getattr(L, name).restype = _i
+        _lib = L
+    return _lib
+
+
+def _ptr(t):
+    """Raw pointer of a torch tensor / numpy array / int / None."""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    if isinstance(t, np.ndarray):
+        return t.ctypes.data
+    return t.data_ptr()
+
+
+def _check(h, st, allow=()):
+    if st != BQ_OK and st not in allow:
+        msg = lib().bq_last_error(h).decode() if h else ""
+        raise BqError(st, f"{lib().bq_status_string(st).decode()}: {msg}")
+    return st
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        return None
+    return stream if isinstance(stream, int) else stream.cuda_stream
+
+
+# ---- the C calls, same names ----------------------------------------------------------------------
+def bq_lattice_create(Lx, Ly, Lz, Lt, bc_phase=None):
+    h = _vp()
+    bc = None
+    if bc_phase is not None:
+        arr = np.asarray(bc_phase, dtype=np.complex128).view(np.float64)
+        bc = (ctypes.c_double * 8)(*arr)
+    st = lib().bq_lattice_create(Lx, Ly, Lz, Lt, bc, ctypes.byref(h))
+    if st != BQ_OK:
+        raise BqError(st, lib().bq_status_string(st).decode())
+    return h
+
+
+def bq_lattice_destroy(h):
+    return lib().bq_lattice_destroy(h)
+
+
+def bq_gauge_load(h, U):
+    """U: canonical complex128 [Lt,Lz,Ly,Lx,4,3,3] numpy array (host) or torch CUDA tensor."""
+    if isinstance(U, np.ndarray):
+        U = np.ascontiguousarray(U, dtype=np.complex128)
+    _check(h, lib().bq_gauge_load(h, _ptr(U)))
+
+
+def bq_field_bytes(h, prec, parity):
+    n = ctypes.c_size_t(0)
+    _check(h, lib().bq_field_bytes(h, prec, parity, ctypes.byref(n)))
+    return n.value
+
+
+def bq_field_import(h, internal, canonical, parity, prec, stream=None):
+    _check(h, lib().bq_field_import(h, _ptr(internal), _ptr(canonical), parity, prec, _stream_ptr(stream)))
+
+
+def bq_field_export(h, canonical, internal, parity, prec, stream=None):
+    _check(h, lib().bq_field_export(h, _ptr(canonical), _ptr(internal), parity, prec, _stream_ptr(stream)))
+
+
+def bq_wilson_apply(h, out, inp, kappa, parity, prec=BQ_FP32, recon=BQ_RECON18, stream=None):
+    _check(h, lib().bq_wilson_apply(h, _ptr(out), _ptr(inp), kappa, parity, prec, recon, _stream_ptr(stream)))
+
+
+def bq_clover_apply(h, csw, kappa, out, inp, parity, inverse, prec):
+    _check(h, lib().bq_clover_apply(h, csw, kappa, _ptr(out), _ptr(inp), parity, int(inverse), prec))
+
+
+def bq_dirac_apply(h, out, inp, kappa, csw, prec, recon=BQ_RECON18, stream=None):
+    _check(h, lib().bq_dirac_apply(h, _ptr(out), _ptr(inp), kappa, csw, prec, recon, _stream_ptr(stream)))
+
+
+def bq_schur_apply(h, out, inp, tmp, kappa, csw, prec, recon=BQ_RECON18, stream=None):
+    _check(h, lib().bq_schur_apply(h, _ptr(out), _ptr(inp), _ptr(tmp), kappa, csw, prec, recon, _stream_ptr(stream)))
+
+
+def bq_solve(h, b, x, kappa, tol, opts: bq_solve_opts | None = None, raise_on_fail=True):
+    """b, x: canonical complex128 arrays (numpy host arrays or torch CUDA tensors); x is in/out.  Returns bq_solve_info."""
+    info = bq_solve_info()
+    st = lib().bq_solve(h, _ptr(b), _ptr(x), kappa, tol, ctypes.byref(opts) if opts is not None else None,
+                        ctypes.byref(info))
+    _check(h, st, allow=() if raise_on_fail else (BQ_ENOTCONVERGED, BQ_EBREAKDOWN))
+    return info
+
+
+def bq_blas_norm2(h, a, prec):
+    r = ctypes.c_double(0)
+    _check(h, lib().bq_blas_norm2(h, _ptr(a), prec, ctypes.byref(r)))
+    return r.value
+
+
+def bq_blas_cdot(h, a, b, prec):
+    r = (ctypes.c_double * 2)()
+    _check(h, lib().bq_blas_cdot(h, _ptr(a), _ptr(b), prec, r))
+    return complex(r[0], r[1])
+
+
+def bq_blas_caxpy(h, alpha, x, y, prec):
+    a = (ctypes.c_double * 2)(complex(alpha).real, complex(alpha).imag)
+    _check(h, lib().bq_blas_caxpy(h, a, _ptr(x), _ptr(y), prec))
+
+
+def bq_blas_bicg_update(h, alpha, omega, p, s, t, rhat, x, r, prec):
+    a = (ctypes.c_double * 2)(complex(alpha).real, complex(alpha).imag)
+    w = (ctypes.c_double * 2)(complex(omega).real, complex(omega).imag)
+    r2 = ctypes.c_double(0)
+    rr = (ctypes.c_double * 2)()
+    _check(h, lib().bq_blas_bicg_update(h, a, w, _ptr(p), _ptr(s), _ptr(t), _ptr(rhat), _ptr(x), _ptr(r), prec,
+                                        ctypes.byref(r2), rr))
+    return r2.value, complex(rr[0], rr[1])
+
+
+# ---- convenience wrapper: owns the handle and allocates internal-layout buffers with torch --------------
+class Lattice:
+    """RAII handle + torch-allocated internal-layout fields.  Pure marshalling; no arithmetic."""
+
+    def __init__(self, L, bc_phase=None):
+        self.L = tuple(int(v) for v in L)
+        self.h = bq_lattice_create(*self.L, bc_phase)
+
+    def close(self):
+        if self.h is not None:
+            bq_lattice_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def field(self, prec, parity=BQ_EVEN):
+        import torch
+        return torch.zeros(bq_field_bytes(self.h, prec, parity), dtype=torch.uint8, device="cuda")
+
+    def import_field(self, canonical, prec, parity):
+        """canonical: complex128 numpy array [Lt,Lz,Ly,Lx,4,3] or torch CUDA tensor -> internal-layout buffer."""
+        import torch
+        if isinstance(canonical, np.ndarray):
+            canonical = torch.from_numpy(np.ascontiguousarray(canonical, dtype=np.complex128)).cuda()
+        buf = self.field(prec, parity)
+        bq_field_import(self.h, buf, canonical, parity, prec)
+        return buf
+
+    def export_field(self, internal, prec, parity):
+        """internal-layout buffer -> complex128 numpy array of the whole lattice (other parity zero)."""
+        import torch
+        Lx, Ly, Lz, Lt = self.L
+        out = torch.zeros((Lt, Lz, Ly, Lx, 4, 3), dtype=torch.complex128, device="cuda")
+        bq_field_export(self.h, out, internal, parity, prec)
+        return out.cpu().numpy()

@@ -1,0 +1,376 @@
+// blas.cu — fused BLAS-1 kernels of the BiCGStab iteration and of the defect-correction outer loop
+// (SURVEY.md §8(a) A6, A8, A9).  See blas.cuh for the work-item and reduction design.
+#include "blas.cuh"
+#include "blas_api.h"
+
+#define BLAS_KERNEL __global__ void __cluster_dims__(BLAS_CLUSTER, 1, 1) __launch_bounds__(BLAS_BLOCK)
+
+// ---------------------------------------------------------------------------------------------------
+// generic reductions
+// ---------------------------------------------------------------------------------------------------
+template <int PREC> BLAS_KERNEL k_norm2(int Vh, const void* __restrict__ a, RedBuf rb, SolverScalars* sc) {
+    using I = Item<PREC>;
+    using C = typename I::C;
+    C acc = 0;
+    const int n = I::count(Vh);
+    for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
+        C v[2 * I::NC];
+        I::load(a, Vh, i, v);
+#pragma unroll
+        for (int k = 0; k < 2 * I::NC; k++) acc += v[k] * v[k];
+    }
+    double red[1] = {(double)acc};
+    grid_reduce<1>(red, rb, [sc](const double* r) { sc->red[0] = r[0]; });
+}
+
+template <int PREC> BLAS_KERNEL k_cdot(int Vh, const void* __restrict__ a, const void* __restrict__ b, RedBuf rb, SolverScalars* sc, int mode) {
+    using I = Item<PREC>;
+    using C = typename I::C;
+    C re = 0, im = 0;
+    const int n = I::count(Vh);
+    for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
+        C x[2 * I::NC], y[2 * I::NC];
+        I::load(a, Vh, i, x);
+        I::load(b, Vh, i, y);
+#pragma unroll
+        for (int k = 0; k < I::NC; k++) {   // conj(x) y
+            re += x[2 * k] * y[2 * k] + x[2 * k + 1] * y[2 * k + 1];
+            im += x[2 * k] * y[2 * k + 1] - x[2 * k + 1] * y[2 * k];
+        }
+    }
+    double red[2] = {(double)re, (double)im};
+    grid_reduce<2>(red, rb, [sc, mode](const double* r) {
+        if (mode == 0) {
+            sc->red[0] = r[0];
+            sc->red[1] = r[1];
+        } else {
+            // (v) alpha = rho / <rhat, v>
+            sc->rhat_v[0] = r[0];
+            sc->rhat_v[1] = r[1];
+            if (r[0] == 0.0 && r[1] == 0.0) {
+                if (!sc->done) sc->done = 2;
+            } else {
+                cdiv(sc->rho, r, sc->alpha);
+            }
+        }
+    });
+}
+
+template <int PREC> BLAS_KERNEL k_caxpy(int Vh, double ar_, double ai_, const void* __restrict__ x, void* __restrict__ y) {
+    using I = Item<PREC>;
+    using C = typename I::C;
+    const C ar = (C)ar_, ai = (C)ai_;
+    const int n = I::count(Vh);
+    for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
+        C xv[2 * I::NC], yv[2 * I::NC];
+        I::load(x, Vh, i, xv);
+        I::load(y, Vh, i, yv);
+#pragma unroll
+        for (int k = 0; k < I::NC; k++) cfma(yv + 2 * k, ar, ai, xv + 2 * k);
+        I::store(y, Vh, i, yv);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// BiCGStab steps
+// ---------------------------------------------------------------------------------------------------
+// r2 = |r|^2; with rhat = r: rho = r2, beta = (rho/1)(1/1) = rho (p = v = 0 makes beta irrelevant), alpha = omega = 1
+template <int PREC> BLAS_KERNEL k_init(int Vh, const void* __restrict__ r, RedBuf rb, SolverScalars* sc, double stop2) {
+    using I = Item<PREC>;
+    using C = typename I::C;
+    C acc = 0;
+    const int n = I::count(Vh);
+    for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
+        C v[2 * I::NC];
+        I::load(r, Vh, i, v);
+#pragma unroll
+        for (int k = 0; k < 2 * I::NC; k++) acc += v[k] * v[k];
+    }
+    double red[1] = {(double)acc};
+    grid_reduce<1>(red, rb, [sc, stop2](const double* r_) {
+        sc->r2 = r_[0];
+        sc->stop2 = stop2;
+        sc->rho[0] = r_[0]; sc->rho[1] = 0;
+        sc->beta[0] = 0; sc->beta[1] = 0;
+        sc->alpha[0] = 1; sc->alpha[1] = 0;
+        sc->omega[0] = 1; sc->omega[1] = 0;
+        sc->iters = 0;
+        sc->done = (r_[0] <= stop2) ? 1 : (r_[0] == 0.0 ? 1 : 0);
+    });
+}
+
+// (i) p = r + beta (p - omega v)
+template <int PREC> BLAS_KERNEL k_p_update(int Vh, const void* __restrict__ r, void* __restrict__ p, const void* __restrict__ v,
+                                           const SolverScalars* __restrict__ sc) {
+    using I = Item<PREC>;
+    using C = typename I::C;
+    if (sc->done) return;
+    const C br = (C)sc->beta[0], bi = (C)sc->beta[1], wr = (C)sc->omega[0], wi = (C)sc->omega[1];
+    const int n = I::count(Vh);
+    for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
+        C rv[2 * I::NC], pv[2 * I::NC], vv[2 * I::NC];
+        I::load(r, Vh, i, rv);
+        I::load(p, Vh, i, pv);
+        I::load(v, Vh, i, vv);
+#pragma unroll
+        for (int k = 0; k < I::NC; k++) {
+            cfma(pv + 2 * k, -wr, -wi, vv + 2 * k);    // p - omega v
+            cfma(rv + 2 * k, br, bi, pv + 2 * k);      // r + beta (.)
+        }
+        I::store(p, Vh, i, rv);
+    }
+}
+
+// (ii) s = r - alpha v
+template <int PREC> BLAS_KERNEL k_s_update(int Vh, const void* __restrict__ r, const void* __restrict__ v, void* __restrict__ s,
+                                           const SolverScalars* __restrict__ sc) {
+    using I = Item<PREC>;
+    using C = typename I::C;
+    if (sc->done) return;
+    const C ar = (C)sc->alpha[0], ai = (C)sc->alpha[1];
+    const int n = I::count(Vh);
+    for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
+        C rv[2 * I::NC], vv[2 * I::NC];
+        I::load(r, Vh, i, rv);
+        I::load(v, Vh, i, vv);
+#pragma unroll
+        for (int k = 0; k < I::NC; k++) cfma(rv + 2 * k, -ar, -ai, vv + 2 * k);
+        I::store(s, Vh, i, rv);
+    }
+}
+
+// (iii) <t,s>, <t,t> in one pass; omega = <t,s>/<t,t>
+template <int PREC> BLAS_KERNEL k_omega(int Vh, const void* __restrict__ t, const void* __restrict__ s, RedBuf rb, SolverScalars* sc) {
+    using I = Item<PREC>;
+    using C = typename I::C;
+    C re = 0, im = 0, tt = 0;
+    const int n = I::count(Vh);
+    for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
+        C x[2 * I::NC], y[2 * I::NC];
+        I::load(t, Vh, i, x);
+        I::load(s, Vh, i, y);
+#pragma unroll
+        for (int k = 0; k < I::NC; k++) {
+            re += x[2 * k] * y[2 * k] + x[2 * k + 1] * y[2 * k + 1];
+            im += x[2 * k] * y[2 * k + 1] - x[2 * k + 1] * y[2 * k];
+            tt += x[2 * k] * x[2 * k] + x[2 * k + 1] * x[2 * k + 1];
+        }
+    }
+    double red[3] = {(double)re, (double)im, (double)tt};
+    grid_reduce<3>(red, rb, [sc](const double* r) {
+        sc->ts[0] = r[0]; sc->ts[1] = r[1]; sc->tt = r[2];
+        if (r[2] == 0.0) {
+            if (!sc->done) sc->done = 2;
+        } else {
+            sc->omega[0] = r[0] / r[2];
+            sc->omega[1] = r[1] / r[2];
+        }
+    });
+}
+
+// (iv) x += alpha p + omega s ; r = s - omega t ; |r|^2 ; <rhat, r>   — one pass over 5 inputs, 2 outputs.
+// The finaliser prepares the next iteration: rho' = <rhat,r>, beta = (rho'/rho)(alpha/omega), rho = rho'.
+template <int PREC> BLAS_KERNEL k_final(int Vh, const void* __restrict__ p, const void* __restrict__ s, const void* __restrict__ t,
+                                        const void* __restrict__ rhat, void* __restrict__ x, void* __restrict__ r, RedBuf rb,
+                                        SolverScalars* sc) {
+    using I = Item<PREC>;
+    using C = typename I::C;
+    if (sc->done) return;   // converged or broken down in an earlier iteration of this batch: x stays frozen
+    const C ar = (C)sc->alpha[0], ai = (C)sc->alpha[1], wr = (C)sc->omega[0], wi = (C)sc->omega[1];
+    C r2 = 0, re = 0, im = 0;
+    const int n = I::count(Vh);
+    for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
+        C xv[2 * I::NC], sv[2 * I::NC], w[2 * I::NC];
+        if constexpr (PREC == BQ_HALF) load_spinor<BQ_FP32>(x, Vh, i, xv);   // fp32 solution accumulator
+        else I::load(x, Vh, i, xv);
+        I::load(p, Vh, i, w);
+#pragma unroll
+        for (int k = 0; k < I::NC; k++) cfma(xv + 2 * k, ar, ai, w + 2 * k);
+        I::load(s, Vh, i, sv);
+#pragma unroll
+        for (int k = 0; k < I::NC; k++) cfma(xv + 2 * k, wr, wi, sv + 2 * k);
+        if constexpr (PREC == BQ_HALF) store_spinor<BQ_FP32>(x, Vh, i, xv);
+        else I::store(x, Vh, i, xv);
+        I::load(t, Vh, i, w);
+#pragma unroll
+        for (int k = 0; k < I::NC; k++) cfma(sv + 2 * k, -wr, -wi, w + 2 * k);   // r = s - omega t
+        I::store(r, Vh, i, sv);
+        if constexpr (PREC == BQ_HALF) I::requantize(sv);       // reductions see r as stored (rounded to half storage)
+        I::load(rhat, Vh, i, w);
+#pragma unroll
+        for (int k = 0; k < I::NC; k++) {
+            r2 += sv[2 * k] * sv[2 * k] + sv[2 * k + 1] * sv[2 * k + 1];
+            re += w[2 * k] * sv[2 * k] + w[2 * k + 1] * sv[2 * k + 1];
+            im += w[2 * k] * sv[2 * k + 1] - w[2 * k + 1] * sv[2 * k];
+        }
+    }
+    double red[3] = {(double)r2, (double)re, (double)im};
+    grid_reduce<3>(red, rb, [sc](const double* q) {
+        sc->r2 = q[0];
+        sc->iters += 1;
+        const double rho_new[2] = {q[1], q[2]};
+        if (q[0] <= sc->stop2) {
+            sc->done = 1;
+        } else if ((rho_new[0] == 0.0 && rho_new[1] == 0.0) || (sc->omega[0] == 0.0 && sc->omega[1] == 0.0)) {
+            sc->done = 2;
+        } else {
+            double a[2], b[2];
+            cdiv(rho_new, sc->rho, a);
+            cdiv(sc->alpha, sc->omega, b);
+            cmuld(a, b, sc->beta);
+        }
+        sc->rho[0] = rho_new[0];
+        sc->rho[1] = rho_new[1];
+    });
+}
+
+// ---------------------------------------------------------------------------------------------------
+// outer loop (fp64)
+// ---------------------------------------------------------------------------------------------------
+BLAS_KERNEL k_outer_residual(int Vh, const void* __restrict__ b, const void* __restrict__ t, void* __restrict__ r, RedBuf rb,
+                             SolverScalars* sc) {
+    using I = Item<BQ_FP64>;
+    double acc = 0;
+    const int n = I::count(Vh);
+    for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
+        double bv[2], tv[2];
+        I::load(b, Vh, i, bv);
+        I::load(t, Vh, i, tv);
+        bv[0] -= tv[0];
+        bv[1] -= tv[1];
+        I::store(r, Vh, i, bv);
+        acc += bv[0] * bv[0] + bv[1] * bv[1];
+    }
+    double red[1] = {acc};
+    grid_reduce<1>(red, rb, [sc](const double* q) {
+        sc->r2 = q[0];
+        sc->red[0] = q[0];
+        sc->rnorm = sqrt(q[0]);
+        sc->scale = q[0] > 0.0 ? 1.0 / sqrt(q[0]) : 0.0;
+    });
+}
+
+template <int PREC_LO> __global__ void __launch_bounds__(128) k_to_low(int Vh, const void* __restrict__ r64, void* __restrict__ lo,
+                                                                      const SolverScalars* __restrict__ sc) {
+    const int h = blockIdx.x * blockDim.x + threadIdx.x;
+    if (h >= Vh) return;
+    const double sca = sc->scale;
+    double v[24];
+    load_spinor<BQ_FP64, true>(r64, Vh, h, v);
+    typename Prec<PREC_LO>::comp w[24];
+#pragma unroll
+    for (int i = 0; i < 24; i++) w[i] = (typename Prec<PREC_LO>::comp)(v[i] * sca);
+    store_spinor<PREC_LO>(lo, Vh, h, w);
+}
+
+template <int EPREC> __global__ void __launch_bounds__(128) k_accumulate(int Vh, const void* __restrict__ e, void* __restrict__ x64,
+                                                                        const SolverScalars* __restrict__ sc) {
+    const int h = blockIdx.x * blockDim.x + threadIdx.x;
+    if (h >= Vh) return;
+    const double rn = sc->rnorm;
+    typename Prec<EPREC>::comp ev[24];
+    load_spinor<EPREC, true>(e, Vh, h, ev);
+    double xv[24];
+    load_spinor<BQ_FP64, true>(x64, Vh, h, xv);
+#pragma unroll
+    for (int i = 0; i < 24; i++) xv[i] += rn * (double)ev[i];
+    store_spinor<BQ_FP64>(x64, Vh, h, xv);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------------
+bq_status blas_ctx_create(bq_lattice* lat, BlasCtx* c) {
+    int dev = 0, sms = 0;
+    BQ_CUDA(lat, cudaGetDevice(&dev));
+    BQ_CUDA(lat, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    c->Vh = lat->g.Vh;
+    // persistent-style grid: 4 CTAs of 256 threads per SM (a multiple of the SM count and of the cluster size),
+    // trimmed for small lattices so that no cluster is empty-handed more than necessary
+    int grid = sms * 4;
+    const int need = (12 * lat->g.Vh + BLAS_BLOCK - 1) / BLAS_BLOCK;
+    if (grid > need) grid = need;
+    grid = ((grid + BLAS_CLUSTER - 1) / BLAS_CLUSTER) * BLAS_CLUSTER;
+    c->grid = grid;
+    c->stream = 0;
+    BQ_CUDA(lat, cudaMalloc(&c->partials, sizeof(double) * 4 * (grid / BLAS_CLUSTER)));
+    BQ_CUDA(lat, cudaMalloc(&c->ticket, sizeof(unsigned int)));
+    BQ_CUDA(lat, cudaMemset(c->ticket, 0, sizeof(unsigned int)));
+    BQ_CUDA(lat, cudaMalloc(&c->sc, sizeof(SolverScalars)));
+    BQ_CUDA(lat, cudaMemset(c->sc, 0, sizeof(SolverScalars)));
+    return BQ_OK;
+}
+
+void blas_ctx_destroy(BlasCtx* c) {
+    if (c->partials) cudaFree(c->partials);
+    if (c->ticket) cudaFree(c->ticket);
+    if (c->sc) cudaFree(c->sc);
+    c->partials = nullptr; c->ticket = nullptr; c->sc = nullptr;
+}
+
+#define DISPATCH_PREC(prec, KERNEL, ...)                                                             \
+    do {                                                                                             \
+        if ((prec) == BQ_FP64) KERNEL<BQ_FP64><<<c.grid, BLAS_BLOCK, 0, c.stream>>>(__VA_ARGS__);    \
+        else if ((prec) == BQ_FP32) KERNEL<BQ_FP32><<<c.grid, BLAS_BLOCK, 0, c.stream>>>(__VA_ARGS__); \
+        else KERNEL<BQ_HALF><<<c.grid, BLAS_BLOCK, 0, c.stream>>>(__VA_ARGS__);                      \
+        BQ_CUDA(lat, cudaGetLastError());                                                            \
+        return BQ_OK;                                                                                \
+    } while (0)
+
+bq_status blas_norm2(bq_lattice* lat, const BlasCtx& c, int prec, const void* a) {
+    RedBuf rb{c.partials, c.ticket};
+    DISPATCH_PREC(prec, k_norm2, c.Vh, a, rb, c.sc);
+}
+bq_status blas_cdot(bq_lattice* lat, const BlasCtx& c, int prec, const void* a, const void* b) {
+    RedBuf rb{c.partials, c.ticket};
+    DISPATCH_PREC(prec, k_cdot, c.Vh, a, b, rb, c.sc, 0);
+}
+bq_status blas_caxpy(bq_lattice* lat, const BlasCtx& c, int prec, double ar, double ai, const void* x, void* y) {
+    DISPATCH_PREC(prec, k_caxpy, c.Vh, ar, ai, x, y);
+}
+bq_status bicg_init(bq_lattice* lat, const BlasCtx& c, int prec, const void* r, double stop2) {
+    RedBuf rb{c.partials, c.ticket};
+    DISPATCH_PREC(prec, k_init, c.Vh, r, rb, c.sc, stop2);
+}
+bq_status bicg_p_update(bq_lattice* lat, const BlasCtx& c, int prec, const void* r, void* p, const void* v) {
+    DISPATCH_PREC(prec, k_p_update, c.Vh, r, p, v, c.sc);
+}
+bq_status bicg_alpha(bq_lattice* lat, const BlasCtx& c, int prec, const void* rhat, const void* v) {
+    RedBuf rb{c.partials, c.ticket};
+    DISPATCH_PREC(prec, k_cdot, c.Vh, rhat, v, rb, c.sc, 1);
+}
+bq_status bicg_s_update(bq_lattice* lat, const BlasCtx& c, int prec, const void* r, const void* v, void* s) {
+    DISPATCH_PREC(prec, k_s_update, c.Vh, r, v, s, c.sc);
+}
+bq_status bicg_omega(bq_lattice* lat, const BlasCtx& c, int prec, const void* t, const void* s) {
+    RedBuf rb{c.partials, c.ticket};
+    DISPATCH_PREC(prec, k_omega, c.Vh, t, s, rb, c.sc);
+}
+bq_status bicg_final(bq_lattice* lat, const BlasCtx& c, int prec, const void* p, const void* s, const void* t, const void* rhat,
+                     void* x, void* r) {
+    RedBuf rb{c.partials, c.ticket};
+    DISPATCH_PREC(prec, k_final, c.Vh, p, s, t, rhat, x, r, rb, c.sc);
+}
+
+bq_status outer_residual(bq_lattice* lat, const BlasCtx& c, const void* b, const void* t, void* r) {
+    RedBuf rb{c.partials, c.ticket};
+    k_outer_residual<<<c.grid, BLAS_BLOCK, 0, c.stream>>>(c.Vh, b, t, r, rb, c.sc);
+    BQ_CUDA(lat, cudaGetLastError());
+    return BQ_OK;
+}
+bq_status outer_to_low(bq_lattice* lat, const BlasCtx& c, int prec_lo, const void* r64, void* lo) {
+    const int grid = (c.Vh + 127) / 128;
+    if (prec_lo == BQ_FP64) k_to_low<BQ_FP64><<<grid, 128, 0, c.stream>>>(c.Vh, r64, lo, c.sc);
+    else if (prec_lo == BQ_FP32) k_to_low<BQ_FP32><<<grid, 128, 0, c.stream>>>(c.Vh, r64, lo, c.sc);
+    else k_to_low<BQ_HALF><<<grid, 128, 0, c.stream>>>(c.Vh, r64, lo, c.sc);
+    BQ_CUDA(lat, cudaGetLastError());
+    return BQ_OK;
+}
+bq_status outer_accumulate(bq_lattice* lat, const BlasCtx& c, int e_prec, const void* e, void* x64) {
+    const int grid = (c.Vh + 127) / 128;
+    if (e_prec == BQ_FP64) k_accumulate<BQ_FP64><<<grid, 128, 0, c.stream>>>(c.Vh, e, x64, c.sc);
+    else if (e_prec == BQ_FP32) k_accumulate<BQ_FP32><<<grid, 128, 0, c.stream>>>(c.Vh, e, x64, c.sc);
+    else return bq_set_error(lat, BQ_EINVAL, "outer_accumulate: accumulator cannot be half");
+    BQ_CUDA(lat, cudaGetLastError());
+    return BQ_OK;
+}

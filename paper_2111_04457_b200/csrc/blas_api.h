@@ -1,0 +1,43 @@
+// blas_api.h — host launchers of the fused BLAS-1 kernels (blas.cu), used by the solver (solve.cu).
+#pragma once
+
+#include "bq_internal.h"
+
+struct SolverScalars;
+
+struct BlasCtx {
+    int Vh;
+    int grid;                 // blocks per launch (multiple of the cluster size)
+    double* partials;         // reduction scratch
+    unsigned int* ticket;
+    SolverScalars* sc;        // device-resident solver state
+    cudaStream_t stream;
+};
+
+bq_status blas_ctx_create(bq_lattice* lat, BlasCtx* ctx);
+void blas_ctx_destroy(BlasCtx* ctx);
+
+// --- generic (results land in sc->red[], no host sync) ---
+bq_status blas_norm2(bq_lattice* lat, const BlasCtx& c, int prec, const void* a);                  // red[0] = |a|^2
+bq_status blas_cdot(bq_lattice* lat, const BlasCtx& c, int prec, const void* a, const void* b);    // red[0..1] = <a,b>
+bq_status blas_caxpy(bq_lattice* lat, const BlasCtx& c, int prec, double ar, double ai, const void* x, void* y);
+
+// --- BiCGStab steps; scalars read from / written to c.sc ---
+// set stop2 and reset the state; then r2 = |r|^2, rho = <rhat,r> = r2 (rhat == r), beta = rho, alpha = omega = 1
+bq_status bicg_init(bq_lattice* lat, const BlasCtx& c, int prec, const void* r, double stop2);
+bq_status bicg_p_update(bq_lattice* lat, const BlasCtx& c, int prec, const void* r, void* p, const void* v);
+bq_status bicg_alpha(bq_lattice* lat, const BlasCtx& c, int prec, const void* rhat, const void* v);
+bq_status bicg_s_update(bq_lattice* lat, const BlasCtx& c, int prec, const void* r, const void* v, void* s);
+bq_status bicg_omega(bq_lattice* lat, const BlasCtx& c, int prec, const void* t, const void* s);
+// x += alpha p + omega s ; r = s - omega t ; r2, rho', beta ; iters++ ; convergence / breakdown flag.
+// For prec == BQ_HALF the accumulator x is an fp32 field (site layout), everything else half storage.
+bq_status bicg_final(bq_lattice* lat, const BlasCtx& c, int prec, const void* p, const void* s, const void* t, const void* rhat,
+                     void* x, void* r);
+
+// --- outer (fp64) loop ---
+// r = b - t (fp64); sc->r2 = red[0] = |r|^2; sc->scale = 1/|r| (0 if r == 0)
+bq_status outer_residual(bq_lattice* lat, const BlasCtx& c, const void* b, const void* t, void* r);
+// lo = convert(r * sc->scale) into precision prec_lo (site-wise; half: per-site norm)
+bq_status outer_to_low(bq_lattice* lat, const BlasCtx& c, int prec_lo, const void* r64, void* lo);
+// x64 += |r| * e_lo   (|r| = sqrt(sc->r2)); e_prec = precision of e (fp32 accumulator when the inner solver is half)
+bq_status outer_accumulate(bq_lattice* lat, const BlasCtx& c, int e_prec, const void* e, void* x64);

@@ -1,0 +1,89 @@
+// bq_internal.h — shared declarations of the CUDA implementation behind include/bq.h.
+// Product code: shares nothing with oracle/ (the gamma-matrix algebra is hard-wired as spin projections
+// in hop.cuh, typed in independently from SURVEY.md Appendix A.2).
+#pragma once
+
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "bq.h"
+
+// ---------------------------------------------------------------------------------------------------
+// Geometry.  Half index h = xh + Lxh*(y + Ly*(z + Lz*t)), xh = x >> 1.
+// ---------------------------------------------------------------------------------------------------
+struct Geom {
+    int L[4];   // Lx, Ly, Lz, Lt
+    int Lxh;    // Lx / 2
+    int Vh;     // sites per parity
+    int V;      // all sites
+};
+
+// reals per site / per link in each store
+constexpr int SPINOR_REALS = 24;
+constexpr int CLOVER_REALS = 72;  // 2 blocks x (6 real diagonal + 15 complex off-diagonal)
+__host__ __device__ constexpr int link_reals(int recon) { return recon == BQ_RECON12 ? 12 : 18; }
+
+__host__ __device__ constexpr size_t prec_real_bytes(int prec) { return prec == BQ_FP64 ? 8 : (prec == BQ_FP32 ? 4 : 2); }
+// bytes per site of a spinor in precision prec (half: 48 B mantissas + 4 B norm)
+__host__ __device__ constexpr size_t spinor_site_bytes(int prec) { return prec == BQ_FP64 ? 192 : (prec == BQ_FP32 ? 96 : 52); }
+
+struct SolverWork;
+
+struct bq_lattice {
+    Geom g;
+    double bc[8];            // 4 x (re, im)
+    int bc_nontrivial[4];    // phase != 1 in that direction
+    double* U_canon;         // device copy of the canonical fp64 gauge field (kept for the clover build)
+    void* gauge[3][2];       // [prec][recon]: [parity][mu][link planes over Vh]
+    bool have_gauge;
+    // clover: [prec][inverse]: [parity][72 reals as planes over Vh]; fp64 always built first
+    void* clover[3][2];
+    bool have_clover;
+    double clover_csw, clover_kappa;
+    SolverWork* work;
+    int* d_flag;             // device int scratch (singular-clover flag etc.)
+    char err[512];
+};
+
+// ---------------------------------------------------------------------------------------------------
+// Error plumbing
+// ---------------------------------------------------------------------------------------------------
+bq_status bq_set_error(bq_lattice* lat, bq_status s, const char* fmt, ...);
+
+#define BQ_CUDA(lat, expr)                                                                              \
+    do {                                                                                                \
+        cudaError_t _e = (expr);                                                                        \
+        if (_e != cudaSuccess)                                                                          \
+            return bq_set_error((lat), _e == cudaErrorMemoryAllocation ? BQ_ENOMEM : BQ_ECUDA,          \
+                                "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e), __FILE__, __LINE__); \
+    } while (0)
+
+#define BQ_TRY(expr)                    \
+    do {                                \
+        bq_status _s = (expr);          \
+        if (_s != BQ_OK) return _s;     \
+    } while (0)
+
+// ---------------------------------------------------------------------------------------------------
+// Internal entry points shared between translation units
+// ---------------------------------------------------------------------------------------------------
+// gauge store of (prec, recon), built on first use from the fp64 18-real store
+bq_status bq_get_gauge(bq_lattice* lat, int prec, int recon, const void** out);
+// clover blocks of (prec, inverse), built on first use; requires bq_clover_build to have run
+bq_status bq_clover_build(bq_lattice* lat, double csw, double kappa);
+bq_status bq_get_clover(bq_lattice* lat, int prec, int inverse, const void** out);
+
+// Hop with epilogue:  out_p = scale * H_{p,1-p} in  [+ z]   (z == nullptr: no xpay).
+// Clover epilogues (cl != nullptr, 72-real blocks of parity p in precision prec):
+//   cl_mode 1: out = scale * C (H in) [+ z]          (C = A^-1 blocks: the "A_oo^-1 H_oe" step)
+//   cl_mode 2: out = C z + scale * H in               (C = A blocks: the "A_ee x - kappa^2 H ..." step)
+bq_status bq_hop(bq_lattice* lat, void* out, const void* in, const void* z, double scale, int out_parity, int prec,
+                 int recon, const void* cl, int cl_mode, cudaStream_t stream);
+// out = C in on one parity (site-diagonal clover multiply)
+bq_status bq_clover_mul(bq_lattice* lat, void* out, const void* in, const void* cl, int prec, cudaStream_t stream);
+
+void bq_solver_free(bq_lattice* lat);
+
+static inline size_t field_bytes_one_parity(const Geom& g, int prec) { return (size_t)g.Vh * spinor_site_bytes(prec); }

@@ -1,0 +1,209 @@
+// hop.cu — the even-odd hopping kernel H_{p,1-p} and bq_wilson_apply / bq_dirac_apply /
+// bq_schur_apply built on it.  One thread per output site; 32 consecutive half-indices per warp so every
+// spinor-plane, link-plane and output access is a 512-byte coalesced request.  Neighbours in y,z,t are whole
+// shifted rows (still coalesced); the x neighbour is the same half-index or +-1 (Appendix A.5), which the L1
+// serves.  Links are read exactly once (streaming / evict-first loads) so that L2 keeps the input spinor,
+// each site of which is gathered by its 8 neighbours; outputs are streamed.
+#include "clover.cuh"
+#include "hop.cuh"
+
+constexpr int HOP_BLOCK = 128;
+
+template <typename C> struct HopArgs {
+    void* out;
+    const void* in;
+    const void* z;        // xpay operand (parity p) or nullptr
+    const void* gf;       // gauge blocks of parity p   (forward links U_mu(x)),    4 blocks of `ublk` bytes
+    const void* gb;       // gauge blocks of parity 1-p (backward links U_mu(x-mu))
+    const void* cl;       // clover blocks of parity p (epilogue) or nullptr
+    size_t ublk;          // bytes of one (parity, mu) gauge block
+    int Lxh, Ly, Lz, Lt, Vh, p;
+    C scale;
+    C phr[4], phi[4];     // boundary phases phi_mu
+    int nontrivial[4];    // phi_mu != 1
+};
+
+// EPI: 0: out = scale*acc;  1: out = z + scale*acc;  2: out = scale * Cl(acc);  3: out = Cl(z) + scale*acc
+template <int PREC, int RECON, int EPI>
+__global__ void __launch_bounds__(HOP_BLOCK, PREC == BQ_FP64 ? 2 : 4)
+hop_kernel(const HopArgs<typename Prec<PREC>::comp> a) {
+    using C = typename Prec<PREC>::comp;
+    const int h = blockIdx.x * HOP_BLOCK + threadIdx.x;
+    if (h >= a.Vh) return;
+    const int Vh = a.Vh;
+    const int xh = h % a.Lxh;
+    int q = h / a.Lxh;
+    const int y = q % a.Ly;
+    q /= a.Ly;
+    const int z = q % a.Lz;
+    const int t = q / a.Lz;
+    const int r = (y + z + t + a.p) & 1;   // x = 2*xh + r
+    const int sy = a.Lxh, sz = a.Lxh * a.Ly, st = sz * a.Lz;
+    const char* gf = static_cast<const char*>(a.gf);
+    const char* gb = static_cast<const char*>(a.gb);
+
+    C acc[24];
+#pragma unroll
+    for (int i = 0; i < 24; i++) acc[i] = 0;
+
+    // ---- x ----
+    {
+        const bool wf = r && (xh == a.Lxh - 1);
+        const int nf = r ? (wf ? h - (a.Lxh - 1) : h + 1) : h;
+        hop_dir<PREC, RECON, 0, true>(acc, a.in, Vh, nf, gf, h, wf && a.nontrivial[0], a.phr[0], a.phi[0]);
+        const bool wb = !r && (xh == 0);
+        const int nb = r ? h : (wb ? h + (a.Lxh - 1) : h - 1);
+        hop_dir<PREC, RECON, 0, false>(acc, a.in, Vh, nb, gb, nb, wb && a.nontrivial[0], a.phr[0], -a.phi[0]);
+    }
+    // ---- y ----
+    {
+        const bool wf = (y == a.Ly - 1);
+        const int nf = wf ? h - (a.Ly - 1) * sy : h + sy;
+        hop_dir<PREC, RECON, 1, true>(acc, a.in, Vh, nf, gf + a.ublk, h, wf && a.nontrivial[1], a.phr[1], a.phi[1]);
+        const bool wb = (y == 0);
+        const int nb = wb ? h + (a.Ly - 1) * sy : h - sy;
+        hop_dir<PREC, RECON, 1, false>(acc, a.in, Vh, nb, gb + a.ublk, nb, wb && a.nontrivial[1], a.phr[1], -a.phi[1]);
+    }
+    // ---- z ----
+    {
+        const bool wf = (z == a.Lz - 1);
+        const int nf = wf ? h - (a.Lz - 1) * sz : h + sz;
+        hop_dir<PREC, RECON, 2, true>(acc, a.in, Vh, nf, gf + 2 * a.ublk, h, wf && a.nontrivial[2], a.phr[2], a.phi[2]);
+        const bool wb = (z == 0);
+        const int nb = wb ? h + (a.Lz - 1) * sz : h - sz;
+        hop_dir<PREC, RECON, 2, false>(acc, a.in, Vh, nb, gb + 2 * a.ublk, nb, wb && a.nontrivial[2], a.phr[2], -a.phi[2]);
+    }
+    // ---- t ----
+    {
+        const bool wf = (t == a.Lt - 1);
+        const int nf = wf ? h - (a.Lt - 1) * st : h + st;
+        hop_dir<PREC, RECON, 3, true>(acc, a.in, Vh, nf, gf + 3 * a.ublk, h, wf && a.nontrivial[3], a.phr[3], a.phi[3]);
+        const bool wb = (t == 0);
+        const int nb = wb ? h + (a.Lt - 1) * st : h - st;
+        hop_dir<PREC, RECON, 3, false>(acc, a.in, Vh, nb, gb + 3 * a.ublk, nb, wb && a.nontrivial[3], a.phr[3], -a.phi[3]);
+    }
+
+    // ---- epilogue ----
+    if (EPI == 2) clover_site_mul<PREC>(a.cl, Vh, h, acc);
+#pragma unroll
+    for (int i = 0; i < 24; i++) acc[i] *= a.scale;
+    if (EPI == 1 || EPI == 3) {
+        C zz[24];
+        load_spinor<PREC, true>(a.z, Vh, h, zz);
+        if (EPI == 3) clover_site_mul<PREC>(a.cl, Vh, h, zz);
+#pragma unroll
+        for (int i = 0; i < 24; i++) acc[i] += zz[i];
+    }
+    store_spinor<PREC, true>(a.out, Vh, h, acc);
+}
+
+template <int PREC, int RECON>
+static bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const void* z, double scale, int p, const void* gauge,
+                            const void* cl, int cl_mode, cudaStream_t stream) {
+    using C = typename Prec<PREC>::comp;
+    const Geom& g = lat->g;
+    HopArgs<C> a;
+    a.out = out; a.in = in; a.z = z; a.cl = cl;
+    a.ublk = link_block_bytes(PREC, RECON, g.Vh);
+    a.gf = static_cast<const char*>(gauge) + (size_t)p * 4 * a.ublk;
+    a.gb = static_cast<const char*>(gauge) + (size_t)(1 - p) * 4 * a.ublk;
+    a.Lxh = g.Lxh; a.Ly = g.L[1]; a.Lz = g.L[2]; a.Lt = g.L[3]; a.Vh = g.Vh; a.p = p;
+    a.scale = (C)scale;
+    for (int mu = 0; mu < 4; mu++) {
+        a.phr[mu] = (C)lat->bc[2 * mu];
+        a.phi[mu] = (C)lat->bc[2 * mu + 1];
+        a.nontrivial[mu] = lat->bc_nontrivial[mu];
+    }
+    const int grid = (g.Vh + HOP_BLOCK - 1) / HOP_BLOCK;
+    int epi;
+    if (cl_mode == 0) epi = z ? 1 : 0;
+    else if (cl_mode == 1 && !z) epi = 2;
+    else if (cl_mode == 2 && z) epi = 3;
+    else return bq_set_error(lat, BQ_EINVAL, "bq_hop: unsupported epilogue (cl_mode=%d, z=%p)", cl_mode, z);
+    switch (epi) {
+        case 0: hop_kernel<PREC, RECON, 0><<<grid, HOP_BLOCK, 0, stream>>>(a); break;
+        case 1: hop_kernel<PREC, RECON, 1><<<grid, HOP_BLOCK, 0, stream>>>(a); break;
+        case 2: hop_kernel<PREC, RECON, 2><<<grid, HOP_BLOCK, 0, stream>>>(a); break;
+        default: hop_kernel<PREC, RECON, 3><<<grid, HOP_BLOCK, 0, stream>>>(a); break;
+    }
+    BQ_CUDA(lat, cudaGetLastError());
+    return BQ_OK;
+}
+
+bq_status bq_hop(bq_lattice* lat, void* out, const void* in, const void* z, double scale, int p, int prec, int recon,
+                 const void* cl, int cl_mode, cudaStream_t stream) {
+    const void* gauge = nullptr;
+    BQ_TRY(bq_get_gauge(lat, prec, recon, &gauge));
+#define BQ_HOP_CASE(P, R) \
+    if (prec == P && recon == R) return launch_hop<P, R>(lat, out, in, z, scale, p, gauge, cl, cl_mode, stream);
+    BQ_HOP_CASE(BQ_FP64, BQ_RECON18)
+    BQ_HOP_CASE(BQ_FP64, BQ_RECON12)
+    BQ_HOP_CASE(BQ_FP32, BQ_RECON18)
+    BQ_HOP_CASE(BQ_FP32, BQ_RECON12)
+    BQ_HOP_CASE(BQ_HALF, BQ_RECON18)
+    BQ_HOP_CASE(BQ_HALF, BQ_RECON12)
+#undef BQ_HOP_CASE
+    return bq_set_error(lat, BQ_EINVAL, "bq_hop: bad prec/recon (%d, %d)", prec, recon);
+}
+
+static bool valid_prec(int p) { return p == BQ_FP64 || p == BQ_FP32 || p == BQ_HALF; }
+static bool valid_recon(int r) { return r == BQ_RECON18 || r == BQ_RECON12; }
+
+extern "C" bq_status bq_wilson_apply(bq_lattice* lat, void* out, const void* in, double kappa, bq_parity parity, bq_prec prec,
+                                     bq_recon recon, void* stream) {
+    if (!lat) return BQ_EINVAL;
+    if (!out || !in || out == in) return bq_set_error(lat, BQ_EINVAL, "bq_wilson_apply: out/in NULL or aliased");
+    if (!valid_prec(prec) || !valid_recon(recon)) return bq_set_error(lat, BQ_EINVAL, "bq_wilson_apply: bad prec/recon");
+    if (!lat->have_gauge) return bq_set_error(lat, BQ_ENOGAUGE, "bq_wilson_apply: no gauge field loaded");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (parity == BQ_EVEN || parity == BQ_ODD)
+        return bq_hop(lat, out, in, nullptr, -kappa, (int)parity, prec, recon, nullptr, 0, s);
+    if (parity != BQ_FULL) return bq_set_error(lat, BQ_EINVAL, "bq_wilson_apply: bad parity %d", (int)parity);
+    return bq_dirac_apply(lat, out, in, kappa, 0.0, prec, recon, stream);
+}
+
+extern "C" bq_status bq_dirac_apply(bq_lattice* lat, void* out, const void* in, double kappa, double csw, bq_prec prec,
+                                    bq_recon recon, void* stream) {
+    if (!lat) return BQ_EINVAL;
+    if (!out || !in || out == in) return bq_set_error(lat, BQ_EINVAL, "bq_dirac_apply: out/in NULL or aliased");
+    if (!valid_prec(prec) || !valid_recon(recon)) return bq_set_error(lat, BQ_EINVAL, "bq_dirac_apply: bad prec/recon");
+    if (!lat->have_gauge) return bq_set_error(lat, BQ_ENOGAUGE, "bq_dirac_apply: no gauge field loaded");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const size_t fb = field_bytes_one_parity(lat->g, prec);
+    char* o = static_cast<char*>(out);
+    const char* i = static_cast<const char*>(in);
+    // out_p = A_pp in_p - kappa H_{p,1-p} in_{1-p}
+    if (csw == 0.0) {
+        BQ_TRY(bq_hop(lat, o, i + fb, i, -kappa, 0, prec, recon, nullptr, 0, s));
+        return bq_hop(lat, o + fb, i, i + fb, -kappa, 1, prec, recon, nullptr, 0, s);
+    }
+    BQ_TRY(bq_clover_build(lat, csw, kappa));
+    const void* cl = nullptr;
+    BQ_TRY(bq_get_clover(lat, prec, 0, &cl));
+    const size_t cb = (size_t)lat->g.Vh * CLOVER_REALS * prec_real_bytes(prec);
+    BQ_TRY(bq_hop(lat, o, i + fb, i, -kappa, 0, prec, recon, cl, 2, s));
+    return bq_hop(lat, o + fb, i, i + fb, -kappa, 1, prec, recon, static_cast<const char*>(cl) + cb, 2, s);
+}
+
+extern "C" bq_status bq_schur_apply(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw,
+                                    bq_prec prec, bq_recon recon, void* stream) {
+    if (!lat) return BQ_EINVAL;
+    if (!out || !in || !tmp || out == in || tmp == in || tmp == out)
+        return bq_set_error(lat, BQ_EINVAL, "bq_schur_apply: NULL or aliased buffers");
+    if (!valid_prec(prec) || !valid_recon(recon)) return bq_set_error(lat, BQ_EINVAL, "bq_schur_apply: bad prec/recon");
+    if (!lat->have_gauge) return bq_set_error(lat, BQ_ENOGAUGE, "bq_schur_apply: no gauge field loaded");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (csw == 0.0) {
+        // tmp_o = -kappa H_oe in_e ;  out_e = in_e + kappa H_eo tmp_o = in_e - kappa^2 H_eo H_oe in_e
+        BQ_TRY(bq_hop(lat, tmp, in, nullptr, -kappa, 1, prec, recon, nullptr, 0, s));
+        return bq_hop(lat, out, tmp, in, kappa, 0, prec, recon, nullptr, 0, s);
+    }
+    BQ_TRY(bq_clover_build(lat, csw, kappa));
+    const void *cl = nullptr, *cli = nullptr;
+    BQ_TRY(bq_get_clover(lat, prec, 0, &cl));
+    BQ_TRY(bq_get_clover(lat, prec, 1, &cli));
+    const size_t cb = (size_t)lat->g.Vh * CLOVER_REALS * prec_real_bytes(prec);
+    // tmp_o = -kappa A_oo^-1 H_oe in_e ;  out_e = A_ee in_e + kappa H_eo tmp_o
+    BQ_TRY(bq_hop(lat, tmp, in, nullptr, -kappa, 1, prec, recon, static_cast<const char*>(cli) + cb, 1, s));
+    return bq_hop(lat, out, tmp, in, kappa, 0, prec, recon, cl, 2, s);
+}

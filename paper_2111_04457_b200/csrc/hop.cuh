@@ -1,0 +1,93 @@
+// hop.cuh — per-site arithmetic of the hopping term of Eq. 1:
+//   (H in)(x) = sum_mu [ (1 - g_mu) U_mu(x) in(x+mu) + (1 + g_mu) U_mu(x-mu)^dag in(x-mu) ]
+// with the spin projection fused into the gather (Euclidean Dirac basis A.1).
+// Writing psi = (u; l), u = spins 0,1 and l = spins 2,3 (each 2 spins x 3 colours):
+//   (1 - g_k) psi = (h; -i s_k h),  h = u + i s_k l          k = x,y,z   (s_k = Pauli matrices)
+//   (1 + g_k) psi = (h; +i s_k h),  h = u - i s_k l
+//   (1 - g_t) psi = (0; 2 l),       (1 + g_t) psi = (2 u; 0)
+// so only the 2-spin h is multiplied by the link: 8 x (12 + 132) + 168 = 1320 flop per site.
+// Index convention of every register array: [2*(3*spin + colour) + reim].
+#pragma once
+
+#include "layout.cuh"
+
+// i*s_k applied to a two-spin object (a0, a1) (3 colours each), result added with sign SGN into (r0, r1):
+//   i s_x (a0,a1) = ( i a1,  i a0);   i s_y (a0,a1) = ( a1, -a0);   i s_z (a0,a1) = ( i a0, -i a1)
+// r += SGN * (i s_k a).   a, r: 12 reals [2*(3*s + c) + reim].
+template <int K, int SGN, typename C> __device__ __forceinline__ void add_isigma(C* r, const C* a) {
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const C a0r = a[2 * c], a0i = a[2 * c + 1], a1r = a[6 + 2 * c], a1i = a[6 + 2 * c + 1];
+        if (K == 0) {         // ( i a1, i a0 ):  i*(x+iy) = -y + ix
+            r[2 * c] += SGN * (-a1i);      r[2 * c + 1] += SGN * a1r;
+            r[6 + 2 * c] += SGN * (-a0i);  r[6 + 2 * c + 1] += SGN * a0r;
+        } else if (K == 1) {  // ( a1, -a0 )
+            r[2 * c] += SGN * a1r;         r[2 * c + 1] += SGN * a1i;
+            r[6 + 2 * c] += SGN * (-a0r);  r[6 + 2 * c + 1] += SGN * (-a0i);
+        } else {              // ( i a0, -i a1 )
+            r[2 * c] += SGN * (-a0i);      r[2 * c + 1] += SGN * a0r;
+            r[6 + 2 * c] += SGN * a1i;     r[6 + 2 * c + 1] += SGN * (-a1r);
+        }
+    }
+}
+
+// chi = U h  (FWD) or U^dagger h (backward) for both spins of the half spinor.  66 flop per spin.
+template <bool DAG, typename C> __device__ __forceinline__ void su3_mul(const C* u, const C* h, C* chi) {
+#pragma unroll
+    for (int s = 0; s < 2; s++)
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            C re = 0, im = 0;
+#pragma unroll
+            for (int b = 0; b < 3; b++) {
+                const C ur = DAG ? u[2 * (3 * b + a)] : u[2 * (3 * a + b)];
+                const C ui = DAG ? -u[2 * (3 * b + a) + 1] : u[2 * (3 * a + b) + 1];
+                const C hr = h[6 * s + 2 * b], hi = h[6 * s + 2 * b + 1];
+                re += ur * hr - ui * hi;
+                im += ur * hi + ui * hr;
+            }
+            chi[6 * s + 2 * a] = re;
+            chi[6 * s + 2 * a + 1] = im;
+        }
+}
+
+template <typename C> __device__ __forceinline__ void phase_mul(C* chi, C pr, C pi) {
+#pragma unroll
+    for (int k = 0; k < 6; k++) {
+        const C r = chi[2 * k], i = chi[2 * k + 1];
+        chi[2 * k] = pr * r - pi * i;
+        chi[2 * k + 1] = pr * i + pi * r;
+    }
+}
+
+// One of the 8 hops.  MU = 0..3, FWD = true: (1 - g_mu) U_mu(x) in(x+mu); false: (1 + g_mu) U_mu(x-mu)^dag in(x-mu).
+//   in     : input spinor field (parity 1-p), nh = half index of the neighbour
+//   ublock : (parity, MU) block of the gauge store; uidx = h (forward: the link lives on x) or nh (backward: on x-mu)
+//   wrap   : this hop crosses the lattice boundary -> multiply by (pr, pi) (phi_mu forward, conj(phi_mu) backward)
+template <int PREC, int RECON, int MU, bool FWD>
+__device__ __forceinline__ void hop_dir(typename Prec<PREC>::comp* acc, const void* in, int Vh, int nh, const void* ublock,
+                                        int uidx, bool wrap, typename Prec<PREC>::comp pr, typename Prec<PREC>::comp pi) {
+    using C = typename Prec<PREC>::comp;
+    C h[12], u[18], chi[12];
+    if (MU < 3) {
+        C psi[24];
+        load_spinor<PREC>(in, Vh, nh, psi);
+#pragma unroll
+        for (int i = 0; i < 12; i++) h[i] = psi[i];           // u
+        add_isigma<MU, FWD ? +1 : -1>(h, psi + 12);           // h = u +- i s_k l
+    } else {
+        // (1 - g_t) psi = (0; 2l): forward needs l only; (1 + g_t) psi = (2u; 0): backward needs u only
+        load_spinor_half<PREC, FWD ? 1 : 0>(in, Vh, nh, h);
+    }
+    load_link<PREC, RECON>(ublock, Vh, uidx, u);
+    su3_mul<!FWD>(u, h, chi);
+    if (wrap) phase_mul(chi, pr, pi);
+    if (MU < 3) {
+#pragma unroll
+        for (int i = 0; i < 12; i++) acc[i] += chi[i];        // upper two spins: h
+        add_isigma<MU, FWD ? -1 : +1>(acc + 12, chi);         // lower two spins: -+ i s_k h
+    } else {
+#pragma unroll
+        for (int i = 0; i < 12; i++) acc[(FWD ? 12 : 0) + i] += 2 * chi[i];
+    }
+}

@@ -1,0 +1,206 @@
+// layout.cuh — device-side access to the even-odd SoA stores (include/bq.h "Internal field layout").
+//
+// A field over Vh sites is a sequence of 16-byte planes: plane k holds, for every half index h, reals
+// [k*W, (k+1)*W) of the site (W = 16/sizeof(real)), so that a warp touches 32 x 16 contiguous bytes per load
+// (the B200 analogue of the paper's "coalesced" GPU layout, and of its SoA vector layout,
+// PAPER.md:99).  Leftover reals (18 = 4*4+2 floats, 18 = 2*8+2 halfs, 12 = 8+4 halfs) live in a narrower
+// trailing plane.  Half-precision spinors carry a trailing fp32 plane with the per-site norm (reading S11).
+#pragma once
+
+#include "bq_internal.h"
+
+template <int PREC> struct Prec;
+template <> struct Prec<BQ_FP64> { using real = double; using comp = double; };
+template <> struct Prec<BQ_FP32> { using real = float; using comp = float; };
+template <> struct Prec<BQ_HALF> { using real = __half; using comp = float; };
+
+// ---- raw loads with a cache policy: default = plain ld.global (L1-cached, normal L2 policy: spinors, of which
+// every site is read by 8 neighbours and must survive in L2); STREAM = ld.global.cs, evict-first streaming
+// (links, clover blocks, BLAS operands: read exactly once).  Both are coherent loads, so a kernel may read and
+// then overwrite the same element (in-place updates) without touching the non-coherent path. ----
+template <bool STREAM, typename V> __device__ __forceinline__ V ld16(const void* p) {
+    if (STREAM) return __ldcs(reinterpret_cast<const V*>(p));
+    return *reinterpret_cast<const V*>(p);
+}
+
+__device__ __forceinline__ void unpack8(const uint4& q, float* f) {
+    const __half2* h = reinterpret_cast<const __half2*>(&q);
+#pragma unroll
+    for (int i = 0; i < 4; i++) {
+        float2 t = __half22float2(h[i]);
+        f[2 * i] = t.x;
+        f[2 * i + 1] = t.y;
+    }
+}
+__device__ __forceinline__ void unpack4(const uint2& q, float* f) {
+    const __half2* h = reinterpret_cast<const __half2*>(&q);
+#pragma unroll
+    for (int i = 0; i < 2; i++) {
+        float2 t = __half22float2(h[i]);
+        f[2 * i] = t.x;
+        f[2 * i + 1] = t.y;
+    }
+}
+__device__ __forceinline__ uint4 pack8(const float* f) {
+    uint4 q;
+    __half2* h = reinterpret_cast<__half2*>(&q);
+#pragma unroll
+    for (int i = 0; i < 4; i++) h[i] = __floats2half2_rn(f[2 * i], f[2 * i + 1]);
+    return q;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Spinor: 24 reals, index 2*(3*spin + colour) + (0 = re, 1 = im)
+// ---------------------------------------------------------------------------------------------------
+template <int PREC, bool STREAM = false>
+__device__ __forceinline__ void load_spinor(const void* base, int Vh, int h, typename Prec<PREC>::comp* v) {
+    const char* b = static_cast<const char*>(base);
+    if constexpr (PREC == BQ_FP64) {
+#pragma unroll
+        for (int k = 0; k < 12; k++) {
+            double2 d = ld16<STREAM, double2>(b + ((size_t)k * Vh + h) * 16);
+            v[2 * k] = d.x;
+            v[2 * k + 1] = d.y;
+        }
+    } else if constexpr (PREC == BQ_FP32) {
+#pragma unroll
+        for (int k = 0; k < 6; k++) {
+            float4 d = ld16<STREAM, float4>(b + ((size_t)k * Vh + h) * 16);
+            v[4 * k] = d.x; v[4 * k + 1] = d.y; v[4 * k + 2] = d.z; v[4 * k + 3] = d.w;
+        }
+    } else {
+        uint4 q[3];
+#pragma unroll
+        for (int k = 0; k < 3; k++) q[k] = ld16<STREAM, uint4>(b + ((size_t)k * Vh + h) * 16);
+        float n = ld16<STREAM, float>(b + (size_t)3 * Vh * 16 + (size_t)h * 4);
+#pragma unroll
+        for (int k = 0; k < 3; k++) unpack8(q[k], v + 8 * k);
+#pragma unroll
+        for (int i = 0; i < 24; i++) v[i] *= n;
+    }
+}
+
+// Upper (W = 0: spins 0,1) or lower (W = 1: spins 2,3) half of a spinor, 12 reals — all the t-direction
+// projectors (1 -+ gamma_4) need.
+template <int PREC, int W>
+__device__ __forceinline__ void load_spinor_half(const void* base, int Vh, int h, typename Prec<PREC>::comp* v) {
+    const char* b = static_cast<const char*>(base);
+    if constexpr (PREC == BQ_FP64) {
+#pragma unroll
+        for (int k = 0; k < 6; k++) {
+            double2 d = ld16<false, double2>(b + ((size_t)(6 * W + k) * Vh + h) * 16);
+            v[2 * k] = d.x;
+            v[2 * k + 1] = d.y;
+        }
+    } else if constexpr (PREC == BQ_FP32) {
+#pragma unroll
+        for (int k = 0; k < 3; k++) {
+            float4 d = ld16<false, float4>(b + ((size_t)(3 * W + k) * Vh + h) * 16);
+            v[4 * k] = d.x; v[4 * k + 1] = d.y; v[4 * k + 2] = d.z; v[4 * k + 3] = d.w;
+        }
+    } else {
+        // reals 0..11 = plane 0 + low 8 bytes of plane 1; reals 12..23 = high 8 bytes of plane 1 + plane 2
+        uint4 q = ld16<false, uint4>(b + ((size_t)(W ? 2 : 0) * Vh + h) * 16);
+        uint2 d = ld16<false, uint2>(b + ((size_t)1 * Vh + h) * 16 + (W ? 8 : 0));
+        float n = ld16<false, float>(b + (size_t)3 * Vh * 16 + (size_t)h * 4);
+        if (W == 0) { unpack8(q, v); unpack4(d, v + 8); }
+        else { unpack4(d, v); unpack8(q, v + 4); }
+#pragma unroll
+        for (int i = 0; i < 12; i++) v[i] *= n;
+    }
+}
+
+template <int PREC, bool STREAM = false>
+__device__ __forceinline__ void store_spinor(void* base, int Vh, int h, const typename Prec<PREC>::comp* v) {
+    char* b = static_cast<char*>(base);
+    if constexpr (PREC == BQ_FP64) {
+#pragma unroll
+        for (int k = 0; k < 12; k++) {
+            double2 d = make_double2(v[2 * k], v[2 * k + 1]);
+            double2* p = reinterpret_cast<double2*>(b + ((size_t)k * Vh + h) * 16);
+            if (STREAM) __stcs(p, d); else *p = d;
+        }
+    } else if constexpr (PREC == BQ_FP32) {
+#pragma unroll
+        for (int k = 0; k < 6; k++) {
+            float4 d = make_float4(v[4 * k], v[4 * k + 1], v[4 * k + 2], v[4 * k + 3]);
+            float4* p = reinterpret_cast<float4*>(b + ((size_t)k * Vh + h) * 16);
+            if (STREAM) __stcs(p, d); else *p = d;
+        }
+    } else {
+        // reading S11: n = max_i |v_i| (fp32); mantissas fp16(v_i / n); zero site -> n = 0, mantissas 0
+        float n = 0.f;
+#pragma unroll
+        for (int i = 0; i < 24; i++) n = fmaxf(n, fabsf(v[i]));
+        float inv = n > 0.f ? 1.0f / n : 0.f;
+        float m[24];
+#pragma unroll
+        for (int i = 0; i < 24; i++) m[i] = v[i] * inv;
+#pragma unroll
+        for (int k = 0; k < 3; k++) {
+            uint4* p = reinterpret_cast<uint4*>(b + ((size_t)k * Vh + h) * 16);
+            uint4 q = pack8(m + 8 * k);
+            if (STREAM) __stcs(p, q); else *p = q;
+        }
+        float* pn = reinterpret_cast<float*>(b + (size_t)3 * Vh * 16 + (size_t)h * 4);
+        if (STREAM) __stcs(pn, n); else *pn = n;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Link: u[2*(3*row + col) + reim], 18 reals; RECON12 stores rows 0,1 and rebuilds row 2 = conj(row0 x row1).
+// `base` points at the (parity, mu) block of the gauge store.
+// ---------------------------------------------------------------------------------------------------
+__host__ __device__ constexpr size_t link_block_bytes(int prec, int recon, int Vh) {
+    return (size_t)link_reals(recon) * prec_real_bytes(prec) * (size_t)Vh;
+}
+
+template <typename C> __device__ __forceinline__ void reconstruct_row2(C* u) {
+    // row2_j = conj(row0_a row1_b - row0_b row1_a), (a, b) = (j+1, j+2) mod 3
+#pragma unroll
+    for (int j = 0; j < 3; j++) {
+        const int a = (j + 1) % 3, b = (j + 2) % 3;
+        C re = (u[2 * a] * u[6 + 2 * b] - u[2 * a + 1] * u[6 + 2 * b + 1]) - (u[2 * b] * u[6 + 2 * a] - u[2 * b + 1] * u[6 + 2 * a + 1]);
+        C im = (u[2 * a] * u[6 + 2 * b + 1] + u[2 * a + 1] * u[6 + 2 * b]) - (u[2 * b] * u[6 + 2 * a + 1] + u[2 * b + 1] * u[6 + 2 * a]);
+        u[12 + 2 * j] = re;
+        u[12 + 2 * j + 1] = -im;
+    }
+}
+
+template <int PREC, int RECON, bool STREAM = true>
+__device__ __forceinline__ void load_link(const void* base, int Vh, int idx, typename Prec<PREC>::comp* u) {
+    const char* b = static_cast<const char*>(base);
+    constexpr int NR = (RECON == BQ_RECON12) ? 12 : 18;
+    if constexpr (PREC == BQ_FP64) {
+#pragma unroll
+        for (int k = 0; k < NR / 2; k++) {
+            double2 d = ld16<STREAM, double2>(b + ((size_t)k * Vh + idx) * 16);
+            u[2 * k] = d.x;
+            u[2 * k + 1] = d.y;
+        }
+    } else if constexpr (PREC == BQ_FP32) {
+#pragma unroll
+        for (int k = 0; k < NR / 4; k++) {
+            float4 d = ld16<STREAM, float4>(b + ((size_t)k * Vh + idx) * 16);
+            u[4 * k] = d.x; u[4 * k + 1] = d.y; u[4 * k + 2] = d.z; u[4 * k + 3] = d.w;
+        }
+        if constexpr (NR == 18) {
+            float2 d = ld16<STREAM, float2>(b + (size_t)4 * Vh * 16 + (size_t)idx * 8);
+            u[16] = d.x; u[17] = d.y;
+        }
+    } else {
+        if constexpr (NR == 18) {
+            uint4 q0 = ld16<STREAM, uint4>(b + ((size_t)0 * Vh + idx) * 16);
+            uint4 q1 = ld16<STREAM, uint4>(b + ((size_t)1 * Vh + idx) * 16);
+            unsigned int r = ld16<STREAM, unsigned int>(b + (size_t)2 * Vh * 16 + (size_t)idx * 4);
+            unpack8(q0, u); unpack8(q1, u + 8);
+            float2 t = __half22float2(*reinterpret_cast<const __half2*>(&r));
+            u[16] = t.x; u[17] = t.y;
+        } else {
+            uint4 q0 = ld16<STREAM, uint4>(b + ((size_t)0 * Vh + idx) * 16);
+            uint2 d = ld16<STREAM, uint2>(b + (size_t)1 * Vh * 16 + (size_t)idx * 8);
+            unpack8(q0, u); unpack4(d, u + 8);
+        }
+    }
+    if constexpr (NR == 12) reconstruct_row2(u);
+}

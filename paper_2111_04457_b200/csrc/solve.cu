@@ -1,0 +1,347 @@
+// solve.cu — bq_solve: even-odd preconditioned BiCGStab with a mixed-precision defect-correction outer loop
+// (the paper's `invert(x, b, nconv, diff)` of a "mixed precision solver").
+//
+//   b^_e = b_e + kappa H_eo A_oo^-1 b_o                                  (A10, fp64)
+//   outer:  r = b^_e - M^ x_e (fp64) ; stop if |r| <= tol |b| ; r_lo = convert(r/|r|)          (A9)
+//           inner BiCGStab  M^ e = r_lo  in fp64 / fp32 / half storage, e0 = 0               (A8)
+//           x_e += |r| e
+//   x_o = A_oo^-1 (b_o + kappa H_oe x_e)                                 (A10, fp64)
+//   M^ = A_ee - kappa^2 H_eo A_oo^-1 H_oe                                (A7; A = 1 for Wilson)
+//
+// All BiCGStab scalars live in device memory (SolverScalars) and are produced by the reduction kernels'
+// finalisers; the host only polls the {done, iters, r2} triple every `check_every` iterations.
+#include <math.h>
+#include <stdlib.h>
+
+#include "blas.cuh"
+#include "blas_api.h"
+
+struct SolverWork {
+    BlasCtx blas;
+    bool blas_ok;
+    // fp64, full lattice [even | odd]
+    void *b, *x;
+    // fp64, one parity
+    void *bhat, *r, *t, *tmp;
+    // inner precision, one parity
+    int inner_prec;
+    void *irhat, *ir, *ip, *iv, *is, *it, *itmp, *ie;
+    SolverScalars* h_sc;   // pinned host mirror
+    cudaEvent_t ev0, ev1;
+};
+
+static void free_inner(SolverWork* w) {
+    void** v[] = {&w->irhat, &w->ir, &w->ip, &w->iv, &w->is, &w->it, &w->itmp, &w->ie};
+    for (void** p : v) {
+        if (*p) cudaFree(*p);
+        *p = nullptr;
+    }
+    w->inner_prec = -1;
+}
+
+void bq_solver_free(bq_lattice* lat) {
+    SolverWork* w = lat->work;
+    if (!w) return;
+    free_inner(w);
+    void** v[] = {&w->b, &w->x, &w->bhat, &w->r, &w->t, &w->tmp};
+    for (void** p : v) {
+        if (*p) cudaFree(*p);
+        *p = nullptr;
+    }
+    if (w->blas_ok) blas_ctx_destroy(&w->blas);
+    if (w->h_sc) cudaFreeHost(w->h_sc);
+    if (w->ev0) cudaEventDestroy(w->ev0);
+    if (w->ev1) cudaEventDestroy(w->ev1);
+    free(w);
+    lat->work = nullptr;
+}
+
+static bq_status get_work(bq_lattice* lat, int inner_prec, SolverWork** out) {
+    const Geom& g = lat->g;
+    if (!lat->work) {
+        SolverWork* w = static_cast<SolverWork*>(calloc(1, sizeof(SolverWork)));
+        if (!w) return bq_set_error(lat, BQ_ENOMEM, "solver workspace: host allocation failed");
+        w->inner_prec = -1;
+        lat->work = w;
+        BQ_TRY(blas_ctx_create(lat, &w->blas));
+        w->blas_ok = true;
+        const size_t fb = field_bytes_one_parity(g, BQ_FP64);
+        BQ_CUDA(lat, cudaMalloc(&w->b, 2 * fb));
+        BQ_CUDA(lat, cudaMalloc(&w->x, 2 * fb));
+        BQ_CUDA(lat, cudaMalloc(&w->bhat, fb));
+        BQ_CUDA(lat, cudaMalloc(&w->r, fb));
+        BQ_CUDA(lat, cudaMalloc(&w->t, fb));
+        BQ_CUDA(lat, cudaMalloc(&w->tmp, fb));
+        BQ_CUDA(lat, cudaMallocHost(&w->h_sc, sizeof(SolverScalars)));
+        BQ_CUDA(lat, cudaEventCreate(&w->ev0));
+        BQ_CUDA(lat, cudaEventCreate(&w->ev1));
+    }
+    SolverWork* w = lat->work;
+    if (w->inner_prec != inner_prec) {
+        free_inner(w);
+        const size_t fb = field_bytes_one_parity(g, inner_prec);
+        void** v[] = {&w->irhat, &w->ir, &w->ip, &w->iv, &w->is, &w->it, &w->itmp};
+        for (void** p : v) BQ_CUDA(lat, cudaMalloc(p, fb));
+        // solution accumulator of the inner solve: fp32 when the inner storage is half
+        BQ_CUDA(lat, cudaMalloc(&w->ie, field_bytes_one_parity(g, inner_prec == BQ_HALF ? BQ_FP32 : inner_prec)));
+        w->inner_prec = inner_prec;
+    }
+    *out = w;
+    return BQ_OK;
+}
+
+// out_e = M^ in_e in precision prec (tmp: odd scratch)
+static bq_status schur(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw, int prec, int recon,
+                       cudaStream_t s) {
+    return bq_schur_apply(lat, out, in, tmp, kappa, csw, (bq_prec)prec, (bq_recon)recon, s);
+}
+
+static bq_status poll(bq_lattice* lat, SolverWork* w) {
+    BQ_CUDA(lat, cudaMemcpyAsync(w->h_sc, w->blas.sc, sizeof(SolverScalars), cudaMemcpyDeviceToHost, w->blas.stream));
+    BQ_CUDA(lat, cudaStreamSynchronize(w->blas.stream));
+    return BQ_OK;
+}
+
+// Inner BiCGStab on M^ e = ir (e0 = 0), stop when |r|^2 <= stop2 or after max_iter iterations.
+// On return w->h_sc holds the final device state.  Textbook van der Vorst recurrences (reading O4).
+static bq_status inner_bicgstab(bq_lattice* lat, SolverWork* w, double kappa, double csw, int prec, int recon, double stop2,
+                                int max_iter, int check_every) {
+    const BlasCtx& c = w->blas;
+    cudaStream_t s = c.stream;
+    const size_t fb = field_bytes_one_parity(lat->g, prec);
+    const size_t eb = field_bytes_one_parity(lat->g, prec == BQ_HALF ? BQ_FP32 : prec);
+    BQ_CUDA(lat, cudaMemsetAsync(w->ie, 0, eb, s));
+    BQ_CUDA(lat, cudaMemsetAsync(w->ip, 0, fb, s));
+    BQ_CUDA(lat, cudaMemsetAsync(w->iv, 0, fb, s));
+    BQ_CUDA(lat, cudaMemcpyAsync(w->irhat, w->ir, fb, cudaMemcpyDeviceToDevice, s));
+    BQ_TRY(bicg_init(lat, c, prec, w->ir, stop2));
+    int launched = 0;
+    for (;;) {
+        const int batch = (max_iter - launched) < check_every ? (max_iter - launched) : check_every;
+        for (int k = 0; k < batch; k++) {
+            BQ_TRY(bicg_p_update(lat, c, prec, w->ir, w->ip, w->iv));                    // p = r + beta (p - omega v)
+            BQ_TRY(schur(lat, w->iv, w->ip, w->itmp, kappa, csw, prec, recon, s));       // v = M^ p
+            BQ_TRY(bicg_alpha(lat, c, prec, w->irhat, w->iv));                           // alpha = rho / <rhat, v>
+            BQ_TRY(bicg_s_update(lat, c, prec, w->ir, w->iv, w->is));                    // s = r - alpha v
+            BQ_TRY(schur(lat, w->it, w->is, w->itmp, kappa, csw, prec, recon, s));       // t = M^ s
+            BQ_TRY(bicg_omega(lat, c, prec, w->it, w->is));                              // omega = <t,s>/<t,t>
+            BQ_TRY(bicg_final(lat, c, prec, w->ip, w->is, w->it, w->irhat, w->ie, w->ir));
+        }
+        launched += batch;
+        BQ_TRY(poll(lat, w));
+        if (w->h_sc->done || launched >= max_iter) break;
+    }
+    return BQ_OK;
+}
+
+extern "C" bq_status bq_solve(bq_lattice* lat, const double* b, double* x, double kappa, double tol, const bq_solve_opts* opts,
+                              bq_solve_info* info) {
+    if (!lat) return BQ_EINVAL;
+    if (info) {
+        info->status = BQ_EINVAL; info->outer_cycles = 0; info->inner_iters = 0; info->restarts = 0;
+        info->true_rel_residual = NAN; info->seconds = 0;
+    }
+    if (!b || !x) return bq_set_error(lat, BQ_EINVAL, "bq_solve: b or x is NULL");
+    if (!(tol > 0.0) || !isfinite(tol)) return bq_set_error(lat, BQ_EINVAL, "bq_solve: tol must be positive");
+    if (!lat->have_gauge) return bq_set_error(lat, BQ_ENOGAUGE, "bq_solve: no gauge field loaded");
+    bq_solve_opts o;
+    if (opts) o = *opts;
+    else { o.inner_prec = BQ_FP32; o.recon = BQ_RECON18; o.csw = 0; o.inner_tol = 0; o.max_inner = 0; o.max_outer = 0; o.check_every = 0; o.stream = nullptr; }
+    if (o.inner_prec != BQ_FP64 && o.inner_prec != BQ_FP32 && o.inner_prec != BQ_HALF) return bq_set_error(lat, BQ_EINVAL, "bq_solve: bad inner_prec");
+    if (o.recon != BQ_RECON18 && o.recon != BQ_RECON12) return bq_set_error(lat, BQ_EINVAL, "bq_solve: bad recon");
+    if (o.stream) return bq_set_error(lat, BQ_EINVAL, "bq_solve: opts->stream must be NULL");
+    const int prec = o.inner_prec;
+    const double inner_tol = o.inner_tol > 0 ? o.inner_tol : (prec == BQ_HALF ? 5e-2 : 1e-5);
+    const int max_inner = o.max_inner > 0 ? o.max_inner : (prec == BQ_HALF ? 100 : 1000);
+    const int max_outer = o.max_outer > 0 ? o.max_outer : 50;
+    const int check_every = o.check_every > 0 ? o.check_every : 8;
+    const double csw = o.csw;
+    const bool clover = csw != 0.0;
+
+    SolverWork* w = nullptr;
+    BQ_TRY(get_work(lat, prec, &w));
+    const BlasCtx& c = w->blas;
+    cudaStream_t s = c.stream;
+    const Geom& g = lat->g;
+    const size_t fb64 = field_bytes_one_parity(g, BQ_FP64);
+    char* bb = static_cast<char*>(w->b);
+    char* xx = static_cast<char*>(w->x);
+    const void *cl64 = nullptr, *cli64 = nullptr;
+    const size_t cb64 = (size_t)g.Vh * CLOVER_REALS * sizeof(double);
+    if (clover) {
+        BQ_TRY(bq_clover_build(lat, csw, kappa));
+        BQ_TRY(bq_get_clover(lat, BQ_FP64, 0, &cl64));
+        BQ_TRY(bq_get_clover(lat, BQ_FP64, 1, &cli64));
+    }
+
+    BQ_CUDA(lat, cudaEventRecord(w->ev0, s));
+    // ---- import b and x0 (canonical, host or device) through a device staging buffer ----
+    {
+        const size_t nb = (size_t)g.V * 24 * sizeof(double);
+        double* stage = nullptr;
+        BQ_CUDA(lat, cudaMalloc(&stage, nb));
+        cudaError_t e = cudaMemcpyAsync(stage, b, nb, cudaMemcpyDefault, s);
+        bq_status st = BQ_OK;
+        if (e == cudaSuccess) st = bq_field_import(lat, w->b, stage, BQ_FULL, BQ_FP64, s);
+        if (e == cudaSuccess && st == BQ_OK) e = cudaMemcpyAsync(stage, x, nb, cudaMemcpyDefault, s);
+        if (e == cudaSuccess && st == BQ_OK) st = bq_field_import(lat, w->x, stage, BQ_FULL, BQ_FP64, s);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        cudaFree(stage);
+        if (e != cudaSuccess) return bq_set_error(lat, BQ_ECUDA, "bq_solve: import failed: %s", cudaGetErrorString(e));
+        BQ_TRY(st);
+    }
+    // |b|^2 over the full lattice (two parities)
+    double bnorm2 = 0;
+    for (int p = 0; p < 2; p++) {
+        BQ_TRY(blas_norm2(lat, c, BQ_FP64, bb + p * fb64));
+        BQ_TRY(poll(lat, w));
+        bnorm2 += w->h_sc->red[0];
+    }
+    const double bnorm = sqrt(bnorm2);
+    bq_status result = BQ_OK;
+    int outer = 0, inner_total = 0, restarts = 0;
+    if (bnorm == 0.0) {
+        BQ_CUDA(lat, cudaMemsetAsync(w->x, 0, 2 * fb64, s));
+    } else {
+        // ---- b^_e = b_e + kappa H_eo A_oo^-1 b_o ----
+        const void* bo = bb + fb64;
+        if (clover) {
+            BQ_TRY(bq_clover_mul(lat, w->tmp, bo, static_cast<const char*>(cli64) + cb64, BQ_FP64, s));
+            bo = w->tmp;
+        }
+        BQ_TRY(bq_hop(lat, w->bhat, bo, bb, kappa, 0, BQ_FP64, BQ_RECON18, nullptr, 0, s));
+        const double target = tol * bnorm;
+        double prev_rnorm = INFINITY;
+        int stalled = 0;
+        for (;;) {
+            // r = b^_e - M^ x_e in fp64
+            BQ_TRY(schur(lat, w->t, xx, w->tmp, kappa, csw, BQ_FP64, BQ_RECON18, s));
+            BQ_TRY(outer_residual(lat, c, w->bhat, w->t, w->r));
+            BQ_TRY(poll(lat, w));
+            const double rnorm = sqrt(w->h_sc->r2);
+            if (!(rnorm == rnorm)) { result = bq_set_error(lat, BQ_EBREAKDOWN, "bq_solve: residual is NaN"); break; }
+            if (rnorm <= target) break;
+            if (outer >= max_outer) { result = bq_set_error(lat, BQ_ENOTCONVERGED, "bq_solve: max_outer reached, |r|/|b| = %.3e", rnorm / bnorm); break; }
+            if (rnorm > 0.5 * prev_rnorm) {
+                if (++stalled >= 4) { result = bq_set_error(lat, BQ_ENOTCONVERGED, "bq_solve: stalled at |r|/|b| = %.3e", rnorm / bnorm); break; }
+            } else stalled = 0;
+            prev_rnorm = rnorm;
+            outer++;
+            // normalised low-precision right-hand side and inner stopping threshold
+            BQ_TRY(outer_to_low(lat, c, prec, w->r, w->ir));
+            double rel = (prec == BQ_FP64) ? 0.9 * target / rnorm : fmax(inner_tol, 0.5 * target / rnorm);
+            BQ_TRY(inner_bicgstab(lat, w, kappa, csw, prec, o.recon, rel * rel, max_inner, check_every));
+            inner_total += w->h_sc->iters;
+            if (w->h_sc->done == 2) restarts++;   // breakdown: the next outer cycle restarts from the true residual
+            if (w->h_sc->done == 2 && w->h_sc->iters == 0 && restarts > 3) {
+                result = bq_set_error(lat, BQ_EBREAKDOWN, "bq_solve: BiCGStab breakdown (rho or <rhat,v> or <t,t> = 0)");
+                break;
+            }
+            // x_e += |r| e   (|r| = sc->rnorm, written by outer_residual; the inner loop does not touch it)
+            BQ_TRY(outer_accumulate(lat, c, prec == BQ_HALF ? BQ_FP32 : prec, w->ie, xx));
+        }
+        // ---- x_o = A_oo^-1 (b_o + kappa H_oe x_e) ----
+        BQ_TRY(bq_hop(lat, xx + fb64, xx, bb + fb64, kappa, 1, BQ_FP64, BQ_RECON18, nullptr, 0, s));
+        if (clover) BQ_TRY(bq_clover_mul(lat, xx + fb64, xx + fb64, static_cast<const char*>(cli64) + cb64, BQ_FP64, s));
+    }
+    // ---- true residual |b - D x| / |b| on the full lattice, fp64 ----
+    double true_rel = 0.0;
+    if (bnorm > 0.0) {
+        // reuse: t (even) and tmp (odd) are one-parity buffers; compute per parity
+        double r2 = 0;
+        for (int p = 0; p < 2; p++) {
+            const void* clp = clover ? static_cast<const char*>(cl64) + p * cb64 : nullptr;
+            BQ_TRY(bq_hop(lat, w->t, xx + (1 - p) * fb64, xx + p * fb64, -kappa, p, BQ_FP64, BQ_RECON18, clp, clover ? 2 : 0, s));
+            BQ_TRY(outer_residual(lat, c, bb + p * fb64, w->t, w->r));
+            BQ_TRY(poll(lat, w));
+            r2 += w->h_sc->r2;
+        }
+        true_rel = sqrt(r2) / bnorm;
+    }
+    // ---- export x ----
+    {
+        const size_t nb = (size_t)g.V * 24 * sizeof(double);
+        double* stage = nullptr;
+        BQ_CUDA(lat, cudaMalloc(&stage, nb));
+        bq_status st = bq_field_export(lat, stage, w->x, BQ_FULL, BQ_FP64, s);
+        cudaError_t e = cudaSuccess;
+        if (st == BQ_OK) e = cudaMemcpyAsync(x, stage, nb, cudaMemcpyDefault, s);
+        if (e == cudaSuccess) e = cudaEventRecord(w->ev1, s);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        cudaFree(stage);
+        if (e != cudaSuccess) return bq_set_error(lat, BQ_ECUDA, "bq_solve: export failed: %s", cudaGetErrorString(e));
+        BQ_TRY(st);
+    }
+    float ms = 0;
+    cudaEventElapsedTime(&ms, w->ev0, w->ev1);
+    if (info) {
+        info->status = result;
+        info->outer_cycles = (prec == BQ_FP64) ? 0 : outer;
+        info->inner_iters = inner_total;
+        info->restarts = (prec == BQ_FP64) ? (outer > 0 ? outer - 1 : 0) + restarts : restarts;
+        info->true_rel_residual = true_rel;
+        info->seconds = ms * 1e-3;
+    }
+    return result;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// BLAS-1 test / benchmark entry points
+// ---------------------------------------------------------------------------------------------------
+static bq_status blas_entry(bq_lattice* lat, int prec, SolverWork** w) {
+    if (!lat) return BQ_EINVAL;
+    if (prec != BQ_FP64 && prec != BQ_FP32 && prec != BQ_HALF) return bq_set_error(lat, BQ_EINVAL, "bad precision");
+    return get_work(lat, lat->work && lat->work->inner_prec >= 0 ? lat->work->inner_prec : BQ_FP32, w);
+}
+
+extern "C" bq_status bq_blas_norm2(bq_lattice* lat, const void* a, bq_prec prec, double* result) {
+    SolverWork* w = nullptr;
+    BQ_TRY(blas_entry(lat, prec, &w));
+    if (!a || !result) return bq_set_error(lat, BQ_EINVAL, "bq_blas_norm2: NULL argument");
+    BQ_TRY(blas_norm2(lat, w->blas, prec, a));
+    BQ_TRY(poll(lat, w));
+    *result = w->h_sc->red[0];
+    return BQ_OK;
+}
+
+extern "C" bq_status bq_blas_cdot(bq_lattice* lat, const void* a, const void* b, bq_prec prec, double* result) {
+    SolverWork* w = nullptr;
+    BQ_TRY(blas_entry(lat, prec, &w));
+    if (!a || !b || !result) return bq_set_error(lat, BQ_EINVAL, "bq_blas_cdot: NULL argument");
+    BQ_TRY(blas_cdot(lat, w->blas, prec, a, b));
+    BQ_TRY(poll(lat, w));
+    result[0] = w->h_sc->red[0];
+    result[1] = w->h_sc->red[1];
+    return BQ_OK;
+}
+
+extern "C" bq_status bq_blas_caxpy(bq_lattice* lat, const double* alpha, const void* x, void* y, bq_prec prec) {
+    SolverWork* w = nullptr;
+    BQ_TRY(blas_entry(lat, prec, &w));
+    if (!alpha || !x || !y) return bq_set_error(lat, BQ_EINVAL, "bq_blas_caxpy: NULL argument");
+    return blas_caxpy(lat, w->blas, prec, alpha[0], alpha[1], x, y);
+}
+
+__global__ void k_set_bicg_scalars(SolverScalars* sc, double ar, double ai, double wr, double wi) {
+    sc->alpha[0] = ar; sc->alpha[1] = ai;
+    sc->omega[0] = wr; sc->omega[1] = wi;
+    sc->rho[0] = 1; sc->rho[1] = 0;
+    sc->done = 0; sc->iters = 0; sc->stop2 = 0;
+}
+
+extern "C" bq_status bq_blas_bicg_update(bq_lattice* lat, const double* alpha, const double* omega, const void* p, const void* s,
+                                         const void* t, const void* rhat, void* x, void* r, bq_prec prec, double* r_norm2,
+                                         double* rhat_r) {
+    SolverWork* w = nullptr;
+    BQ_TRY(blas_entry(lat, prec, &w));
+    if (!alpha || !omega || !p || !s || !t || !rhat || !x || !r || !r_norm2 || !rhat_r)
+        return bq_set_error(lat, BQ_EINVAL, "bq_blas_bicg_update: NULL argument");
+    k_set_bicg_scalars<<<1, 1, 0, w->blas.stream>>>(w->blas.sc, alpha[0], alpha[1], omega[0], omega[1]);
+    BQ_CUDA(lat, cudaGetLastError());
+    BQ_TRY(bicg_final(lat, w->blas, prec, p, s, t, rhat, x, r));
+    BQ_TRY(poll(lat, w));
+    *r_norm2 = w->h_sc->r2;
+    rhat_r[0] = w->h_sc->rho[0];
+    rhat_r[1] = w->h_sc->rho[1];
+    return BQ_OK;
+}

@@ -1,0 +1,75 @@
+"""C-ABI library checks that need no GPU: libbq.so builds, loads and exports every symbol include/bq.h declares;
+argument validation that happens before any device work; no silent CPU fallback."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def bq():
+    from paper_2111_04457_b200 import build
+    build.build()
+    from paper_2111_04457_b200 import bq as _bq
+    return _bq
+
+
+def declared_symbols():
+    with open(os.path.join(ROOT, "include", "bq.h")) as f:
+        text = re.sub(r"/\*.*?\*/", "", f.read(), flags=re.S)
+    return sorted(set(re.findall(r"\b(bq_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_every_declared_symbol_is_exported(bq):
+    lib = bq.lib()
+    names = declared_symbols()
+    assert set(names) == set(bq.EXPORTS), "binding and header disagree"
+    for n in names:
+        assert hasattr(lib, n), f"libbq.so does not export {n}"
+
+
+def test_struct_layouts_match_header(bq):
+    assert ctypes.sizeof(bq.bq_solve_opts) == 48
+    assert ctypes.sizeof(bq.bq_solve_info) == 32
+
+
+def test_status_strings(bq):
+    lib = bq.lib()
+    seen = {lib.bq_status_string(s).decode() for s in range(10)}
+    assert len(seen) == 10 and "unknown status" not in seen
+
+
+def test_extent_and_phase_validation_precede_device_work(bq):
+    for L in ((3, 4, 4, 4), (4, 4, 4, 5), (0, 4, 4, 4), (4, 1, 4, 4)):
+        with pytest.raises(bq.BqError) as e:
+            bq.bq_lattice_create(*L)
+        assert e.value.status == bq.BQ_EODD_EXTENT
+    with pytest.raises(bq.BqError) as e:
+        bq.bq_lattice_create(4, 4, 4, 4, [1, 1, 1, 0.5])       # |phase| != 1
+    assert e.value.status == bq.BQ_EINVAL
+    with pytest.raises(bq.BqError) as e:
+        bq.bq_lattice_create(2048, 2048, 1024, 2)               # V >= 2^31
+    assert e.value.status == bq.BQ_EINVAL
+
+
+def test_no_cpu_fallback(bq):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a device is present")
+    with pytest.raises(bq.BqError) as e:
+        bq.bq_lattice_create(4, 4, 4, 4)
+    assert e.value.status == bq.BQ_ECUDA
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_2111_04457_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h", ".c")):
+                with open(os.path.join(dirpath, f)) as fh:
+                    src = fh.read()
+                assert "oracle" not in src.replace("the oracle", "").replace("oracle/", "").replace("CPU oracle", "").replace(
+                    "oracle's", ""), f"{f} mentions the oracle module"

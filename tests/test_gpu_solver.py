@@ -1,0 +1,170 @@
+"""GPU parity for the fused BLAS-1 kernels (A6) and bq_solve (A7-A10) against numpy / the CPU oracle.
+
+Solves: any x with true residual |b - D x|/|b| <= tol is correct; the residual is recomputed
+here with the ORACLE's operator, never trusted from the library.  Iteration counts are reported, not matched.
+"""
+import numpy as np
+import pytest
+
+from oracle import bqo
+from paper_2111_04457_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def bq():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_2111_04457_b200 import bq as _bq
+    _bq.lib()
+    return _bq
+
+
+def even_part(L, psi):
+    return np.where((inputs.site_parity(L) == 0)[..., None, None], psi, 0)
+
+
+# storage rounding of the operands, then sums of ~N products: tolerances relative to |a||b|
+BLAS_TOL = {0: 1e-13, 1: 2e-6, 2: 2e-3}
+
+
+@pytest.mark.parametrize("prec", [0, 1, 2])
+@pytest.mark.parametrize("L", [(4, 4, 4, 4), (8, 6, 6, 10)])
+def test_blas_reductions_and_axpy(bq, prec, L):
+    a = even_part(L, inputs.spinor(L, 41))
+    b = even_part(L, inputs.spinor(L, 42, inputs.STREAM_TEST))
+    with bq.Lattice(L) as lat:
+        da, db = lat.import_field(a, prec, bq.BQ_EVEN), lat.import_field(b, prec, bq.BQ_EVEN)
+        # compare against numpy on the values as stored (export = exact view of the stored numbers)
+        sa, sb = lat.export_field(da, prec, bq.BQ_EVEN), lat.export_field(db, prec, bq.BQ_EVEN)
+        n2 = bq.bq_blas_norm2(lat.h, da, prec)
+        assert abs(n2 - np.vdot(sa, sa).real) <= 1e-6 * n2 if prec else abs(n2 - np.vdot(sa, sa).real) <= 1e-13 * n2
+        assert abs(n2 - np.vdot(a, a).real) <= 2 * BLAS_TOL[prec] * n2 + 1e-13 * n2
+        dot = bq.bq_blas_cdot(lat.h, da, db, prec)
+        scale = np.linalg.norm(a) * np.linalg.norm(b)
+        assert abs(dot - np.vdot(sa, sb)) <= (1e-6 if prec else 1e-13) * scale
+        assert abs(dot - np.vdot(a, b)) <= BLAS_TOL[prec] * scale
+        # bitwise reproducible reductions
+        assert bq.bq_blas_cdot(lat.h, da, db, prec) == dot and bq.bq_blas_norm2(lat.h, da, prec) == n2
+        alpha = 0.3 - 0.7j
+        bq.bq_blas_caxpy(lat.h, alpha, da, db, prec)
+        got = lat.export_field(db, prec, bq.BQ_EVEN)
+        ref = sb + alpha * sa
+        tol = {0: 1e-15, 1: 3e-7, 2: 1e-3}[prec]
+        assert np.abs(got - ref).max() <= tol * np.abs(ref).max()
+
+
+@pytest.mark.parametrize("prec", [0, 1, 2])
+def test_blas_bicg_update(bq, prec):
+    L = (8, 4, 4, 6)
+    vec = [even_part(L, inputs.spinor(L, 50 + k)) for k in range(6)]
+    alpha, omega = 0.8 + 0.1j, 0.6 - 0.2j
+    with bq.Lattice(L) as lat:
+        xprec = bq.BQ_FP32 if prec == bq.BQ_HALF else prec
+        p, s, t, rhat, r = [lat.import_field(v, prec, bq.BQ_EVEN) for v in vec[:5]]
+        x = lat.import_field(vec[5], xprec, bq.BQ_EVEN)
+        sp, ss, st, srhat = [lat.export_field(d, prec, bq.BQ_EVEN) for d in (p, s, t, rhat)]
+        sx = lat.export_field(x, xprec, bq.BQ_EVEN)
+        r2, rr = bq.bq_blas_bicg_update(lat.h, alpha, omega, p, s, t, rhat, x, r, prec)
+        x_ref = sx + alpha * sp + omega * ss
+        r_ref = ss - omega * st
+        tol = {0: 1e-15, 1: 5e-7, 2: 1e-3}[prec]
+        assert np.abs(lat.export_field(x, xprec, bq.BQ_EVEN) - x_ref).max() <= (5e-7 if prec else 1e-15) * np.abs(x_ref).max()
+        got_r = lat.export_field(r, prec, bq.BQ_EVEN)
+        assert np.abs(got_r - r_ref).max() <= tol * np.abs(r_ref).max()
+        rtol = {0: 1e-13, 1: 1e-6, 2: 1e-6}[prec]     # reductions are over r as stored
+        assert abs(r2 - np.vdot(got_r, got_r).real) <= rtol * r2
+        assert abs(rr - np.vdot(srhat, got_r)) <= rtol * np.linalg.norm(srhat) * np.linalg.norm(got_r)
+
+
+# ---------------------------------------------------------------------------------------------------
+# solves
+# ---------------------------------------------------------------------------------------------------
+def oracle_residual(U, x, b, kappa, A=None):
+    return np.linalg.norm(b - bqo.dirac_apply(U, x, kappa, A=A)) / np.linalg.norm(b)
+
+
+def test_config1_solve_fp64(bq, cfg1):
+    """BASELINE.json config 1: 4^4 fp64 BiCGStab to 1e-12."""
+    U, b, kappa, L = cfg1["U"], cfg1["b"], cfg1["kappa"], cfg1["L"]
+    x = np.zeros_like(b)
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        opts = bq.bq_solve_opts(inner_prec=bq.BQ_FP64)
+        info = bq.bq_solve(lat.h, b, x, kappa, 1e-12, opts)
+    assert info.status == 0 and info.true_rel_residual <= 1e-12
+    assert oracle_residual(U, x, b, kappa) <= 1e-12
+    x_ref, oinfo = bqo.bicgstab(U, b, kappa, tol=1e-13)
+    assert np.linalg.norm(x - x_ref) / np.linalg.norm(x_ref) < 1e-10
+    assert 0 < info.inner_iters < 200
+    print("config1 fp64: iters", info.inner_iters, "restarts", info.restarts, "oracle iters (full D)", oinfo["iters"])
+
+
+@pytest.mark.parametrize("inner,recon", [(1, 0), (1, 1), (2, 0), (2, 1)])
+def test_mixed_precision_wilson_solve(bq, inner, recon):
+    L = (8, 8, 8, 8)
+    kappa = 0.1235
+    U = inputs.gauge(L, 61, 0.7)
+    b = inputs.spinor(L, 61)
+    import torch
+    xd = torch.zeros(b.shape, dtype=torch.complex128, device="cuda")     # device-resident b and x
+    bd = torch.from_numpy(b).cuda()
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        opts = bq.bq_solve_opts(inner_prec=inner, recon=recon)
+        info = bq.bq_solve(lat.h, bd, xd, kappa, 1e-10, opts)
+    x = xd.cpu().numpy()
+    res = oracle_residual(U, x, b, kappa)
+    print(f"inner={inner} recon={recon}: outer {info.outer_cycles} inner iters {info.inner_iters} true res {res:.2e}")
+    assert info.status == 0 and res <= 1e-10 and abs(res - info.true_rel_residual) < 1e-11
+    assert info.outer_cycles >= 2
+
+
+@pytest.mark.parametrize("inner", [0, 1, 2])
+def test_clover_solve(bq, inner):
+    L = (8, 4, 8, 8)
+    csw, kappa = 1.0, 0.1215
+    U = inputs.gauge(L, 62, 0.5)
+    b = inputs.spinor(L, 62)
+    A = bqo.clover_build(U, csw, kappa)
+    x = np.zeros_like(b)
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        opts = bq.bq_solve_opts(inner_prec=inner, csw=csw)
+        info = bq.bq_solve(lat.h, b, x, kappa, 1e-10, opts)
+    res = oracle_residual(U, x, b, kappa, A=A)
+    print(f"clover inner={inner}: outer {info.outer_cycles} iters {info.inner_iters} res {res:.2e}")
+    assert info.status == 0 and res <= 1e-10
+    x_ref, _ = bqo.bicgstab(U, b, kappa, tol=1e-12, A=A)
+    assert np.linalg.norm(x - x_ref) / np.linalg.norm(x_ref) < 1e-8
+
+
+def test_solve_with_initial_guess_and_zero_rhs(bq, cfg1):
+    U, b, kappa, L = cfg1["U"], cfg1["b"], cfg1["kappa"], cfg1["L"]
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        x = np.zeros_like(b)
+        info0 = bq.bq_solve(lat.h, b, x, kappa, 1e-10)
+        x1 = x.copy()
+        info1 = bq.bq_solve(lat.h, b, x1, kappa, 1e-10)             # start from the solution: nothing to do
+        assert info1.inner_iters == 0 and np.array_equal(np.isfinite(x1), np.ones_like(x1, dtype=bool))
+        assert oracle_residual(U, x1, b, kappa) <= 1e-10
+        xz = inputs.spinor(L, 5)
+        infoz = bq.bq_solve(lat.h, np.zeros_like(b), xz, kappa, 1e-10)
+        assert infoz.status == 0 and np.all(xz == 0)
+        assert info0.inner_iters > 0
+
+
+def test_solve_reports_non_convergence(bq, cfg1):
+    U, b, kappa, L = cfg1["U"], cfg1["b"], cfg1["kappa"], cfg1["L"]
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        x = np.zeros_like(b)
+        opts = bq.bq_solve_opts(inner_prec=bq.BQ_FP32, max_inner=2, max_outer=2, check_every=1)
+        info = bq.bq_solve(lat.h, b, x, kappa, 1e-12, opts, raise_on_fail=False)
+        assert info.status == bq.BQ_ENOTCONVERGED
+        # x holds the best iterate and the reported residual is the true one
+        assert abs(oracle_residual(U, x, b, kappa) - info.true_rel_residual) < 1e-9
+        with pytest.raises(bq.BqError):
+            bq.bq_solve(lat.h, b, x, kappa, -1.0)
