@@ -164,6 +164,10 @@ typedef struct {
 bq_status bq_solve(bq_lattice* lat, const double* b, double* x, double kappa, double tol, const bq_solve_opts* opts,
                    bq_solve_info* info);
 
+/* Launch accounting for benchmarks: out[0] = kernels launched through this handle since creation,
+ * out[1..3] = hop-kernel launches with fp64 / fp32 / half storage (each is 1320 flop x Vh sites). */
+bq_status bq_get_counters(const bq_lattice* lat, unsigned long long* out /*[4]*/);
+
 /* Fused BLAS-1 on one-parity internal-layout fields, exposed for tests and benchmarks.
  * All complex scalars are (re, im) pairs of doubles on the HOST; results are written to HOST doubles after a
  * stream synchronise.  <a,b> = sum conj(a_i) b_i.  Reductions are accumulated in fp64 for BQ_FP64 and in fp32

@@ -26,7 +26,7 @@ EXPORTS = [
     "bq_lattice_create", "bq_lattice_destroy", "bq_status_string", "bq_last_error", "bq_gauge_load",
     "bq_field_bytes", "bq_field_import", "bq_field_export", "bq_wilson_apply", "bq_clover_apply",
     "bq_dirac_apply", "bq_schur_apply", "bq_solve", "bq_blas_norm2", "bq_blas_cdot", "bq_blas_caxpy",
-    "bq_blas_bicg_update",
+    "bq_blas_bicg_update", "bq_get_counters",
 ]
 
 
@@ -78,6 +78,7 @@ def lib():
         L.bq_blas_cdot.argtypes = [_vp, _vp, _vp, _i, _dp]
         L.bq_blas_caxpy.argtypes = [_vp, _dp, _vp, _vp, _i]
         L.bq_blas_bicg_update.argtypes = [_vp, _dp, _dp, _vp, _vp, _vp, _vp, _vp, _vp, _i, _dp, _dp]
+        L.bq_get_counters.argtypes = [_vp, ctypes.POINTER(ctypes.c_ulonglong)]
         for name in EXPORTS:
             if name not in ("bq_status_string", "bq_last_error"):
                 getattr(L, name).restype = _i
@@ -170,6 +171,13 @@ def bq_solve(h, b, x, kappa, tol, opts: bq_solve_opts | None = None, raise_on_fa
                         ctypes.byref(info))
     _check(h, st, allow=() if raise_on_fail else (BQ_ENOTCONVERGED, BQ_EBREAKDOWN))
     return info
+
+
+def bq_get_counters(h):
+    """{'launches': all kernels, 'hop_fp64' / 'hop_fp32' / 'hop_half': hop-kernel launches} since handle creation."""
+    out = (ctypes.c_ulonglong * 4)()
+    _check(h, lib().bq_get_counters(h, out))
+    return {"launches": out[0], "hop_fp64": out[1], "hop_fp32": out[2], "hop_half": out[3]}
 
 
 def bq_blas_norm2(h, a, prec):

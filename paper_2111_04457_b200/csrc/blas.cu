@@ -313,7 +313,7 @@ void blas_ctx_destroy(BlasCtx* c) {
         if ((prec) == BQ_FP64) KERNEL<BQ_FP64><<<c.grid, BLAS_BLOCK, 0, c.stream>>>(__VA_ARGS__);    \
         else if ((prec) == BQ_FP32) KERNEL<BQ_FP32><<<c.grid, BLAS_BLOCK, 0, c.stream>>>(__VA_ARGS__); \
         else KERNEL<BQ_HALF><<<c.grid, BLAS_BLOCK, 0, c.stream>>>(__VA_ARGS__);                      \
-        BQ_CUDA(lat, cudaGetLastError());                                                            \
+        BQ_CHECK_LAUNCH(lat);                                                            \
         return BQ_OK;                                                                                \
     } while (0)
 
@@ -355,7 +355,7 @@ bq_status bicg_final(bq_lattice* lat, const BlasCtx& c, int prec, const void* p,
 bq_status outer_residual(bq_lattice* lat, const BlasCtx& c, const void* b, const void* t, void* r) {
     RedBuf rb{c.partials, c.ticket};
     k_outer_residual<<<c.grid, BLAS_BLOCK, 0, c.stream>>>(c.Vh, b, t, r, rb, c.sc);
-    BQ_CUDA(lat, cudaGetLastError());
+    BQ_CHECK_LAUNCH(lat);
     return BQ_OK;
 }
 bq_status outer_to_low(bq_lattice* lat, const BlasCtx& c, int prec_lo, const void* r64, void* lo) {
@@ -363,7 +363,7 @@ bq_status outer_to_low(bq_lattice* lat, const BlasCtx& c, int prec_lo, const voi
     if (prec_lo == BQ_FP64) k_to_low<BQ_FP64><<<grid, 128, 0, c.stream>>>(c.Vh, r64, lo, c.sc);
     else if (prec_lo == BQ_FP32) k_to_low<BQ_FP32><<<grid, 128, 0, c.stream>>>(c.Vh, r64, lo, c.sc);
     else k_to_low<BQ_HALF><<<grid, 128, 0, c.stream>>>(c.Vh, r64, lo, c.sc);
-    BQ_CUDA(lat, cudaGetLastError());
+    BQ_CHECK_LAUNCH(lat);
     return BQ_OK;
 }
 bq_status outer_accumulate(bq_lattice* lat, const BlasCtx& c, int e_prec, const void* e, void* x64) {
@@ -371,6 +371,6 @@ bq_status outer_accumulate(bq_lattice* lat, const BlasCtx& c, int e_prec, const 
     if (e_prec == BQ_FP64) k_accumulate<BQ_FP64><<<grid, 128, 0, c.stream>>>(c.Vh, e, x64, c.sc);
     else if (e_prec == BQ_FP32) k_accumulate<BQ_FP32><<<grid, 128, 0, c.stream>>>(c.Vh, e, x64, c.sc);
     else return bq_set_error(lat, BQ_EINVAL, "outer_accumulate: accumulator cannot be half");
-    BQ_CUDA(lat, cudaGetLastError());
+    BQ_CHECK_LAUNCH(lat);
     return BQ_OK;
 }

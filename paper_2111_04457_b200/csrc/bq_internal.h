@@ -44,6 +44,8 @@ struct bq_lattice {
     double clover_csw, clover_kappa;
     SolverWork* work;
     int* d_flag;             // device int scratch (singular-clover flag etc.)
+    unsigned long long n_launch;      // kernels launched through this handle
+    unsigned long long n_hop[3];      // hop-kernel launches per storage precision
     char err[512];
 };
 
@@ -60,7 +62,14 @@ bq_status bq_set_error(bq_lattice* lat, bq_status s, const char* fmt, ...);
                                 "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e), __FILE__, __LINE__); \
     } while (0)
 
-#define BQ_TRY(expr)                    \
+// after every kernel launch: count it (bq_get_counters) and pick up launch errors
+#define BQ_CHECK_LAUNCH(lat)                 \
+    do {                                     \
+        (lat)->n_launch++;                   \
+        BQ_CUDA((lat), cudaGetLastError());  \
+    } while (0)
+
+#define BQ_TRY(expr)                  \
     do {                                \
         bq_status _s = (expr);          \
         if (_s != BQ_OK) return _s;     \

@@ -242,7 +242,7 @@ bq_status bq_clover_build(bq_lattice* lat, double csw, double kappa) {
     BQ_CUDA(lat, cudaMemset(lat->d_flag, 0, sizeof(int)));
     clover_build_kernel<<<(g.V + 63) / 64, 64>>>(g, lat->U_canon, csw * kappa, static_cast<double*>(lat->clover[BQ_FP64][0]),
                                                 static_cast<double*>(lat->clover[BQ_FP64][1]), lat->d_flag);
-    BQ_CUDA(lat, cudaGetLastError());
+    BQ_CHECK_LAUNCH(lat);
     int flag = 0;
     BQ_CUDA(lat, cudaMemcpy(&flag, lat->d_flag, sizeof(int), cudaMemcpyDeviceToHost));
     if (flag) return bq_set_error(lat, BQ_ESINGULAR_CLOVER, "clover block not positive definite (csw=%g kappa=%g)", csw, kappa);
@@ -290,7 +290,7 @@ bq_status bq_clover_mul(bq_lattice* lat, void* out, const void* in, const void* 
     if (prec == BQ_FP64) clover_mul_kernel<BQ_FP64><<<grid, 128, 0, stream>>>(Vh, out, in, cl);
     else if (prec == BQ_FP32) clover_mul_kernel<BQ_FP32><<<grid, 128, 0, stream>>>(Vh, out, in, cl);
     else clover_mul_kernel<BQ_HALF><<<grid, 128, 0, stream>>>(Vh, out, in, cl);
-    BQ_CUDA(lat, cudaGetLastError());
+    BQ_CHECK_LAUNCH(lat);
     return BQ_OK;
 }
 

@@ -126,7 +126,15 @@ static bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const vo
         case 2: hop_kernel<PREC, RECON, 2><<<grid, HOP_BLOCK, 0, stream>>>(a); break;
         default: hop_kernel<PREC, RECON, 3><<<grid, HOP_BLOCK, 0, stream>>>(a); break;
     }
-    BQ_CUDA(lat, cudaGetLastError());
+    BQ_CHECK_LAUNCH(lat);
+    lat->n_hop[PREC]++;
+    return BQ_OK;
+}
+
+extern "C" bq_status bq_get_counters(const bq_lattice* lat, unsigned long long* out) {
+    if (!lat || !out) return BQ_EINVAL;
+    out[0] = lat->n_launch;
+    for (int p = 0; p < 3; p++) out[1 + p] = lat->n_hop[p];
     return BQ_OK;
 }
 

@@ -197,7 +197,7 @@ extern "C" bq_status bq_gauge_load(bq_lattice* lat, const double* U) {
     BQ_CUDA(lat, cudaMalloc(&lat->gauge[BQ_FP64][BQ_RECON18], 8 * link_block_bytes(BQ_FP64, BQ_RECON18, g.Vh)));
     const int n = 8 * g.Vh;
     gauge_relayout_kernel<<<(n + 255) / 256, 256>>>(g, lat->U_canon, static_cast<double2*>(lat->gauge[BQ_FP64][BQ_RECON18]));
-    BQ_CUDA(lat, cudaGetLastError());
+    BQ_CHECK_LAUNCH(lat);
     BQ_CUDA(lat, cudaDeviceSynchronize());
     lat->have_gauge = true;
     return BQ_OK;
@@ -303,7 +303,7 @@ static bq_status import_export(bq_lattice* lat, void* internal, double* canon, b
             else if (prec == BQ_FP32) export_kernel<BQ_FP32><<<grid, 128, 0, s>>>(g, p, canon, buf);
             else export_kernel<BQ_HALF><<<grid, 128, 0, s>>>(g, p, canon, buf);
         }
-        BQ_CUDA(lat, cudaGetLastError());
+        BQ_CHECK_LAUNCH(lat);
     }
     return BQ_OK;
 }

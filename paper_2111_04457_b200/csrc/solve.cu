@@ -337,7 +337,7 @@ extern "C" bq_status bq_blas_bicg_update(bq_lattice* lat, const double* alpha, c
     if (!alpha || !omega || !p || !s || !t || !rhat || !x || !r || !r_norm2 || !rhat_r)
         return bq_set_error(lat, BQ_EINVAL, "bq_blas_bicg_update: NULL argument");
     k_set_bicg_scalars<<<1, 1, 0, w->blas.stream>>>(w->blas.sc, alpha[0], alpha[1], omega[0], omega[1]);
-    BQ_CUDA(lat, cudaGetLastError());
+    BQ_CHECK_LAUNCH(lat);
     BQ_TRY(bicg_final(lat, w->blas, prec, p, s, t, rhat, x, r));
     BQ_TRY(poll(lat, w));
     *r_norm2 = w->h_sc->r2;
