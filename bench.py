@@ -43,8 +43,8 @@ FALLBACK_HBM_GBS = 6650.0
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
-    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=4000)
+    ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--lattice", default="32,32,32,64")
     ap.add_argument("--prec", default="fp32", choices=["fp64", "fp32", "half"])
@@ -83,7 +83,7 @@ class ClockSampler:
         try:
             self.f = open(self.path, "w")
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={q}", "--format=csv,noheader,nounits",
-                                          "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+                                          "-lms", "50"], stdout=self.f, stderr=subprocess.DEVNULL)
         except Exception:
             self.proc = None
 
@@ -133,7 +133,7 @@ def oracle_hop_sample(U, psi, kappa, L, seconds_target=10.0):
     t0 = time.perf_counter()
     bqo.dirac_apply_sites(U, masked, kappa, probe)
     rate = len(probe) / (time.perf_counter() - t0)
-    n = int(min(len(even_sites) * 8, max(len(probe), rate * seconds_target)))
+    n = int(max(len(probe), rate * seconds_target))           # about seconds_target of CPU work
     reps, rem = divmod(n, len(even_sites))
     t0 = time.perf_counter()
     done = 0

@@ -13,7 +13,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libbq.so")
+LIB_PATH = os.environ.get("BQ_LIB", os.path.join(_HERE, "libbq.so"))   # BQ_LIB: load another build of the same library
 
 # enums (include/bq.h)
 BQ_OK, BQ_EINVAL, BQ_EODD_EXTENT, BQ_ENOGAUGE, BQ_ENOCLOVER, BQ_ESINGULAR_CLOVER, BQ_ECUDA, BQ_ENOMEM, \

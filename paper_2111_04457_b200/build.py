@@ -49,8 +49,13 @@ def _source_hash() -> str:
     return h.hexdigest()
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    h = _source_hash()
+def build(force: bool = False, verbose: bool = False, extra_flags=(), lib_path: str | None = None) -> str:
+    """Default: the in-tree libbq.so.  extra_flags / lib_path build a tuning variant (e.g. -DHOP_BLOCK=64) elsewhere."""
+    variant = lib_path is not None
+    LIB = lib_path or globals()["LIB"]
+    STAMP = LIB + ".stamp"
+    OBJDIR = os.path.join(os.path.dirname(LIB), "build_" + os.path.basename(LIB)) if variant else globals()["OBJDIR"]
+    h = _source_hash() + " ".join(extra_flags)
     if not force and os.path.exists(LIB) and os.path.exists(STAMP):
         with open(STAMP) as f:
             if f.read().strip() == h:
@@ -60,7 +65,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
     def compile_one(unit: str) -> str:
         obj = os.path.join(OBJDIR, unit.replace(".cu", ".o"))
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, unit), "-o", obj]
+        cmd = [nvcc] + NVCC_FLAGS + list(extra_flags) + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, unit), "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError(f"nvcc failed for {unit}:\n{r.stdout}\n{r.stderr}")

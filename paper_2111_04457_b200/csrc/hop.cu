@@ -7,7 +7,16 @@
 #include "clover.cuh"
 #include "hop.cuh"
 
-constexpr int HOP_BLOCK = 128;
+// Launch shape: HOP_BLOCK threads per CTA, HOP_MINB_* resident CTAs per SM asked of ptxas (register cap).
+#ifndef HOP_BLOCK
+#define HOP_BLOCK 128
+#endif
+#ifndef HOP_MINB_LO
+#define HOP_MINB_LO 4   // fp32 / half storage
+#endif
+#ifndef HOP_MINB_64
+#define HOP_MINB_64 2   // fp64
+#endif
 
 template <typename C> struct HopArgs {
     void* out;
@@ -20,12 +29,12 @@ template <typename C> struct HopArgs {
     int Lxh, Ly, Lz, Lt, Vh, p;
     C scale;
     C phr[4], phi[4];     // boundary phases phi_mu
-    int nontrivial[4];    // phi_mu != 1
 };
 
 // EPI: 0: out = scale*acc;  1: out = z + scale*acc;  2: out = scale * Cl(acc);  3: out = Cl(z) + scale*acc
-template <int PREC, int RECON, int EPI>
-__global__ void __launch_bounds__(HOP_BLOCK, PREC == BQ_FP64 ? 2 : 4)
+// CPLX: false = all boundary phases real (+-1), true = general complex phases (see hop_dir)
+template <int PREC, int RECON, int EPI, bool CPLX>
+__global__ void __launch_bounds__(HOP_BLOCK, PREC == BQ_FP64 ? HOP_MINB_64 : HOP_MINB_LO)
 hop_kernel(const HopArgs<typename Prec<PREC>::comp> a) {
     using C = typename Prec<PREC>::comp;
     const int h = blockIdx.x * HOP_BLOCK + threadIdx.x;
@@ -41,6 +50,7 @@ hop_kernel(const HopArgs<typename Prec<PREC>::comp> a) {
     const int sy = a.Lxh, sz = a.Lxh * a.Ly, st = sz * a.Lz;
     const char* gf = static_cast<const char*>(a.gf);
     const char* gb = static_cast<const char*>(a.gb);
+    const C one = 1, zero = 0;
 
     C acc[24];
 #pragma unroll
@@ -50,37 +60,37 @@ hop_kernel(const HopArgs<typename Prec<PREC>::comp> a) {
     {
         const bool wf = r && (xh == a.Lxh - 1);
         const int nf = r ? (wf ? h - (a.Lxh - 1) : h + 1) : h;
-        hop_dir<PREC, RECON, 0, true>(acc, a.in, Vh, nf, gf, h, wf && a.nontrivial[0], a.phr[0], a.phi[0]);
+        hop_dir<PREC, RECON, 0, true, CPLX>(acc, a.in, Vh, nf, gf, h, wf ? a.phr[0] : one, wf ? a.phi[0] : zero);
         const bool wb = !r && (xh == 0);
         const int nb = r ? h : (wb ? h + (a.Lxh - 1) : h - 1);
-        hop_dir<PREC, RECON, 0, false>(acc, a.in, Vh, nb, gb, nb, wb && a.nontrivial[0], a.phr[0], -a.phi[0]);
+        hop_dir<PREC, RECON, 0, false, CPLX>(acc, a.in, Vh, nb, gb, nb, wb ? a.phr[0] : one, wb ? -a.phi[0] : zero);
     }
     // ---- y ----
     {
         const bool wf = (y == a.Ly - 1);
         const int nf = wf ? h - (a.Ly - 1) * sy : h + sy;
-        hop_dir<PREC, RECON, 1, true>(acc, a.in, Vh, nf, gf + a.ublk, h, wf && a.nontrivial[1], a.phr[1], a.phi[1]);
+        hop_dir<PREC, RECON, 1, true, CPLX>(acc, a.in, Vh, nf, gf + a.ublk, h, wf ? a.phr[1] : one, wf ? a.phi[1] : zero);
         const bool wb = (y == 0);
         const int nb = wb ? h + (a.Ly - 1) * sy : h - sy;
-        hop_dir<PREC, RECON, 1, false>(acc, a.in, Vh, nb, gb + a.ublk, nb, wb && a.nontrivial[1], a.phr[1], -a.phi[1]);
+        hop_dir<PREC, RECON, 1, false, CPLX>(acc, a.in, Vh, nb, gb + a.ublk, nb, wb ? a.phr[1] : one, wb ? -a.phi[1] : zero);
     }
     // ---- z ----
     {
         const bool wf = (z == a.Lz - 1);
         const int nf = wf ? h - (a.Lz - 1) * sz : h + sz;
-        hop_dir<PREC, RECON, 2, true>(acc, a.in, Vh, nf, gf + 2 * a.ublk, h, wf && a.nontrivial[2], a.phr[2], a.phi[2]);
+        hop_dir<PREC, RECON, 2, true, CPLX>(acc, a.in, Vh, nf, gf + 2 * a.ublk, h, wf ? a.phr[2] : one, wf ? a.phi[2] : zero);
         const bool wb = (z == 0);
         const int nb = wb ? h + (a.Lz - 1) * sz : h - sz;
-        hop_dir<PREC, RECON, 2, false>(acc, a.in, Vh, nb, gb + 2 * a.ublk, nb, wb && a.nontrivial[2], a.phr[2], -a.phi[2]);
+        hop_dir<PREC, RECON, 2, false, CPLX>(acc, a.in, Vh, nb, gb + 2 * a.ublk, nb, wb ? a.phr[2] : one, wb ? -a.phi[2] : zero);
     }
     // ---- t ----
     {
         const bool wf = (t == a.Lt - 1);
         const int nf = wf ? h - (a.Lt - 1) * st : h + st;
-        hop_dir<PREC, RECON, 3, true>(acc, a.in, Vh, nf, gf + 3 * a.ublk, h, wf && a.nontrivial[3], a.phr[3], a.phi[3]);
+        hop_dir<PREC, RECON, 3, true, CPLX>(acc, a.in, Vh, nf, gf + 3 * a.ublk, h, wf ? a.phr[3] : one, wf ? a.phi[3] : zero);
         const bool wb = (t == 0);
         const int nb = wb ? h + (a.Lt - 1) * st : h - st;
-        hop_dir<PREC, RECON, 3, false>(acc, a.in, Vh, nb, gb + 3 * a.ublk, nb, wb && a.nontrivial[3], a.phr[3], -a.phi[3]);
+        hop_dir<PREC, RECON, 3, false, CPLX>(acc, a.in, Vh, nb, gb + 3 * a.ublk, nb, wb ? a.phr[3] : one, wb ? -a.phi[3] : zero);
     }
 
     // ---- epilogue ----
@@ -109,10 +119,11 @@ static bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const vo
     a.gb = static_cast<const char*>(gauge) + (size_t)(1 - p) * 4 * a.ublk;
     a.Lxh = g.Lxh; a.Ly = g.L[1]; a.Lz = g.L[2]; a.Lt = g.L[3]; a.Vh = g.Vh; a.p = p;
     a.scale = (C)scale;
+    bool cplx = false;
     for (int mu = 0; mu < 4; mu++) {
         a.phr[mu] = (C)lat->bc[2 * mu];
         a.phi[mu] = (C)lat->bc[2 * mu + 1];
-        a.nontrivial[mu] = lat->bc_nontrivial[mu];
+        if (lat->bc[2 * mu + 1] != 0.0) cplx = true;
     }
     const int grid = (g.Vh + HOP_BLOCK - 1) / HOP_BLOCK;
     int epi;
@@ -120,12 +131,18 @@ static bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const vo
     else if (cl_mode == 1 && !z) epi = 2;
     else if (cl_mode == 2 && z) epi = 3;
     else return bq_set_error(lat, BQ_EINVAL, "bq_hop: unsupported epilogue (cl_mode=%d, z=%p)", cl_mode, z);
+#define BQ_HOP_LAUNCH(E)                                                                   \
+    do {                                                                                   \
+        if (cplx) hop_kernel<PREC, RECON, E, true><<<grid, HOP_BLOCK, 0, stream>>>(a);      \
+        else hop_kernel<PREC, RECON, E, false><<<grid, HOP_BLOCK, 0, stream>>>(a);          \
+    } while (0)
     switch (epi) {
-        case 0: hop_kernel<PREC, RECON, 0><<<grid, HOP_BLOCK, 0, stream>>>(a); break;
-        case 1: hop_kernel<PREC, RECON, 1><<<grid, HOP_BLOCK, 0, stream>>>(a); break;
-        case 2: hop_kernel<PREC, RECON, 2><<<grid, HOP_BLOCK, 0, stream>>>(a); break;
-        default: hop_kernel<PREC, RECON, 3><<<grid, HOP_BLOCK, 0, stream>>>(a); break;
+        case 0: BQ_HOP_LAUNCH(0); break;
+        case 1: BQ_HOP_LAUNCH(1); break;
+        case 2: BQ_HOP_LAUNCH(2); break;
+        default: BQ_HOP_LAUNCH(3); break;
     }
+#undef BQ_HOP_LAUNCH
     BQ_CHECK_LAUNCH(lat);
     lat->n_hop[PREC]++;
     return BQ_OK;

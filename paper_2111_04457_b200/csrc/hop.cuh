@@ -11,22 +11,22 @@
 
 #include "layout.cuh"
 
-// i*s_k applied to a two-spin object (a0, a1) (3 colours each), result added with sign SGN into (r0, r1):
+// i*s_k applied to a two-spin object (a0, a1) (3 colours each), added with a scalar weight w into (r0, r1):
 //   i s_x (a0,a1) = ( i a1,  i a0);   i s_y (a0,a1) = ( a1, -a0);   i s_z (a0,a1) = ( i a0, -i a1)
-// r += SGN * (i s_k a).   a, r: 12 reals [2*(3*s + c) + reim].
-template <int K, int SGN, typename C> __device__ __forceinline__ void add_isigma(C* r, const C* a) {
+// r += w * (i s_k a).   a, r: 12 reals [2*(3*s + c) + reim].  Each line is one FMA (the sign rides on the operand).
+template <int K, typename C> __device__ __forceinline__ void add_isigma(C* r, const C* a, const C w) {
 #pragma unroll
     for (int c = 0; c < 3; c++) {
         const C a0r = a[2 * c], a0i = a[2 * c + 1], a1r = a[6 + 2 * c], a1i = a[6 + 2 * c + 1];
         if (K == 0) {         // ( i a1, i a0 ):  i*(x+iy) = -y + ix
-            r[2 * c] += SGN * (-a1i);      r[2 * c + 1] += SGN * a1r;
-            r[6 + 2 * c] += SGN * (-a0i);  r[6 + 2 * c + 1] += SGN * a0r;
+            r[2 * c] += w * (-a1i);      r[2 * c + 1] += w * a1r;
+            r[6 + 2 * c] += w * (-a0i);  r[6 + 2 * c + 1] += w * a0r;
         } else if (K == 1) {  // ( a1, -a0 )
-            r[2 * c] += SGN * a1r;         r[2 * c + 1] += SGN * a1i;
-            r[6 + 2 * c] += SGN * (-a0r);  r[6 + 2 * c + 1] += SGN * (-a0i);
+            r[2 * c] += w * a1r;         r[2 * c + 1] += w * a1i;
+            r[6 + 2 * c] += w * (-a0r);  r[6 + 2 * c + 1] += w * (-a0i);
         } else {              // ( i a0, -i a1 )
-            r[2 * c] += SGN * (-a0i);      r[2 * c + 1] += SGN * a0r;
-            r[6 + 2 * c] += SGN * a1i;     r[6 + 2 * c + 1] += SGN * (-a1r);
+            r[2 * c] += w * (-a0i);      r[2 * c + 1] += w * a0r;
+            r[6 + 2 * c] += w * a1i;     r[6 + 2 * c + 1] += w * (-a1r);
         }
     }
 }
@@ -63,10 +63,12 @@ template <typename C> __device__ __forceinline__ void phase_mul(C* chi, C pr, C 
 // One of the 8 hops.  MU = 0..3, FWD = true: (1 - g_mu) U_mu(x) in(x+mu); false: (1 + g_mu) U_mu(x-mu)^dag in(x-mu).
 //   in     : input spinor field (parity 1-p), nh = half index of the neighbour
 //   ublock : (parity, MU) block of the gauge store; uidx = h (forward: the link lives on x) or nh (backward: on x-mu)
-//   wrap   : this hop crosses the lattice boundary -> multiply by (pr, pi) (phi_mu forward, conj(phi_mu) backward)
-template <int PREC, int RECON, int MU, bool FWD>
+//   (pr, pi): boundary factor of this hop — phi_mu (forward) / conj(phi_mu) (backward) if it wraps, else (1, 0).
+//   CPLX = false: every phase is real (+-1): pi is ignored and pr rides on the accumulation FMAs (no branch, no
+//   extra instruction).  CPLX = true: general phases, one branch-free complex multiply of the half spinor.
+template <int PREC, int RECON, int MU, bool FWD, bool CPLX>
 __device__ __forceinline__ void hop_dir(typename Prec<PREC>::comp* acc, const void* in, int Vh, int nh, const void* ublock,
-                                        int uidx, bool wrap, typename Prec<PREC>::comp pr, typename Prec<PREC>::comp pi) {
+                                        int uidx, typename Prec<PREC>::comp pr, typename Prec<PREC>::comp pi) {
     using C = typename Prec<PREC>::comp;
     C h[12], u[18], chi[12];
     if (MU < 3) {
@@ -74,20 +76,25 @@ __device__ __forceinline__ void hop_dir(typename Prec<PREC>::comp* acc, const vo
         load_spinor<PREC>(in, Vh, nh, psi);
 #pragma unroll
         for (int i = 0; i < 12; i++) h[i] = psi[i];           // u
-        add_isigma<MU, FWD ? +1 : -1>(h, psi + 12);           // h = u +- i s_k l
+        add_isigma<MU>(h, psi + 12, C(FWD ? 1 : -1));         // h = u +- i s_k l
     } else {
         // (1 - g_t) psi = (0; 2l): forward needs l only; (1 + g_t) psi = (2u; 0): backward needs u only
         load_spinor_half<PREC, FWD ? 1 : 0>(in, Vh, nh, h);
     }
     load_link<PREC, RECON>(ublock, Vh, uidx, u);
     su3_mul<!FWD>(u, h, chi);
-    if (wrap) phase_mul(chi, pr, pi);
+    C w = pr;
+    if (CPLX) {
+        phase_mul(chi, pr, pi);
+        w = C(1);
+    }
     if (MU < 3) {
 #pragma unroll
-        for (int i = 0; i < 12; i++) acc[i] += chi[i];        // upper two spins: h
-        add_isigma<MU, FWD ? -1 : +1>(acc + 12, chi);         // lower two spins: -+ i s_k h
+        for (int i = 0; i < 12; i++) acc[i] += w * chi[i];    // upper two spins: h
+        add_isigma<MU>(acc + 12, chi, FWD ? -w : w);          // lower two spins: -+ i s_k h
     } else {
+        const C w2 = 2 * w;
 #pragma unroll
-        for (int i = 0; i < 12; i++) acc[(FWD ? 12 : 0) + i] += 2 * chi[i];
+        for (int i = 0; i < 12; i++) acc[(FWD ? 12 : 0) + i] += w2 * chi[i];
     }
 }
