@@ -138,8 +138,8 @@ template <int NRED, class Fin> __device__ __forceinline__ void grid_reduce(doubl
 // complex helpers on (re, im) pairs
 template <typename C> __device__ __forceinline__ void cfma(C* y, C ar, C ai, const C* x) {   // y += a x
     const C xr = x[0], xi = x[1];
-    y[0] += ar * xr - ai * xi;
-    y[1] += ar * xi + ai * xr;
+    y[0] = mad(-ai, xi, mad(ar, xr, y[0]));
+    y[1] = mad(ai, xr, mad(ar, xi, y[1]));
 }
 __device__ __forceinline__ void cdiv(const double* a, const double* b, double* q) {   // q = a / b
     const double d = b[0] * b[0] + b[1] * b[1];

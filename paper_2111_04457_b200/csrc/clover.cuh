@@ -21,10 +21,10 @@ template <typename C> __device__ __forceinline__ void herm6_mul(const C* b, cons
             const int k = i * (i - 1) / 2 + j;
             const C lr = b[6 + 2 * k], li = b[6 + 2 * k + 1];
             // y_i += L_ij x_j ;  y_j += conj(L_ij) x_i
-            y[2 * i] += lr * x[2 * j] - li * x[2 * j + 1];
-            y[2 * i + 1] += lr * x[2 * j + 1] + li * x[2 * j];
-            y[2 * j] += lr * x[2 * i] + li * x[2 * i + 1];
-            y[2 * j + 1] += lr * x[2 * i + 1] - li * x[2 * i];
+            y[2 * i] = mad(-li, x[2 * j + 1], mad(lr, x[2 * j], y[2 * i]));
+            y[2 * i + 1] = mad(li, x[2 * j], mad(lr, x[2 * j + 1], y[2 * i + 1]));
+            y[2 * j] = mad(li, x[2 * i + 1], mad(lr, x[2 * i], y[2 * j]));
+            y[2 * j + 1] = mad(-li, x[2 * i], mad(lr, x[2 * i + 1], y[2 * j + 1]));
         }
 }
 

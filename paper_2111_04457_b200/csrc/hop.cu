@@ -27,11 +27,12 @@ template <typename C> struct HopArgs {
     const void* cl;       // clover blocks of parity p (epilogue) or nullptr
     size_t ublk;          // bytes of one (parity, mu) gauge block
     int Lxh, Ly, Lz, Lt, Vh, p;
-    C scale;
-    C phr[4], phi[4];     // boundary phases phi_mu
+    C scale;              // epilogue scale: weight of a hop that does not wrap
+    C phr[4], phi[4];     // scale x boundary phase phi_mu: weight of a hop that wraps in direction mu
 };
 
 // EPI: 0: out = scale*acc;  1: out = z + scale*acc;  2: out = scale * Cl(acc);  3: out = Cl(z) + scale*acc
+// (acc = H in; `scale` is carried by the per-direction weights, so acc arrives at the epilogue already scaled)
 // CPLX: false = all boundary phases real (+-1), true = general complex phases (see hop_dir)
 template <int PREC, int RECON, int EPI, bool CPLX>
 __global__ void __launch_bounds__(HOP_BLOCK, PREC == BQ_FP64 ? HOP_MINB_64 : HOP_MINB_LO)
@@ -50,7 +51,7 @@ hop_kernel(const HopArgs<typename Prec<PREC>::comp> a) {
     const int sy = a.Lxh, sz = a.Lxh * a.Ly, st = sz * a.Lz;
     const char* gf = static_cast<const char*>(a.gf);
     const char* gb = static_cast<const char*>(a.gb);
-    const C one = 1, zero = 0;
+    const C one = a.scale, zero = 0;   // weight of an interior hop (the epilogue scale rides on the accumulation)
 
     C acc[24];
 #pragma unroll
@@ -94,9 +95,7 @@ hop_kernel(const HopArgs<typename Prec<PREC>::comp> a) {
     }
 
     // ---- epilogue ----
-    if (EPI == 2) clover_site_mul<PREC>(a.cl, Vh, h, acc);
-#pragma unroll
-    for (int i = 0; i < 24; i++) acc[i] *= a.scale;
+    if (EPI == 2) clover_site_mul<PREC>(a.cl, Vh, h, acc);   // linear: the scale already inside acc commutes with it
     if (EPI == 1 || EPI == 3) {
         C zz[24];
         load_spinor<PREC, true>(a.z, Vh, h, zz);
@@ -121,8 +120,8 @@ static bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const vo
     a.scale = (C)scale;
     bool cplx = false;
     for (int mu = 0; mu < 4; mu++) {
-        a.phr[mu] = (C)lat->bc[2 * mu];
-        a.phi[mu] = (C)lat->bc[2 * mu + 1];
+        a.phr[mu] = (C)(scale * lat->bc[2 * mu]);
+        a.phi[mu] = (C)(scale * lat->bc[2 * mu + 1]);
         if (lat->bc[2 * mu + 1] != 0.0) cplx = true;
     }
     const int grid = (g.Vh + HOP_BLOCK - 1) / HOP_BLOCK;

@@ -32,19 +32,28 @@ template <int K, typename C> __device__ __forceinline__ void add_isigma(C* r, co
 }
 
 // chi = U h  (FWD) or U^dagger h (backward) for both spins of the half spinor.  66 flop per spin.
+// Written as explicit FMA chains (1 FMUL + 5 FFMA per real output): `re += ur*hr - ui*hi` costs three
+// instructions per term (FMUL, FFMA, FADD) because C forbids the reassociation.
 template <bool DAG, typename C> __device__ __forceinline__ void su3_mul(const C* u, const C* h, C* chi) {
 #pragma unroll
     for (int s = 0; s < 2; s++)
 #pragma unroll
         for (int a = 0; a < 3; a++) {
-            C re = 0, im = 0;
+            C re, im;
 #pragma unroll
             for (int b = 0; b < 3; b++) {
                 const C ur = DAG ? u[2 * (3 * b + a)] : u[2 * (3 * a + b)];
                 const C ui = DAG ? -u[2 * (3 * b + a) + 1] : u[2 * (3 * a + b) + 1];
                 const C hr = h[6 * s + 2 * b], hi = h[6 * s + 2 * b + 1];
-                re += ur * hr - ui * hi;
-                im += ur * hi + ui * hr;
+                if (b == 0) {
+                    re = ur * hr;
+                    im = ur * hi;
+                } else {
+                    re = mad(ur, hr, re);
+                    im = mad(ur, hi, im);
+                }
+                re = mad(-ui, hi, re);
+                im = mad(ui, hr, im);
             }
             chi[6 * s + 2 * a] = re;
             chi[6 * s + 2 * a + 1] = im;
@@ -55,31 +64,34 @@ template <typename C> __device__ __forceinline__ void phase_mul(C* chi, C pr, C 
 #pragma unroll
     for (int k = 0; k < 6; k++) {
         const C r = chi[2 * k], i = chi[2 * k + 1];
-        chi[2 * k] = pr * r - pi * i;
-        chi[2 * k + 1] = pr * i + pi * r;
+        chi[2 * k] = mad(-pi, i, pr * r);
+        chi[2 * k + 1] = mad(pi, r, pr * i);
     }
 }
 
 // One of the 8 hops.  MU = 0..3, FWD = true: (1 - g_mu) U_mu(x) in(x+mu); false: (1 + g_mu) U_mu(x-mu)^dag in(x-mu).
 //   in     : input spinor field (parity 1-p), nh = half index of the neighbour
 //   ublock : (parity, MU) block of the gauge store; uidx = h (forward: the link lives on x) or nh (backward: on x-mu)
-//   (pr, pi): boundary factor of this hop — phi_mu (forward) / conj(phi_mu) (backward) if it wraps, else (1, 0).
+//   (pr, pi): weight of this hop = epilogue scale x boundary factor — phi_mu (forward) / conj(phi_mu) (backward) if
+//   the hop wraps, else 1.
 //   CPLX = false: every phase is real (+-1): pi is ignored and pr rides on the accumulation FMAs (no branch, no
 //   extra instruction).  CPLX = true: general phases, one branch-free complex multiply of the half spinor.
+//   Half storage: the neighbour's site norm is folded into the same weight (chi is linear in the spinor), so the
+//   mantissas are never rescaled on their own.
 template <int PREC, int RECON, int MU, bool FWD, bool CPLX>
 __device__ __forceinline__ void hop_dir(typename Prec<PREC>::comp* acc, const void* in, int Vh, int nh, const void* ublock,
                                         int uidx, typename Prec<PREC>::comp pr, typename Prec<PREC>::comp pi) {
     using C = typename Prec<PREC>::comp;
-    C h[12], u[18], chi[12];
+    C h[12], u[18], chi[12], n;
     if (MU < 3) {
         C psi[24];
-        load_spinor<PREC>(in, Vh, nh, psi);
+        load_spinor_raw<PREC>(in, Vh, nh, psi, n);
 #pragma unroll
         for (int i = 0; i < 12; i++) h[i] = psi[i];           // u
         add_isigma<MU>(h, psi + 12, C(FWD ? 1 : -1));         // h = u +- i s_k l
     } else {
         // (1 - g_t) psi = (0; 2l): forward needs l only; (1 + g_t) psi = (2u; 0): backward needs u only
-        load_spinor_half<PREC, FWD ? 1 : 0>(in, Vh, nh, h);
+        load_spinor_half_raw<PREC, FWD ? 1 : 0>(in, Vh, nh, h, n);
     }
     load_link<PREC, RECON>(ublock, Vh, uidx, u);
     su3_mul<!FWD>(u, h, chi);
@@ -88,13 +100,14 @@ __device__ __forceinline__ void hop_dir(typename Prec<PREC>::comp* acc, const vo
         phase_mul(chi, pr, pi);
         w = C(1);
     }
+    if (PREC == BQ_HALF) w *= n;
     if (MU < 3) {
 #pragma unroll
-        for (int i = 0; i < 12; i++) acc[i] += w * chi[i];    // upper two spins: h
-        add_isigma<MU>(acc + 12, chi, FWD ? -w : w);          // lower two spins: -+ i s_k h
+        for (int i = 0; i < 12; i++) acc[i] = mad(w, chi[i], acc[i]);   // upper two spins: h
+        add_isigma<MU>(acc + 12, chi, FWD ? -w : w);                    // lower two spins: -+ i s_k h
     } else {
         const C w2 = 2 * w;
 #pragma unroll
-        for (int i = 0; i < 12; i++) acc[(FWD ? 12 : 0) + i] += w2 * chi[i];
+        for (int i = 0; i < 12; i++) acc[(FWD ? 12 : 0) + i] = mad(w2, chi[i], acc[(FWD ? 12 : 0) + i]);
     }
 }

@@ -14,6 +14,10 @@ template <> struct Prec<BQ_FP64> { using real = double; using comp = double; };
 template <> struct Prec<BQ_FP32> { using real = float; using comp = float; };
 template <> struct Prec<BQ_HALF> { using real = __half; using comp = float; };
 
+// a*b + c in one rounding, spelled out so that complex products compile to FMA chains (1 FMUL + n FFMA).
+__device__ __forceinline__ float mad(float a, float b, float c) { return __fmaf_rn(a, b, c); }
+__device__ __forceinline__ double mad(double a, double b, double c) { return __fma_rn(a, b, c); }
+
 // ---- raw loads with a cache policy: default = plain ld.global (L1-cached, normal L2 policy: spinors, of which
 // every site is read by 8 neighbours and must survive in L2); STREAM = ld.global.cs, evict-first streaming
 // (links, clover blocks, BLAS operands: read exactly once).  Both are coherent loads, so a kernel may read and
@@ -52,9 +56,13 @@ __device__ __forceinline__ uint4 pack8(const float* f) {
 // ---------------------------------------------------------------------------------------------------
 // Spinor: 24 reals, index 2*(3*spin + colour) + (0 = re, 1 = im)
 // ---------------------------------------------------------------------------------------------------
+// Raw form: for BQ_HALF the 24 fp16 mantissas come back un-scaled and the site norm in `n` (the hop kernel folds n
+// into the per-direction weight of its accumulation FMAs, saving 24 multiplies per gather); n = 1 otherwise.
 template <int PREC, bool STREAM = false>
-__device__ __forceinline__ void load_spinor(const void* base, int Vh, int h, typename Prec<PREC>::comp* v) {
+__device__ __forceinline__ void load_spinor_raw(const void* base, int Vh, int h, typename Prec<PREC>::comp* v,
+                                                typename Prec<PREC>::comp& n) {
     const char* b = static_cast<const char*>(base);
+    n = 1;
     if constexpr (PREC == BQ_FP64) {
 #pragma unroll
         for (int k = 0; k < 12; k++) {
@@ -72,9 +80,17 @@ __device__ __forceinline__ void load_spinor(const void* base, int Vh, int h, typ
         uint4 q[3];
 #pragma unroll
         for (int k = 0; k < 3; k++) q[k] = ld16<STREAM, uint4>(b + ((size_t)k * Vh + h) * 16);
-        float n = ld16<STREAM, float>(b + (size_t)3 * Vh * 16 + (size_t)h * 4);
+        n = ld16<STREAM, float>(b + (size_t)3 * Vh * 16 + (size_t)h * 4);
 #pragma unroll
         for (int k = 0; k < 3; k++) unpack8(q[k], v + 8 * k);
+    }
+}
+
+template <int PREC, bool STREAM = false>
+__device__ __forceinline__ void load_spinor(const void* base, int Vh, int h, typename Prec<PREC>::comp* v) {
+    typename Prec<PREC>::comp n;
+    load_spinor_raw<PREC, STREAM>(base, Vh, h, v, n);
+    if constexpr (PREC == BQ_HALF) {
 #pragma unroll
         for (int i = 0; i < 24; i++) v[i] *= n;
     }
@@ -83,8 +99,10 @@ __device__ __forceinline__ void load_spinor(const void* base, int Vh, int h, typ
 // Upper (W = 0: spins 0,1) or lower (W = 1: spins 2,3) half of a spinor, 12 reals — all the t-direction
 // projectors (1 -+ gamma_4) need.
 template <int PREC, int W>
-__device__ __forceinline__ void load_spinor_half(const void* base, int Vh, int h, typename Prec<PREC>::comp* v) {
+__device__ __forceinline__ void load_spinor_half_raw(const void* base, int Vh, int h, typename Prec<PREC>::comp* v,
+                                                     typename Prec<PREC>::comp& n) {
     const char* b = static_cast<const char*>(base);
+    n = 1;
     if constexpr (PREC == BQ_FP64) {
 #pragma unroll
         for (int k = 0; k < 6; k++) {
@@ -102,11 +120,9 @@ __device__ __forceinline__ void load_spinor_half(const void* base, int Vh, int h
         // reals 0..11 = plane 0 + low 8 bytes of plane 1; reals 12..23 = high 8 bytes of plane 1 + plane 2
         uint4 q = ld16<false, uint4>(b + ((size_t)(W ? 2 : 0) * Vh + h) * 16);
         uint2 d = ld16<false, uint2>(b + ((size_t)1 * Vh + h) * 16 + (W ? 8 : 0));
-        float n = ld16<false, float>(b + (size_t)3 * Vh * 16 + (size_t)h * 4);
+        n = ld16<false, float>(b + (size_t)3 * Vh * 16 + (size_t)h * 4);
         if (W == 0) { unpack8(q, v); unpack4(d, v + 8); }
         else { unpack4(d, v); unpack8(q, v + 4); }
-#pragma unroll
-        for (int i = 0; i < 12; i++) v[i] *= n;
     }
 }
 
@@ -156,14 +172,22 @@ __host__ __device__ constexpr size_t link_block_bytes(int prec, int recon, int V
 }
 
 template <typename C> __device__ __forceinline__ void reconstruct_row2(C* u) {
-    // row2_j = conj(row0_a row1_b - row0_b row1_a), (a, b) = (j+1, j+2) mod 3
+    // row2_j = conj(row0_a row1_b - row0_b row1_a), (a, b) = (j+1, j+2) mod 3; FMA chains: 8 instructions per entry
 #pragma unroll
     for (int j = 0; j < 3; j++) {
         const int a = (j + 1) % 3, b = (j + 2) % 3;
-        C re = (u[2 * a] * u[6 + 2 * b] - u[2 * a + 1] * u[6 + 2 * b + 1]) - (u[2 * b] * u[6 + 2 * a] - u[2 * b + 1] * u[6 + 2 * a + 1]);
-        C im = (u[2 * a] * u[6 + 2 * b + 1] + u[2 * a + 1] * u[6 + 2 * b]) - (u[2 * b] * u[6 + 2 * a + 1] + u[2 * b + 1] * u[6 + 2 * a]);
+        const C ar = u[2 * a], ai = u[2 * a + 1], br = u[2 * b], bi = u[2 * b + 1];                    // row 0
+        const C cr = u[6 + 2 * a], ci = u[6 + 2 * a + 1], dr = u[6 + 2 * b], di = u[6 + 2 * b + 1];    // row 1
+        C re = ar * dr;
+        re = mad(-ai, di, re);
+        re = mad(-br, cr, re);
+        re = mad(bi, ci, re);
+        C im = br * ci;            // -Im(row0_a row1_b - row0_b row1_a)
+        im = mad(bi, cr, im);
+        im = mad(-ar, di, im);
+        im = mad(-ai, dr, im);
         u[12 + 2 * j] = re;
-        u[12 + 2 * j + 1] = -im;
+        u[12 + 2 * j + 1] = im;
     }
 }
 
