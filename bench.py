@@ -121,29 +121,23 @@ class ClockSampler:
         return out
 
 
-def oracle_hop_sample(U, psi, kappa, L, seconds_target=10.0):
+def oracle_hop_sample(U, psi, kappa, L, seconds_target=12.0):
     """The CPU oracle computing (D [0; psi_odd])(x) at a sample of EVEN sites = the same hop, 1320 flop/site."""
     from oracle import bqo
     from paper_2111_04457_b200 import inputs
     par = inputs.site_parity(L).ravel()
     even_sites = np.nonzero(par == 0)[0]
     masked = np.where((inputs.site_parity(L) == 1)[..., None, None], psi, 0)
-    # calibrate on a small stride sample, then size the sample for ~seconds_target
-    probe = even_sites[:: max(1, len(even_sites) // 65536)]
-    t0 = time.perf_counter()
-    bqo.dirac_apply_sites(U, masked, kappa, probe)
-    rate = len(probe) / (time.perf_counter() - t0)
-    n = int(max(len(probe), rate * seconds_target))           # about seconds_target of CPU work
-    reps, rem = divmod(n, len(even_sites))
+    bqo.dirac_apply_sites(U, masked, kappa, even_sites[:4096])     # spin up the thread team
+    # whole passes over the even sites until about seconds_target of CPU work has been done
     t0 = time.perf_counter()
     done = 0
-    for _ in range(reps):
+    while True:
         bqo.dirac_apply_sites(U, masked, kappa, even_sites)
         done += len(even_sites)
-    if rem:
-        bqo.dirac_apply_sites(U, masked, kappa, even_sites[:rem])
-        done += rem
-    dt = time.perf_counter() - t0
+        dt = time.perf_counter() - t0
+        if dt >= seconds_target:
+            break
     return {"value": FLOP_PER_SITE * done / dt / 1e9, "unit": "GFlop/s", "cores": bqo.num_threads(), "kind": "oracle",
             "sample": f"{done} even-site hop evaluations ({done / len(even_sites):.2f} passes over the even sites) "
                       f"of the same lattice and inputs, oracle/bqo.c dirac_apply_sites, {dt:.1f} s"}, dt, done
@@ -197,17 +191,12 @@ def main():
         return
 
     import torch
-    import torch.distributed as dist
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
+    from paper_2111_04457_b200 import bq, build, inputs, replicas
+    rank, local_rank, world = replicas.env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
     torch.cuda.set_device(local_rank)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-
-    from paper_2111_04457_b200 import bq, build, inputs
+    replicas.init("nccl", torch.device("cuda", local_rank))
     build.build()
     bq.lib()
     prec, recon = PREC_ID[args.prec], (0 if args.recon == 18 else 1)
@@ -217,10 +206,7 @@ def main():
     U = inputs.gauge(L, seed, 0.5)
     psi = inputs.spinor(L, seed)
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+    barrier = replicas.barrier
 
     lat = bq.Lattice(L)
     bq.bq_gauge_load(lat.h, U)
@@ -242,10 +228,7 @@ def main():
     clocks = sampler.stop()
     c1 = bq.bq_get_counters(lat.h)
     launches = int(c1["launches"] - c0["launches"])
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = replicas.max_over_ranks(ms)
     ms_per_step = ms / args.steps
     gflops = world * FLOP_PER_SITE * Vh / (ms_per_step * 1e-3) / 1e9
     bps = BYTES_PER_SITE[(args.prec, args.recon)]
@@ -283,11 +266,7 @@ def main():
             if it > 0:
                 times.append(dt); infos.append(info)
                 hops.append(sum(int(k1[k] - k0[k]) for k in ("hop_fp64", "hop_fp32", "hop_half")))
-        dt = max(times)
-        if world > 1:
-            t = torch.tensor([dt], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = replicas.max_over_ranks(max(times))
         nbytes = b_host.numel() * 16
         e2e = {"value": world * FLOP_PER_SITE * Vh * hops[-1] / dt / 1e9, "unit": "GFlop/s",
                "h2d_bytes_per_step": 2 * nbytes, "d2h_bytes_per_step": nbytes,
@@ -301,9 +280,7 @@ def main():
     if rank == 0 and world == 1 and not args.skip_cpu:
         cpu, _, _ = oracle_hop_sample(U, psi, kappa, L)
     lat.close()
-    if world > 1:
-        dist.barrier()
-        dist.destroy_process_group()
+    replicas.finish()
     if rank != 0:
         return
     line = {

@@ -148,9 +148,10 @@ __device__ bool invert_herm6(const c64 (*A)[6], c64 (*Ainv)[6]) {
     return true;
 }
 
-// 72 reals of site h into the fp64 clover store: real r -> plane r/2, slot r%2
+// 72 reals of site h into the fp64 clover store: real r -> 16-byte word r/2, slot r%2
 __device__ __forceinline__ void store_clover64(double* base, int Vh, int h, const double* c) {
-    for (int k = 0; k < 36; k++) reinterpret_cast<double2*>(base)[(size_t)k * Vh + h] = make_double2(c[2 * k], c[2 * k + 1]);
+    char* b = reinterpret_cast<char*>(base);
+    for (int k = 0; k < 36; k++) *reinterpret_cast<double2*>(b + CloverAddr<BQ_FP64>::word(Vh, h, k)) = make_double2(c[2 * k], c[2 * k + 1]);
 }
 
 __global__ void clover_build_kernel(Geom g, const double* __restrict__ U, double ck, double* __restrict__ A_out,
@@ -205,24 +206,24 @@ __global__ void clover_build_kernel(Geom g, const double* __restrict__ U, double
     store_clover64(Ainv_out + pb, g.Vh, h, packed_inv);
 }
 
-// fp64 clover store -> fp32 / half store (same plane rule: real r -> plane r/W, slot r%W)
+// fp64 clover store -> fp32 / half store (same word rule: real r -> word r/W, slot r%W)
 template <int PREC> __global__ void clover_convert_kernel(int Vh, const double* __restrict__ src, void* __restrict__ dst_) {
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;   // (p, h)
     if (idx >= 2 * Vh) return;
     const int p = idx / Vh, h = idx % Vh;
-    const double2* s = reinterpret_cast<const double2*>(src + (size_t)p * CLOVER_REALS * Vh);
+    const char* s = reinterpret_cast<const char*>(src + (size_t)p * CLOVER_REALS * Vh);
     float f[72];
     for (int k = 0; k < 36; k++) {
-        const double2 d = s[(size_t)k * Vh + h];
+        const double2 d = *reinterpret_cast<const double2*>(s + CloverAddr<BQ_FP64>::word(Vh, h, k));
         f[2 * k] = (float)d.x;
         f[2 * k + 1] = (float)d.y;
     }
     char* dst = static_cast<char*>(dst_) + (size_t)p * CLOVER_REALS * prec_real_bytes(PREC) * Vh;
     if (PREC == BQ_FP32) {
         for (int k = 0; k < 18; k++)
-            reinterpret_cast<float4*>(dst)[(size_t)k * Vh + h] = make_float4(f[4 * k], f[4 * k + 1], f[4 * k + 2], f[4 * k + 3]);
+            *reinterpret_cast<float4*>(dst + CloverAddr<BQ_FP32>::word(Vh, h, k)) = make_float4(f[4 * k], f[4 * k + 1], f[4 * k + 2], f[4 * k + 3]);
     } else {
-        for (int k = 0; k < 9; k++) reinterpret_cast<uint4*>(dst)[(size_t)k * Vh + h] = pack8(f + 8 * k);
+        for (int k = 0; k < 9; k++) *reinterpret_cast<uint4*>(dst + CloverAddr<BQ_HALF>::word(Vh, h, k)) = pack8(f + 8 * k);
     }
 }
 

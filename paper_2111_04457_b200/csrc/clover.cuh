@@ -28,29 +28,30 @@ template <typename C> __device__ __forceinline__ void herm6_mul(const C* b, cons
         }
 }
 
-// 36 reals of chirality block BLK (0: B+, 1: B-) of site h.  Clover store: 72 reals per site as 16-byte planes.
+// 36 reals of chirality block BLK (0: B+, 1: B-) of site h.  Clover store: 72 reals per site as 16-byte words (layout.cuh).
 template <int PREC, int BLK, bool STREAM = true>
 __device__ __forceinline__ void load_clover_block(const void* base, int Vh, int h, typename Prec<PREC>::comp* c) {
+    using A = CloverAddr<PREC>;
     const char* b = static_cast<const char*>(base);
     if constexpr (PREC == BQ_FP64) {
 #pragma unroll
         for (int k = 0; k < 18; k++) {
-            double2 d = ld16<STREAM, double2>(b + ((size_t)(18 * BLK + k) * Vh + h) * 16);
+            double2 d = ld16<STREAM, double2>(b + A::word(Vh, h, 18 * BLK + k));
             c[2 * k] = d.x;
             c[2 * k + 1] = d.y;
         }
     } else if constexpr (PREC == BQ_FP32) {
 #pragma unroll
         for (int k = 0; k < 9; k++) {
-            float4 d = ld16<STREAM, float4>(b + ((size_t)(9 * BLK + k) * Vh + h) * 16);
+            float4 d = ld16<STREAM, float4>(b + A::word(Vh, h, 9 * BLK + k));
             c[4 * k] = d.x; c[4 * k + 1] = d.y; c[4 * k + 2] = d.z; c[4 * k + 3] = d.w;
         }
     } else {
         // 72 halfs = 9 planes of 8; block 0 = planes 0..3 + low half of plane 4, block 1 = high half of 4 + planes 5..8
         uint4 q[4];
 #pragma unroll
-        for (int k = 0; k < 4; k++) q[k] = ld16<STREAM, uint4>(b + ((size_t)((BLK ? 5 : 0) + k) * Vh + h) * 16);
-        uint2 d = ld16<STREAM, uint2>(b + ((size_t)4 * Vh + h) * 16 + (BLK ? 8 : 0));
+        for (int k = 0; k < 4; k++) q[k] = ld16<STREAM, uint4>(b + A::word(Vh, h, (BLK ? 5 : 0) + k));
+        uint2 d = ld16<STREAM, uint2>(b + A::word(Vh, h, 4) + (BLK ? 8 : 0));
         if (BLK == 0) {
 #pragma unroll
             for (int k = 0; k < 4; k++) unpack8(q[k], c + 8 * k);

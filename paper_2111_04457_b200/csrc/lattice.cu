@@ -131,58 +131,32 @@ __device__ __forceinline__ int canonical_site(const Geom& g, int p, int h) {
 // ---------------------------------------------------------------------------------------------------
 // gauge store
 // ---------------------------------------------------------------------------------------------------
-// canonical U[s][mu][3][3][2] (fp64)  ->  fp64 18-real even-odd SoA store [p][mu][9 planes of double2][Vh]
-__global__ void gauge_relayout_kernel(Geom g, const double* __restrict__ U, double2* __restrict__ out) {
+// canonical U[s][mu][3][3][2] (fp64)  ->  fp64 18-real even-odd store [p][mu][link store over Vh]
+__global__ void gauge_relayout_kernel(Geom g, const double* __restrict__ U, void* __restrict__ out) {
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;   // (p, mu, h) flattened, h fastest
     if (idx >= 8 * g.Vh) return;
     const int h = idx % g.Vh, pm = idx / g.Vh, mu = pm & 3, p = pm >> 2;
     const int s = canonical_site(g, p, h);
     const double2* src = reinterpret_cast<const double2*>(U + ((size_t)s * 4 + mu) * 18);
-    double2* dst = out + (size_t)pm * 9 * g.Vh + h;
+    double u[18];
 #pragma unroll
-    for (int k = 0; k < 9; k++) dst[(size_t)k * g.Vh] = src[k];
+    for (int k = 0; k < 9; k++) {
+        const double2 d = src[k];
+        u[2 * k] = d.x;
+        u[2 * k + 1] = d.y;
+    }
+    store_link<BQ_FP64, BQ_RECON18>(static_cast<char*>(out) + (size_t)pm * link_block_bytes(BQ_FP64, BQ_RECON18, g.Vh), g.Vh, h, u);
 }
 
 // fp64 18-real store -> store of (PREC, RECON): plain rounding (links have entries in [-1,1]: fp16 needs no norm)
 template <int PREC, int RECON>
-__global__ void gauge_convert_kernel(int Vh, const double2* __restrict__ src, void* __restrict__ dst_) {
+__global__ void gauge_convert_kernel(int Vh, const void* __restrict__ src, void* __restrict__ dst) {
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= 8 * Vh) return;
     const int h = idx % Vh, pm = idx / Vh;
-    constexpr int NR = (RECON == BQ_RECON12) ? 12 : 18;
     double u[18];
-#pragma unroll
-    for (int k = 0; k < 9; k++) {
-        const double2 d = src[((size_t)pm * 9 + k) * Vh + h];
-        u[2 * k] = d.x;
-        u[2 * k + 1] = d.y;
-    }
-    char* dst = static_cast<char*>(dst_) + (size_t)pm * link_block_bytes(PREC, RECON, Vh);
-    if constexpr (PREC == BQ_FP64) {
-#pragma unroll
-        for (int k = 0; k < NR / 2; k++) reinterpret_cast<double2*>(dst)[(size_t)k * Vh + h] = make_double2(u[2 * k], u[2 * k + 1]);
-    } else if constexpr (PREC == BQ_FP32) {
-#pragma unroll
-        for (int k = 0; k < NR / 4; k++)
-            reinterpret_cast<float4*>(dst)[(size_t)k * Vh + h] =
-                make_float4((float)u[4 * k], (float)u[4 * k + 1], (float)u[4 * k + 2], (float)u[4 * k + 3]);
-        if (NR == 18) reinterpret_cast<float2*>(dst + (size_t)4 * Vh * 16)[h] = make_float2((float)u[16], (float)u[17]);
-    } else {
-        float f[18];
-#pragma unroll
-        for (int i = 0; i < 18; i++) f[i] = (float)u[i];
-        reinterpret_cast<uint4*>(dst)[h] = pack8(f);
-        if (NR == 18) {
-            reinterpret_cast<uint4*>(dst)[(size_t)Vh + h] = pack8(f + 8);
-            reinterpret_cast<__half2*>(dst + (size_t)2 * Vh * 16)[h] = __floats2half2_rn(f[16], f[17]);
-        } else {
-            uint2 d;
-            __half2* hh = reinterpret_cast<__half2*>(&d);
-            hh[0] = __floats2half2_rn(f[8], f[9]);
-            hh[1] = __floats2half2_rn(f[10], f[11]);
-            reinterpret_cast<uint2*>(dst + (size_t)Vh * 16)[h] = d;
-        }
-    }
+    load_link<BQ_FP64, BQ_RECON18>(static_cast<const char*>(src) + (size_t)pm * link_block_bytes(BQ_FP64, BQ_RECON18, Vh), Vh, h, u);
+    store_link<PREC, RECON>(static_cast<char*>(dst) + (size_t)pm * link_block_bytes(PREC, RECON, Vh), Vh, h, u);
 }
 
 extern "C" bq_status bq_gauge_load(bq_lattice* lat, const double* U) {
@@ -196,7 +170,7 @@ extern "C" bq_status bq_gauge_load(bq_lattice* lat, const double* U) {
     BQ_CUDA(lat, cudaMemcpy(lat->U_canon, U, nbytes, cudaMemcpyDefault));   // host or device source
     BQ_CUDA(lat, cudaMalloc(&lat->gauge[BQ_FP64][BQ_RECON18], 8 * link_block_bytes(BQ_FP64, BQ_RECON18, g.Vh)));
     const int n = 8 * g.Vh;
-    gauge_relayout_kernel<<<(n + 255) / 256, 256>>>(g, lat->U_canon, static_cast<double2*>(lat->gauge[BQ_FP64][BQ_RECON18]));
+    gauge_relayout_kernel<<<(n + 255) / 256, 256>>>(g, lat->U_canon, lat->gauge[BQ_FP64][BQ_RECON18]);
     BQ_CHECK_LAUNCH(lat);
     BQ_CUDA(lat, cudaDeviceSynchronize());
     lat->have_gauge = true;
@@ -210,7 +184,7 @@ bq_status bq_get_gauge(bq_lattice* lat, int prec, int recon, const void** out) {
         const Geom& g = lat->g;
         void* dst = nullptr;
         BQ_CUDA(lat, cudaMalloc(&dst, 8 * link_block_bytes(prec, recon, g.Vh)));
-        const double2* src = static_cast<const double2*>(lat->gauge[BQ_FP64][BQ_RECON18]);
+        const void* src = lat->gauge[BQ_FP64][BQ_RECON18];
         const int n = 8 * g.Vh, grid = (n + 255) / 256;
         if (prec == BQ_FP64) gauge_convert_kernel<BQ_FP64, BQ_RECON12><<<grid, 256>>>(g.Vh, src, dst);
         else if (prec == BQ_FP32 && recon == BQ_RECON18) gauge_convert_kernel<BQ_FP32, BQ_RECON18><<<grid, 256>>>(g.Vh, src, dst);
@@ -262,10 +236,11 @@ __global__ void import_kernel(Geom g, int p, const double* __restrict__ canon, v
         float f[24];
 #pragma unroll
         for (int i = 0; i < 24; i++) f[i] = (float)(v[i] * inv);
+        using A = SpinorAddr<BQ_HALF>;
         char* b = static_cast<char*>(internal);
 #pragma unroll
-        for (int k = 0; k < 3; k++) reinterpret_cast<uint4*>(b)[(size_t)k * g.Vh + h] = pack8(f + 8 * k);
-        reinterpret_cast<float*>(b + (size_t)3 * g.Vh * 16)[h] = n;
+        for (int k = 0; k < 3; k++) *reinterpret_cast<uint4*>(b + A::word(g.Vh, h, k)) = pack8(f + 8 * k);
+        *reinterpret_cast<float*>(b + A::tail(g.Vh, h)) = n;
     }
 }
 
