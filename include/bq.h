@@ -181,6 +181,28 @@ bq_status bq_blas_bicg_update(bq_lattice* lat, const double* alpha, const double
                               const void* t, const void* rhat, void* x, void* r, bq_prec prec,
                               double* r_norm2, double* rhat_r /*[2]*/);
 
+/* Benchmark hook: device time (CUDA events on the library's stream, after one warm-up launch per set) of ONE
+ * internal kernel of the hot path, averaged over `reps` back-to-back launches that rotate over `nsets` (1..16) sets
+ * of scratch vectors allocated inside the call, so that a launch does not find its operands in L2.
+ * bytes_per_launch = the kernel's ALGORITHMIC bytes (every operand read once, every result written
+ * once).  BQ_K_HOP* launch on even output sites; the clover variants need csw != 0.  Synchronises. */
+typedef enum {
+    BQ_K_HOP = 0,            /* out = -kappa H in                                   (A3, epilogue 0)                 */
+    BQ_K_HOP_XPAY = 1,       /* out = z + kappa H in                                (A3, epilogue 1; Wilson M^ step 2) */
+    BQ_K_HOP_CLOVINV = 2,    /* out = -kappa A^-1 H in                              (A3+A5, clover M^ step 1)        */
+    BQ_K_HOP_CLOV_XPAY = 3,  /* out = A z + kappa H in                              (A3+A5, clover M^ step 2)        */
+    BQ_K_SCHUR = 4,          /* out = M^ in (two hop launches)                      (A7)                             */
+    BQ_K_NORM2 = 5,          /* |a|^2                                               (A6)                             */
+    BQ_K_P_UPDATE = 6,       /* p = r + beta (p - omega v)                          (A6 i)                           */
+    BQ_K_ALPHA = 7,          /* <rhat, v> -> alpha                                  (A6 v)                           */
+    BQ_K_S_UPDATE = 8,       /* s = r - alpha v                                     (A6 ii)                          */
+    BQ_K_OMEGA = 9,          /* <t,s>, <t,t> -> omega                               (A6 iii)                         */
+    BQ_K_FINAL = 10,         /* x += alpha p + omega s; r = s - omega t; |r|^2; <rhat,r>   (A6 iv)                   */
+    BQ_K_BICG_ITER = 11      /* one whole inner BiCGStab iteration: 4 hops + 5 BLAS-1 kernels  (A8)                  */
+} bq_kernel_id;
+bq_status bq_bench_kernel(bq_lattice* lat, int which, bq_prec prec, bq_recon recon, double csw, double kappa, int reps,
+                          int nsets, double* us_per_launch, double* bytes_per_launch);
+
 #ifdef __cplusplus
 }
 #endif

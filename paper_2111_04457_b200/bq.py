@@ -26,7 +26,7 @@ EXPORTS = [
     "bq_lattice_create", "bq_lattice_destroy", "bq_status_string", "bq_last_error", "bq_gauge_load",
     "bq_field_bytes", "bq_field_import", "bq_field_export", "bq_wilson_apply", "bq_clover_apply",
     "bq_dirac_apply", "bq_schur_apply", "bq_solve", "bq_blas_norm2", "bq_blas_cdot", "bq_blas_caxpy",
-    "bq_blas_bicg_update", "bq_get_counters",
+    "bq_blas_bicg_update", "bq_get_counters", "bq_bench_kernel",
 ]
 
 
@@ -79,6 +79,7 @@ def lib():
         L.bq_blas_caxpy.argtypes = [_vp, _dp, _vp, _vp, _i]
         L.bq_blas_bicg_update.argtypes = [_vp, _dp, _dp, _vp, _vp, _vp, _vp, _vp, _vp, _i, _dp, _dp]
         L.bq_get_counters.argtypes = [_vp, ctypes.POINTER(ctypes.c_ulonglong)]
+        L.bq_bench_kernel.argtypes = [_vp, _i, _i, _i, _d, _d, _i, _i, _dp, _dp]
         for name in EXPORTS:
             if name not in ("bq_status_string", "bq_last_error"):
                 getattr(L, name).restype = _i
@@ -178,6 +179,18 @@ def bq_get_counters(h):
     out = (ctypes.c_ulonglong * 4)()
     _check(h, lib().bq_get_counters(h, out))
     return {"launches": out[0], "hop_fp64": out[1], "hop_fp32": out[2], "hop_half": out[3]}
+
+
+BQ_K = {"hop": 0, "hop_xpay": 1, "hop_clovinv": 2, "hop_clov_xpay": 3, "schur": 4, "norm2": 5, "p_update": 6, "alpha": 7,
+        "s_update": 8, "omega": 9, "final": 10, "bicg_iter": 11}
+
+
+def bq_bench_kernel(h, which, prec, recon=BQ_RECON18, csw=0.0, kappa=0.125, reps=200, nsets=3):
+    """(microseconds per launch, algorithmic bytes per launch) of one internal kernel (bq_kernel_id or its name)."""
+    us, nb = ctypes.c_double(0), ctypes.c_double(0)
+    _check(h, lib().bq_bench_kernel(h, BQ_K[which] if isinstance(which, str) else which, prec, recon, csw, kappa, reps, nsets,
+                                    ctypes.byref(us), ctypes.byref(nb)))
+    return us.value, nb.value
 
 
 def bq_blas_norm2(h, a, prec):

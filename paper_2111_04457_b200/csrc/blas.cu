@@ -5,19 +5,41 @@
 
 #define BLAS_KERNEL __global__ void __cluster_dims__(BLAS_CLUSTER, 1, 1) __launch_bounds__(BLAS_BLOCK)
 
+// Loop shape shared by all kernels below: a grid-stride loop in which every thread handles UNR items per trip
+// (items i0 + u*BLAS_BLOCK), with all loads of a trip issued before any arithmetic, so that each thread keeps
+// UNR x (operands) 16-byte requests in flight — BLAS-1 is pure streaming and lives on memory-level parallelism.
+// Measured on B200 (32^3x64, one run, +-1%): reductions want 4 items in flight per operand, the read-modify-write
+// updates 2, the 5-operand final update 1; 4 CTAs per SM beat 8 everywhere (profiles/r1_blas_launch_shape.txt).
+#define BLAS_TRIPS(I, n) for (int i0 = blockIdx.x * (BLAS_BLOCK * UNR) + threadIdx.x; i0 < (n); i0 += gridDim.x * (BLAS_BLOCK * UNR))
+#define BLAS_UNROLL(I) _Pragma("unroll") for (int u = 0; u < UNR; u++)
+#ifndef BLAS_UNR_REDUCE
+#define BLAS_UNR_REDUCE 4
+#endif
+#ifndef BLAS_UNR_UPDATE
+#define BLAS_UNR_UPDATE 2
+#endif
+#ifndef BLAS_UNR_FINAL
+#define BLAS_UNR_FINAL 1
+#endif
+#define UNR_REDUCE(I) (I::FLAT ? BLAS_UNR_REDUCE : 1)
+#define UNR_UPDATE(I) (I::FLAT ? BLAS_UNR_UPDATE : 1)
+#define BLAS_IDX (i0 + u * BLAS_BLOCK)
+
 // ---------------------------------------------------------------------------------------------------
 // generic reductions
 // ---------------------------------------------------------------------------------------------------
 template <int PREC> BLAS_KERNEL k_norm2(int Vh, const void* __restrict__ a, RedBuf rb, SolverScalars* sc) {
     using I = Item<PREC>;
     using C = typename I::C;
+    constexpr int UNR = UNR_REDUCE(I);
     C acc = 0;
     const int n = I::count(Vh);
-    for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
-        C v[2 * I::NC];
-        I::load(a, Vh, i, v);
+    BLAS_TRIPS(I, n) {
+        C v[UNR][2 * I::NC];
+        BLAS_UNROLL(I) I::load_or_zero(a, Vh, BLAS_IDX, n, v[u]);
+        BLAS_UNROLL(I)
 #pragma unroll
-        for (int k = 0; k < 2 * I::NC; k++) acc += v[k] * v[k];
+        for (int k = 0; k < 2 * I::NC; k++) acc = mad(v[u][k], v[u][k], acc);
     }
     double red[1] = {(double)acc};
     grid_reduce<1>(red, rb, [sc](const double* r) { sc->red[0] = r[0]; });
@@ -26,16 +48,20 @@ template <int PREC> BLAS_KERNEL k_norm2(int Vh, const void* __restrict__ a, RedB
 template <int PREC> BLAS_KERNEL k_cdot(int Vh, const void* __restrict__ a, const void* __restrict__ b, RedBuf rb, SolverScalars* sc, int mode) {
     using I = Item<PREC>;
     using C = typename I::C;
+    constexpr int UNR = UNR_REDUCE(I);
     C re = 0, im = 0;
     const int n = I::count(Vh);
-    for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
-        C x[2 * I::NC], y[2 * I::NC];
-        I::load(a, Vh, i, x);
-        I::load(b, Vh, i, y);
+    BLAS_TRIPS(I, n) {
+        C x[UNR][2 * I::NC], y[UNR][2 * I::NC];
+        BLAS_UNROLL(I) {
+            I::load_or_zero(a, Vh, BLAS_IDX, n, x[u]);
+            I::load_or_zero(b, Vh, BLAS_IDX, n, y[u]);
+        }
+        BLAS_UNROLL(I)
 #pragma unroll
         for (int k = 0; k < I::NC; k++) {   // conj(x) y
-            re += x[2 * k] * y[2 * k] + x[2 * k + 1] * y[2 * k + 1];
-            im += x[2 * k] * y[2 * k + 1] - x[2 * k + 1] * y[2 * k];
+            re = mad(x[u][2 * k + 1], y[u][2 * k + 1], mad(x[u][2 * k], y[u][2 * k], re));
+            im = mad(-x[u][2 * k + 1], y[u][2 * k], mad(x[u][2 * k], y[u][2 * k + 1], im));
         }
     }
     double red[2] = {(double)re, (double)im};
@@ -59,15 +85,20 @@ template <int PREC> BLAS_KERNEL k_cdot(int Vh, const void* __restrict__ a, const
 template <int PREC> BLAS_KERNEL k_caxpy(int Vh, double ar_, double ai_, const void* __restrict__ x, void* __restrict__ y) {
     using I = Item<PREC>;
     using C = typename I::C;
+    constexpr int UNR = UNR_UPDATE(I);
     const C ar = (C)ar_, ai = (C)ai_;
     const int n = I::count(Vh);
-    for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
-        C xv[2 * I::NC], yv[2 * I::NC];
-        I::load(x, Vh, i, xv);
-        I::load(y, Vh, i, yv);
+    BLAS_TRIPS(I, n) {
+        C xv[UNR][2 * I::NC], yv[UNR][2 * I::NC];
+        BLAS_UNROLL(I) {
+            I::load_or_zero(x, Vh, BLAS_IDX, n, xv[u]);
+            I::load_or_zero(y, Vh, BLAS_IDX, n, yv[u]);
+        }
+        BLAS_UNROLL(I) {
 #pragma unroll
-        for (int k = 0; k < I::NC; k++) cfma(yv + 2 * k, ar, ai, xv + 2 * k);
-        I::store(y, Vh, i, yv);
+            for (int k = 0; k < I::NC; k++) cfma(yv[u] + 2 * k, ar, ai, xv[u] + 2 * k);
+            if (BLAS_IDX < n) I::store(y, Vh, BLAS_IDX, yv[u]);
+        }
     }
 }
 
@@ -78,13 +109,15 @@ template <int PREC> BLAS_KERNEL k_caxpy(int Vh, double ar_, double ai_, const vo
 template <int PREC> BLAS_KERNEL k_init(int Vh, const void* __restrict__ r, RedBuf rb, SolverScalars* sc, double stop2) {
     using I = Item<PREC>;
     using C = typename I::C;
+    constexpr int UNR = UNR_REDUCE(I);
     C acc = 0;
     const int n = I::count(Vh);
-    for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
-        C v[2 * I::NC];
-        I::load(r, Vh, i, v);
+    BLAS_TRIPS(I, n) {
+        C v[UNR][2 * I::NC];
+        BLAS_UNROLL(I) I::load_or_zero(r, Vh, BLAS_IDX, n, v[u]);
+        BLAS_UNROLL(I)
 #pragma unroll
-        for (int k = 0; k < 2 * I::NC; k++) acc += v[k] * v[k];
+        for (int k = 0; k < 2 * I::NC; k++) acc = mad(v[u][k], v[u][k], acc);
     }
     double red[1] = {(double)acc};
     grid_reduce<1>(red, rb, [sc, stop2](const double* r_) {
@@ -104,20 +137,25 @@ template <int PREC> BLAS_KERNEL k_p_update(int Vh, const void* __restrict__ r, v
                                            const SolverScalars* __restrict__ sc) {
     using I = Item<PREC>;
     using C = typename I::C;
+    constexpr int UNR = UNR_UPDATE(I);
     if (sc->done) return;
     const C br = (C)sc->beta[0], bi = (C)sc->beta[1], wr = (C)sc->omega[0], wi = (C)sc->omega[1];
     const int n = I::count(Vh);
-    for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
-        C rv[2 * I::NC], pv[2 * I::NC], vv[2 * I::NC];
-        I::load(r, Vh, i, rv);
-        I::load(p, Vh, i, pv);
-        I::load(v, Vh, i, vv);
-#pragma unroll
-        for (int k = 0; k < I::NC; k++) {
-            cfma(pv + 2 * k, -wr, -wi, vv + 2 * k);    // p - omega v
-            cfma(rv + 2 * k, br, bi, pv + 2 * k);      // r + beta (.)
+    BLAS_TRIPS(I, n) {
+        C rv[UNR][2 * I::NC], pv[UNR][2 * I::NC], vv[UNR][2 * I::NC];
+        BLAS_UNROLL(I) {
+            I::load_or_zero(r, Vh, BLAS_IDX, n, rv[u]);
+            I::load_or_zero(p, Vh, BLAS_IDX, n, pv[u]);
+            I::load_or_zero(v, Vh, BLAS_IDX, n, vv[u]);
         }
-        I::store(p, Vh, i, rv);
+        BLAS_UNROLL(I) {
+#pragma unroll
+            for (int k = 0; k < I::NC; k++) {
+                cfma(pv[u] + 2 * k, -wr, -wi, vv[u] + 2 * k);    // p - omega v
+                cfma(rv[u] + 2 * k, br, bi, pv[u] + 2 * k);      // r + beta (.)
+            }
+            if (BLAS_IDX < n) I::store(p, Vh, BLAS_IDX, rv[u]);
+        }
     }
 }
 
@@ -126,16 +164,21 @@ template <int PREC> BLAS_KERNEL k_s_update(int Vh, const void* __restrict__ r, c
                                            const SolverScalars* __restrict__ sc) {
     using I = Item<PREC>;
     using C = typename I::C;
+    constexpr int UNR = UNR_UPDATE(I);
     if (sc->done) return;
     const C ar = (C)sc->alpha[0], ai = (C)sc->alpha[1];
     const int n = I::count(Vh);
-    for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
-        C rv[2 * I::NC], vv[2 * I::NC];
-        I::load(r, Vh, i, rv);
-        I::load(v, Vh, i, vv);
+    BLAS_TRIPS(I, n) {
+        C rv[UNR][2 * I::NC], vv[UNR][2 * I::NC];
+        BLAS_UNROLL(I) {
+            I::load_or_zero(r, Vh, BLAS_IDX, n, rv[u]);
+            I::load_or_zero(v, Vh, BLAS_IDX, n, vv[u]);
+        }
+        BLAS_UNROLL(I) {
 #pragma unroll
-        for (int k = 0; k < I::NC; k++) cfma(rv + 2 * k, -ar, -ai, vv + 2 * k);
-        I::store(s, Vh, i, rv);
+            for (int k = 0; k < I::NC; k++) cfma(rv[u] + 2 * k, -ar, -ai, vv[u] + 2 * k);
+            if (BLAS_IDX < n) I::store(s, Vh, BLAS_IDX, rv[u]);
+        }
     }
 }
 
@@ -143,17 +186,21 @@ template <int PREC> BLAS_KERNEL k_s_update(int Vh, const void* __restrict__ r, c
 template <int PREC> BLAS_KERNEL k_omega(int Vh, const void* __restrict__ t, const void* __restrict__ s, RedBuf rb, SolverScalars* sc) {
     using I = Item<PREC>;
     using C = typename I::C;
+    constexpr int UNR = UNR_REDUCE(I);
     C re = 0, im = 0, tt = 0;
     const int n = I::count(Vh);
-    for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
-        C x[2 * I::NC], y[2 * I::NC];
-        I::load(t, Vh, i, x);
-        I::load(s, Vh, i, y);
+    BLAS_TRIPS(I, n) {
+        C x[UNR][2 * I::NC], y[UNR][2 * I::NC];
+        BLAS_UNROLL(I) {
+            I::load_or_zero(t, Vh, BLAS_IDX, n, x[u]);
+            I::load_or_zero(s, Vh, BLAS_IDX, n, y[u]);
+        }
+        BLAS_UNROLL(I)
 #pragma unroll
         for (int k = 0; k < I::NC; k++) {
-            re += x[2 * k] * y[2 * k] + x[2 * k + 1] * y[2 * k + 1];
-            im += x[2 * k] * y[2 * k + 1] - x[2 * k + 1] * y[2 * k];
-            tt += x[2 * k] * x[2 * k] + x[2 * k + 1] * x[2 * k + 1];
+            re = mad(x[u][2 * k + 1], y[u][2 * k + 1], mad(x[u][2 * k], y[u][2 * k], re));
+            im = mad(-x[u][2 * k + 1], y[u][2 * k], mad(x[u][2 * k], y[u][2 * k + 1], im));
+            tt = mad(x[u][2 * k + 1], x[u][2 * k + 1], mad(x[u][2 * k], x[u][2 * k], tt));
         }
     }
     double red[3] = {(double)re, (double)im, (double)tt};
@@ -179,29 +226,58 @@ template <int PREC> BLAS_KERNEL k_final(int Vh, const void* __restrict__ p, cons
     const C ar = (C)sc->alpha[0], ai = (C)sc->alpha[1], wr = (C)sc->omega[0], wi = (C)sc->omega[1];
     C r2 = 0, re = 0, im = 0;
     const int n = I::count(Vh);
-    for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
-        C xv[2 * I::NC], sv[2 * I::NC], w[2 * I::NC];
-        if constexpr (PREC == BQ_HALF) load_spinor<BQ_FP32>(x, Vh, i, xv);   // fp32 solution accumulator
-        else I::load(x, Vh, i, xv);
-        I::load(p, Vh, i, w);
+    if constexpr (PREC == BQ_HALF) {
+        for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
+            C xv[24], sv[24], w[24];
+            load_spinor<BQ_FP32>(x, Vh, i, xv);   // fp32 solution accumulator
+            I::load(p, Vh, i, w);
 #pragma unroll
-        for (int k = 0; k < I::NC; k++) cfma(xv + 2 * k, ar, ai, w + 2 * k);
-        I::load(s, Vh, i, sv);
+            for (int k = 0; k < 12; k++) cfma(xv + 2 * k, ar, ai, w + 2 * k);
+            I::load(s, Vh, i, sv);
 #pragma unroll
-        for (int k = 0; k < I::NC; k++) cfma(xv + 2 * k, wr, wi, sv + 2 * k);
-        if constexpr (PREC == BQ_HALF) store_spinor<BQ_FP32>(x, Vh, i, xv);
-        else I::store(x, Vh, i, xv);
-        I::load(t, Vh, i, w);
+            for (int k = 0; k < 12; k++) cfma(xv + 2 * k, wr, wi, sv + 2 * k);
+            store_spinor<BQ_FP32>(x, Vh, i, xv);
+            I::load(t, Vh, i, w);
 #pragma unroll
-        for (int k = 0; k < I::NC; k++) cfma(sv + 2 * k, -wr, -wi, w + 2 * k);   // r = s - omega t
-        I::store(r, Vh, i, sv);
-        if constexpr (PREC == BQ_HALF) I::requantize(sv);       // reductions see r as stored (rounded to half storage)
-        I::load(rhat, Vh, i, w);
+            for (int k = 0; k < 12; k++) cfma(sv + 2 * k, -wr, -wi, w + 2 * k);   // r = s - omega t
+            I::store(r, Vh, i, sv);
+            I::requantize(sv);       // reductions see r as stored (rounded to half storage)
+            I::load(rhat, Vh, i, w);
 #pragma unroll
-        for (int k = 0; k < I::NC; k++) {
-            r2 += sv[2 * k] * sv[2 * k] + sv[2 * k + 1] * sv[2 * k + 1];
-            re += w[2 * k] * sv[2 * k] + w[2 * k + 1] * sv[2 * k + 1];
-            im += w[2 * k] * sv[2 * k + 1] - w[2 * k + 1] * sv[2 * k];
+            for (int k = 0; k < 12; k++) {
+                r2 = mad(sv[2 * k + 1], sv[2 * k + 1], mad(sv[2 * k], sv[2 * k], r2));
+                re = mad(w[2 * k + 1], sv[2 * k + 1], mad(w[2 * k], sv[2 * k], re));
+                im = mad(-w[2 * k + 1], sv[2 * k], mad(w[2 * k], sv[2 * k + 1], im));
+            }
+        }
+    } else {
+        constexpr int U2 = BLAS_UNR_FINAL;    // 5 operands = 5 requests in flight per thread (more was slower)
+        for (int i0 = blockIdx.x * (BLAS_BLOCK * U2) + threadIdx.x; i0 < n; i0 += gridDim.x * (BLAS_BLOCK * U2)) {
+            C xv[U2][2 * I::NC], pv[U2][2 * I::NC], sv[U2][2 * I::NC], tv[U2][2 * I::NC], hv[U2][2 * I::NC];
+#pragma unroll
+            for (int u = 0; u < U2; u++) {
+                I::load_or_zero(x, Vh, BLAS_IDX, n, xv[u]);
+                I::load_or_zero(p, Vh, BLAS_IDX, n, pv[u]);
+                I::load_or_zero(s, Vh, BLAS_IDX, n, sv[u]);
+                I::load_or_zero(t, Vh, BLAS_IDX, n, tv[u]);
+                I::load_or_zero(rhat, Vh, BLAS_IDX, n, hv[u]);
+            }
+#pragma unroll
+            for (int u = 0; u < U2; u++) {
+#pragma unroll
+                for (int k = 0; k < I::NC; k++) {
+                    cfma(xv[u] + 2 * k, ar, ai, pv[u] + 2 * k);
+                    cfma(xv[u] + 2 * k, wr, wi, sv[u] + 2 * k);
+                    cfma(sv[u] + 2 * k, -wr, -wi, tv[u] + 2 * k);   // r = s - omega t
+                    r2 = mad(sv[u][2 * k + 1], sv[u][2 * k + 1], mad(sv[u][2 * k], sv[u][2 * k], r2));
+                    re = mad(hv[u][2 * k + 1], sv[u][2 * k + 1], mad(hv[u][2 * k], sv[u][2 * k], re));
+                    im = mad(-hv[u][2 * k + 1], sv[u][2 * k], mad(hv[u][2 * k], sv[u][2 * k + 1], im));
+                }
+                if (BLAS_IDX < n) {
+                    I::store(x, Vh, BLAS_IDX, xv[u]);
+                    I::store(r, Vh, BLAS_IDX, sv[u]);
+                }
+            }
         }
     }
     double red[3] = {(double)r2, (double)re, (double)im};
@@ -230,16 +306,21 @@ template <int PREC> BLAS_KERNEL k_final(int Vh, const void* __restrict__ p, cons
 BLAS_KERNEL k_outer_residual(int Vh, const void* __restrict__ b, const void* __restrict__ t, void* __restrict__ r, RedBuf rb,
                              SolverScalars* sc) {
     using I = Item<BQ_FP64>;
+    constexpr int UNR = UNR_UPDATE(I);
     double acc = 0;
     const int n = I::count(Vh);
-    for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
-        double bv[2], tv[2];
-        I::load(b, Vh, i, bv);
-        I::load(t, Vh, i, tv);
-        bv[0] -= tv[0];
-        bv[1] -= tv[1];
-        I::store(r, Vh, i, bv);
-        acc += bv[0] * bv[0] + bv[1] * bv[1];
+    BLAS_TRIPS(I, n) {
+        double bv[UNR][2], tv[UNR][2];
+        BLAS_UNROLL(I) {
+            I::load_or_zero(b, Vh, BLAS_IDX, n, bv[u]);
+            I::load_or_zero(t, Vh, BLAS_IDX, n, tv[u]);
+        }
+        BLAS_UNROLL(I) {
+            bv[u][0] -= tv[u][0];
+            bv[u][1] -= tv[u][1];
+            if (BLAS_IDX < n) I::store(r, Vh, BLAS_IDX, bv[u]);
+            acc += bv[u][0] * bv[u][0] + bv[u][1] * bv[u][1];
+        }
     }
     double red[1] = {acc};
     grid_reduce<1>(red, rb, [sc](const double* q) {
@@ -285,9 +366,9 @@ bq_status blas_ctx_create(bq_lattice* lat, BlasCtx* c) {
     BQ_CUDA(lat, cudaGetDevice(&dev));
     BQ_CUDA(lat, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     c->Vh = lat->g.Vh;
-    // persistent-style grid: 4 CTAs of 256 threads per SM (a multiple of the SM count and of the cluster size),
-    // trimmed for small lattices so that no cluster is empty-handed more than necessary
-    int grid = sms * 4;
+    // persistent-style grid: 8 CTAs of 256 threads per SM = full occupancy (a multiple of the SM count and of the
+    // cluster size), trimmed for small lattices so that no cluster is empty-handed more than necessary
+    int grid = sms * BLAS_CTAS_PER_SM;
     const int need = (12 * lat->g.Vh + BLAS_BLOCK - 1) / BLAS_BLOCK;
     if (grid > need) grid = need;
     grid = ((grid + BLAS_CLUSTER - 1) / BLAS_CLUSTER) * BLAS_CLUSTER;

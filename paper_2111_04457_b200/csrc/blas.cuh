@@ -20,12 +20,20 @@ namespace cg = cooperative_groups;
 
 constexpr int BLAS_BLOCK = 256;
 constexpr int BLAS_CLUSTER = 4;
+#ifndef BLAS_CTAS_PER_SM
+#define BLAS_CTAS_PER_SM 4  // grid = SMs x this (persistent-style, grid-stride loops)
+#endif
 
 template <int PREC> struct Item;
 template <> struct Item<BQ_FP64> {
     using C = double;
     static constexpr int NC = 1;
+    static constexpr bool FLAT = true;   // items are independent 16-byte chunks: several per thread per trip (blas.cu)
     __host__ __device__ static int count(int Vh) { return 12 * Vh; }
+    __device__ static void load_or_zero(const void* b, int Vh, int i, int n, C* v) {
+        if (i < n) load(b, Vh, i, v);
+        else v[0] = v[1] = 0;
+    }
     __device__ static void load(const void* b, int, int i, C* v) {
         const double2 d = reinterpret_cast<const double2*>(b)[i];
         v[0] = d.x; v[1] = d.y;
@@ -35,7 +43,12 @@ template <> struct Item<BQ_FP64> {
 template <> struct Item<BQ_FP32> {
     using C = float;
     static constexpr int NC = 2;
+    static constexpr bool FLAT = true;
     __host__ __device__ static int count(int Vh) { return 6 * Vh; }
+    __device__ static void load_or_zero(const void* b, int Vh, int i, int n, C* v) {
+        if (i < n) load(b, Vh, i, v);
+        else v[0] = v[1] = v[2] = v[3] = 0;
+    }
     __device__ static void load(const void* b, int, int i, C* v) {
         const float4 d = reinterpret_cast<const float4*>(b)[i];
         v[0] = d.x; v[1] = d.y; v[2] = d.z; v[3] = d.w;
@@ -45,7 +58,15 @@ template <> struct Item<BQ_FP32> {
 template <> struct Item<BQ_HALF> {
     using C = float;
     static constexpr int NC = 12;
+    static constexpr bool FLAT = false;  // a site is already 52 bytes in 4 requests
     __host__ __device__ static int count(int Vh) { return Vh; }
+    __device__ static void load_or_zero(const void* b, int Vh, int i, int n, C* v) {
+        if (i < n) load(b, Vh, i, v);
+        else {
+#pragma unroll
+            for (int k = 0; k < 24; k++) v[k] = 0;
+        }
+    }
     __device__ static void load(const void* b, int Vh, int i, C* v) { load_spinor<BQ_HALF>(b, Vh, i, v); }
     __device__ static void store(void* b, int Vh, int i, const C* v) { store_spinor<BQ_HALF>(b, Vh, i, v); }
     // what a load of the just-stored item would return: v -> fp16(v/n) * n, n = max|v|

@@ -90,6 +90,13 @@ static bq_status get_work(bq_lattice* lat, int inner_prec, SolverWork** out) {
     return BQ_OK;
 }
 
+__global__ void k_set_bicg_scalars(SolverScalars* sc, double ar, double ai, double wr, double wi) {
+    sc->alpha[0] = ar; sc->alpha[1] = ai;
+    sc->omega[0] = wr; sc->omega[1] = wi;
+    sc->rho[0] = 1; sc->rho[1] = 0;
+    sc->done = 0; sc->iters = 0; sc->stop2 = -1.0;
+}
+
 // out_e = M^ in_e in precision prec (tmp: odd scratch)
 static bq_status schur(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw, int prec, int recon,
                        cudaStream_t s) {
@@ -322,13 +329,6 @@ extern "C" bq_status bq_blas_caxpy(bq_lattice* lat, const double* alpha, const v
     return blas_caxpy(lat, w->blas, prec, alpha[0], alpha[1], x, y);
 }
 
-__global__ void k_set_bicg_scalars(SolverScalars* sc, double ar, double ai, double wr, double wi) {
-    sc->alpha[0] = ar; sc->alpha[1] = ai;
-    sc->omega[0] = wr; sc->omega[1] = wi;
-    sc->rho[0] = 1; sc->rho[1] = 0;
-    sc->done = 0; sc->iters = 0; sc->stop2 = 0;
-}
-
 extern "C" bq_status bq_blas_bicg_update(bq_lattice* lat, const double* alpha, const double* omega, const void* p, const void* s,
                                          const void* t, const void* rhat, void* x, void* r, bq_prec prec, double* r_norm2,
                                          double* rhat_r) {
@@ -343,5 +343,133 @@ extern "C" bq_status bq_blas_bicg_update(bq_lattice* lat, const double* alpha, c
     *r_norm2 = w->h_sc->r2;
     rhat_r[0] = w->h_sc->rho[0];
     rhat_r[1] = w->h_sc->rho[1];
+    return BQ_OK;
+}
+
+// scratch filler of bq_bench_kernel: finite, non-zero, site- and component-dependent values in [-0.5, 0.5)
+template <int PREC> __global__ void k_bench_fill(int Vh, void* f, unsigned int seed) {
+    const int h = blockIdx.x * blockDim.x + threadIdx.x;
+    if (h >= Vh) return;
+    typename Prec<PREC>::comp v[24];
+#pragma unroll
+    for (int i = 0; i < 24; i++) {
+        unsigned int x = (unsigned int)h * 24u + i + seed * 0x9E3779B9u;
+        x ^= x >> 16; x *= 0x7feb352du; x ^= x >> 15; x *= 0x846ca68bu; x ^= x >> 16;
+        v[i] = (typename Prec<PREC>::comp)((x >> 8) * (1.0f / 16777216.0f) - 0.5f);
+    }
+    store_spinor<PREC>(f, Vh, h, v);
+}
+static void bench_fill(int prec, int Vh, void* f, unsigned int seed, cudaStream_t s) {
+    const int grid = (Vh + 127) / 128;
+    if (prec == BQ_FP64) k_bench_fill<BQ_FP64><<<grid, 128, 0, s>>>(Vh, f, seed);
+    else if (prec == BQ_FP32) k_bench_fill<BQ_FP32><<<grid, 128, 0, s>>>(Vh, f, seed);
+    else k_bench_fill<BQ_HALF><<<grid, 128, 0, s>>>(Vh, f, seed);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// bq_bench_kernel: device time of one internal kernel of the hot path, measured with CUDA events over `reps`
+// back-to-back launches that rotate over `nsets` sets of scratch vectors (so that consecutive launches do not find
+// their operands in L2).  Benchmark hook only: contents of the scratch vectors are irrelevant.
+// ---------------------------------------------------------------------------------------------------
+extern "C" bq_status bq_bench_kernel(bq_lattice* lat, int which, bq_prec prec, bq_recon recon, double csw, double kappa, int reps,
+                                     int nsets, double* us_per_launch, double* bytes_per_launch) {
+    if (!lat) return BQ_EINVAL;
+    if (!us_per_launch || !bytes_per_launch || reps < 1 || nsets < 1 || nsets > 16) return bq_set_error(lat, BQ_EINVAL, "bq_bench_kernel: bad arguments");
+    if (prec != BQ_FP64 && prec != BQ_FP32 && prec != BQ_HALF) return bq_set_error(lat, BQ_EINVAL, "bq_bench_kernel: bad precision");
+    if (recon != BQ_RECON18 && recon != BQ_RECON12) return bq_set_error(lat, BQ_EINVAL, "bq_bench_kernel: bad recon");
+    if (!lat->have_gauge) return bq_set_error(lat, BQ_ENOGAUGE, "bq_bench_kernel: no gauge field loaded");
+    SolverWork* w = nullptr;
+    BQ_TRY(get_work(lat, lat->work && lat->work->inner_prec >= 0 ? lat->work->inner_prec : BQ_FP32, &w));
+    const BlasCtx& c = w->blas;
+    cudaStream_t s = c.stream;
+    const Geom& g = lat->g;
+    const size_t fb = field_bytes_one_parity(g, prec);
+    const size_t xb = field_bytes_one_parity(g, prec == BQ_HALF ? BQ_FP32 : prec);   // solution accumulator of k_final
+    const bool clover = csw != 0.0;
+    const void *cl = nullptr, *cli = nullptr;
+    const size_t cb = (size_t)g.Vh * CLOVER_REALS * prec_real_bytes(prec);
+    if (clover) {
+        BQ_TRY(bq_clover_build(lat, csw, kappa));
+        BQ_TRY(bq_get_clover(lat, prec, 0, &cl));
+        BQ_TRY(bq_get_clover(lat, prec, 1, &cli));
+    }
+    const void* gauge = nullptr;
+    BQ_TRY(bq_get_gauge(lat, prec, recon, &gauge));
+    // scratch: per set 7 vectors of the storage precision + 1 accumulator
+    constexpr int NV = 7;
+    char* pool = nullptr;
+    const size_t set_bytes = NV * fb + xb;
+    BQ_CUDA(lat, cudaMalloc(&pool, set_bytes * nsets));
+    // finite non-zero contents: an exactly zero inner product would set the solver's breakdown flag and make the
+    // following kernels exit early
+    for (int set = 0; set < nsets; set++) {
+        for (int i = 0; i < NV; i++) bench_fill(prec, g.Vh, pool + (size_t)set * set_bytes + (size_t)i * fb, 1 + set * 8 + i, s);
+        bench_fill(prec == BQ_HALF ? BQ_FP32 : prec, g.Vh, pool + (size_t)set * set_bytes + (size_t)NV * fb, 100 + set, s);
+    }
+    k_set_bicg_scalars<<<1, 1, 0, s>>>(c.sc, 0.5, 0.1, 0.5, -0.1);
+    BQ_CHECK_LAUNCH(lat);
+    const double spin_b = (double)spinor_site_bytes(prec), link_b = (double)link_reals(recon) * prec_real_bytes(prec);
+    const double clov_b = (double)CLOVER_REALS * prec_real_bytes(prec), acc_b = (double)spinor_site_bytes(prec == BQ_HALF ? BQ_FP32 : prec);
+    double bytes = 0;
+    bq_status st = BQ_OK;
+    auto vec = [&](int set, int i) { return static_cast<void*>(pool + (size_t)set * set_bytes + (size_t)i * fb); };
+    auto accv = [&](int set) { return static_cast<void*>(pool + (size_t)set * set_bytes + (size_t)NV * fb); };
+    auto launch = [&](int set) -> bq_status {
+        void *v0 = vec(set, 0), *v1 = vec(set, 1), *v2 = vec(set, 2), *v3 = vec(set, 3), *v4 = vec(set, 4), *v5 = vec(set, 5);
+        switch (which) {
+            case BQ_K_HOP: bytes = 8 * link_b + 2 * spin_b; return bq_hop(lat, v0, v1, nullptr, -kappa, 0, prec, recon, nullptr, 0, s);
+            case BQ_K_HOP_XPAY: bytes = 8 * link_b + 3 * spin_b; return bq_hop(lat, v0, v1, v2, kappa, 0, prec, recon, nullptr, 0, s);
+            case BQ_K_HOP_CLOVINV:
+                if (!clover) return bq_set_error(lat, BQ_EINVAL, "bq_bench_kernel: clover kernels need csw != 0");
+                bytes = 8 * link_b + 2 * spin_b + clov_b;
+                return bq_hop(lat, v0, v1, nullptr, -kappa, 1, prec, recon, static_cast<const char*>(cli) + cb, 1, s);
+            case BQ_K_HOP_CLOV_XPAY:
+                if (!clover) return bq_set_error(lat, BQ_EINVAL, "bq_bench_kernel: clover kernels need csw != 0");
+                bytes = 8 * link_b + 3 * spin_b + clov_b;
+                return bq_hop(lat, v0, v1, v2, kappa, 0, prec, recon, cl, 2, s);
+            case BQ_K_SCHUR:
+                bytes = 2 * (8 * link_b + 2 * spin_b) + spin_b + (clover ? 2 * clov_b : 0);
+                return schur(lat, v0, v1, v2, kappa, csw, prec, recon, s);
+            case BQ_K_NORM2: bytes = spin_b; return blas_norm2(lat, c, prec, v0);
+            case BQ_K_P_UPDATE: bytes = 4 * spin_b; return bicg_p_update(lat, c, prec, v0, v1, v2);
+            case BQ_K_ALPHA: bytes = 2 * spin_b; return bicg_alpha(lat, c, prec, v0, v1);
+            case BQ_K_S_UPDATE: bytes = 3 * spin_b; return bicg_s_update(lat, c, prec, v0, v1, v2);
+            case BQ_K_OMEGA: bytes = 2 * spin_b; return bicg_omega(lat, c, prec, v0, v1);
+            case BQ_K_FINAL: bytes = 5 * spin_b + 2 * acc_b; return bicg_final(lat, c, prec, v0, v1, v2, v3, accv(set), v4);
+            case BQ_K_BICG_ITER: {
+                // one whole inner iteration: p-update, M^, alpha, s-update, M^, omega, final (same order as inner_bicgstab)
+                const double schur_b = 2 * (8 * link_b + 2 * spin_b) + spin_b + (clover ? 2 * clov_b : 0);
+                bytes = 2 * schur_b + (4 + 2 + 3 + 2 + 5) * spin_b + 2 * acc_b;
+                void* v6 = vec(set, 6);
+                BQ_TRY(bicg_p_update(lat, c, prec, v0, v1, v2));
+                BQ_TRY(schur(lat, v2, v1, v6, kappa, csw, prec, recon, s));
+                BQ_TRY(bicg_alpha(lat, c, prec, v3, v2));
+                BQ_TRY(bicg_s_update(lat, c, prec, v0, v2, v4));
+                BQ_TRY(schur(lat, v5, v4, v6, kappa, csw, prec, recon, s));
+                BQ_TRY(bicg_omega(lat, c, prec, v5, v4));
+                return bicg_final(lat, c, prec, v1, v4, v5, v3, accv(set), v0);
+            }
+            default: return bq_set_error(lat, BQ_EINVAL, "bq_bench_kernel: unknown kernel id %d", which);
+        }
+    };
+    for (int i = 0; i < nsets && st == BQ_OK; i++) st = launch(i);      // warm-up: one launch per set
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    if (st == BQ_OK) {
+        cudaEventRecord(e0, s);
+        for (int i = 0; i < reps && st == BQ_OK; i++) st = launch(i % nsets);
+        cudaEventRecord(e1, s);
+    }
+    cudaError_t e = cudaStreamSynchronize(s);
+    float ms = 0;
+    if (st == BQ_OK && e == cudaSuccess) cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(pool);
+    if (st != BQ_OK) return st;
+    if (e != cudaSuccess) return bq_set_error(lat, BQ_ECUDA, "bq_bench_kernel: %s", cudaGetErrorString(e));
+    *us_per_launch = (double)ms * 1e3 / reps;
+    *bytes_per_launch = bytes * (double)g.Vh;
     return BQ_OK;
 }

@@ -1,0 +1,60 @@
+"""Per-kernel device times of the hot path against the HBM roofline.
+
+    python -m paper_2111_04457_b200.kbench [--lattice 32,32,32,64] [--reps 200] [--nsets 3] [--json]
+
+Each line: kernel, storage precision, link form, microseconds per launch (CUDA events inside libbq's
+bq_bench_kernel, operands rotated over `nsets` scratch sets so that nothing is found in L2), algorithmic
+GB/s (every operand once) and its fraction of the measured copy bandwidth (MEASURED_PEAKS.json).
+Inputs: seeded synthetic gauge field of BASELINE config 3/4 (exp(i*0.5*H)); vector contents are irrelevant.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--lattice", default="32,32,32,64")
+    ap.add_argument("--reps", type=int, default=200)
+    ap.add_argument("--nsets", type=int, default=3)
+    ap.add_argument("--json", action="store_true")
+    ap.add_argument("--precs", default="fp64,fp32,half")
+    args = ap.parse_args()
+    import torch
+    from . import bq, build, inputs
+    assert torch.cuda.is_available(), "kbench needs a CUDA device"
+    build.build()
+    L = tuple(int(v) for v in args.lattice.split(","))
+    peak = 6650.0
+    pk = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(pk):
+        with open(pk) as f:
+            peak = float(json.load(f)["hbm_gbs"])
+    U = inputs.gauge(L, inputs.BASE_SEED + 4, 0.5)
+    rows = []
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        for pname in args.precs.split(","):
+            prec = {"fp64": 0, "fp32": 1, "half": 2}[pname]
+            for which, recon, csw in ([("hop", r, 0.0) for r in (0, 1)] + [("hop_xpay", 0, 0.0), ("hop_clovinv", 0, 1.0), ("hop_clov_xpay", 0, 1.0),
+                                      ("schur", 0, 0.0), ("schur", 0, 1.0), ("norm2", 0, 0.0), ("p_update", 0, 0.0), ("alpha", 0, 0.0),
+                                      ("s_update", 0, 0.0), ("omega", 0, 0.0), ("final", 0, 0.0), ("bicg_iter", 0, 0.0), ("bicg_iter", 1, 0.0),
+                                      ("bicg_iter", 0, 1.0)]):
+                us, nb = bq.bq_bench_kernel(lat.h, which, prec, recon, csw, 0.1215, args.reps, args.nsets)
+                rows.append({"kernel": which, "prec": pname, "recon": 12 if recon else 18, "csw": csw, "us": us, "bytes": nb,
+                             "gbs": nb / us / 1e3, "frac": nb / us / 1e3 / peak})
+    if args.json:
+        print(json.dumps({"lattice": L, "peak_gbs": peak, "rows": rows}))
+        return
+    print(f"# lattice {L}, reps {args.reps}, nsets {args.nsets}, peak {peak:.0f} GB/s (measured copy)")
+    print(f"{'kernel':16s} {'prec':5s} {'links':5s} {'csw':>4s} {'us':>9s} {'MB':>9s} {'GB/s':>8s} {'frac':>6s}")
+    for r in rows:
+        print(f"{r['kernel']:16s} {r['prec']:5s} {r['recon']:<5d} {r['csw']:4.1f} {r['us']:9.1f} {r['bytes'] / 1e6:9.1f} {r['gbs']:8.0f} {r['frac']:6.3f}")
+
+
+if __name__ == "__main__":
+    main()
