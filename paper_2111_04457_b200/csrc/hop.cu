@@ -12,7 +12,10 @@
 #define HOP_BLOCK 128
 #endif
 #ifndef HOP_MINB_LO
-#define HOP_MINB_LO 4   // fp32 / half storage
+#define HOP_MINB_LO 4   // fp32 storage
+#endif
+#ifndef HOP_MINB_HALF
+#define HOP_MINB_HALF 4 // half storage
 #endif
 #ifndef HOP_MINB_64
 #define HOP_MINB_64 2   // fp64
@@ -35,7 +38,7 @@ template <typename C> struct HopArgs {
 // (acc = H in; `scale` is carried by the per-direction weights, so acc arrives at the epilogue already scaled)
 // CPLX: false = all boundary phases real (+-1), true = general complex phases (see hop_dir)
 template <int PREC, int RECON, int EPI, bool CPLX>
-__global__ void __launch_bounds__(HOP_BLOCK, PREC == BQ_FP64 ? HOP_MINB_64 : HOP_MINB_LO)
+__global__ void __launch_bounds__(HOP_BLOCK, PREC == BQ_FP64 ? HOP_MINB_64 : (PREC == BQ_FP32 ? HOP_MINB_LO : HOP_MINB_HALF))
 hop_kernel(const HopArgs<typename Prec<PREC>::comp> a) {
     using C = typename Prec<PREC>::comp;
     const int h = blockIdx.x * HOP_BLOCK + threadIdx.x;
