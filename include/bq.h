@@ -164,6 +164,15 @@ typedef struct {
 bq_status bq_solve(bq_lattice* lat, const double* b, double* x, double kappa, double tol, const bq_solve_opts* opts,
                    bq_solve_info* info);
 
+/* The same operator with the BiCGStab inner products fused into the epilogue of its second hop kernel (SURVEY A6
+ * (iii), (v): no separate reduction pass over the result), exposed for tests:
+ *   w != NULL: dots[0..1] = <w, out>;      w == NULL: dots[0..1] = <out, in>, dots[2] = <out, out>
+ * (<a,b> = sum conj(a_i) b_i).  The sums are taken over the values of out BEFORE they are rounded to the storage
+ * precision (BQ_HALF: before the per-site renormalisation), per thread in the compute type, in fp64 across threads,
+ * in a fixed order.  w: internal-layout even-site field of precision prec.  dots: HOST doubles.  Synchronises. */
+bq_status bq_schur_apply_dots(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw,
+                              bq_prec prec, bq_recon recon, const void* w, double* dots /*[3]*/);
+
 /* Launch accounting for benchmarks: out[0] = kernels launched through this handle since creation,
  * out[1..3] = hop-kernel launches with fp64 / fp32 / half storage (each is 1320 flop x Vh sites). */
 bq_status bq_get_counters(const bq_lattice* lat, unsigned long long* out /*[4]*/);
@@ -198,7 +207,11 @@ typedef enum {
     BQ_K_S_UPDATE = 8,       /* s = r - alpha v                                     (A6 ii)                          */
     BQ_K_OMEGA = 9,          /* <t,s>, <t,t> -> omega                               (A6 iii)                         */
     BQ_K_FINAL = 10,         /* x += alpha p + omega s; r = s - omega t; |r|^2; <rhat,r>   (A6 iv)                   */
-    BQ_K_BICG_ITER = 11      /* one whole inner BiCGStab iteration: 4 hops + 5 BLAS-1 kernels  (A8)                  */
+    BQ_K_BICG_ITER = 11,     /* one whole inner BiCGStab iteration as bq_solve runs it: 4 hops (two of them with
+                                fused inner products) + 3 BLAS-1 kernels                    (A8)                     */
+    BQ_K_HOP_XPAY_ALPHA = 12,   /* out = [A] z + kappa H in and <w, out> -> alpha           (A3 [+A5] + A6 v)        */
+    BQ_K_HOP_XPAY_OMEGA = 13,   /* out = [A] z + kappa H in and <out,z>, <out,out> -> omega  (A3 [+A5] + A6 iii)     */
+    BQ_K_BICG_ITER_UNFUSED = 14 /* the same iteration with the two inner products as separate kernels (4 + 5)        */
 } bq_kernel_id;
 bq_status bq_bench_kernel(bq_lattice* lat, int which, bq_prec prec, bq_recon recon, double csw, double kappa, int reps,
                           int nsets, double* us_per_launch, double* bytes_per_launch);

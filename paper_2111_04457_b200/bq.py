@@ -26,7 +26,7 @@ EXPORTS = [
     "bq_lattice_create", "bq_lattice_destroy", "bq_status_string", "bq_last_error", "bq_gauge_load",
     "bq_field_bytes", "bq_field_import", "bq_field_export", "bq_wilson_apply", "bq_clover_apply",
     "bq_dirac_apply", "bq_schur_apply", "bq_solve", "bq_blas_norm2", "bq_blas_cdot", "bq_blas_caxpy",
-    "bq_blas_bicg_update", "bq_get_counters", "bq_bench_kernel",
+    "bq_blas_bicg_update", "bq_get_counters", "bq_bench_kernel", "bq_schur_apply_dots",
 ]
 
 
@@ -73,6 +73,7 @@ def lib():
         L.bq_clover_apply.argtypes = [_vp, _d, _d, _vp, _vp, _i, _i, _i]
         L.bq_dirac_apply.argtypes = [_vp, _vp, _vp, _d, _d, _i, _i, _vp]
         L.bq_schur_apply.argtypes = [_vp, _vp, _vp, _vp, _d, _d, _i, _i, _vp]
+        L.bq_schur_apply_dots.argtypes = [_vp, _vp, _vp, _vp, _d, _d, _i, _i, _vp, _dp]
         L.bq_solve.argtypes = [_vp, _vp, _vp, _d, _d, ctypes.POINTER(bq_solve_opts), ctypes.POINTER(bq_solve_info)]
         L.bq_blas_norm2.argtypes = [_vp, _vp, _i, _dp]
         L.bq_blas_cdot.argtypes = [_vp, _vp, _vp, _i, _dp]
@@ -165,6 +166,15 @@ def bq_schur_apply(h, out, inp, tmp, kappa, csw, prec, recon=BQ_RECON18, stream=
     _check(h, lib().bq_schur_apply(h, _ptr(out), _ptr(inp), _ptr(tmp), kappa, csw, prec, recon, _stream_ptr(stream)))
 
 
+def bq_schur_apply_dots(h, out, inp, tmp, kappa, csw, prec, recon=BQ_RECON18, w=None):
+    """out = M^ inp with the inner products fused into the hop epilogue: w given -> <w,out>; else (<out,inp>, <out,out>)."""
+    r = (ctypes.c_double * 3)()
+    _check(h, lib().bq_schur_apply_dots(h, _ptr(out), _ptr(inp), _ptr(tmp), kappa, csw, prec, recon, _ptr(w), r))
+    if w is not None:
+        return complex(r[0], r[1])
+    return complex(r[0], r[1]), r[2]
+
+
 def bq_solve(h, b, x, kappa, tol, opts: bq_solve_opts | None = None, raise_on_fail=True):
     """b, x: canonical complex128 arrays (numpy host arrays or torch CUDA tensors); x is in/out.  Returns bq_solve_info."""
     info = bq_solve_info()
@@ -182,7 +192,8 @@ def bq_get_counters(h):
 
 
 BQ_K = {"hop": 0, "hop_xpay": 1, "hop_clovinv": 2, "hop_clov_xpay": 3, "schur": 4, "norm2": 5, "p_update": 6, "alpha": 7,
-        "s_update": 8, "omega": 9, "final": 10, "bicg_iter": 11}
+        "s_update": 8, "omega": 9, "final": 10, "bicg_iter": 11, "hop_xpay_alpha": 12, "hop_xpay_omega": 13,
+        "bicg_iter_unfused": 14}
 
 
 def bq_bench_kernel(h, which, prec, recon=BQ_RECON18, csw=0.0, kappa=0.125, reps=200, nsets=3):

@@ -70,14 +70,7 @@ template <int PREC> BLAS_KERNEL k_cdot(int Vh, const void* __restrict__ a, const
             sc->red[0] = r[0];
             sc->red[1] = r[1];
         } else {
-            // (v) alpha = rho / <rhat, v>
-            sc->rhat_v[0] = r[0];
-            sc->rhat_v[1] = r[1];
-            if (r[0] == 0.0 && r[1] == 0.0) {
-                if (!sc->done) sc->done = 2;
-            } else {
-                cdiv(sc->rho, r, sc->alpha);
-            }
+            fin_alpha(sc, r);   // (v) alpha = rho / <rhat, v>
         }
     });
 }
@@ -204,15 +197,7 @@ template <int PREC> BLAS_KERNEL k_omega(int Vh, const void* __restrict__ t, cons
         }
     }
     double red[3] = {(double)re, (double)im, (double)tt};
-    grid_reduce<3>(red, rb, [sc](const double* r) {
-        sc->ts[0] = r[0]; sc->ts[1] = r[1]; sc->tt = r[2];
-        if (r[2] == 0.0) {
-            if (!sc->done) sc->done = 2;
-        } else {
-            sc->omega[0] = r[0] / r[2];
-            sc->omega[1] = r[1] / r[2];
-        }
-    });
+    grid_reduce<3>(red, rb, [sc](const double* r) { fin_omega(sc, r); });
 }
 
 // (iv) x += alpha p + omega s ; r = s - omega t ; |r|^2 ; <rhat, r>   — one pass over 5 inputs, 2 outputs.

@@ -157,6 +157,31 @@ template <int NRED, class Fin> __device__ __forceinline__ void grid_reduce(doubl
 }
 
 // complex helpers on (re, im) pairs
+__device__ __forceinline__ void cdiv(const double* a, const double* b, double* q);
+
+// Finalisers of the two inner products of a BiCGStab iteration, shared by the stand-alone reduction kernels
+// (blas.cu) and by the hop kernel's fused reduction epilogues (hop.cu).
+// (v)   r = <rhat, v>:            alpha = rho / <rhat, v>
+__device__ __forceinline__ void fin_alpha(SolverScalars* sc, const double* r) {
+    sc->rhat_v[0] = r[0];
+    sc->rhat_v[1] = r[1];
+    if (r[0] == 0.0 && r[1] == 0.0) {
+        if (!sc->done) sc->done = 2;
+    } else {
+        cdiv(sc->rho, r, sc->alpha);
+    }
+}
+// (iii) r = (<t,s>, <t,t>):       omega = <t,s> / <t,t>
+__device__ __forceinline__ void fin_omega(SolverScalars* sc, const double* r) {
+    sc->ts[0] = r[0]; sc->ts[1] = r[1]; sc->tt = r[2];
+    if (r[2] == 0.0) {
+        if (!sc->done) sc->done = 2;
+    } else {
+        sc->omega[0] = r[0] / r[2];
+        sc->omega[1] = r[1] / r[2];
+    }
+}
+
 template <typename C> __device__ __forceinline__ void cfma(C* y, C ar, C ai, const C* x) {   // y += a x
     const C xr = x[0], xi = x[1];
     y[0] = mad(-ai, xi, mad(ar, xr, y[0]));

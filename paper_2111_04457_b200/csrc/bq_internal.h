@@ -30,6 +30,7 @@ __host__ __device__ constexpr size_t prec_real_bytes(int prec) { return prec == 
 __host__ __device__ constexpr size_t spinor_site_bytes(int prec) { return prec == BQ_FP64 ? 192 : (prec == BQ_FP32 ? 96 : 52); }
 
 struct SolverWork;
+struct SolverScalars;
 
 struct bq_lattice {
     Geom g;
@@ -44,6 +45,7 @@ struct bq_lattice {
     double clover_csw, clover_kappa;
     SolverWork* work;
     int* d_flag;             // device int scratch (singular-clover flag etc.)
+    double* hop_partials;    // per-CTA partial sums of the hop kernel's fused reduction epilogues (lazily allocated)
     unsigned long long n_launch;      // kernels launched through this handle
     unsigned long long n_hop[3];      // hop-kernel launches per storage precision
     char err[512];
@@ -88,8 +90,18 @@ bq_status bq_get_clover(bq_lattice* lat, int prec, int inverse, const void** out
 // Clover epilogues (cl != nullptr, 72-real blocks of parity p in precision prec):
 //   cl_mode 1: out = scale * C (H in) [+ z]          (C = A^-1 blocks: the "A_oo^-1 H_oe" step)
 //   cl_mode 2: out = C z + scale * H in               (C = A blocks: the "A_ee x - kappa^2 H ..." step)
+// Fused reduction epilogue (xpay forms only), accumulated on the values before they are rounded to storage:
+//   mode 1: <w, out> -> sc->rhat_v, sc->alpha = sc->rho / <w, out>;   mode 2: <out, z>, <out, out> -> sc->ts, tt, omega
+struct HopRed {
+    int mode;
+    const void* w;
+    SolverScalars* sc;
+};
 bq_status bq_hop(bq_lattice* lat, void* out, const void* in, const void* z, double scale, int out_parity, int prec,
-                 int recon, const void* cl, int cl_mode, cudaStream_t stream);
+                 int recon, const void* cl, int cl_mode, cudaStream_t stream, const HopRed* red = nullptr);
+// out_e = M^ in_e (see bq_schur_apply) with an optional fused reduction on out in the second hop
+bq_status bq_schur_red(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw, int prec, int recon,
+                       cudaStream_t stream, const HopRed* red);
 // out = C in on one parity (site-diagonal clover multiply)
 bq_status bq_clover_mul(bq_lattice* lat, void* out, const void* in, const void* cl, int prec, cudaStream_t stream);
 

@@ -4,6 +4,7 @@
 // shifted rows (still coalesced); the x neighbour is the same half-index or +-1 (Appendix A.5), which the L1
 // serves.  Links are read exactly once (streaming / evict-first loads) so that L2 keeps the input spinor,
 // each site of which is gathered by its 8 neighbours; outputs are streamed.
+#include "blas.cuh"
 #include "clover.cuh"
 #include "hop.cuh"
 
@@ -32,17 +33,74 @@ template <typename C> struct HopArgs {
     int Lxh, Ly, Lz, Lt, Vh, p;
     C scale;              // epilogue scale: weight of a hop that does not wrap
     C phr[4], phi[4];     // scale x boundary phase phi_mu: weight of a hop that wraps in direction mu
+    // fused reduction epilogue (RED != 0)
+    const void* w;        // RED 1: left operand of <w, out>
+    double* partials;     // [grid][NRED]: one partial sum per CTA
 };
+
+// Grid-wide sum for the hop kernel's reduction epilogues (no clusters here: the hop grid is one CTA per 128 sites).
+// Per CTA: warp shuffles -> shared memory -> one partial per CTA, stored and forgotten (no ticket, no fence: a CTA
+// that waited ~2 us for an atomic's return at the end of its ~10 us life cost the memory-bound hop 15-20 %).
+// A one-CTA kernel launched right behind the hop (k_hop_red_final) adds the partials — each thread a fixed strided
+// subset in index order, then a fixed-order tree — and runs the finaliser.  The order of every addition is fixed,
+// so the result is bitwise reproducible.
+template <int NRED> __device__ __forceinline__ void hop_block_partial(const double* v, double* partials) {
+    __shared__ double s_w[NRED][HOP_BLOCK / 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < NRED; k++) {
+        const double x = warp_sum(v[k]);
+        if (lane == 0) s_w[k][warp] = x;
+    }
+    __syncthreads();
+    if (threadIdx.x < NRED) {
+        double a = 0;
+#pragma unroll
+        for (int i = 0; i < HOP_BLOCK / 32; i++) a += s_w[threadIdx.x][i];
+        partials[(size_t)blockIdx.x * NRED + threadIdx.x] = a;
+    }
+}
+
+constexpr int HOP_RED_FINAL_BLOCK = 1024;
+// MODE 1: NRED = 2, fin_alpha;  MODE 2: NRED = 3, fin_omega
+template <int MODE> __global__ void __launch_bounds__(HOP_RED_FINAL_BLOCK) k_hop_red_final(const double* __restrict__ partials, int n,
+                                                                                        SolverScalars* sc) {
+    constexpr int NRED = MODE == 1 ? 2 : 3;
+    __shared__ double s_w[NRED][HOP_RED_FINAL_BLOCK / 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double acc[NRED];
+#pragma unroll
+    for (int k = 0; k < NRED; k++) acc[k] = 0;
+#pragma unroll 4
+    for (int c = threadIdx.x; c < n; c += HOP_RED_FINAL_BLOCK)
+#pragma unroll
+        for (int k = 0; k < NRED; k++) acc[k] += partials[(size_t)c * NRED + k];
+#pragma unroll
+    for (int k = 0; k < NRED; k++) {
+        const double x = warp_sum(acc[k]);
+        if (lane == 0) s_w[k][warp] = x;
+    }
+    __syncthreads();
+    if (warp == 0) {
+        double red[NRED];
+#pragma unroll
+        for (int k = 0; k < NRED; k++) red[k] = warp_sum(s_w[k][lane]);
+        if (lane == 0) {
+            if (MODE == 1) fin_alpha(sc, red);
+            else fin_omega(sc, red);
+        }
+    }
+}
 
 // EPI: 0: out = scale*acc;  1: out = z + scale*acc;  2: out = scale * Cl(acc);  3: out = Cl(z) + scale*acc
 // (acc = H in; `scale` is carried by the per-direction weights, so acc arrives at the epilogue already scaled)
 // CPLX: false = all boundary phases real (+-1), true = general complex phases (see hop_dir)
-template <int PREC, int RECON, int EPI, bool CPLX>
-__global__ void __launch_bounds__(HOP_BLOCK, PREC == BQ_FP64 ? HOP_MINB_64 : (PREC == BQ_FP32 ? HOP_MINB_LO : HOP_MINB_HALF))
-hop_kernel(const HopArgs<typename Prec<PREC>::comp> a) {
+// RED: fused inner products of the BiCGStab iteration on the value just computed (before it is rounded to the
+// storage precision), so that the solver needs no separate reduction pass over it:
+//   0: none;  1: <w, out> -> alpha = rho / <w, out>;  2 (EPI 1, 3 only): <out, z>, <out, out> -> omega
+template <int PREC, int RECON, int EPI, bool CPLX, int RED>
+__device__ __forceinline__ void hop_site(const HopArgs<typename Prec<PREC>::comp>& a, const int h, typename Prec<PREC>::comp* red) {
     using C = typename Prec<PREC>::comp;
-    const int h = blockIdx.x * HOP_BLOCK + threadIdx.x;
-    if (h >= a.Vh) return;
     const int Vh = a.Vh;
     const int xh = h % a.Lxh;
     int q = h / a.Lxh;
@@ -102,16 +160,57 @@ hop_kernel(const HopArgs<typename Prec<PREC>::comp> a) {
     if (EPI == 1 || EPI == 3) {
         C zz[24];
         load_spinor<PREC, true>(a.z, Vh, h, zz);
-        if (EPI == 3) clover_site_mul<PREC>(a.cl, Vh, h, zz);
+        if (EPI == 3) {
+            C az[24];
 #pragma unroll
-        for (int i = 0; i < 24; i++) acc[i] += zz[i];
+            for (int i = 0; i < 24; i++) az[i] = zz[i];
+            clover_site_mul<PREC>(a.cl, Vh, h, az);
+#pragma unroll
+            for (int i = 0; i < 24; i++) acc[i] += az[i];
+        } else {
+#pragma unroll
+            for (int i = 0; i < 24; i++) acc[i] += zz[i];
+        }
+        if (RED == 2) {   // <out, z> = sum conj(out) z ;  <out, out>
+#pragma unroll
+            for (int k = 0; k < 12; k++) {
+                red[0] = mad(acc[2 * k + 1], zz[2 * k + 1], mad(acc[2 * k], zz[2 * k], red[0]));
+                red[1] = mad(-acc[2 * k + 1], zz[2 * k], mad(acc[2 * k], zz[2 * k + 1], red[1]));
+                red[2] = mad(acc[2 * k + 1], acc[2 * k + 1], mad(acc[2 * k], acc[2 * k], red[2]));
+            }
+        }
+    }
+    if (RED == 1) {       // <w, out> = sum conj(w) out
+        C wv[24];
+        load_spinor<PREC, true>(a.w, Vh, h, wv);
+#pragma unroll
+        for (int k = 0; k < 12; k++) {
+            red[0] = mad(wv[2 * k + 1], acc[2 * k + 1], mad(wv[2 * k], acc[2 * k], red[0]));
+            red[1] = mad(-wv[2 * k + 1], acc[2 * k], mad(wv[2 * k], acc[2 * k + 1], red[1]));
+        }
     }
     store_spinor<PREC, true>(a.out, Vh, h, acc);
 }
 
+template <int PREC, int RECON, int EPI, bool CPLX, int RED>
+__global__ void __launch_bounds__(HOP_BLOCK, PREC == BQ_FP64 ? HOP_MINB_64 : (PREC == BQ_FP32 ? HOP_MINB_LO : HOP_MINB_HALF))
+hop_kernel(const HopArgs<typename Prec<PREC>::comp> a) {
+    using C = typename Prec<PREC>::comp;
+    const int h = blockIdx.x * HOP_BLOCK + threadIdx.x;
+    if (RED == 0) {
+        if (h >= a.Vh) return;
+        hop_site<PREC, RECON, EPI, CPLX, 0>(a, h, nullptr);
+    } else {
+        C red[3] = {0, 0, 0};
+        if (h < a.Vh) hop_site<PREC, RECON, EPI, CPLX, RED>(a, h, red);
+        const double v[3] = {(double)red[0], (double)red[1], (double)red[2]};
+        hop_block_partial<RED == 1 ? 2 : 3>(v, a.partials);
+    }
+}
+
 template <int PREC, int RECON>
 static bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const void* z, double scale, int p, const void* gauge,
-                            const void* cl, int cl_mode, cudaStream_t stream) {
+                            const void* cl, int cl_mode, const HopRed* red, cudaStream_t stream) {
     using C = typename Prec<PREC>::comp;
     const Geom& g = lat->g;
     HopArgs<C> a;
@@ -128,25 +227,44 @@ static bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const vo
         if (lat->bc[2 * mu + 1] != 0.0) cplx = true;
     }
     const int grid = (g.Vh + HOP_BLOCK - 1) / HOP_BLOCK;
+    const int rmode = red ? red->mode : 0;
+    a.w = nullptr; a.partials = nullptr;
+    if (rmode) {
+        if ((rmode != 1 && rmode != 2) || !red->sc || (rmode == 1 && !red->w) || !z)
+            return bq_set_error(lat, BQ_EINVAL, "bq_hop: bad fused reduction (mode %d)", rmode);
+        if (!lat->hop_partials) BQ_CUDA(lat, cudaMalloc(&lat->hop_partials, sizeof(double) * 3 * grid));
+        a.w = red->w; a.partials = lat->hop_partials;
+    }
     int epi;
     if (cl_mode == 0) epi = z ? 1 : 0;
     else if (cl_mode == 1 && !z) epi = 2;
     else if (cl_mode == 2 && z) epi = 3;
     else return bq_set_error(lat, BQ_EINVAL, "bq_hop: unsupported epilogue (cl_mode=%d, z=%p)", cl_mode, z);
-#define BQ_HOP_LAUNCH(E)                                                                   \
+#define BQ_HOP_LAUNCH(E, R)                                                                \
     do {                                                                                   \
-        if (cplx) hop_kernel<PREC, RECON, E, true><<<grid, HOP_BLOCK, 0, stream>>>(a);      \
-        else hop_kernel<PREC, RECON, E, false><<<grid, HOP_BLOCK, 0, stream>>>(a);          \
+        if (cplx) hop_kernel<PREC, RECON, E, true, R><<<grid, HOP_BLOCK, 0, stream>>>(a);   \
+        else hop_kernel<PREC, RECON, E, false, R><<<grid, HOP_BLOCK, 0, stream>>>(a);       \
     } while (0)
-    switch (epi) {
-        case 0: BQ_HOP_LAUNCH(0); break;
-        case 1: BQ_HOP_LAUNCH(1); break;
-        case 2: BQ_HOP_LAUNCH(2); break;
-        default: BQ_HOP_LAUNCH(3); break;
+    // fused reductions exist for the xpay epilogues only (the second hop of M^, which produces v and t)
+    switch (epi * 3 + rmode) {
+        case 0: BQ_HOP_LAUNCH(0, 0); break;
+        case 3: BQ_HOP_LAUNCH(1, 0); break;
+        case 4: BQ_HOP_LAUNCH(1, 1); break;
+        case 5: BQ_HOP_LAUNCH(1, 2); break;
+        case 6: BQ_HOP_LAUNCH(2, 0); break;
+        case 9: BQ_HOP_LAUNCH(3, 0); break;
+        case 10: BQ_HOP_LAUNCH(3, 1); break;
+        case 11: BQ_HOP_LAUNCH(3, 2); break;
+        default: return bq_set_error(lat, BQ_EINVAL, "bq_hop: epilogue %d has no fused reduction %d", epi, rmode);
     }
 #undef BQ_HOP_LAUNCH
     BQ_CHECK_LAUNCH(lat);
     lat->n_hop[PREC]++;
+    if (rmode) {
+        if (rmode == 1) k_hop_red_final<1><<<1, HOP_RED_FINAL_BLOCK, 0, stream>>>(lat->hop_partials, grid, red->sc);
+        else k_hop_red_final<2><<<1, HOP_RED_FINAL_BLOCK, 0, stream>>>(lat->hop_partials, grid, red->sc);
+        BQ_CHECK_LAUNCH(lat);
+    }
     return BQ_OK;
 }
 
@@ -158,11 +276,11 @@ extern "C" bq_status bq_get_counters(const bq_lattice* lat, unsigned long long* 
 }
 
 bq_status bq_hop(bq_lattice* lat, void* out, const void* in, const void* z, double scale, int p, int prec, int recon,
-                 const void* cl, int cl_mode, cudaStream_t stream) {
+                 const void* cl, int cl_mode, cudaStream_t stream, const HopRed* red) {
     const void* gauge = nullptr;
     BQ_TRY(bq_get_gauge(lat, prec, recon, &gauge));
 #define BQ_HOP_CASE(P, R) \
-    if (prec == P && recon == R) return launch_hop<P, R>(lat, out, in, z, scale, p, gauge, cl, cl_mode, stream);
+    if (prec == P && recon == R) return launch_hop<P, R>(lat, out, in, z, scale, p, gauge, cl, cl_mode, red, stream);
     BQ_HOP_CASE(BQ_FP64, BQ_RECON18)
     BQ_HOP_CASE(BQ_FP64, BQ_RECON12)
     BQ_HOP_CASE(BQ_FP32, BQ_RECON18)
@@ -214,16 +332,20 @@ extern "C" bq_status bq_dirac_apply(bq_lattice* lat, void* out, const void* in, 
 
 extern "C" bq_status bq_schur_apply(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw,
                                     bq_prec prec, bq_recon recon, void* stream) {
+    return bq_schur_red(lat, out, in, tmp, kappa, csw, prec, recon, static_cast<cudaStream_t>(stream), nullptr);
+}
+
+bq_status bq_schur_red(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw, int prec, int recon,
+                       cudaStream_t s, const HopRed* red) {
     if (!lat) return BQ_EINVAL;
     if (!out || !in || !tmp || out == in || tmp == in || tmp == out)
         return bq_set_error(lat, BQ_EINVAL, "bq_schur_apply: NULL or aliased buffers");
     if (!valid_prec(prec) || !valid_recon(recon)) return bq_set_error(lat, BQ_EINVAL, "bq_schur_apply: bad prec/recon");
     if (!lat->have_gauge) return bq_set_error(lat, BQ_ENOGAUGE, "bq_schur_apply: no gauge field loaded");
-    cudaStream_t s = static_cast<cudaStream_t>(stream);
     if (csw == 0.0) {
         // tmp_o = -kappa H_oe in_e ;  out_e = in_e + kappa H_eo tmp_o = in_e - kappa^2 H_eo H_oe in_e
         BQ_TRY(bq_hop(lat, tmp, in, nullptr, -kappa, 1, prec, recon, nullptr, 0, s));
-        return bq_hop(lat, out, tmp, in, kappa, 0, prec, recon, nullptr, 0, s);
+        return bq_hop(lat, out, tmp, in, kappa, 0, prec, recon, nullptr, 0, s, red);
     }
     BQ_TRY(bq_clover_build(lat, csw, kappa));
     const void *cl = nullptr, *cli = nullptr;
@@ -232,5 +354,5 @@ extern "C" bq_status bq_schur_apply(bq_lattice* lat, void* out, const void* in, 
     const size_t cb = (size_t)lat->g.Vh * CLOVER_REALS * prec_real_bytes(prec);
     // tmp_o = -kappa A_oo^-1 H_oe in_e ;  out_e = A_ee in_e + kappa H_eo tmp_o
     BQ_TRY(bq_hop(lat, tmp, in, nullptr, -kappa, 1, prec, recon, static_cast<const char*>(cli) + cb, 1, s));
-    return bq_hop(lat, out, tmp, in, kappa, 0, prec, recon, cl, 2, s);
+    return bq_hop(lat, out, tmp, in, kappa, 0, prec, recon, cl, 2, s, red);
 }

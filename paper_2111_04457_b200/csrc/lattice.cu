@@ -102,6 +102,7 @@ extern "C" bq_status bq_lattice_destroy(bq_lattice* lat) {
     free_clover(lat);
     bq_solver_free(lat);
     if (lat->d_flag) cudaFree(lat->d_flag);
+    if (lat->hop_partials) cudaFree(lat->hop_partials);
     free(lat);
     return BQ_OK;
 }

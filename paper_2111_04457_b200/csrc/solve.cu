@@ -99,8 +99,8 @@ __global__ void k_set_bicg_scalars(SolverScalars* sc, double ar, double ai, doub
 
 // out_e = M^ in_e in precision prec (tmp: odd scratch)
 static bq_status schur(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw, int prec, int recon,
-                       cudaStream_t s) {
-    return bq_schur_apply(lat, out, in, tmp, kappa, csw, (bq_prec)prec, (bq_recon)recon, s);
+                       cudaStream_t s, const HopRed* red = nullptr) {
+    return bq_schur_red(lat, out, in, tmp, kappa, csw, prec, recon, s, red);
 }
 
 static bq_status poll(bq_lattice* lat, SolverWork* w) {
@@ -123,15 +123,15 @@ static bq_status inner_bicgstab(bq_lattice* lat, SolverWork* w, double kappa, do
     BQ_CUDA(lat, cudaMemcpyAsync(w->irhat, w->ir, fb, cudaMemcpyDeviceToDevice, s));
     BQ_TRY(bicg_init(lat, c, prec, w->ir, stop2));
     int launched = 0;
+    // the two inner products on v and t ride on the second hop of M^ (hop.cu, RED epilogues): 7 kernels per iteration
+    const HopRed red_alpha{1, w->irhat, c.sc}, red_omega{2, nullptr, c.sc};
     for (;;) {
         const int batch = (max_iter - launched) < check_every ? (max_iter - launched) : check_every;
         for (int k = 0; k < batch; k++) {
-            BQ_TRY(bicg_p_update(lat, c, prec, w->ir, w->ip, w->iv));                    // p = r + beta (p - omega v)
-            BQ_TRY(schur(lat, w->iv, w->ip, w->itmp, kappa, csw, prec, recon, s));       // v = M^ p
-            BQ_TRY(bicg_alpha(lat, c, prec, w->irhat, w->iv));                           // alpha = rho / <rhat, v>
-            BQ_TRY(bicg_s_update(lat, c, prec, w->ir, w->iv, w->is));                    // s = r - alpha v
-            BQ_TRY(schur(lat, w->it, w->is, w->itmp, kappa, csw, prec, recon, s));       // t = M^ s
-            BQ_TRY(bicg_omega(lat, c, prec, w->it, w->is));                              // omega = <t,s>/<t,t>
+            BQ_TRY(bicg_p_update(lat, c, prec, w->ir, w->ip, w->iv));                          // p = r + beta (p - omega v)
+            BQ_TRY(schur(lat, w->iv, w->ip, w->itmp, kappa, csw, prec, recon, s, &red_alpha)); // v = M^ p; alpha = rho/<rhat,v>
+            BQ_TRY(bicg_s_update(lat, c, prec, w->ir, w->iv, w->is));                          // s = r - alpha v
+            BQ_TRY(schur(lat, w->it, w->is, w->itmp, kappa, csw, prec, recon, s, &red_omega)); // t = M^ s; omega = <t,s>/<t,t>
             BQ_TRY(bicg_final(lat, c, prec, w->ip, w->is, w->it, w->irhat, w->ie, w->ir));
         }
         launched += batch;
@@ -346,6 +346,27 @@ extern "C" bq_status bq_blas_bicg_update(bq_lattice* lat, const double* alpha, c
     return BQ_OK;
 }
 
+extern "C" bq_status bq_schur_apply_dots(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw,
+                                         bq_prec prec, bq_recon recon, const void* w_vec, double* dots) {
+    SolverWork* w = nullptr;
+    BQ_TRY(blas_entry(lat, prec, &w));
+    if (!dots) return bq_set_error(lat, BQ_EINVAL, "bq_schur_apply_dots: dots is NULL");
+    const HopRed red{w_vec ? 1 : 2, w_vec, w->blas.sc};
+    k_set_bicg_scalars<<<1, 1, 0, w->blas.stream>>>(w->blas.sc, 1, 0, 1, 0);   // rho = 1: alpha = 1 / <w, out>
+    BQ_CHECK_LAUNCH(lat);
+    BQ_TRY(bq_schur_red(lat, out, in, tmp, kappa, csw, prec, recon, w->blas.stream, &red));
+    BQ_TRY(poll(lat, w));
+    if (w_vec) {
+        dots[0] = w->h_sc->rhat_v[0];
+        dots[1] = w->h_sc->rhat_v[1];
+    } else {
+        dots[0] = w->h_sc->ts[0];
+        dots[1] = w->h_sc->ts[1];
+        dots[2] = w->h_sc->tt;
+    }
+    return BQ_OK;
+}
+
 // scratch filler of bq_bench_kernel: finite, non-zero, site- and component-dependent values in [-0.5, 0.5)
 template <int PREC> __global__ void k_bench_fill(int Vh, void* f, unsigned int seed) {
     const int h = blockIdx.x * blockDim.x + threadIdx.x;
@@ -436,17 +457,31 @@ extern "C" bq_status bq_bench_kernel(bq_lattice* lat, int which, bq_prec prec, b
             case BQ_K_S_UPDATE: bytes = 3 * spin_b; return bicg_s_update(lat, c, prec, v0, v1, v2);
             case BQ_K_OMEGA: bytes = 2 * spin_b; return bicg_omega(lat, c, prec, v0, v1);
             case BQ_K_FINAL: bytes = 5 * spin_b + 2 * acc_b; return bicg_final(lat, c, prec, v0, v1, v2, v3, accv(set), v4);
+            case BQ_K_HOP_XPAY_ALPHA: {
+                bytes = 8 * link_b + 4 * spin_b + (clover ? clov_b : 0);
+                const HopRed red{1, v3, c.sc};
+                return bq_hop(lat, v0, v1, v2, kappa, 0, prec, recon, clover ? cl : nullptr, clover ? 2 : 0, s, &red);
+            }
+            case BQ_K_HOP_XPAY_OMEGA: {
+                bytes = 8 * link_b + 3 * spin_b + (clover ? clov_b : 0);
+                const HopRed red{2, nullptr, c.sc};
+                return bq_hop(lat, v0, v1, v2, kappa, 0, prec, recon, clover ? cl : nullptr, clover ? 2 : 0, s, &red);
+            }
+            case BQ_K_BICG_ITER_UNFUSED:
             case BQ_K_BICG_ITER: {
-                // one whole inner iteration: p-update, M^, alpha, s-update, M^, omega, final (same order as inner_bicgstab)
+                // one whole inner iteration (same order as inner_bicgstab): p-update, M^ (+ <rhat,v>), s-update,
+                // M^ (+ <t,s>, <t,t>), final; the UNFUSED form runs the two inner products as separate kernels
+                const bool fused = which == BQ_K_BICG_ITER;
                 const double schur_b = 2 * (8 * link_b + 2 * spin_b) + spin_b + (clover ? 2 * clov_b : 0);
-                bytes = 2 * schur_b + (4 + 2 + 3 + 2 + 5) * spin_b + 2 * acc_b;
+                bytes = 2 * schur_b + (4 + 3 + 5) * spin_b + 2 * acc_b + (fused ? 1 : 4) * spin_b;
                 void* v6 = vec(set, 6);
+                const HopRed red_alpha{1, v3, c.sc}, red_omega{2, nullptr, c.sc};
                 BQ_TRY(bicg_p_update(lat, c, prec, v0, v1, v2));
-                BQ_TRY(schur(lat, v2, v1, v6, kappa, csw, prec, recon, s));
-                BQ_TRY(bicg_alpha(lat, c, prec, v3, v2));
+                BQ_TRY(schur(lat, v2, v1, v6, kappa, csw, prec, recon, s, fused ? &red_alpha : nullptr));
+                if (!fused) BQ_TRY(bicg_alpha(lat, c, prec, v3, v2));
                 BQ_TRY(bicg_s_update(lat, c, prec, v0, v2, v4));
-                BQ_TRY(schur(lat, v5, v4, v6, kappa, csw, prec, recon, s));
-                BQ_TRY(bicg_omega(lat, c, prec, v5, v4));
+                BQ_TRY(schur(lat, v5, v4, v6, kappa, csw, prec, recon, s, fused ? &red_omega : nullptr));
+                if (!fused) BQ_TRY(bicg_omega(lat, c, prec, v5, v4));
                 return bicg_final(lat, c, prec, v1, v4, v5, v3, accv(set), v0);
             }
             default: return bq_set_error(lat, BQ_EINVAL, "bq_bench_kernel: unknown kernel id %d", which);

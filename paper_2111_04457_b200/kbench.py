@@ -42,8 +42,10 @@ def main():
             prec = {"fp64": 0, "fp32": 1, "half": 2}[pname]
             for which, recon, csw in ([("hop", r, 0.0) for r in (0, 1)] + [("hop_xpay", 0, 0.0), ("hop_clovinv", 0, 1.0), ("hop_clov_xpay", 0, 1.0),
                                       ("schur", 0, 0.0), ("schur", 0, 1.0), ("norm2", 0, 0.0), ("p_update", 0, 0.0), ("alpha", 0, 0.0),
-                                      ("s_update", 0, 0.0), ("omega", 0, 0.0), ("final", 0, 0.0), ("bicg_iter", 0, 0.0), ("bicg_iter", 1, 0.0),
-                                      ("bicg_iter", 0, 1.0)]):
+                                      ("s_update", 0, 0.0), ("omega", 0, 0.0), ("final", 0, 0.0), ("hop_xpay_alpha", 0, 0.0),
+                                      ("hop_xpay_omega", 0, 0.0), ("hop_xpay_alpha", 0, 1.0), ("hop_xpay_omega", 0, 1.0),
+                                      ("bicg_iter_unfused", 0, 0.0), ("bicg_iter", 0, 0.0), ("bicg_iter", 1, 0.0),
+                                      ("bicg_iter_unfused", 0, 1.0), ("bicg_iter", 0, 1.0)]):
                 us, nb = bq.bq_bench_kernel(lat.h, which, prec, recon, csw, 0.1215, args.reps, args.nsets)
                 rows.append({"kernel": which, "prec": pname, "recon": 12 if recon else 18, "csw": csw, "us": us, "bytes": nb,
                              "gbs": nb / us / 1e3, "frac": nb / us / 1e3 / peak})
@@ -51,9 +53,9 @@ def main():
         print(json.dumps({"lattice": L, "peak_gbs": peak, "rows": rows}))
         return
     print(f"# lattice {L}, reps {args.reps}, nsets {args.nsets}, peak {peak:.0f} GB/s (measured copy)")
-    print(f"{'kernel':16s} {'prec':5s} {'links':5s} {'csw':>4s} {'us':>9s} {'MB':>9s} {'GB/s':>8s} {'frac':>6s}")
+    print(f"{'kernel':18s} {'prec':5s} {'links':5s} {'csw':>4s} {'us':>9s} {'MB':>9s} {'GB/s':>8s} {'frac':>6s}")
     for r in rows:
-        print(f"{r['kernel']:16s} {r['prec']:5s} {r['recon']:<5d} {r['csw']:4.1f} {r['us']:9.1f} {r['bytes'] / 1e6:9.1f} {r['gbs']:8.0f} {r['frac']:6.3f}")
+        print(f"{r['kernel']:18s} {r['prec']:5s} {r['recon']:<5d} {r['csw']:4.1f} {r['us']:9.1f} {r['bytes'] / 1e6:9.1f} {r['gbs']:8.0f} {r['frac']:6.3f}")
 
 
 if __name__ == "__main__":

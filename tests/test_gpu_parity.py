@@ -210,6 +210,52 @@ def test_wilson_clover_dirac_and_schur(bq, prec, recon):
         assert relmax(lat.export_field(o, prec, bq.BQ_EVEN), ref) < 2 * TOL[prec]
 
 
+@pytest.mark.parametrize("prec", PRECS)
+@pytest.mark.parametrize("csw", [0.0, 1.0])
+@pytest.mark.parametrize("L", [(4, 4, 6, 8), (6, 6, 4, 10)])
+def test_schur_fused_inner_products(bq, prec, csw, L):
+    """A6 (iii), (v) fused into the hop epilogue: <w, M^x>, <M^x, x>, <M^x, M^x> against the oracle's operator and
+    numpy sums; the output field itself must equal the unfused bq_schur_apply (bit for bit in fp64 / fp32; in half
+    storage the two kernel instantiations may contract `z*n + acc` differently, so there to one fp16 ulp)."""
+    import torch
+    kappa = 0.1215
+    U, psi = make_case(L, 34, 0.5)
+    wv = inputs.spinor(L, 35)
+    even = (inputs.site_parity(L) == 0)[..., None, None]
+    A = bqo.clover_build(U, csw, kappa) if csw else None
+    Ainv = bqo.site_matrix_invert(A) if csw else None
+    xe_ref, w_ref = np.where(even, psi, 0), np.where(even, wv, 0)
+    ref = bqo.schur_apply(U, xe_ref, kappa, A=A, Ainv=Ainv)
+    # storage-rounding bound of an inner product, relative to |a||b| (DESIGN.md section 3)
+    tol = {0: 1e-13, 1: 2e-6, 2: 2e-3}[prec]
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        xe = lat.import_field(psi, prec, bq.BQ_EVEN)
+        we = lat.import_field(wv, prec, bq.BQ_EVEN)
+        o, o2, tmp = lat.field(prec, bq.BQ_EVEN), lat.field(prec, bq.BQ_EVEN), lat.field(prec, bq.BQ_ODD)
+        bq.bq_schur_apply(lat.h, o2, xe, tmp, kappa, csw, prec)
+        nr, nx, nw = np.linalg.norm(ref), np.linalg.norm(xe_ref), np.linalg.norm(w_ref)
+        unfused = lat.export_field(o2, prec, bq.BQ_EVEN)
+
+        def same_field():
+            if prec != 2:
+                return torch.equal(o, o2)
+            return relmax(lat.export_field(o, prec, bq.BQ_EVEN), unfused) < 2.0 ** -10
+
+        for rep in range(2):    # twice: no state may be left behind by the first launch
+            wd = bq.bq_schur_apply_dots(lat.h, o, xe, tmp, kappa, csw, prec, w=we)
+            assert same_field()
+            assert abs(wd - np.vdot(w_ref, ref)) < tol * nw * nr
+            ts, tt = bq.bq_schur_apply_dots(lat.h, o, xe, tmp, kappa, csw, prec)
+            assert same_field()
+            assert abs(ts - np.vdot(ref, xe_ref)) < tol * nr * nx
+            assert abs(tt - np.vdot(ref, ref).real) < tol * nr * nr
+            if rep == 0:
+                first = (wd, ts, tt)
+            else:
+                assert first == (wd, ts, tt)      # fixed summation order: bitwise reproducible
+
+
 def test_clover_rebuilds_on_new_gauge_or_parameters(bq):
     L = (4, 4, 4, 4)
     psi = inputs.spinor(L, 33)
