@@ -24,14 +24,17 @@
  * g_4 = diag(1,1,-1,-1).
  *
  * Internal (device-side) field layout, produced by bq_field_import and consumed by the apply calls:
- * even-odd (checkerboard) structure-of-arrays.  parity p = (x+y+z+t)&1, half index
- * h = (x>>1) + (Lx/2)*(y + Ly*(z + Lz*t)), Vh = V/2.  A one-parity spinor is a sequence of 16-byte
- * "planes", plane k holding for every h the reals [k*W, (k+1)*W) of the site's 24 (W = 16/sizeof(real)):
- *   BQ_FP64: 12 planes of double2   (Vh*192 bytes)
- *   BQ_FP32:  6 planes of float4    (Vh* 96 bytes)
- *   BQ_HALF:  3 planes of 8 x fp16 mantissas v_i/n, then one plane of fp32 n = max_i|v_i| (Vh*52 bytes)
- * so a warp reads 32 consecutive sites x 128 bits per load.  A BQ_FULL buffer is the even block
+ * even-odd (checkerboard), site-vectorised, tiled structure of arrays.  parity p = (x+y+z+t)&1, half index
+ * h = (x>>1) + (Lx/2)*(y + Ly*(z + Lz*t)), Vh = V/2 (a multiple of 8).  A site's S bytes are cut into 16-byte
+ * words (word k = reals [k*W, (k+1)*W) of the site's 24, W = 16/sizeof(real)); sites are grouped in tiles of 8
+ * consecutive half indices; inside a tile, word k of the 8 sites is one contiguous 128-byte plane:
+ *     address(h, k) = base + (h >> 3)*8*S + k*128 + (h & 7)*16
+ *   BQ_FP64: 12 words of double2               S = 192   (Vh*192 bytes)
+ *   BQ_FP32:  6 words of float4                S =  96   (Vh* 96 bytes)
+ *   BQ_HALF:  3 words of 8 x fp16 mantissas v_i/n, then a 4-byte fp32 n = max_i|v_i|   S = 52   (Vh*52 bytes)
+ * so a warp of 32 consecutive h reads four whole 128-byte lines per load.  A BQ_FULL buffer is the even block
  * followed by the odd block.  bq_field_bytes gives the sizes.  Buffers must be 16-byte aligned.
+ * A multi-right-hand-side buffer (the *_multi calls) is nrhs such fields one after the other.
  *
  * Ownership: the caller (PyTorch in this repo) allocates and frees every field buffer and passes raw
  * DEVICE pointers; the library never keeps them after the call returns.  The handle owns its gauge
@@ -133,6 +136,16 @@ bq_status bq_dirac_apply(bq_lattice* lat, void* out, const void* in, double kapp
 bq_status bq_schur_apply(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw,
                          bq_prec prec, bq_recon recon, void* stream);
 
+/* Multi-right-hand-side forms (the paper's use case is the 12 spin-colour sources of one
+ * propagator on one gauge field): the same operators applied to nrhs fields in ONE launch per hop, so
+ * that every link is fetched from HBM once for all right-hand sides (compulsory traffic per site and rhs: 8/nrhs links
+ * + 2 spinors).  in / out / tmp: nrhs internal-layout fields one after the other (rhs k at byte offset
+ * k * bq_field_bytes(prec, parity)); results equal nrhs separate single-field calls bit for bit. */
+bq_status bq_wilson_apply_multi(bq_lattice* lat, void* out, const void* in, int nrhs, double kappa, bq_parity parity,
+                                bq_prec prec, bq_recon recon, void* stream);
+bq_status bq_schur_apply_multi(bq_lattice* lat, void* out, const void* in, void* tmp, int nrhs, double kappa, double csw,
+                               bq_prec prec, bq_recon recon, void* stream);
+
 typedef struct {
     int inner_prec;    /* bq_prec: BQ_FP64 = plain fp64 BiCGStab, no outer loop; BQ_FP32 / BQ_HALF = defect correction */
     int recon;         /* bq_recon used by the inner operator (the fp64 outer operator always uses 18 reals)          */
@@ -163,6 +176,17 @@ typedef struct {
  * Errors: BQ_ENOGAUGE, BQ_EINVAL (tol <= 0, NULLs), BQ_ENOTCONVERGED, BQ_EBREAKDOWN, BQ_ESINGULAR_CLOVER, BQ_ECUDA. */
 bq_status bq_solve(bq_lattice* lat, const double* b, double* x, double kappa, double tol, const bq_solve_opts* opts,
                    bq_solve_info* info);
+
+/* The same solve for nrhs right-hand sides at once (Fig. 1 of the paper loops over the 12 spin-colour
+ * sources of a propagator on one configuration).  b, x: nrhs canonical fp64 fields one after the other
+ * (24*V doubles each), HOST or DEVICE.  All right-hand sides advance together: every hop of the batched BiCGStab is ONE
+ * multi-rhs kernel launch (links read once for the batch), every BLAS-1 step one batched launch; each right-hand side
+ * keeps its own device-resident scalars, stops on its own criterion (its iterate is frozen from then on) and gets its
+ * own entry of info[nrhs] (seconds = device time of the whole call).  The mathematics per right-hand side is that of
+ * bq_solve.  Returns BQ_OK only if every right-hand side converged; otherwise the status of the failure, with
+ * info[k].true_rel_residual telling which ones did. */
+bq_status bq_solve_multi(bq_lattice* lat, const double* b, double* x, int nrhs, double kappa, double tol,
+                         const bq_solve_opts* opts, bq_solve_info* info /*[nrhs]*/);
 
 /* The same operator with the BiCGStab inner products fused into the epilogue of its second hop kernel (SURVEY A6
  * (iii), (v): no separate reduction pass over the result), exposed for tests:
@@ -215,6 +239,12 @@ typedef enum {
 } bq_kernel_id;
 bq_status bq_bench_kernel(bq_lattice* lat, int which, bq_prec prec, bq_recon recon, double csw, double kappa, int reps,
                           int nsets, double* us_per_launch, double* bytes_per_launch);
+
+/* The same for the multi-rhs kernels (BQ_K_HOP, BQ_K_HOP_XPAY, BQ_K_HOP_CLOVINV, BQ_K_HOP_CLOV_XPAY, BQ_K_SCHUR):
+ * one launch processes nrhs right-hand sides; bytes_per_launch counts links and clover blocks once and the spinors
+ * once per right-hand side. */
+bq_status bq_bench_kernel_multi(bq_lattice* lat, int which, bq_prec prec, bq_recon recon, double csw, double kappa,
+                                int nrhs, int reps, int nsets, double* us_per_launch, double* bytes_per_launch);
 
 #ifdef __cplusplus
 }

@@ -27,6 +27,7 @@ EXPORTS = [
     "bq_field_bytes", "bq_field_import", "bq_field_export", "bq_wilson_apply", "bq_clover_apply",
     "bq_dirac_apply", "bq_schur_apply", "bq_solve", "bq_blas_norm2", "bq_blas_cdot", "bq_blas_caxpy",
     "bq_blas_bicg_update", "bq_get_counters", "bq_bench_kernel", "bq_schur_apply_dots",
+    "bq_wilson_apply_multi", "bq_schur_apply_multi", "bq_bench_kernel_multi", "bq_solve_multi",
 ]
 
 
@@ -75,12 +76,16 @@ def lib():
         L.bq_schur_apply.argtypes = [_vp, _vp, _vp, _vp, _d, _d, _i, _i, _vp]
         L.bq_schur_apply_dots.argtypes = [_vp, _vp, _vp, _vp, _d, _d, _i, _i, _vp, _dp]
         L.bq_solve.argtypes = [_vp, _vp, _vp, _d, _d, ctypes.POINTER(bq_solve_opts), ctypes.POINTER(bq_solve_info)]
+        L.bq_solve_multi.argtypes = [_vp, _vp, _vp, _i, _d, _d, ctypes.POINTER(bq_solve_opts), ctypes.POINTER(bq_solve_info)]
         L.bq_blas_norm2.argtypes = [_vp, _vp, _i, _dp]
         L.bq_blas_cdot.argtypes = [_vp, _vp, _vp, _i, _dp]
         L.bq_blas_caxpy.argtypes = [_vp, _dp, _vp, _vp, _i]
         L.bq_blas_bicg_update.argtypes = [_vp, _dp, _dp, _vp, _vp, _vp, _vp, _vp, _vp, _i, _dp, _dp]
         L.bq_get_counters.argtypes = [_vp, ctypes.POINTER(ctypes.c_ulonglong)]
         L.bq_bench_kernel.argtypes = [_vp, _i, _i, _i, _d, _d, _i, _i, _dp, _dp]
+        L.bq_wilson_apply_multi.argtypes = [_vp, _vp, _vp, _i, _d, _i, _i, _i, _vp]
+        L.bq_schur_apply_multi.argtypes = [_vp, _vp, _vp, _vp, _i, _d, _d, _i, _i, _vp]
+        L.bq_bench_kernel_multi.argtypes = [_vp, _i, _i, _i, _d, _d, _i, _i, _i, _dp, _dp]
         for name in EXPORTS:
             if name not in ("bq_status_string", "bq_last_error"):
                 getattr(L, name).restype = _i
@@ -166,6 +171,15 @@ def bq_schur_apply(h, out, inp, tmp, kappa, csw, prec, recon=BQ_RECON18, stream=
     _check(h, lib().bq_schur_apply(h, _ptr(out), _ptr(inp), _ptr(tmp), kappa, csw, prec, recon, _stream_ptr(stream)))
 
 
+def bq_wilson_apply_multi(h, out, inp, nrhs, kappa, parity, prec=BQ_FP32, recon=BQ_RECON18, stream=None):
+    _check(h, lib().bq_wilson_apply_multi(h, _ptr(out), _ptr(inp), nrhs, kappa, parity, prec, recon, _stream_ptr(stream)))
+
+
+def bq_schur_apply_multi(h, out, inp, tmp, nrhs, kappa, csw, prec, recon=BQ_RECON18, stream=None):
+    _check(h, lib().bq_schur_apply_multi(h, _ptr(out), _ptr(inp), _ptr(tmp), nrhs, kappa, csw, prec, recon,
+                                         _stream_ptr(stream)))
+
+
 def bq_schur_apply_dots(h, out, inp, tmp, kappa, csw, prec, recon=BQ_RECON18, w=None):
     """out = M^ inp with the inner products fused into the hop epilogue: w given -> <w,out>; else (<out,inp>, <out,out>)."""
     r = (ctypes.c_double * 3)()
@@ -182,6 +196,14 @@ def bq_solve(h, b, x, kappa, tol, opts: bq_solve_opts | None = None, raise_on_fa
                         ctypes.byref(info))
     _check(h, st, allow=() if raise_on_fail else (BQ_ENOTCONVERGED, BQ_EBREAKDOWN))
     return info
+
+
+def bq_solve_multi(h, b, x, nrhs, kappa, tol, opts: bq_solve_opts | None = None, raise_on_fail=True):
+    """b, x: [nrhs, Lt,Lz,Ly,Lx,4,3] complex128 (numpy host arrays or torch CUDA tensors); x is in/out.  Returns [bq_solve_info]."""
+    infos = (bq_solve_info * nrhs)()
+    st = lib().bq_solve_multi(h, _ptr(b), _ptr(x), nrhs, kappa, tol, ctypes.byref(opts) if opts is not None else None, infos)
+    _check(h, st, allow=() if raise_on_fail else (BQ_ENOTCONVERGED, BQ_EBREAKDOWN))
+    return list(infos)
 
 
 def bq_get_counters(h):
@@ -201,6 +223,14 @@ def bq_bench_kernel(h, which, prec, recon=BQ_RECON18, csw=0.0, kappa=0.125, reps
     us, nb = ctypes.c_double(0), ctypes.c_double(0)
     _check(h, lib().bq_bench_kernel(h, BQ_K[which] if isinstance(which, str) else which, prec, recon, csw, kappa, reps, nsets,
                                     ctypes.byref(us), ctypes.byref(nb)))
+    return us.value, nb.value
+
+
+def bq_bench_kernel_multi(h, which, prec, nrhs, recon=BQ_RECON18, csw=0.0, kappa=0.125, reps=50, nsets=2):
+    """(microseconds per launch, algorithmic bytes per launch) of one multi-rhs kernel; a launch covers nrhs fields."""
+    us, nb = ctypes.c_double(0), ctypes.c_double(0)
+    _check(h, lib().bq_bench_kernel_multi(h, BQ_K[which] if isinstance(which, str) else which, prec, recon, csw, kappa, nrhs,
+                                          reps, nsets, ctypes.byref(us), ctypes.byref(nb)))
     return us.value, nb.value
 
 

@@ -28,10 +28,11 @@
 // ---------------------------------------------------------------------------------------------------
 // generic reductions
 // ---------------------------------------------------------------------------------------------------
-template <int PREC> BLAS_KERNEL k_norm2(int Vh, const void* __restrict__ a, RedBuf rb, SolverScalars* sc) {
+template <int PREC> BLAS_KERNEL k_norm2(int Vh, const void* __restrict__ a, RedBuf rb, SolverScalars* sc, size_t stride) {
     using I = Item<PREC>;
     using C = typename I::C;
     constexpr int UNR = UNR_REDUCE(I);
+    a = rhs_field(a, stride); sc += blockIdx.y; rb = rhs_redbuf(rb);
     C acc = 0;
     const int n = I::count(Vh);
     BLAS_TRIPS(I, n) {
@@ -45,10 +46,12 @@ template <int PREC> BLAS_KERNEL k_norm2(int Vh, const void* __restrict__ a, RedB
     grid_reduce<1>(red, rb, [sc](const double* r) { sc->red[0] = r[0]; });
 }
 
-template <int PREC> BLAS_KERNEL k_cdot(int Vh, const void* __restrict__ a, const void* __restrict__ b, RedBuf rb, SolverScalars* sc, int mode) {
+template <int PREC> BLAS_KERNEL k_cdot(int Vh, const void* __restrict__ a, const void* __restrict__ b, RedBuf rb, SolverScalars* sc, int mode,
+                                       size_t stride) {
     using I = Item<PREC>;
     using C = typename I::C;
     constexpr int UNR = UNR_REDUCE(I);
+    a = rhs_field(a, stride); b = rhs_field(b, stride); sc += blockIdx.y; rb = rhs_redbuf(rb);
     C re = 0, im = 0;
     const int n = I::count(Vh);
     BLAS_TRIPS(I, n) {
@@ -99,10 +102,14 @@ template <int PREC> BLAS_KERNEL k_caxpy(int Vh, double ar_, double ai_, const vo
 // BiCGStab steps
 // ---------------------------------------------------------------------------------------------------
 // r2 = |r|^2; with rhat = r: rho = r2, beta = (rho/1)(1/1) = rho (p = v = 0 makes beta irrelevant), alpha = omega = 1
-template <int PREC> BLAS_KERNEL k_init(int Vh, const void* __restrict__ r, RedBuf rb, SolverScalars* sc, double stop2) {
+// stop2s != nullptr: one stopping threshold per right-hand side (device array), else `stop2` for all
+template <int PREC> BLAS_KERNEL k_init(int Vh, const void* __restrict__ r, RedBuf rb, SolverScalars* sc, double stop2,
+                                       const double* __restrict__ stop2s, size_t stride) {
     using I = Item<PREC>;
     using C = typename I::C;
     constexpr int UNR = UNR_REDUCE(I);
+    r = rhs_field(r, stride); sc += blockIdx.y; rb = rhs_redbuf(rb);
+    if (stop2s) stop2 = stop2s[blockIdx.y];
     C acc = 0;
     const int n = I::count(Vh);
     BLAS_TRIPS(I, n) {
@@ -127,10 +134,11 @@ template <int PREC> BLAS_KERNEL k_init(int Vh, const void* __restrict__ r, RedBu
 
 // (i) p = r + beta (p - omega v)
 template <int PREC> BLAS_KERNEL k_p_update(int Vh, const void* __restrict__ r, void* __restrict__ p, const void* __restrict__ v,
-                                           const SolverScalars* __restrict__ sc) {
+                                           const SolverScalars* __restrict__ sc, size_t stride) {
     using I = Item<PREC>;
     using C = typename I::C;
     constexpr int UNR = UNR_UPDATE(I);
+    r = rhs_field(r, stride); p = rhs_field(p, stride); v = rhs_field(v, stride); sc += blockIdx.y;
     if (sc->done) return;
     const C br = (C)sc->beta[0], bi = (C)sc->beta[1], wr = (C)sc->omega[0], wi = (C)sc->omega[1];
     const int n = I::count(Vh);
@@ -154,10 +162,11 @@ template <int PREC> BLAS_KERNEL k_p_update(int Vh, const void* __restrict__ r, v
 
 // (ii) s = r - alpha v
 template <int PREC> BLAS_KERNEL k_s_update(int Vh, const void* __restrict__ r, const void* __restrict__ v, void* __restrict__ s,
-                                           const SolverScalars* __restrict__ sc) {
+                                           const SolverScalars* __restrict__ sc, size_t stride) {
     using I = Item<PREC>;
     using C = typename I::C;
     constexpr int UNR = UNR_UPDATE(I);
+    r = rhs_field(r, stride); v = rhs_field(v, stride); s = rhs_field(s, stride); sc += blockIdx.y;
     if (sc->done) return;
     const C ar = (C)sc->alpha[0], ai = (C)sc->alpha[1];
     const int n = I::count(Vh);
@@ -176,10 +185,12 @@ template <int PREC> BLAS_KERNEL k_s_update(int Vh, const void* __restrict__ r, c
 }
 
 // (iii) <t,s>, <t,t> in one pass; omega = <t,s>/<t,t>
-template <int PREC> BLAS_KERNEL k_omega(int Vh, const void* __restrict__ t, const void* __restrict__ s, RedBuf rb, SolverScalars* sc) {
+template <int PREC> BLAS_KERNEL k_omega(int Vh, const void* __restrict__ t, const void* __restrict__ s, RedBuf rb, SolverScalars* sc,
+                                        size_t stride) {
     using I = Item<PREC>;
     using C = typename I::C;
     constexpr int UNR = UNR_REDUCE(I);
+    t = rhs_field(t, stride); s = rhs_field(s, stride); sc += blockIdx.y; rb = rhs_redbuf(rb);
     C re = 0, im = 0, tt = 0;
     const int n = I::count(Vh);
     BLAS_TRIPS(I, n) {
@@ -204,9 +215,11 @@ template <int PREC> BLAS_KERNEL k_omega(int Vh, const void* __restrict__ t, cons
 // The finaliser prepares the next iteration: rho' = <rhat,r>, beta = (rho'/rho)(alpha/omega), rho = rho'.
 template <int PREC> BLAS_KERNEL k_final(int Vh, const void* __restrict__ p, const void* __restrict__ s, const void* __restrict__ t,
                                         const void* __restrict__ rhat, void* __restrict__ x, void* __restrict__ r, RedBuf rb,
-                                        SolverScalars* sc) {
+                                        SolverScalars* sc, size_t stride, size_t xstride) {
     using I = Item<PREC>;
     using C = typename I::C;
+    p = rhs_field(p, stride); s = rhs_field(s, stride); t = rhs_field(t, stride); rhat = rhs_field(rhat, stride);
+    r = rhs_field(r, stride); x = rhs_field(x, xstride); sc += blockIdx.y; rb = rhs_redbuf(rb);
     if (sc->done) return;   // converged or broken down in an earlier iteration of this batch: x stays frozen
     const C ar = (C)sc->alpha[0], ai = (C)sc->alpha[1], wr = (C)sc->omega[0], wi = (C)sc->omega[1];
     C r2 = 0, re = 0, im = 0;
@@ -289,9 +302,10 @@ template <int PREC> BLAS_KERNEL k_final(int Vh, const void* __restrict__ p, cons
 // outer loop (fp64)
 // ---------------------------------------------------------------------------------------------------
 BLAS_KERNEL k_outer_residual(int Vh, const void* __restrict__ b, const void* __restrict__ t, void* __restrict__ r, RedBuf rb,
-                             SolverScalars* sc) {
+                             SolverScalars* sc, size_t bstride, size_t stride) {
     using I = Item<BQ_FP64>;
     constexpr int UNR = UNR_UPDATE(I);
+    b = rhs_field(b, bstride); t = rhs_field(t, stride); r = rhs_field(r, stride); sc += blockIdx.y; rb = rhs_redbuf(rb);
     double acc = 0;
     const int n = I::count(Vh);
     BLAS_TRIPS(I, n) {
@@ -317,9 +331,10 @@ BLAS_KERNEL k_outer_residual(int Vh, const void* __restrict__ b, const void* __r
 }
 
 template <int PREC_LO> __global__ void __launch_bounds__(128) k_to_low(int Vh, const void* __restrict__ r64, void* __restrict__ lo,
-                                                                      const SolverScalars* __restrict__ sc) {
+                                                                      const SolverScalars* __restrict__ sc, size_t stride64, size_t stride_lo) {
     const int h = blockIdx.x * blockDim.x + threadIdx.x;
     if (h >= Vh) return;
+    r64 = rhs_field(r64, stride64); lo = rhs_field(lo, stride_lo); sc += blockIdx.y;
     const double sca = sc->scale;
     double v[24];
     load_spinor<BQ_FP64, true>(r64, Vh, h, v);
@@ -330,9 +345,10 @@ template <int PREC_LO> __global__ void __launch_bounds__(128) k_to_low(int Vh, c
 }
 
 template <int EPREC> __global__ void __launch_bounds__(128) k_accumulate(int Vh, const void* __restrict__ e, void* __restrict__ x64,
-                                                                        const SolverScalars* __restrict__ sc) {
+                                                                        const SolverScalars* __restrict__ sc, size_t estride, size_t xstride) {
     const int h = blockIdx.x * blockDim.x + threadIdx.x;
     if (h >= Vh) return;
+    e = rhs_field(e, estride); x64 = rhs_field(x64, xstride); sc += blockIdx.y;
     const double rn = sc->rnorm;
     typename Prec<EPREC>::comp ev[24];
     load_spinor<EPREC, true>(e, Vh, h, ev);
@@ -351,7 +367,7 @@ bq_status blas_ctx_create(bq_lattice* lat, BlasCtx* c) {
     BQ_CUDA(lat, cudaGetDevice(&dev));
     BQ_CUDA(lat, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     c->Vh = lat->g.Vh;
-    // persistent-style grid: 8 CTAs of 256 threads per SM = full occupancy (a multiple of the SM count and of the
+    // persistent-style grid: BLAS_CTAS_PER_SM CTAs of 256 threads per SM (a multiple of the SM count and of the
     // cluster size), trimmed for small lattices so that no cluster is empty-handed more than necessary
     int grid = sms * BLAS_CTAS_PER_SM;
     const int need = (12 * lat->g.Vh + BLAS_BLOCK - 1) / BLAS_BLOCK;
@@ -359,11 +375,23 @@ bq_status blas_ctx_create(bq_lattice* lat, BlasCtx* c) {
     grid = ((grid + BLAS_CLUSTER - 1) / BLAS_CLUSTER) * BLAS_CLUSTER;
     c->grid = grid;
     c->stream = 0;
-    BQ_CUDA(lat, cudaMalloc(&c->partials, sizeof(double) * 4 * (grid / BLAS_CLUSTER)));
-    BQ_CUDA(lat, cudaMalloc(&c->ticket, sizeof(unsigned int)));
-    BQ_CUDA(lat, cudaMemset(c->ticket, 0, sizeof(unsigned int)));
-    BQ_CUDA(lat, cudaMalloc(&c->sc, sizeof(SolverScalars)));
-    BQ_CUDA(lat, cudaMemset(c->sc, 0, sizeof(SolverScalars)));
+    c->nrhs = 1; c->stride = 0; c->xstride = 0; c->stride64 = 0;
+    c->cap = 0; c->partials = nullptr; c->ticket = nullptr; c->sc = nullptr; c->stop2s = nullptr;
+    return blas_ctx_reserve(lat, c, 1);
+}
+
+// scratch and solver states for up to nrhs right-hand sides
+bq_status blas_ctx_reserve(bq_lattice* lat, BlasCtx* c, int nrhs) {
+    if (nrhs <= c->cap) return BQ_OK;
+    blas_ctx_destroy(c);
+    c->pstride = 4 * (c->grid / BLAS_CLUSTER);
+    BQ_CUDA(lat, cudaMalloc(&c->partials, sizeof(double) * c->pstride * nrhs));
+    BQ_CUDA(lat, cudaMalloc(&c->ticket, sizeof(unsigned int) * nrhs));
+    BQ_CUDA(lat, cudaMemset(c->ticket, 0, sizeof(unsigned int) * nrhs));
+    BQ_CUDA(lat, cudaMalloc(&c->sc, sizeof(SolverScalars) * nrhs));
+    BQ_CUDA(lat, cudaMemset(c->sc, 0, sizeof(SolverScalars) * nrhs));
+    BQ_CUDA(lat, cudaMalloc(&c->stop2s, sizeof(double) * nrhs));
+    c->cap = nrhs;
     return BQ_OK;
 }
 
@@ -371,71 +399,79 @@ void blas_ctx_destroy(BlasCtx* c) {
     if (c->partials) cudaFree(c->partials);
     if (c->ticket) cudaFree(c->ticket);
     if (c->sc) cudaFree(c->sc);
-    c->partials = nullptr; c->ticket = nullptr; c->sc = nullptr;
+    if (c->stop2s) cudaFree(c->stop2s);
+    c->partials = nullptr; c->ticket = nullptr; c->sc = nullptr; c->stop2s = nullptr; c->cap = 0;
 }
 
-#define DISPATCH_PREC(prec, KERNEL, ...)                                                             \
-    do {                                                                                             \
-        if ((prec) == BQ_FP64) KERNEL<BQ_FP64><<<c.grid, BLAS_BLOCK, 0, c.stream>>>(__VA_ARGS__);    \
-        else if ((prec) == BQ_FP32) KERNEL<BQ_FP32><<<c.grid, BLAS_BLOCK, 0, c.stream>>>(__VA_ARGS__); \
-        else KERNEL<BQ_HALF><<<c.grid, BLAS_BLOCK, 0, c.stream>>>(__VA_ARGS__);                      \
-        BQ_CHECK_LAUNCH(lat);                                                            \
-        return BQ_OK;                                                                                \
+// c.nrhs right-hand sides per launch (gridDim.y), operand fields c.stride bytes apart (storage precision of the call)
+#define DISPATCH_PREC(prec, KERNEL, ...)                                                          \
+    do {                                                                                          \
+        const dim3 g_(c.grid, c.nrhs);                                                            \
+        if ((prec) == BQ_FP64) KERNEL<BQ_FP64><<<g_, BLAS_BLOCK, 0, c.stream>>>(__VA_ARGS__);     \
+        else if ((prec) == BQ_FP32) KERNEL<BQ_FP32><<<g_, BLAS_BLOCK, 0, c.stream>>>(__VA_ARGS__); \
+        else KERNEL<BQ_HALF><<<g_, BLAS_BLOCK, 0, c.stream>>>(__VA_ARGS__);                       \
+        BQ_CHECK_LAUNCH(lat);                                                                     \
+        return BQ_OK;                                                                             \
     } while (0)
 
 bq_status blas_norm2(bq_lattice* lat, const BlasCtx& c, int prec, const void* a) {
-    RedBuf rb{c.partials, c.ticket};
-    DISPATCH_PREC(prec, k_norm2, c.Vh, a, rb, c.sc);
+    RedBuf rb{c.partials, c.ticket, c.pstride};
+    DISPATCH_PREC(prec, k_norm2, c.Vh, a, rb, c.sc, c.stride);
 }
 bq_status blas_cdot(bq_lattice* lat, const BlasCtx& c, int prec, const void* a, const void* b) {
-    RedBuf rb{c.partials, c.ticket};
-    DISPATCH_PREC(prec, k_cdot, c.Vh, a, b, rb, c.sc, 0);
+    RedBuf rb{c.partials, c.ticket, c.pstride};
+    DISPATCH_PREC(prec, k_cdot, c.Vh, a, b, rb, c.sc, 0, c.stride);
 }
 bq_status blas_caxpy(bq_lattice* lat, const BlasCtx& c, int prec, double ar, double ai, const void* x, void* y) {
-    DISPATCH_PREC(prec, k_caxpy, c.Vh, ar, ai, x, y);
+    const BlasCtx one = blas_single(c);
+    {
+        const BlasCtx& c = one;
+        DISPATCH_PREC(prec, k_caxpy, c.Vh, ar, ai, x, y);
+    }
+    return BQ_OK;
 }
-bq_status bicg_init(bq_lattice* lat, const BlasCtx& c, int prec, const void* r, double stop2) {
-    RedBuf rb{c.partials, c.ticket};
-    DISPATCH_PREC(prec, k_init, c.Vh, r, rb, c.sc, stop2);
+bq_status bicg_init(bq_lattice* lat, const BlasCtx& c, int prec, const void* r, double stop2, bool per_rhs_stop2) {
+    RedBuf rb{c.partials, c.ticket, c.pstride};
+    DISPATCH_PREC(prec, k_init, c.Vh, r, rb, c.sc, stop2, per_rhs_stop2 ? c.stop2s : nullptr, c.stride);
 }
 bq_status bicg_p_update(bq_lattice* lat, const BlasCtx& c, int prec, const void* r, void* p, const void* v) {
-    DISPATCH_PREC(prec, k_p_update, c.Vh, r, p, v, c.sc);
+    DISPATCH_PREC(prec, k_p_update, c.Vh, r, p, v, c.sc, c.stride);
 }
 bq_status bicg_alpha(bq_lattice* lat, const BlasCtx& c, int prec, const void* rhat, const void* v) {
-    RedBuf rb{c.partials, c.ticket};
-    DISPATCH_PREC(prec, k_cdot, c.Vh, rhat, v, rb, c.sc, 1);
+    RedBuf rb{c.partials, c.ticket, c.pstride};
+    DISPATCH_PREC(prec, k_cdot, c.Vh, rhat, v, rb, c.sc, 1, c.stride);
 }
 bq_status bicg_s_update(bq_lattice* lat, const BlasCtx& c, int prec, const void* r, const void* v, void* s) {
-    DISPATCH_PREC(prec, k_s_update, c.Vh, r, v, s, c.sc);
+    DISPATCH_PREC(prec, k_s_update, c.Vh, r, v, s, c.sc, c.stride);
 }
 bq_status bicg_omega(bq_lattice* lat, const BlasCtx& c, int prec, const void* t, const void* s) {
-    RedBuf rb{c.partials, c.ticket};
-    DISPATCH_PREC(prec, k_omega, c.Vh, t, s, rb, c.sc);
+    RedBuf rb{c.partials, c.ticket, c.pstride};
+    DISPATCH_PREC(prec, k_omega, c.Vh, t, s, rb, c.sc, c.stride);
 }
 bq_status bicg_final(bq_lattice* lat, const BlasCtx& c, int prec, const void* p, const void* s, const void* t, const void* rhat,
                      void* x, void* r) {
-    RedBuf rb{c.partials, c.ticket};
-    DISPATCH_PREC(prec, k_final, c.Vh, p, s, t, rhat, x, r, rb, c.sc);
+    RedBuf rb{c.partials, c.ticket, c.pstride};
+    DISPATCH_PREC(prec, k_final, c.Vh, p, s, t, rhat, x, r, rb, c.sc, c.stride, c.xstride);
 }
 
-bq_status outer_residual(bq_lattice* lat, const BlasCtx& c, const void* b, const void* t, void* r) {
-    RedBuf rb{c.partials, c.ticket};
-    k_outer_residual<<<c.grid, BLAS_BLOCK, 0, c.stream>>>(c.Vh, b, t, r, rb, c.sc);
+bq_status outer_residual(bq_lattice* lat, const BlasCtx& c, const void* b, size_t bstride, const void* t, void* r) {
+    RedBuf rb{c.partials, c.ticket, c.pstride};
+    k_outer_residual<<<dim3(c.grid, c.nrhs), BLAS_BLOCK, 0, c.stream>>>(c.Vh, b, t, r, rb, c.sc, bstride, c.stride64);
     BQ_CHECK_LAUNCH(lat);
     return BQ_OK;
 }
 bq_status outer_to_low(bq_lattice* lat, const BlasCtx& c, int prec_lo, const void* r64, void* lo) {
-    const int grid = (c.Vh + 127) / 128;
-    if (prec_lo == BQ_FP64) k_to_low<BQ_FP64><<<grid, 128, 0, c.stream>>>(c.Vh, r64, lo, c.sc);
-    else if (prec_lo == BQ_FP32) k_to_low<BQ_FP32><<<grid, 128, 0, c.stream>>>(c.Vh, r64, lo, c.sc);
-    else k_to_low<BQ_HALF><<<grid, 128, 0, c.stream>>>(c.Vh, r64, lo, c.sc);
+    const dim3 grid((c.Vh + 127) / 128, c.nrhs);
+    if (prec_lo == BQ_FP64) k_to_low<BQ_FP64><<<grid, 128, 0, c.stream>>>(c.Vh, r64, lo, c.sc, c.stride64, c.stride);
+    else if (prec_lo == BQ_FP32) k_to_low<BQ_FP32><<<grid, 128, 0, c.stream>>>(c.Vh, r64, lo, c.sc, c.stride64, c.stride);
+    else k_to_low<BQ_HALF><<<grid, 128, 0, c.stream>>>(c.Vh, r64, lo, c.sc, c.stride64, c.stride);
     BQ_CHECK_LAUNCH(lat);
     return BQ_OK;
 }
-bq_status outer_accumulate(bq_lattice* lat, const BlasCtx& c, int e_prec, const void* e, void* x64) {
-    const int grid = (c.Vh + 127) / 128;
-    if (e_prec == BQ_FP64) k_accumulate<BQ_FP64><<<grid, 128, 0, c.stream>>>(c.Vh, e, x64, c.sc);
-    else if (e_prec == BQ_FP32) k_accumulate<BQ_FP32><<<grid, 128, 0, c.stream>>>(c.Vh, e, x64, c.sc);
+bq_status outer_accumulate(bq_lattice* lat, const BlasCtx& c, int e_prec, const void* e, void* x64, size_t x64stride) {
+    const dim3 grid((c.Vh + 127) / 128, c.nrhs);
+    if (e_prec == BQ_FP64) k_accumulate<BQ_FP64><<<grid, 128, 0, c.stream>>>(c.Vh, e, x64, c.sc, c.xstride, x64stride);
+    else if (e_prec == BQ_FP32) k_accumulate<BQ_FP32><<<grid, 128, 0, c.stream>>>(c.Vh, e, x64, c.sc, c.xstride, x64stride);
     else return bq_set_error(lat, BQ_EINVAL, "outer_accumulate: accumulator cannot be half");
     BQ_CHECK_LAUNCH(lat);
     return BQ_OK;

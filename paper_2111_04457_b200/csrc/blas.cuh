@@ -94,9 +94,20 @@ struct SolverScalars {
 };
 
 struct RedBuf {
-    double* partials;        // [clusters][NRED]
-    unsigned int* ticket;
+    double* partials;        // [rhs][clusters][4]
+    unsigned int* ticket;    // [rhs]
+    int pstride;             // doubles of partials per right-hand side
 };
+
+// Batched (multi-rhs) launches: gridDim.y = right-hand sides; blockIdx.y selects the operand fields (`stride` bytes
+// apart), the BiCGStab state sc[rhs] and the reduction scratch of that right-hand side.  gridDim.y = 1 is the plain case.
+__device__ __forceinline__ const void* rhs_field(const void* p, size_t stride) { return static_cast<const char*>(p) + blockIdx.y * stride; }
+__device__ __forceinline__ void* rhs_field(void* p, size_t stride) { return static_cast<char*>(p) + blockIdx.y * stride; }
+__device__ __forceinline__ RedBuf rhs_redbuf(RedBuf rb) {
+    rb.partials += (size_t)blockIdx.y * rb.pstride;
+    rb.ticket += blockIdx.y;
+    return rb;
+}
 
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll

@@ -46,6 +46,7 @@ struct bq_lattice {
     SolverWork* work;
     int* d_flag;             // device int scratch (singular-clover flag etc.)
     double* hop_partials;    // per-CTA partial sums of the hop kernel's fused reduction epilogues (lazily allocated)
+    size_t hop_partials_cap; // doubles allocated there
     unsigned long long n_launch;      // kernels launched through this handle
     unsigned long long n_hop[3];      // hop-kernel launches per storage precision
     char err[512];
@@ -97,11 +98,18 @@ struct HopRed {
     const void* w;
     SolverScalars* sc;
 };
+// Multi-rhs form: every operand is an array of nrhs one-parity fields, s_* bytes apart; red->sc is an array of nrhs
+// SolverScalars (one BiCGStab state per right-hand side).
+struct HopMulti {
+    int nrhs;
+    size_t s_in, s_out, s_z, s_w;
+};
 bq_status bq_hop(bq_lattice* lat, void* out, const void* in, const void* z, double scale, int out_parity, int prec,
-                 int recon, const void* cl, int cl_mode, cudaStream_t stream, const HopRed* red = nullptr);
+                 int recon, const void* cl, int cl_mode, cudaStream_t stream, const HopRed* red = nullptr,
+                 const HopMulti* multi = nullptr);
 // out_e = M^ in_e (see bq_schur_apply) with an optional fused reduction on out in the second hop
 bq_status bq_schur_red(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw, int prec, int recon,
-                       cudaStream_t stream, const HopRed* red);
+                       cudaStream_t stream, const HopRed* red, int nrhs = 0 /* 0: single field; >= 1: arrays of nrhs fields */);
 // out = C in on one parity (site-diagonal clover multiply)
 bq_status bq_clover_mul(bq_lattice* lat, void* out, const void* in, const void* cl, int prec, cudaStream_t stream);
 

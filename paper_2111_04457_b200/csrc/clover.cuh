@@ -65,20 +65,20 @@ __device__ __forceinline__ void load_clover_block(const void* base, int Vh, int 
 }
 
 // v <- C(x) v for the spinor v (24 reals) of site h, C = the two stored blocks (A or A^-1).
-template <int PREC>
+template <int PREC, bool STREAM = true>
 __device__ __forceinline__ void clover_site_mul(const void* cl, int Vh, int h, typename Prec<PREC>::comp* v) {
     using C = typename Prec<PREC>::comp;
     C chi[12], yp[12], ym[12];
     {
         C blk[36];
-        load_clover_block<PREC, 0>(cl, Vh, h, blk);
+        load_clover_block<PREC, 0, STREAM>(cl, Vh, h, blk);
 #pragma unroll
         for (int i = 0; i < 12; i++) chi[i] = v[i] + v[12 + i];
         herm6_mul(blk, chi, yp);
     }
     {
         C blk[36];
-        load_clover_block<PREC, 1>(cl, Vh, h, blk);
+        load_clover_block<PREC, 1, STREAM>(cl, Vh, h, blk);
 #pragma unroll
         for (int i = 0; i < 12; i++) chi[i] = v[i] - v[12 + i];
         herm6_mul(blk, chi, ym);

@@ -35,7 +35,10 @@ template <typename C> struct HopArgs {
     C phr[4], phi[4];     // scale x boundary phase phi_mu: weight of a hop that wraps in direction mu
     // fused reduction epilogue (RED != 0)
     const void* w;        // RED 1: left operand of <w, out>
-    double* partials;     // [grid][NRED]: one partial sum per CTA
+    double* partials;     // [rhs][grid][NRED]: one partial sum per CTA (and right-hand side)
+    // multi-rhs form (hop_kernel_mrhs): nrhs fields per operand, `s_*` bytes apart; T tiles of 8 sites per CTA
+    int nrhs, T;
+    size_t s_in, s_out, s_z, s_w;
 };
 
 // Grid-wide sum for the hop kernel's reduction epilogues (no clusters here: the hop grid is one CTA per 128 sites).
@@ -63,9 +66,12 @@ template <int NRED> __device__ __forceinline__ void hop_block_partial(const doub
 
 constexpr int HOP_RED_FINAL_BLOCK = 1024;
 // MODE 1: NRED = 2, fin_alpha;  MODE 2: NRED = 3, fin_omega
+// One CTA per right-hand side (blockIdx.x): partials [rhs][n][NRED], scalars sc[rhs].
 template <int MODE> __global__ void __launch_bounds__(HOP_RED_FINAL_BLOCK) k_hop_red_final(const double* __restrict__ partials, int n,
                                                                                         SolverScalars* sc) {
     constexpr int NRED = MODE == 1 ? 2 : 3;
+    partials += (size_t)blockIdx.x * n * NRED;
+    sc += blockIdx.x;
     __shared__ double s_w[NRED][HOP_RED_FINAL_BLOCK / 32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double acc[NRED];
@@ -98,8 +104,10 @@ template <int MODE> __global__ void __launch_bounds__(HOP_RED_FINAL_BLOCK) k_hop
 // RED: fused inner products of the BiCGStab iteration on the value just computed (before it is rounded to the
 // storage precision), so that the solver needs no separate reduction pass over it:
 //   0: none;  1: <w, out> -> alpha = rho / <w, out>;  2 (EPI 1, 3 only): <out, z>, <out, out> -> omega
-template <int PREC, int RECON, int EPI, bool CPLX, int RED>
-__device__ __forceinline__ void hop_site(const HopArgs<typename Prec<PREC>::comp>& a, const int h, typename Prec<PREC>::comp* red) {
+// in / out / zp / wp: the operand fields of this thread's right-hand side; LSTREAM: see hop_dir.
+template <int PREC, int RECON, int EPI, bool CPLX, int RED, bool LSTREAM = true>
+__device__ __forceinline__ void hop_site(const HopArgs<typename Prec<PREC>::comp>& a, const int h, const void* in, void* out,
+                                         const void* zp, const void* wp, typename Prec<PREC>::comp* red) {
     using C = typename Prec<PREC>::comp;
     const int Vh = a.Vh;
     const int xh = h % a.Lxh;
@@ -122,49 +130,49 @@ __device__ __forceinline__ void hop_site(const HopArgs<typename Prec<PREC>::comp
     {
         const bool wf = r && (xh == a.Lxh - 1);
         const int nf = r ? (wf ? h - (a.Lxh - 1) : h + 1) : h;
-        hop_dir<PREC, RECON, 0, true, CPLX>(acc, a.in, Vh, nf, gf, h, wf ? a.phr[0] : one, wf ? a.phi[0] : zero);
+        hop_dir<PREC, RECON, 0, true, CPLX, LSTREAM>(acc, in, Vh, nf, gf, h, wf ? a.phr[0] : one, wf ? a.phi[0] : zero);
         const bool wb = !r && (xh == 0);
         const int nb = r ? h : (wb ? h + (a.Lxh - 1) : h - 1);
-        hop_dir<PREC, RECON, 0, false, CPLX>(acc, a.in, Vh, nb, gb, nb, wb ? a.phr[0] : one, wb ? -a.phi[0] : zero);
+        hop_dir<PREC, RECON, 0, false, CPLX, LSTREAM>(acc, in, Vh, nb, gb, nb, wb ? a.phr[0] : one, wb ? -a.phi[0] : zero);
     }
     // ---- y ----
     {
         const bool wf = (y == a.Ly - 1);
         const int nf = wf ? h - (a.Ly - 1) * sy : h + sy;
-        hop_dir<PREC, RECON, 1, true, CPLX>(acc, a.in, Vh, nf, gf + a.ublk, h, wf ? a.phr[1] : one, wf ? a.phi[1] : zero);
+        hop_dir<PREC, RECON, 1, true, CPLX, LSTREAM>(acc, in, Vh, nf, gf + a.ublk, h, wf ? a.phr[1] : one, wf ? a.phi[1] : zero);
         const bool wb = (y == 0);
         const int nb = wb ? h + (a.Ly - 1) * sy : h - sy;
-        hop_dir<PREC, RECON, 1, false, CPLX>(acc, a.in, Vh, nb, gb + a.ublk, nb, wb ? a.phr[1] : one, wb ? -a.phi[1] : zero);
+        hop_dir<PREC, RECON, 1, false, CPLX, LSTREAM>(acc, in, Vh, nb, gb + a.ublk, nb, wb ? a.phr[1] : one, wb ? -a.phi[1] : zero);
     }
     // ---- z ----
     {
         const bool wf = (z == a.Lz - 1);
         const int nf = wf ? h - (a.Lz - 1) * sz : h + sz;
-        hop_dir<PREC, RECON, 2, true, CPLX>(acc, a.in, Vh, nf, gf + 2 * a.ublk, h, wf ? a.phr[2] : one, wf ? a.phi[2] : zero);
+        hop_dir<PREC, RECON, 2, true, CPLX, LSTREAM>(acc, in, Vh, nf, gf + 2 * a.ublk, h, wf ? a.phr[2] : one, wf ? a.phi[2] : zero);
         const bool wb = (z == 0);
         const int nb = wb ? h + (a.Lz - 1) * sz : h - sz;
-        hop_dir<PREC, RECON, 2, false, CPLX>(acc, a.in, Vh, nb, gb + 2 * a.ublk, nb, wb ? a.phr[2] : one, wb ? -a.phi[2] : zero);
+        hop_dir<PREC, RECON, 2, false, CPLX, LSTREAM>(acc, in, Vh, nb, gb + 2 * a.ublk, nb, wb ? a.phr[2] : one, wb ? -a.phi[2] : zero);
     }
     // ---- t ----
     {
         const bool wf = (t == a.Lt - 1);
         const int nf = wf ? h - (a.Lt - 1) * st : h + st;
-        hop_dir<PREC, RECON, 3, true, CPLX>(acc, a.in, Vh, nf, gf + 3 * a.ublk, h, wf ? a.phr[3] : one, wf ? a.phi[3] : zero);
+        hop_dir<PREC, RECON, 3, true, CPLX, LSTREAM>(acc, in, Vh, nf, gf + 3 * a.ublk, h, wf ? a.phr[3] : one, wf ? a.phi[3] : zero);
         const bool wb = (t == 0);
         const int nb = wb ? h + (a.Lt - 1) * st : h - st;
-        hop_dir<PREC, RECON, 3, false, CPLX>(acc, a.in, Vh, nb, gb + 3 * a.ublk, nb, wb ? a.phr[3] : one, wb ? -a.phi[3] : zero);
+        hop_dir<PREC, RECON, 3, false, CPLX, LSTREAM>(acc, in, Vh, nb, gb + 3 * a.ublk, nb, wb ? a.phr[3] : one, wb ? -a.phi[3] : zero);
     }
 
     // ---- epilogue ----
-    if (EPI == 2) clover_site_mul<PREC>(a.cl, Vh, h, acc);   // linear: the scale already inside acc commutes with it
+    if (EPI == 2) clover_site_mul<PREC, LSTREAM>(a.cl, Vh, h, acc);   // linear: the scale already inside acc commutes with it
     if (EPI == 1 || EPI == 3) {
         C zz[24];
-        load_spinor<PREC, true>(a.z, Vh, h, zz);
+        load_spinor<PREC, true>(zp, Vh, h, zz);
         if (EPI == 3) {
             C az[24];
 #pragma unroll
             for (int i = 0; i < 24; i++) az[i] = zz[i];
-            clover_site_mul<PREC>(a.cl, Vh, h, az);
+            clover_site_mul<PREC, LSTREAM>(a.cl, Vh, h, az);
 #pragma unroll
             for (int i = 0; i < 24; i++) acc[i] += az[i];
         } else {
@@ -182,14 +190,14 @@ __device__ __forceinline__ void hop_site(const HopArgs<typename Prec<PREC>::comp
     }
     if (RED == 1) {       // <w, out> = sum conj(w) out
         C wv[24];
-        load_spinor<PREC, true>(a.w, Vh, h, wv);
+        load_spinor<PREC, true>(wp, Vh, h, wv);
 #pragma unroll
         for (int k = 0; k < 12; k++) {
             red[0] = mad(wv[2 * k + 1], acc[2 * k + 1], mad(wv[2 * k], acc[2 * k], red[0]));
             red[1] = mad(-wv[2 * k + 1], acc[2 * k], mad(wv[2 * k], acc[2 * k + 1], red[1]));
         }
     }
-    store_spinor<PREC, true>(a.out, Vh, h, acc);
+    store_spinor<PREC, true>(out, Vh, h, acc);
 }
 
 template <int PREC, int RECON, int EPI, bool CPLX, int RED>
@@ -199,18 +207,72 @@ hop_kernel(const HopArgs<typename Prec<PREC>::comp> a) {
     const int h = blockIdx.x * HOP_BLOCK + threadIdx.x;
     if (RED == 0) {
         if (h >= a.Vh) return;
-        hop_site<PREC, RECON, EPI, CPLX, 0>(a, h, nullptr);
+        hop_site<PREC, RECON, EPI, CPLX, 0>(a, h, a.in, a.out, a.z, a.w, nullptr);
     } else {
         C red[3] = {0, 0, 0};
-        if (h < a.Vh) hop_site<PREC, RECON, EPI, CPLX, RED>(a, h, red);
+        if (h < a.Vh) hop_site<PREC, RECON, EPI, CPLX, RED>(a, h, a.in, a.out, a.z, a.w, red);
         const double v[3] = {(double)red[0], (double)red[1], (double)red[2]};
         hop_block_partial<RED == 1 ? 2 : 3>(v, a.partials);
     }
 }
 
+// ---------------------------------------------------------------------------------------------------
+// Multi-right-hand-side hop (the paper's workload is the 12 spin-colour sources of a
+// propagator on ONE gauge field).  One thread per (site, rhs); the 8 sites of a tile are the
+// fastest index, then the rhs, then the tile:  thread q*8 + s8 of a CTA handles site 8*(T*blockIdx.x + q / nrhs) + s8
+// of right-hand side q % nrhs.  A warp is therefore 8 sites x 4 right-hand sides: every spinor load instruction reads
+// four whole 128-byte planes (one per rhs field), and every link load instruction reads ONE 128-byte plane that its
+// four 8-lane groups share (identical addresses merge in the load unit).  All nrhs right-hand sides of a tile live in
+// the same CTA, so a link plane is fetched from L2/DRAM once per CTA and found in L1 by the other warps: compulsory
+// DRAM traffic per (site, rhs) drops from 8 links + 2 spinors to 8/nrhs links + 2 spinors (fp32/18: 768 -> 240 B at
+// nrhs = 12).  Links are read with the default cache policy here (not evict-first).
+// ---------------------------------------------------------------------------------------------------
+constexpr int HOP_MRHS_MAX = 16;      // right-hand sides per launch (8 * nrhs * T <= 128 threads)
+
+template <int NRED> __device__ __forceinline__ void hop_block_partial_mrhs(const double* v, double* partials, int nrhs, int T) {
+    __shared__ double s_g[NRED][HOP_BLOCK / 8];
+#pragma unroll
+    for (int k = 0; k < NRED; k++) {
+        double x = v[k];
+        x += __shfl_xor_sync(0xffffffffu, x, 4);
+        x += __shfl_xor_sync(0xffffffffu, x, 2);
+        x += __shfl_xor_sync(0xffffffffu, x, 1);
+        if ((threadIdx.x & 7) == 0) s_g[k][threadIdx.x >> 3] = x;
+    }
+    __syncthreads();
+    if (threadIdx.x < nrhs * NRED) {
+        const int rhs = threadIdx.x / NRED, k = threadIdx.x % NRED;
+        double a = 0;
+        for (int t = 0; t < T; t++) a += s_g[k][t * nrhs + rhs];
+        partials[((size_t)rhs * gridDim.x + blockIdx.x) * NRED + k] = a;
+    }
+}
+
+template <int PREC, int RECON, int EPI, bool CPLX, int RED>
+__global__ void __launch_bounds__(HOP_BLOCK, PREC == BQ_FP64 ? HOP_MINB_64 : (PREC == BQ_FP32 ? HOP_MINB_LO : HOP_MINB_HALF))
+hop_kernel_mrhs(const HopArgs<typename Prec<PREC>::comp> a) {
+    using C = typename Prec<PREC>::comp;
+    const int q = threadIdx.x >> 3, s8 = threadIdx.x & 7;
+    const int rhs = q % a.nrhs, tl = q / a.nrhs;
+    const int h = (blockIdx.x * a.T + tl) * 8 + s8;
+    const bool live = tl < a.T && h < a.Vh;     // the CTA is padded to whole warps
+    const char* in = static_cast<const char*>(a.in) + (size_t)rhs * a.s_in;
+    char* out = static_cast<char*>(a.out) + (size_t)rhs * a.s_out;
+    const char* zp = a.z ? static_cast<const char*>(a.z) + (size_t)rhs * a.s_z : nullptr;
+    const char* wp = a.w ? static_cast<const char*>(a.w) + (size_t)rhs * a.s_w : nullptr;
+    if (RED == 0) {
+        if (live) hop_site<PREC, RECON, EPI, CPLX, 0, false>(a, h, in, out, zp, wp, nullptr);
+    } else {
+        C red[3] = {0, 0, 0};
+        if (live) hop_site<PREC, RECON, EPI, CPLX, RED, false>(a, h, in, out, zp, wp, red);
+        const double v[3] = {(double)red[0], (double)red[1], (double)red[2]};
+        hop_block_partial_mrhs<RED == 1 ? 2 : 3>(v, a.partials, a.nrhs, a.T);
+    }
+}
+
 template <int PREC, int RECON>
 static bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const void* z, double scale, int p, const void* gauge,
-                            const void* cl, int cl_mode, const HopRed* red, cudaStream_t stream) {
+                            const void* cl, int cl_mode, const HopRed* red, cudaStream_t stream, const HopMulti* m) {
     using C = typename Prec<PREC>::comp;
     const Geom& g = lat->g;
     HopArgs<C> a;
@@ -226,13 +288,26 @@ static bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const vo
         a.phi[mu] = (C)(scale * lat->bc[2 * mu + 1]);
         if (lat->bc[2 * mu + 1] != 0.0) cplx = true;
     }
-    const int grid = (g.Vh + HOP_BLOCK - 1) / HOP_BLOCK;
+    // launch shape: one thread per site (128 per CTA), or — multi-rhs — T tiles x nrhs x 8 sites per CTA, padded to warps
+    const bool multi = m != nullptr;
+    const int nrhs = multi ? m->nrhs : 1;
+    a.nrhs = nrhs;
+    a.T = multi ? (HOP_BLOCK / 8 / nrhs > 0 ? HOP_BLOCK / 8 / nrhs : 1) : 0;
+    a.s_in = multi ? m->s_in : 0; a.s_out = multi ? m->s_out : 0; a.s_z = multi ? m->s_z : 0; a.s_w = multi ? m->s_w : 0;
+    const int block = multi ? ((8 * nrhs * a.T + 31) / 32) * 32 : HOP_BLOCK;
+    const int grid = multi ? (g.Vh / 8 + a.T - 1) / a.T : (g.Vh + HOP_BLOCK - 1) / HOP_BLOCK;
     const int rmode = red ? red->mode : 0;
     a.w = nullptr; a.partials = nullptr;
     if (rmode) {
         if ((rmode != 1 && rmode != 2) || !red->sc || (rmode == 1 && !red->w) || !z)
             return bq_set_error(lat, BQ_EINVAL, "bq_hop: bad fused reduction (mode %d)", rmode);
-        if (!lat->hop_partials) BQ_CUDA(lat, cudaMalloc(&lat->hop_partials, sizeof(double) * 3 * grid));
+        const size_t need = (size_t)3 * grid * nrhs;
+        if (lat->hop_partials_cap < need) {
+            if (lat->hop_partials) BQ_CUDA(lat, cudaFree(lat->hop_partials));
+            lat->hop_partials = nullptr; lat->hop_partials_cap = 0;
+            BQ_CUDA(lat, cudaMalloc(&lat->hop_partials, sizeof(double) * need));
+            lat->hop_partials_cap = need;
+        }
         a.w = red->w; a.partials = lat->hop_partials;
     }
     int epi;
@@ -240,10 +315,15 @@ static bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const vo
     else if (cl_mode == 1 && !z) epi = 2;
     else if (cl_mode == 2 && z) epi = 3;
     else return bq_set_error(lat, BQ_EINVAL, "bq_hop: unsupported epilogue (cl_mode=%d, z=%p)", cl_mode, z);
-#define BQ_HOP_LAUNCH(E, R)                                                                \
-    do {                                                                                   \
-        if (cplx) hop_kernel<PREC, RECON, E, true, R><<<grid, HOP_BLOCK, 0, stream>>>(a);   \
-        else hop_kernel<PREC, RECON, E, false, R><<<grid, HOP_BLOCK, 0, stream>>>(a);       \
+#define BQ_HOP_LAUNCH(E, R)                                                                         \
+    do {                                                                                            \
+        if (multi) {                                                                                \
+            if (cplx) hop_kernel_mrhs<PREC, RECON, E, true, R><<<grid, block, 0, stream>>>(a);       \
+            else hop_kernel_mrhs<PREC, RECON, E, false, R><<<grid, block, 0, stream>>>(a);           \
+        } else {                                                                                    \
+            if (cplx) hop_kernel<PREC, RECON, E, true, R><<<grid, HOP_BLOCK, 0, stream>>>(a);        \
+            else hop_kernel<PREC, RECON, E, false, R><<<grid, HOP_BLOCK, 0, stream>>>(a);            \
+        }                                                                                           \
     } while (0)
     // fused reductions exist for the xpay epilogues only (the second hop of M^, which produces v and t)
     switch (epi * 3 + rmode) {
@@ -259,10 +339,10 @@ static bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const vo
     }
 #undef BQ_HOP_LAUNCH
     BQ_CHECK_LAUNCH(lat);
-    lat->n_hop[PREC]++;
+    lat->n_hop[PREC] += nrhs;     // counted per right-hand side: each is 1320 flop x Vh sites
     if (rmode) {
-        if (rmode == 1) k_hop_red_final<1><<<1, HOP_RED_FINAL_BLOCK, 0, stream>>>(lat->hop_partials, grid, red->sc);
-        else k_hop_red_final<2><<<1, HOP_RED_FINAL_BLOCK, 0, stream>>>(lat->hop_partials, grid, red->sc);
+        if (rmode == 1) k_hop_red_final<1><<<nrhs, HOP_RED_FINAL_BLOCK, 0, stream>>>(lat->hop_partials, grid, red->sc);
+        else k_hop_red_final<2><<<nrhs, HOP_RED_FINAL_BLOCK, 0, stream>>>(lat->hop_partials, grid, red->sc);
         BQ_CHECK_LAUNCH(lat);
     }
     return BQ_OK;
@@ -276,11 +356,26 @@ extern "C" bq_status bq_get_counters(const bq_lattice* lat, unsigned long long* 
 }
 
 bq_status bq_hop(bq_lattice* lat, void* out, const void* in, const void* z, double scale, int p, int prec, int recon,
-                 const void* cl, int cl_mode, cudaStream_t stream, const HopRed* red) {
+                 const void* cl, int cl_mode, cudaStream_t stream, const HopRed* red, const HopMulti* m) {
     const void* gauge = nullptr;
     BQ_TRY(bq_get_gauge(lat, prec, recon, &gauge));
+    if (m && m->nrhs < 1) return bq_set_error(lat, BQ_EINVAL, "bq_hop: nrhs must be >= 1");
+    if (m && m->nrhs > HOP_MRHS_MAX) {
+        // more right-hand sides than one CTA shape holds: equal chunks of <= HOP_MRHS_MAX, one launch each
+        const int nchunk = (m->nrhs + HOP_MRHS_MAX - 1) / HOP_MRHS_MAX, per = (m->nrhs + nchunk - 1) / nchunk;
+        for (int r0 = 0; r0 < m->nrhs; r0 += per) {
+            HopMulti c = *m;
+            c.nrhs = (m->nrhs - r0) < per ? (m->nrhs - r0) : per;
+            HopRed rc;
+            if (red) { rc = *red; rc.sc = red->sc + r0; if (rc.w) rc.w = static_cast<const char*>(red->w) + (size_t)r0 * m->s_w; }
+            BQ_TRY(bq_hop(lat, static_cast<char*>(out) + (size_t)r0 * m->s_out, static_cast<const char*>(in) + (size_t)r0 * m->s_in,
+                          z ? static_cast<const char*>(z) + (size_t)r0 * m->s_z : nullptr, scale, p, prec, recon, cl, cl_mode, stream,
+                          red ? &rc : nullptr, &c));
+        }
+        return BQ_OK;
+    }
 #define BQ_HOP_CASE(P, R) \
-    if (prec == P && recon == R) return launch_hop<P, R>(lat, out, in, z, scale, p, gauge, cl, cl_mode, red, stream);
+    if (prec == P && recon == R) return launch_hop<P, R>(lat, out, in, z, scale, p, gauge, cl, cl_mode, red, stream, m);
     BQ_HOP_CASE(BQ_FP64, BQ_RECON18)
     BQ_HOP_CASE(BQ_FP64, BQ_RECON12)
     BQ_HOP_CASE(BQ_FP32, BQ_RECON18)
@@ -332,20 +427,23 @@ extern "C" bq_status bq_dirac_apply(bq_lattice* lat, void* out, const void* in, 
 
 extern "C" bq_status bq_schur_apply(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw,
                                     bq_prec prec, bq_recon recon, void* stream) {
-    return bq_schur_red(lat, out, in, tmp, kappa, csw, prec, recon, static_cast<cudaStream_t>(stream), nullptr);
+    return bq_schur_red(lat, out, in, tmp, kappa, csw, prec, recon, static_cast<cudaStream_t>(stream), nullptr, 0);
 }
 
 bq_status bq_schur_red(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw, int prec, int recon,
-                       cudaStream_t s, const HopRed* red) {
+                       cudaStream_t s, const HopRed* red, int nrhs) {
     if (!lat) return BQ_EINVAL;
     if (!out || !in || !tmp || out == in || tmp == in || tmp == out)
         return bq_set_error(lat, BQ_EINVAL, "bq_schur_apply: NULL or aliased buffers");
     if (!valid_prec(prec) || !valid_recon(recon)) return bq_set_error(lat, BQ_EINVAL, "bq_schur_apply: bad prec/recon");
     if (!lat->have_gauge) return bq_set_error(lat, BQ_ENOGAUGE, "bq_schur_apply: no gauge field loaded");
+    const size_t fb = field_bytes_one_parity(lat->g, prec);
+    const HopMulti mm{nrhs, fb, fb, fb, fb};
+    const HopMulti* m = nrhs >= 1 ? &mm : nullptr;
     if (csw == 0.0) {
         // tmp_o = -kappa H_oe in_e ;  out_e = in_e + kappa H_eo tmp_o = in_e - kappa^2 H_eo H_oe in_e
-        BQ_TRY(bq_hop(lat, tmp, in, nullptr, -kappa, 1, prec, recon, nullptr, 0, s));
-        return bq_hop(lat, out, tmp, in, kappa, 0, prec, recon, nullptr, 0, s, red);
+        BQ_TRY(bq_hop(lat, tmp, in, nullptr, -kappa, 1, prec, recon, nullptr, 0, s, nullptr, m));
+        return bq_hop(lat, out, tmp, in, kappa, 0, prec, recon, nullptr, 0, s, red, m);
     }
     BQ_TRY(bq_clover_build(lat, csw, kappa));
     const void *cl = nullptr, *cli = nullptr;
@@ -353,6 +451,38 @@ bq_status bq_schur_red(bq_lattice* lat, void* out, const void* in, void* tmp, do
     BQ_TRY(bq_get_clover(lat, prec, 1, &cli));
     const size_t cb = (size_t)lat->g.Vh * CLOVER_REALS * prec_real_bytes(prec);
     // tmp_o = -kappa A_oo^-1 H_oe in_e ;  out_e = A_ee in_e + kappa H_eo tmp_o
-    BQ_TRY(bq_hop(lat, tmp, in, nullptr, -kappa, 1, prec, recon, static_cast<const char*>(cli) + cb, 1, s));
-    return bq_hop(lat, out, tmp, in, kappa, 0, prec, recon, cl, 2, s, red);
+    BQ_TRY(bq_hop(lat, tmp, in, nullptr, -kappa, 1, prec, recon, static_cast<const char*>(cli) + cb, 1, s, nullptr, m));
+    return bq_hop(lat, out, tmp, in, kappa, 0, prec, recon, cl, 2, s, red, m);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// multi-rhs entry points
+// ---------------------------------------------------------------------------------------------------
+extern "C" bq_status bq_wilson_apply_multi(bq_lattice* lat, void* out, const void* in, int nrhs, double kappa, bq_parity parity,
+                                           bq_prec prec, bq_recon recon, void* stream) {
+    if (!lat) return BQ_EINVAL;
+    if (!out || !in || out == in) return bq_set_error(lat, BQ_EINVAL, "bq_wilson_apply_multi: out/in NULL or aliased");
+    if (nrhs < 1) return bq_set_error(lat, BQ_EINVAL, "bq_wilson_apply_multi: nrhs must be >= 1");
+    if (!valid_prec(prec) || !valid_recon(recon)) return bq_set_error(lat, BQ_EINVAL, "bq_wilson_apply_multi: bad prec/recon");
+    if (!lat->have_gauge) return bq_set_error(lat, BQ_ENOGAUGE, "bq_wilson_apply_multi: no gauge field loaded");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const size_t fb = field_bytes_one_parity(lat->g, prec);
+    if (parity == BQ_EVEN || parity == BQ_ODD) {
+        const HopMulti m{nrhs, fb, fb, fb, fb};
+        return bq_hop(lat, out, in, nullptr, -kappa, (int)parity, prec, recon, nullptr, 0, s, nullptr, &m);
+    }
+    if (parity != BQ_FULL) return bq_set_error(lat, BQ_EINVAL, "bq_wilson_apply_multi: bad parity %d", (int)parity);
+    // [rhs][even | odd] buffers: out_p = in_p - kappa H_{p,1-p} in_{1-p}
+    const HopMulti m{nrhs, 2 * fb, 2 * fb, 2 * fb, 2 * fb};
+    char* o = static_cast<char*>(out);
+    const char* i = static_cast<const char*>(in);
+    BQ_TRY(bq_hop(lat, o, i + fb, i, -kappa, 0, prec, recon, nullptr, 0, s, nullptr, &m));
+    return bq_hop(lat, o + fb, i, i + fb, -kappa, 1, prec, recon, nullptr, 0, s, nullptr, &m);
+}
+
+extern "C" bq_status bq_schur_apply_multi(bq_lattice* lat, void* out, const void* in, void* tmp, int nrhs, double kappa, double csw,
+                                          bq_prec prec, bq_recon recon, void* stream) {
+    if (!lat) return BQ_EINVAL;
+    if (nrhs < 1) return bq_set_error(lat, BQ_EINVAL, "bq_schur_apply_multi: nrhs must be >= 1");
+    return bq_schur_red(lat, out, in, tmp, kappa, csw, prec, recon, static_cast<cudaStream_t>(stream), nullptr, nrhs);
 }

@@ -78,7 +78,9 @@ template <typename C> __device__ __forceinline__ void phase_mul(C* chi, C pr, C 
 //   extra instruction).  CPLX = true: general phases, one branch-free complex multiply of the half spinor.
 //   Half storage: the neighbour's site norm is folded into the same weight (chi is linear in the spinor), so the
 //   mantissas are never rescaled on their own.
-template <int PREC, int RECON, int MU, bool FWD, bool CPLX>
+//   LSTREAM: links read with the streaming (evict-first) policy — right when each link is used once (one right-hand
+//   side); the multi-rhs kernel reads them with the default policy so that the other right-hand sides hit in L1/L2.
+template <int PREC, int RECON, int MU, bool FWD, bool CPLX, bool LSTREAM = true>
 __device__ __forceinline__ void hop_dir(typename Prec<PREC>::comp* acc, const void* in, int Vh, int nh, const void* ublock,
                                         int uidx, typename Prec<PREC>::comp pr, typename Prec<PREC>::comp pi) {
     using C = typename Prec<PREC>::comp;
@@ -93,7 +95,7 @@ __device__ __forceinline__ void hop_dir(typename Prec<PREC>::comp* acc, const vo
         // (1 - g_t) psi = (0; 2l): forward needs l only; (1 + g_t) psi = (2u; 0): backward needs u only
         load_spinor_half_raw<PREC, FWD ? 1 : 0>(in, Vh, nh, h, n);
     }
-    load_link<PREC, RECON>(ublock, Vh, uidx, u);
+    load_link<PREC, RECON, LSTREAM>(ublock, Vh, uidx, u);
     su3_mul<!FWD>(u, h, chi);
     C w = pr;
     if (CPLX) {

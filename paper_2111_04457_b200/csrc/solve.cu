@@ -19,14 +19,16 @@
 struct SolverWork {
     BlasCtx blas;
     bool blas_ok;
-    // fp64, full lattice [even | odd]
+    int nrhs;              // right-hand sides the buffers below are sized for
+    // fp64, full lattice, [rhs][even | odd]
     void *b, *x;
-    // fp64, one parity
+    // fp64, one parity, [rhs]
     void *bhat, *r, *t, *tmp;
-    // inner precision, one parity
+    // inner precision, one parity, [rhs]
     int inner_prec;
     void *irhat, *ir, *ip, *iv, *is, *it, *itmp, *ie;
-    SolverScalars* h_sc;   // pinned host mirror
+    SolverScalars* h_sc;   // pinned host mirror, [rhs]
+    double* h_stop2;       // pinned host staging of the per-rhs inner thresholds, [rhs]
     cudaEvent_t ev0, ev1;
 };
 
@@ -39,24 +41,31 @@ static void free_inner(SolverWork* w) {
     w->inner_prec = -1;
 }
 
-void bq_solver_free(bq_lattice* lat) {
-    SolverWork* w = lat->work;
-    if (!w) return;
-    free_inner(w);
+static void free_outer(SolverWork* w) {
     void** v[] = {&w->b, &w->x, &w->bhat, &w->r, &w->t, &w->tmp};
     for (void** p : v) {
         if (*p) cudaFree(*p);
         *p = nullptr;
     }
-    if (w->blas_ok) blas_ctx_destroy(&w->blas);
     if (w->h_sc) cudaFreeHost(w->h_sc);
+    if (w->h_stop2) cudaFreeHost(w->h_stop2);
+    w->h_sc = nullptr; w->h_stop2 = nullptr;
+    w->nrhs = 0;
+}
+
+void bq_solver_free(bq_lattice* lat) {
+    SolverWork* w = lat->work;
+    if (!w) return;
+    free_inner(w);
+    free_outer(w);
+    if (w->blas_ok) blas_ctx_destroy(&w->blas);
     if (w->ev0) cudaEventDestroy(w->ev0);
     if (w->ev1) cudaEventDestroy(w->ev1);
     free(w);
     lat->work = nullptr;
 }
 
-static bq_status get_work(bq_lattice* lat, int inner_prec, SolverWork** out) {
+static bq_status get_work(bq_lattice* lat, int inner_prec, SolverWork** out, int nrhs = 1) {
     const Geom& g = lat->g;
     if (!lat->work) {
         SolverWork* w = static_cast<SolverWork*>(calloc(1, sizeof(SolverWork)));
@@ -65,27 +74,36 @@ static bq_status get_work(bq_lattice* lat, int inner_prec, SolverWork** out) {
         lat->work = w;
         BQ_TRY(blas_ctx_create(lat, &w->blas));
         w->blas_ok = true;
-        const size_t fb = field_bytes_one_parity(g, BQ_FP64);
+        BQ_CUDA(lat, cudaEventCreate(&w->ev0));
+        BQ_CUDA(lat, cudaEventCreate(&w->ev1));
+    }
+    SolverWork* w = lat->work;
+    if (w->nrhs < nrhs) {
+        free_outer(w);
+        free_inner(w);
+        BQ_TRY(blas_ctx_reserve(lat, &w->blas, nrhs));
+        const size_t fb = field_bytes_one_parity(g, BQ_FP64) * nrhs;
         BQ_CUDA(lat, cudaMalloc(&w->b, 2 * fb));
         BQ_CUDA(lat, cudaMalloc(&w->x, 2 * fb));
         BQ_CUDA(lat, cudaMalloc(&w->bhat, fb));
         BQ_CUDA(lat, cudaMalloc(&w->r, fb));
         BQ_CUDA(lat, cudaMalloc(&w->t, fb));
         BQ_CUDA(lat, cudaMalloc(&w->tmp, fb));
-        BQ_CUDA(lat, cudaMallocHost(&w->h_sc, sizeof(SolverScalars)));
-        BQ_CUDA(lat, cudaEventCreate(&w->ev0));
-        BQ_CUDA(lat, cudaEventCreate(&w->ev1));
+        BQ_CUDA(lat, cudaMallocHost(&w->h_sc, sizeof(SolverScalars) * nrhs));
+        BQ_CUDA(lat, cudaMallocHost(&w->h_stop2, sizeof(double) * nrhs));
+        w->nrhs = nrhs;
     }
-    SolverWork* w = lat->work;
     if (w->inner_prec != inner_prec) {
         free_inner(w);
-        const size_t fb = field_bytes_one_parity(g, inner_prec);
+        const size_t fb = field_bytes_one_parity(g, inner_prec) * w->nrhs;
         void** v[] = {&w->irhat, &w->ir, &w->ip, &w->iv, &w->is, &w->it, &w->itmp};
         for (void** p : v) BQ_CUDA(lat, cudaMalloc(p, fb));
         // solution accumulator of the inner solve: fp32 when the inner storage is half
-        BQ_CUDA(lat, cudaMalloc(&w->ie, field_bytes_one_parity(g, inner_prec == BQ_HALF ? BQ_FP32 : inner_prec)));
+        BQ_CUDA(lat, cudaMalloc(&w->ie, field_bytes_one_parity(g, inner_prec == BQ_HALF ? BQ_FP32 : inner_prec) * w->nrhs));
         w->inner_prec = inner_prec;
     }
+    // batch shape of the BLAS launches: plain single-field launches until a multi-rhs solve says otherwise
+    w->blas.nrhs = 1; w->blas.stride = 0; w->blas.xstride = 0; w->blas.stride64 = 0;
     *out = w;
     return BQ_OK;
 }
@@ -97,66 +115,79 @@ __global__ void k_set_bicg_scalars(SolverScalars* sc, double ar, double ai, doub
     sc->done = 0; sc->iters = 0; sc->stop2 = -1.0;
 }
 
-// out_e = M^ in_e in precision prec (tmp: odd scratch)
+// out_e = M^ in_e in precision prec (tmp: odd scratch); nrhs = 0: single fields, >= 1: arrays of nrhs fields
 static bq_status schur(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw, int prec, int recon,
-                       cudaStream_t s, const HopRed* red = nullptr) {
-    return bq_schur_red(lat, out, in, tmp, kappa, csw, prec, recon, s, red);
+                       cudaStream_t s, const HopRed* red = nullptr, int nrhs = 0) {
+    return bq_schur_red(lat, out, in, tmp, kappa, csw, prec, recon, s, red, nrhs);
 }
 
+// copy the device-resident solver states of the nrhs right-hand sides of the current batch to w->h_sc
 static bq_status poll(bq_lattice* lat, SolverWork* w) {
-    BQ_CUDA(lat, cudaMemcpyAsync(w->h_sc, w->blas.sc, sizeof(SolverScalars), cudaMemcpyDeviceToHost, w->blas.stream));
+    BQ_CUDA(lat, cudaMemcpyAsync(w->h_sc, w->blas.sc, sizeof(SolverScalars) * w->blas.nrhs, cudaMemcpyDeviceToHost, w->blas.stream));
     BQ_CUDA(lat, cudaStreamSynchronize(w->blas.stream));
     return BQ_OK;
 }
 
-// Inner BiCGStab on M^ e = ir (e0 = 0), stop when |r|^2 <= stop2 or after max_iter iterations.
-// On return w->h_sc holds the final device state.  Textbook van der Vorst recurrences (reading O4).
-static bq_status inner_bicgstab(bq_lattice* lat, SolverWork* w, double kappa, double csw, int prec, int recon, double stop2,
-                                int max_iter, int check_every) {
+// Inner BiCGStab on M^ e = ir (e0 = 0) for every right-hand side of the batch (w->blas.nrhs), each with its own
+// device-resident scalars; rhs k stops when |r_k|^2 <= w->h_stop2[k] or after max_iter iterations.  A right-hand
+// side that has stopped keeps its iterate frozen (its update kernels exit early) while the others go on; the hop
+// kernels always process the whole batch.  On return w->h_sc holds the final device states.
+// Textbook van der Vorst recurrences (reading O4).
+static bq_status inner_bicgstab(bq_lattice* lat, SolverWork* w, double kappa, double csw, int prec, int recon, int max_iter,
+                                int check_every) {
     const BlasCtx& c = w->blas;
     cudaStream_t s = c.stream;
-    const size_t fb = field_bytes_one_parity(lat->g, prec);
-    const size_t eb = field_bytes_one_parity(lat->g, prec == BQ_HALF ? BQ_FP32 : prec);
+    const int n = c.nrhs, mrhs = n > 1 ? n : 0;
+    const size_t fb = field_bytes_one_parity(lat->g, prec) * n;
+    const size_t eb = field_bytes_one_parity(lat->g, prec == BQ_HALF ? BQ_FP32 : prec) * n;
     BQ_CUDA(lat, cudaMemsetAsync(w->ie, 0, eb, s));
     BQ_CUDA(lat, cudaMemsetAsync(w->ip, 0, fb, s));
     BQ_CUDA(lat, cudaMemsetAsync(w->iv, 0, fb, s));
     BQ_CUDA(lat, cudaMemcpyAsync(w->irhat, w->ir, fb, cudaMemcpyDeviceToDevice, s));
-    BQ_TRY(bicg_init(lat, c, prec, w->ir, stop2));
+    BQ_CUDA(lat, cudaMemcpyAsync(c.stop2s, w->h_stop2, sizeof(double) * n, cudaMemcpyHostToDevice, s));
+    BQ_TRY(bicg_init(lat, c, prec, w->ir, 0.0, true));
     int launched = 0;
     // the two inner products on v and t ride on the second hop of M^ (hop.cu, RED epilogues): 7 kernels per iteration
     const HopRed red_alpha{1, w->irhat, c.sc}, red_omega{2, nullptr, c.sc};
     for (;;) {
         const int batch = (max_iter - launched) < check_every ? (max_iter - launched) : check_every;
         for (int k = 0; k < batch; k++) {
-            BQ_TRY(bicg_p_update(lat, c, prec, w->ir, w->ip, w->iv));                          // p = r + beta (p - omega v)
-            BQ_TRY(schur(lat, w->iv, w->ip, w->itmp, kappa, csw, prec, recon, s, &red_alpha)); // v = M^ p; alpha = rho/<rhat,v>
-            BQ_TRY(bicg_s_update(lat, c, prec, w->ir, w->iv, w->is));                          // s = r - alpha v
-            BQ_TRY(schur(lat, w->it, w->is, w->itmp, kappa, csw, prec, recon, s, &red_omega)); // t = M^ s; omega = <t,s>/<t,t>
+            BQ_TRY(bicg_p_update(lat, c, prec, w->ir, w->ip, w->iv));                                // p = r + beta (p - omega v)
+            BQ_TRY(schur(lat, w->iv, w->ip, w->itmp, kappa, csw, prec, recon, s, &red_alpha, mrhs)); // v = M^ p; alpha = rho/<rhat,v>
+            BQ_TRY(bicg_s_update(lat, c, prec, w->ir, w->iv, w->is));                                // s = r - alpha v
+            BQ_TRY(schur(lat, w->it, w->is, w->itmp, kappa, csw, prec, recon, s, &red_omega, mrhs)); // t = M^ s; omega = <t,s>/<t,t>
             BQ_TRY(bicg_final(lat, c, prec, w->ip, w->is, w->it, w->irhat, w->ie, w->ir));
         }
         launched += batch;
         BQ_TRY(poll(lat, w));
-        if (w->h_sc->done || launched >= max_iter) break;
+        bool all_done = true;
+        for (int k = 0; k < n; k++) all_done = all_done && w->h_sc[k].done;
+        if (all_done || launched >= max_iter) break;
     }
     return BQ_OK;
 }
 
-extern "C" bq_status bq_solve(bq_lattice* lat, const double* b, double* x, double kappa, double tol, const bq_solve_opts* opts,
-                              bq_solve_info* info) {
+// bq_solve (nrhs = 1, single-field kernels) and bq_solve_multi (nrhs >= 1 right-hand sides solved together with the
+// multi-rhs kernels: one gauge-field read per hop for the whole batch).  b, x: nrhs canonical fields one after the other.
+static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrhs, bool multi, double kappa, double tol,
+                            const bq_solve_opts* opts, bq_solve_info* info) {
     if (!lat) return BQ_EINVAL;
-    if (info) {
-        info->status = BQ_EINVAL; info->outer_cycles = 0; info->inner_iters = 0; info->restarts = 0;
-        info->true_rel_residual = NAN; info->seconds = 0;
-    }
-    if (!b || !x) return bq_set_error(lat, BQ_EINVAL, "bq_solve: b or x is NULL");
-    if (!(tol > 0.0) || !isfinite(tol)) return bq_set_error(lat, BQ_EINVAL, "bq_solve: tol must be positive");
-    if (!lat->have_gauge) return bq_set_error(lat, BQ_ENOGAUGE, "bq_solve: no gauge field loaded");
+    const char* fn = multi ? "bq_solve_multi" : "bq_solve";
+    if (info)
+        for (int k = 0; k < (nrhs > 0 ? nrhs : 0); k++) {
+            info[k].status = BQ_EINVAL; info[k].outer_cycles = 0; info[k].inner_iters = 0; info[k].restarts = 0;
+            info[k].true_rel_residual = NAN; info[k].seconds = 0;
+        }
+    if (nrhs < 1) return bq_set_error(lat, BQ_EINVAL, "%s: nrhs must be >= 1", fn);
+    if (!b || !x) return bq_set_error(lat, BQ_EINVAL, "%s: b or x is NULL", fn);
+    if (!(tol > 0.0) || !isfinite(tol)) return bq_set_error(lat, BQ_EINVAL, "%s: tol must be positive", fn);
+    if (!lat->have_gauge) return bq_set_error(lat, BQ_ENOGAUGE, "%s: no gauge field loaded", fn);
     bq_solve_opts o;
     if (opts) o = *opts;
     else { o.inner_prec = BQ_FP32; o.recon = BQ_RECON18; o.csw = 0; o.inner_tol = 0; o.max_inner = 0; o.max_outer = 0; o.check_every = 0; o.stream = nullptr; }
-    if (o.inner_prec != BQ_FP64 && o.inner_prec != BQ_FP32 && o.inner_prec != BQ_HALF) return bq_set_error(lat, BQ_EINVAL, "bq_solve: bad inner_prec");
-    if (o.recon != BQ_RECON18 && o.recon != BQ_RECON12) return bq_set_error(lat, BQ_EINVAL, "bq_solve: bad recon");
-    if (o.stream) return bq_set_error(lat, BQ_EINVAL, "bq_solve: opts->stream must be NULL");
+    if (o.inner_prec != BQ_FP64 && o.inner_prec != BQ_FP32 && o.inner_prec != BQ_HALF) return bq_set_error(lat, BQ_EINVAL, "%s: bad inner_prec", fn);
+    if (o.recon != BQ_RECON18 && o.recon != BQ_RECON12) return bq_set_error(lat, BQ_EINVAL, "%s: bad recon", fn);
+    if (o.stream) return bq_set_error(lat, BQ_EINVAL, "%s: opts->stream must be NULL", fn);
     const int prec = o.inner_prec;
     const double inner_tol = o.inner_tol > 0 ? o.inner_tol : (prec == BQ_HALF ? 5e-2 : 1e-5);
     const int max_inner = o.max_inner > 0 ? o.max_inner : (prec == BQ_HALF ? 100 : 1000);
@@ -164,14 +195,19 @@ extern "C" bq_status bq_solve(bq_lattice* lat, const double* b, double* x, doubl
     const int check_every = o.check_every > 0 ? o.check_every : 8;
     const double csw = o.csw;
     const bool clover = csw != 0.0;
+    const int n = nrhs, mrhs = multi ? n : 0;      // mrhs = 0 selects the single-field kernels
 
     SolverWork* w = nullptr;
-    BQ_TRY(get_work(lat, prec, &w));
-    const BlasCtx& c = w->blas;
-    cudaStream_t s = c.stream;
+    BQ_TRY(get_work(lat, prec, &w, n));
     const Geom& g = lat->g;
     const size_t fb64 = field_bytes_one_parity(g, BQ_FP64);
-    char* bb = static_cast<char*>(w->b);
+    w->blas.nrhs = n;
+    w->blas.stride = field_bytes_one_parity(g, prec);
+    w->blas.xstride = field_bytes_one_parity(g, prec == BQ_HALF ? BQ_FP32 : prec);
+    w->blas.stride64 = fb64;
+    const BlasCtx& c = w->blas;
+    cudaStream_t s = c.stream;
+    char* bb = static_cast<char*>(w->b);     // [rhs][even | odd], 2*fb64 per rhs
     char* xx = static_cast<char*>(w->x);
     const void *cl64 = nullptr, *cli64 = nullptr;
     const size_t cb64 = (size_t)g.Vh * CLOVER_REALS * sizeof(double);
@@ -180,6 +216,9 @@ extern "C" bq_status bq_solve(bq_lattice* lat, const double* b, double* x, doubl
         BQ_TRY(bq_get_clover(lat, BQ_FP64, 0, &cl64));
         BQ_TRY(bq_get_clover(lat, BQ_FP64, 1, &cli64));
     }
+    // operand strides of the fp64 hops: full-lattice fields (b, x) are 2*fb64 apart, one-parity work vectors fb64
+    const HopMulti* none = nullptr;
+    auto hm = [&](size_t s_in, size_t s_out, size_t s_z) { return HopMulti{n, s_in, s_out, s_z, 0}; };
 
     BQ_CUDA(lat, cudaEventRecord(w->ev0, s));
     // ---- import b and x0 (canonical, host or device) through a device staging buffer ----
@@ -187,109 +226,188 @@ extern "C" bq_status bq_solve(bq_lattice* lat, const double* b, double* x, doubl
         const size_t nb = (size_t)g.V * 24 * sizeof(double);
         double* stage = nullptr;
         BQ_CUDA(lat, cudaMalloc(&stage, nb));
-        cudaError_t e = cudaMemcpyAsync(stage, b, nb, cudaMemcpyDefault, s);
+        cudaError_t e = cudaSuccess;
         bq_status st = BQ_OK;
-        if (e == cudaSuccess) st = bq_field_import(lat, w->b, stage, BQ_FULL, BQ_FP64, s);
-        if (e == cudaSuccess && st == BQ_OK) e = cudaMemcpyAsync(stage, x, nb, cudaMemcpyDefault, s);
-        if (e == cudaSuccess && st == BQ_OK) st = bq_field_import(lat, w->x, stage, BQ_FULL, BQ_FP64, s);
+        for (int k = 0; k < n && e == cudaSuccess && st == BQ_OK; k++) {
+            e = cudaMemcpyAsync(stage, reinterpret_cast<const char*>(b) + (size_t)k * nb, nb, cudaMemcpyDefault, s);
+            if (e == cudaSuccess) st = bq_field_import(lat, bb + (size_t)k * 2 * fb64, stage, BQ_FULL, BQ_FP64, s);
+            if (e == cudaSuccess && st == BQ_OK) e = cudaMemcpyAsync(stage, reinterpret_cast<const char*>(x) + (size_t)k * nb, nb, cudaMemcpyDefault, s);
+            if (e == cudaSuccess && st == BQ_OK) st = bq_field_import(lat, xx + (size_t)k * 2 * fb64, stage, BQ_FULL, BQ_FP64, s);
+        }
         if (e == cudaSuccess) e = cudaStreamSynchronize(s);
         cudaFree(stage);
-        if (e != cudaSuccess) return bq_set_error(lat, BQ_ECUDA, "bq_solve: import failed: %s", cudaGetErrorString(e));
+        if (e != cudaSuccess) return bq_set_error(lat, BQ_ECUDA, "%s: import failed: %s", fn, cudaGetErrorString(e));
         BQ_TRY(st);
     }
-    // |b|^2 over the full lattice (two parities)
-    double bnorm2 = 0;
-    for (int p = 0; p < 2; p++) {
-        BQ_TRY(blas_norm2(lat, c, BQ_FP64, bb + p * fb64));
-        BQ_TRY(poll(lat, w));
-        bnorm2 += w->h_sc->red[0];
-    }
-    const double bnorm = sqrt(bnorm2);
+    // |b_k|^2 over the full lattice (two parities)
+    double* bnorm = static_cast<double*>(calloc(5 * (size_t)n, sizeof(double)));
+    int* ik = static_cast<int*>(calloc(4 * (size_t)n, sizeof(int)));
+    if (!bnorm || !ik) { free(bnorm); free(ik); return bq_set_error(lat, BQ_ENOMEM, "%s: host allocation failed", fn); }
+    double *target = bnorm + n, *prev_rnorm = bnorm + 2 * n, *rnorm = bnorm + 3 * n, *true_rel = bnorm + 4 * n;
+    int *stalled = ik, *inner_total = ik + n, *restarts = ik + 2 * n, *cycles = ik + 3 * n;
     bq_status result = BQ_OK;
-    int outer = 0, inner_total = 0, restarts = 0;
-    if (bnorm == 0.0) {
-        BQ_CUDA(lat, cudaMemsetAsync(w->x, 0, 2 * fb64, s));
-    } else {
+    // every early exit below goes through `fail` so that the host scratch is released
+#define SOLVE_TRY(expr)                         \
+    do {                                        \
+        bq_status _s = (expr);                  \
+        if (_s != BQ_OK) { free(bnorm); free(ik); return _s; } \
+    } while (0)
+    {
+        BlasCtx cb = c;
+        cb.stride = 2 * fb64;
+        for (int p = 0; p < 2; p++) {
+            SOLVE_TRY(blas_norm2(lat, cb, BQ_FP64, bb + p * fb64));
+            SOLVE_TRY(poll(lat, w));
+            for (int k = 0; k < n; k++) bnorm[k] += w->h_sc[k].red[0];
+        }
+    }
+    bool any_nonzero = false;
+    for (int k = 0; k < n; k++) {
+        bnorm[k] = sqrt(bnorm[k]);
+        target[k] = tol * bnorm[k];
+        prev_rnorm[k] = INFINITY;
+        any_nonzero = any_nonzero || bnorm[k] > 0.0;
+    }
+    int outer = 0;
+    // a zero right-hand side has the solution x = 0 (and is "converged" from the start: |r| <= 0 needs x = 0)
+    for (int k = 0; k < n; k++)
+        if (bnorm[k] == 0.0) {
+            cudaError_t e = cudaMemsetAsync(xx + (size_t)k * 2 * fb64, 0, 2 * fb64, s);
+            if (e != cudaSuccess) { free(bnorm); free(ik); return bq_set_error(lat, BQ_ECUDA, "%s: memset failed", fn); }
+        }
+    if (any_nonzero) {
         // ---- b^_e = b_e + kappa H_eo A_oo^-1 b_o ----
         const void* bo = bb + fb64;
+        size_t bo_stride = 2 * fb64;
         if (clover) {
-            BQ_TRY(bq_clover_mul(lat, w->tmp, bo, static_cast<const char*>(cli64) + cb64, BQ_FP64, s));
+            for (int k = 0; k < n; k++)
+                SOLVE_TRY(bq_clover_mul(lat, static_cast<char*>(w->tmp) + (size_t)k * fb64, bb + (size_t)k * 2 * fb64 + fb64,
+                                        static_cast<const char*>(cli64) + cb64, BQ_FP64, s));
             bo = w->tmp;
+            bo_stride = fb64;
         }
-        BQ_TRY(bq_hop(lat, w->bhat, bo, bb, kappa, 0, BQ_FP64, BQ_RECON18, nullptr, 0, s));
-        const double target = tol * bnorm;
-        double prev_rnorm = INFINITY;
-        int stalled = 0;
+        {
+            const HopMulti m = hm(bo_stride, fb64, 2 * fb64);
+            SOLVE_TRY(bq_hop(lat, w->bhat, bo, bb, kappa, 0, BQ_FP64, BQ_RECON18, nullptr, 0, s, nullptr, multi ? &m : none));
+        }
         for (;;) {
             // r = b^_e - M^ x_e in fp64
-            BQ_TRY(schur(lat, w->t, xx, w->tmp, kappa, csw, BQ_FP64, BQ_RECON18, s));
-            BQ_TRY(outer_residual(lat, c, w->bhat, w->t, w->r));
-            BQ_TRY(poll(lat, w));
-            const double rnorm = sqrt(w->h_sc->r2);
-            if (!(rnorm == rnorm)) { result = bq_set_error(lat, BQ_EBREAKDOWN, "bq_solve: residual is NaN"); break; }
-            if (rnorm <= target) break;
-            if (outer >= max_outer) { result = bq_set_error(lat, BQ_ENOTCONVERGED, "bq_solve: max_outer reached, |r|/|b| = %.3e", rnorm / bnorm); break; }
-            if (rnorm > 0.5 * prev_rnorm) {
-                if (++stalled >= 4) { result = bq_set_error(lat, BQ_ENOTCONVERGED, "bq_solve: stalled at |r|/|b| = %.3e", rnorm / bnorm); break; }
-            } else stalled = 0;
-            prev_rnorm = rnorm;
-            outer++;
-            // normalised low-precision right-hand side and inner stopping threshold
-            BQ_TRY(outer_to_low(lat, c, prec, w->r, w->ir));
-            double rel = (prec == BQ_FP64) ? 0.9 * target / rnorm : fmax(inner_tol, 0.5 * target / rnorm);
-            BQ_TRY(inner_bicgstab(lat, w, kappa, csw, prec, o.recon, rel * rel, max_inner, check_every));
-            inner_total += w->h_sc->iters;
-            if (w->h_sc->done == 2) restarts++;   // breakdown: the next outer cycle restarts from the true residual
-            if (w->h_sc->done == 2 && w->h_sc->iters == 0 && restarts > 3) {
-                result = bq_set_error(lat, BQ_EBREAKDOWN, "bq_solve: BiCGStab breakdown (rho or <rhat,v> or <t,t> = 0)");
-                break;
+            {
+                // x_e of rhs k lives at xx + k*2*fb64: Schur with input stride 2*fb64 = two hops by hand
+                const HopMulti m1 = hm(2 * fb64, fb64, 0), m2 = hm(fb64, fb64, 2 * fb64);
+                if (!clover) {
+                    SOLVE_TRY(bq_hop(lat, w->tmp, xx, nullptr, -kappa, 1, BQ_FP64, BQ_RECON18, nullptr, 0, s, nullptr, multi ? &m1 : none));
+                    SOLVE_TRY(bq_hop(lat, w->t, w->tmp, xx, kappa, 0, BQ_FP64, BQ_RECON18, nullptr, 0, s, nullptr, multi ? &m2 : none));
+                } else {
+                    SOLVE_TRY(bq_hop(lat, w->tmp, xx, nullptr, -kappa, 1, BQ_FP64, BQ_RECON18, static_cast<const char*>(cli64) + cb64, 1, s, nullptr, multi ? &m1 : none));
+                    SOLVE_TRY(bq_hop(lat, w->t, w->tmp, xx, kappa, 0, BQ_FP64, BQ_RECON18, cl64, 2, s, nullptr, multi ? &m2 : none));
+                }
             }
+            SOLVE_TRY(outer_residual(lat, c, w->bhat, fb64, w->t, w->r));
+            SOLVE_TRY(poll(lat, w));
+            bool all_conv = true, nan = false, stall = false;
+            double worst = 0;
+            for (int k = 0; k < n; k++) {
+                rnorm[k] = sqrt(w->h_sc[k].r2);
+                if (!(rnorm[k] == rnorm[k])) nan = true;
+                if (bnorm[k] == 0.0 || rnorm[k] <= target[k]) continue;
+                all_conv = false;
+                if (rnorm[k] / bnorm[k] > worst) worst = rnorm[k] / bnorm[k];
+                if (rnorm[k] > 0.5 * prev_rnorm[k]) {
+                    if (++stalled[k] >= 4) stall = true;
+                } else stalled[k] = 0;
+                prev_rnorm[k] = rnorm[k];
+            }
+            if (nan) { result = bq_set_error(lat, BQ_EBREAKDOWN, "%s: residual is NaN", fn); break; }
+            if (all_conv) break;
+            if (outer >= max_outer) { result = bq_set_error(lat, BQ_ENOTCONVERGED, "%s: max_outer reached, |r|/|b| = %.3e", fn, worst); break; }
+            if (stall) { result = bq_set_error(lat, BQ_ENOTCONVERGED, "%s: stalled at |r|/|b| = %.3e", fn, worst); break; }
+            outer++;
+            // normalised low-precision right-hand sides and inner stopping thresholds; a right-hand side that has
+            // already converged gets an infinite threshold: its inner solve stops at once with e = 0
+            SOLVE_TRY(outer_to_low(lat, c, prec, w->r, w->ir));
+            for (int k = 0; k < n; k++) {
+                if (bnorm[k] == 0.0 || rnorm[k] <= target[k]) { w->h_stop2[k] = INFINITY; continue; }
+                const double rel = (prec == BQ_FP64) ? 0.9 * target[k] / rnorm[k] : fmax(inner_tol, 0.5 * target[k] / rnorm[k]);
+                w->h_stop2[k] = rel * rel;
+                cycles[k]++;
+            }
+            SOLVE_TRY(inner_bicgstab(lat, w, kappa, csw, prec, o.recon, max_inner, check_every));
+            bool dead = false;
+            for (int k = 0; k < n; k++) {
+                inner_total[k] += w->h_sc[k].iters;
+                if (w->h_sc[k].done == 2) {   // breakdown: the next outer cycle restarts from the true residual
+                    restarts[k]++;
+                    if (w->h_sc[k].iters == 0 && restarts[k] > 3) dead = true;
+                }
+            }
+            if (dead) { result = bq_set_error(lat, BQ_EBREAKDOWN, "%s: BiCGStab breakdown (rho or <rhat,v> or <t,t> = 0)", fn); break; }
             // x_e += |r| e   (|r| = sc->rnorm, written by outer_residual; the inner loop does not touch it)
-            BQ_TRY(outer_accumulate(lat, c, prec == BQ_HALF ? BQ_FP32 : prec, w->ie, xx));
+            SOLVE_TRY(outer_accumulate(lat, c, prec == BQ_HALF ? BQ_FP32 : prec, w->ie, xx, 2 * fb64));
         }
         // ---- x_o = A_oo^-1 (b_o + kappa H_oe x_e) ----
-        BQ_TRY(bq_hop(lat, xx + fb64, xx, bb + fb64, kappa, 1, BQ_FP64, BQ_RECON18, nullptr, 0, s));
-        if (clover) BQ_TRY(bq_clover_mul(lat, xx + fb64, xx + fb64, static_cast<const char*>(cli64) + cb64, BQ_FP64, s));
-    }
-    // ---- true residual |b - D x| / |b| on the full lattice, fp64 ----
-    double true_rel = 0.0;
-    if (bnorm > 0.0) {
-        // reuse: t (even) and tmp (odd) are one-parity buffers; compute per parity
-        double r2 = 0;
+        {
+            const HopMulti m = hm(2 * fb64, 2 * fb64, 2 * fb64);
+            SOLVE_TRY(bq_hop(lat, xx + fb64, xx, bb + fb64, kappa, 1, BQ_FP64, BQ_RECON18, nullptr, 0, s, nullptr, multi ? &m : none));
+        }
+        if (clover)
+            for (int k = 0; k < n; k++)
+                SOLVE_TRY(bq_clover_mul(lat, xx + (size_t)k * 2 * fb64 + fb64, xx + (size_t)k * 2 * fb64 + fb64,
+                                        static_cast<const char*>(cli64) + cb64, BQ_FP64, s));
+        // ---- true residual |b - D x| / |b| on the full lattice, fp64 ----
         for (int p = 0; p < 2; p++) {
             const void* clp = clover ? static_cast<const char*>(cl64) + p * cb64 : nullptr;
-            BQ_TRY(bq_hop(lat, w->t, xx + (1 - p) * fb64, xx + p * fb64, -kappa, p, BQ_FP64, BQ_RECON18, clp, clover ? 2 : 0, s));
-            BQ_TRY(outer_residual(lat, c, bb + p * fb64, w->t, w->r));
-            BQ_TRY(poll(lat, w));
-            r2 += w->h_sc->r2;
+            const HopMulti m = hm(2 * fb64, fb64, 2 * fb64);
+            SOLVE_TRY(bq_hop(lat, w->t, xx + (1 - p) * fb64, xx + p * fb64, -kappa, p, BQ_FP64, BQ_RECON18, clp, clover ? 2 : 0, s, nullptr,
+                             multi ? &m : none));
+            SOLVE_TRY(outer_residual(lat, c, bb + p * fb64, 2 * fb64, w->t, w->r));
+            SOLVE_TRY(poll(lat, w));
+            for (int k = 0; k < n; k++) true_rel[k] += w->h_sc[k].r2;
         }
-        true_rel = sqrt(r2) / bnorm;
+        for (int k = 0; k < n; k++) true_rel[k] = bnorm[k] > 0.0 ? sqrt(true_rel[k]) / bnorm[k] : 0.0;
     }
     // ---- export x ----
     {
         const size_t nb = (size_t)g.V * 24 * sizeof(double);
         double* stage = nullptr;
-        BQ_CUDA(lat, cudaMalloc(&stage, nb));
-        bq_status st = bq_field_export(lat, stage, w->x, BQ_FULL, BQ_FP64, s);
-        cudaError_t e = cudaSuccess;
-        if (st == BQ_OK) e = cudaMemcpyAsync(x, stage, nb, cudaMemcpyDefault, s);
+        cudaError_t e = cudaMalloc(&stage, nb);
+        bq_status st = BQ_OK;
+        for (int k = 0; k < n && e == cudaSuccess && st == BQ_OK; k++) {
+            st = bq_field_export(lat, stage, xx + (size_t)k * 2 * fb64, BQ_FULL, BQ_FP64, s);
+            if (st == BQ_OK) e = cudaMemcpyAsync(reinterpret_cast<char*>(x) + (size_t)k * nb, stage, nb, cudaMemcpyDefault, s);
+        }
         if (e == cudaSuccess) e = cudaEventRecord(w->ev1, s);
         if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-        cudaFree(stage);
-        if (e != cudaSuccess) return bq_set_error(lat, BQ_ECUDA, "bq_solve: export failed: %s", cudaGetErrorString(e));
-        BQ_TRY(st);
+        if (stage) cudaFree(stage);
+        if (e != cudaSuccess) { free(bnorm); free(ik); return bq_set_error(lat, BQ_ECUDA, "%s: export failed: %s", fn, cudaGetErrorString(e)); }
+        SOLVE_TRY(st);
     }
+#undef SOLVE_TRY
     float ms = 0;
     cudaEventElapsedTime(&ms, w->ev0, w->ev1);
-    if (info) {
-        info->status = result;
-        info->outer_cycles = (prec == BQ_FP64) ? 0 : outer;
-        info->inner_iters = inner_total;
-        info->restarts = (prec == BQ_FP64) ? (outer > 0 ? outer - 1 : 0) + restarts : restarts;
-        info->true_rel_residual = true_rel;
-        info->seconds = ms * 1e-3;
-    }
+    if (info)
+        for (int k = 0; k < n; k++) {
+            info[k].status = result;
+            info[k].outer_cycles = (prec == BQ_FP64) ? 0 : cycles[k];
+            info[k].inner_iters = inner_total[k];
+            info[k].restarts = (prec == BQ_FP64) ? (cycles[k] > 0 ? cycles[k] - 1 : 0) + restarts[k] : restarts[k];
+            info[k].true_rel_residual = true_rel[k];
+            info[k].seconds = ms * 1e-3;     // device time of the whole call (all right-hand sides together)
+        }
+    free(bnorm);
+    free(ik);
+    w->blas.nrhs = 1;
     return result;
+}
+
+extern "C" bq_status bq_solve(bq_lattice* lat, const double* b, double* x, double kappa, double tol, const bq_solve_opts* opts,
+                              bq_solve_info* info) {
+    return solve_impl(lat, b, x, 1, false, kappa, tol, opts, info);
+}
+
+extern "C" bq_status bq_solve_multi(bq_lattice* lat, const double* b, double* x, int nrhs, double kappa, double tol,
+                                    const bq_solve_opts* opts, bq_solve_info* info) {
+    return solve_impl(lat, b, x, nrhs, true, kappa, tol, opts, info);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -504,6 +622,83 @@ extern "C" bq_status bq_bench_kernel(bq_lattice* lat, int which, bq_prec prec, b
     cudaFree(pool);
     if (st != BQ_OK) return st;
     if (e != cudaSuccess) return bq_set_error(lat, BQ_ECUDA, "bq_bench_kernel: %s", cudaGetErrorString(e));
+    *us_per_launch = (double)ms * 1e3 / reps;
+    *bytes_per_launch = bytes * (double)g.Vh;
+    return BQ_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// bq_bench_kernel_multi: the same measurement for the multi-rhs kernels.  Algorithmic bytes per launch: links and
+// clover blocks once, spinors once per right-hand side.
+// ---------------------------------------------------------------------------------------------------
+extern "C" bq_status bq_bench_kernel_multi(bq_lattice* lat, int which, bq_prec prec, bq_recon recon, double csw, double kappa,
+                                           int nrhs, int reps, int nsets, double* us_per_launch, double* bytes_per_launch) {
+    if (!lat) return BQ_EINVAL;
+    if (!us_per_launch || !bytes_per_launch || reps < 1 || nsets < 1 || nsets > 16 || nrhs < 1)
+        return bq_set_error(lat, BQ_EINVAL, "bq_bench_kernel_multi: bad arguments");
+    if (prec != BQ_FP64 && prec != BQ_FP32 && prec != BQ_HALF) return bq_set_error(lat, BQ_EINVAL, "bq_bench_kernel_multi: bad precision");
+    if (recon != BQ_RECON18 && recon != BQ_RECON12) return bq_set_error(lat, BQ_EINVAL, "bq_bench_kernel_multi: bad recon");
+    if (!lat->have_gauge) return bq_set_error(lat, BQ_ENOGAUGE, "bq_bench_kernel_multi: no gauge field loaded");
+    const Geom& g = lat->g;
+    cudaStream_t s = 0;
+    const size_t fb = field_bytes_one_parity(g, prec);
+    const bool clover = csw != 0.0;
+    const void *cl = nullptr, *cli = nullptr;
+    const size_t cb = (size_t)g.Vh * CLOVER_REALS * prec_real_bytes(prec);
+    if (clover) {
+        BQ_TRY(bq_clover_build(lat, csw, kappa));
+        BQ_TRY(bq_get_clover(lat, prec, 0, &cl));
+        BQ_TRY(bq_get_clover(lat, prec, 1, &cli));
+    }
+    const void* gauge = nullptr;
+    BQ_TRY(bq_get_gauge(lat, prec, recon, &gauge));
+    constexpr int NV = 3;     // per set: out, in, z/tmp — each an array of nrhs fields
+    char* pool = nullptr;
+    const size_t vec_bytes = fb * nrhs, set_bytes = NV * vec_bytes;
+    BQ_CUDA(lat, cudaMalloc(&pool, set_bytes * nsets));
+    for (int set = 0; set < nsets; set++)
+        for (int i = 0; i < NV * nrhs; i++) bench_fill(prec, g.Vh, pool + (size_t)set * set_bytes + (size_t)i * fb, 1 + set * 64 + i, s);
+    const double spin_b = (double)spinor_site_bytes(prec), link_b = (double)link_reals(recon) * prec_real_bytes(prec);
+    const double clov_b = (double)CLOVER_REALS * prec_real_bytes(prec);
+    double bytes = 0;
+    bq_status st = BQ_OK;
+    const HopMulti m{nrhs, fb, fb, fb, fb};
+    auto launch = [&](int set) -> bq_status {
+        void *v0 = pool + (size_t)set * set_bytes, *v1 = pool + (size_t)set * set_bytes + vec_bytes, *v2 = pool + (size_t)set * set_bytes + 2 * vec_bytes;
+        switch (which) {
+            case BQ_K_HOP: bytes = 8 * link_b + nrhs * 2 * spin_b; return bq_hop(lat, v0, v1, nullptr, -kappa, 0, prec, recon, nullptr, 0, s, nullptr, &m);
+            case BQ_K_HOP_XPAY: bytes = 8 * link_b + nrhs * 3 * spin_b; return bq_hop(lat, v0, v1, v2, kappa, 0, prec, recon, nullptr, 0, s, nullptr, &m);
+            case BQ_K_HOP_CLOVINV:
+                if (!clover) return bq_set_error(lat, BQ_EINVAL, "bq_bench_kernel_multi: clover kernels need csw != 0");
+                bytes = 8 * link_b + clov_b + nrhs * 2 * spin_b;
+                return bq_hop(lat, v0, v1, nullptr, -kappa, 1, prec, recon, static_cast<const char*>(cli) + cb, 1, s, nullptr, &m);
+            case BQ_K_HOP_CLOV_XPAY:
+                if (!clover) return bq_set_error(lat, BQ_EINVAL, "bq_bench_kernel_multi: clover kernels need csw != 0");
+                bytes = 8 * link_b + clov_b + nrhs * 3 * spin_b;
+                return bq_hop(lat, v0, v1, v2, kappa, 0, prec, recon, cl, 2, s, nullptr, &m);
+            case BQ_K_SCHUR:
+                bytes = 2 * (8 * link_b + nrhs * 2 * spin_b) + nrhs * spin_b + (clover ? 2 * clov_b : 0);
+                return bq_schur_red(lat, v0, v1, v2, kappa, csw, prec, recon, s, nullptr, nrhs);
+            default: return bq_set_error(lat, BQ_EINVAL, "bq_bench_kernel_multi: unsupported kernel id %d", which);
+        }
+    };
+    for (int i = 0; i < nsets && st == BQ_OK; i++) st = launch(i);
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    if (st == BQ_OK) {
+        cudaEventRecord(e0, s);
+        for (int i = 0; i < reps && st == BQ_OK; i++) st = launch(i % nsets);
+        cudaEventRecord(e1, s);
+    }
+    cudaError_t e = cudaStreamSynchronize(s);
+    float ms = 0;
+    if (st == BQ_OK && e == cudaSuccess) cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(pool);
+    if (st != BQ_OK) return st;
+    if (e != cudaSuccess) return bq_set_error(lat, BQ_ECUDA, "bq_bench_kernel_multi: %s", cudaGetErrorString(e));
     *us_per_launch = (double)ms * 1e3 / reps;
     *bytes_per_launch = bytes * (double)g.Vh;
     return BQ_OK;

@@ -23,7 +23,10 @@ def main():
     ap.add_argument("--nsets", type=int, default=3)
     ap.add_argument("--json", action="store_true")
     ap.add_argument("--precs", default="fp64,fp32,half")
+    ap.add_argument("--nrhs", default="2,4,8,12,16", help="right-hand sides per launch for the multi-rhs lines ('' = none)")
+    ap.add_argument("--only", default="", help="comma-separated kernel names to run (e.g. 'hop,hop x12'); default all")
     args = ap.parse_args()
+    only = [v.strip() for v in args.only.split(",") if v.strip()]
     import torch
     from . import bq, build, inputs
     assert torch.cuda.is_available(), "kbench needs a CUDA device"
@@ -46,16 +49,29 @@ def main():
                                       ("hop_xpay_omega", 0, 0.0), ("hop_xpay_alpha", 0, 1.0), ("hop_xpay_omega", 0, 1.0),
                                       ("bicg_iter_unfused", 0, 0.0), ("bicg_iter", 0, 0.0), ("bicg_iter", 1, 0.0),
                                       ("bicg_iter_unfused", 0, 1.0), ("bicg_iter", 0, 1.0)]):
+                if only and which not in only:
+                    continue
                 us, nb = bq.bq_bench_kernel(lat.h, which, prec, recon, csw, 0.1215, args.reps, args.nsets)
                 rows.append({"kernel": which, "prec": pname, "recon": 12 if recon else 18, "csw": csw, "us": us, "bytes": nb,
                              "gbs": nb / us / 1e3, "frac": nb / us / 1e3 / peak})
+        # multi-rhs kernels: one launch covers nrhs right-hand sides; bytes count the links once
+        for pname in args.precs.split(","):
+            prec = {"fp64": 0, "fp32": 1, "half": 2}[pname]
+            for nrhs in [int(v) for v in args.nrhs.split(",") if v]:
+                for which, recon, csw in (("hop", 0, 0.0), ("hop", 1, 0.0), ("schur", 0, 0.0), ("schur", 0, 1.0)):
+                    if only and f"{which} x{nrhs}" not in only:
+                        continue
+                    us, nb = bq.bq_bench_kernel_multi(lat.h, which, prec, nrhs, recon, csw, 0.1215, max(8, args.reps // nrhs), 2)
+                    rows.append({"kernel": f"{which} x{nrhs}", "prec": pname, "recon": 12 if recon else 18, "csw": csw, "us": us,
+                                 "bytes": nb, "gbs": nb / us / 1e3, "frac": nb / us / 1e3 / peak, "nrhs": nrhs, "us_per_rhs": us / nrhs})
     if args.json:
         print(json.dumps({"lattice": L, "peak_gbs": peak, "rows": rows}))
         return
     print(f"# lattice {L}, reps {args.reps}, nsets {args.nsets}, peak {peak:.0f} GB/s (measured copy)")
     print(f"{'kernel':18s} {'prec':5s} {'links':5s} {'csw':>4s} {'us':>9s} {'MB':>9s} {'GB/s':>8s} {'frac':>6s}")
     for r in rows:
-        print(f"{r['kernel']:18s} {r['prec']:5s} {r['recon']:<5d} {r['csw']:4.1f} {r['us']:9.1f} {r['bytes'] / 1e6:9.1f} {r['gbs']:8.0f} {r['frac']:6.3f}")
+        tail = f"   {r['us_per_rhs']:7.1f} us/rhs" if "nrhs" in r else ""
+        print(f"{r['kernel']:18s} {r['prec']:5s} {r['recon']:<5d} {r['csw']:4.1f} {r['us']:9.1f} {r['bytes'] / 1e6:9.1f} {r['gbs']:8.0f} {r['frac']:6.3f}{tail}")
 
 
 if __name__ == "__main__":
