@@ -240,7 +240,8 @@ typedef enum {
 bq_status bq_bench_kernel(bq_lattice* lat, int which, bq_prec prec, bq_recon recon, double csw, double kappa, int reps,
                           int nsets, double* us_per_launch, double* bytes_per_launch);
 
-/* The same for the multi-rhs kernels (BQ_K_HOP, BQ_K_HOP_XPAY, BQ_K_HOP_CLOVINV, BQ_K_HOP_CLOV_XPAY, BQ_K_SCHUR):
+/* The same for the multi-rhs kernels (BQ_K_HOP, BQ_K_HOP_XPAY, BQ_K_HOP_CLOVINV, BQ_K_HOP_CLOV_XPAY, BQ_K_SCHUR,
+ * BQ_K_BICG_ITER = one batched inner iteration of bq_solve_multi):
  * one launch processes nrhs right-hand sides; bytes_per_launch counts links and clover blocks once and the spinors
  * once per right-hand side. */
 bq_status bq_bench_kernel_multi(bq_lattice* lat, int which, bq_prec prec, bq_recon recon, double csw, double kappa,

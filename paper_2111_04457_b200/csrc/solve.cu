@@ -652,12 +652,28 @@ extern "C" bq_status bq_bench_kernel_multi(bq_lattice* lat, int which, bq_prec p
     }
     const void* gauge = nullptr;
     BQ_TRY(bq_get_gauge(lat, prec, recon, &gauge));
-    constexpr int NV = 3;     // per set: out, in, z/tmp — each an array of nrhs fields
+    const bool iter = which == BQ_K_BICG_ITER;
+    const int NV = iter ? 8 : 3;     // per set: out, in, z/tmp (+ the BiCGStab vectors) — each an array of nrhs fields
+    const size_t xb = field_bytes_one_parity(g, prec == BQ_HALF ? BQ_FP32 : prec);
+    SolverWork* w = nullptr;
+    if (iter) {
+        BQ_TRY(get_work(lat, lat->work && lat->work->inner_prec >= 0 ? lat->work->inner_prec : BQ_FP32, &w));
+        BQ_TRY(blas_ctx_reserve(lat, &w->blas, nrhs));
+        w->blas.nrhs = nrhs; w->blas.stride = fb; w->blas.xstride = xb; w->blas.stride64 = field_bytes_one_parity(g, BQ_FP64);
+        s = w->blas.stream;
+        for (int k = 0; k < nrhs; k++) {
+            k_set_bicg_scalars<<<1, 1, 0, s>>>(w->blas.sc + k, 0.5, 0.1, 0.5, -0.1);
+            BQ_CHECK_LAUNCH(lat);
+        }
+    }
     char* pool = nullptr;
-    const size_t vec_bytes = fb * nrhs, set_bytes = NV * vec_bytes;
+    const size_t vec_bytes = (fb > xb ? fb : xb) * nrhs, set_bytes = NV * vec_bytes;
     BQ_CUDA(lat, cudaMalloc(&pool, set_bytes * nsets));
     for (int set = 0; set < nsets; set++)
-        for (int i = 0; i < NV * nrhs; i++) bench_fill(prec, g.Vh, pool + (size_t)set * set_bytes + (size_t)i * fb, 1 + set * 64 + i, s);
+        for (int i = 0; i < NV; i++)
+            for (int k = 0; k < nrhs; k++)
+                bench_fill(i == 7 && prec == BQ_HALF ? BQ_FP32 : prec, g.Vh,
+                           pool + (size_t)set * set_bytes + (size_t)i * vec_bytes + (size_t)k * (i == 7 ? xb : fb), 1 + set * 256 + i * 16 + k, s);
     const double spin_b = (double)spinor_site_bytes(prec), link_b = (double)link_reals(recon) * prec_real_bytes(prec);
     const double clov_b = (double)CLOVER_REALS * prec_real_bytes(prec);
     double bytes = 0;
@@ -679,6 +695,22 @@ extern "C" bq_status bq_bench_kernel_multi(bq_lattice* lat, int which, bq_prec p
             case BQ_K_SCHUR:
                 bytes = 2 * (8 * link_b + nrhs * 2 * spin_b) + nrhs * spin_b + (clover ? 2 * clov_b : 0);
                 return bq_schur_red(lat, v0, v1, v2, kappa, csw, prec, recon, s, nullptr, nrhs);
+            case BQ_K_BICG_ITER: {
+                // one whole batched inner iteration as bq_solve_multi runs it (7 launches + 2 one-CTA-per-rhs finalisers)
+                const BlasCtx& c = w->blas;
+                char* base = pool + (size_t)set * set_bytes;
+                void *r = base, *p = base + vec_bytes, *v = base + 2 * vec_bytes, *rhat = base + 3 * vec_bytes, *sv = base + 4 * vec_bytes,
+                     *t = base + 5 * vec_bytes, *tmp = base + 6 * vec_bytes, *x = base + 7 * vec_bytes;
+                const double schur_b = 2 * (8 * link_b + nrhs * 2 * spin_b) + nrhs * spin_b + (clover ? 2 * clov_b : 0);
+                const double acc_b = (double)spinor_site_bytes(prec == BQ_HALF ? BQ_FP32 : prec);
+                bytes = 2 * schur_b + nrhs * ((4 + 3 + 5 + 1) * spin_b + 2 * acc_b);
+                const HopRed red_alpha{1, rhat, c.sc}, red_omega{2, nullptr, c.sc};
+                BQ_TRY(bicg_p_update(lat, c, prec, r, p, v));
+                BQ_TRY(bq_schur_red(lat, v, p, tmp, kappa, csw, prec, recon, s, &red_alpha, nrhs));
+                BQ_TRY(bicg_s_update(lat, c, prec, r, v, sv));
+                BQ_TRY(bq_schur_red(lat, t, sv, tmp, kappa, csw, prec, recon, s, &red_omega, nrhs));
+                return bicg_final(lat, c, prec, p, sv, t, rhat, x, r);
+            }
             default: return bq_set_error(lat, BQ_EINVAL, "bq_bench_kernel_multi: unsupported kernel id %d", which);
         }
     };
@@ -697,6 +729,7 @@ extern "C" bq_status bq_bench_kernel_multi(bq_lattice* lat, int which, bq_prec p
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     cudaFree(pool);
+    if (w) w->blas.nrhs = 1;
     if (st != BQ_OK) return st;
     if (e != cudaSuccess) return bq_set_error(lat, BQ_ECUDA, "bq_bench_kernel_multi: %s", cudaGetErrorString(e));
     *us_per_launch = (double)ms * 1e3 / reps;

@@ -24,6 +24,8 @@ def main():
     ap.add_argument("--json", action="store_true")
     ap.add_argument("--precs", default="fp64,fp32,half")
     ap.add_argument("--nrhs", default="2,4,8,12,16", help="right-hand sides per launch for the multi-rhs lines ('' = none)")
+    ap.add_argument("--solve", type=int, default=0, metavar="NRHS",
+                    help="also time bq_solve_multi on NRHS point sources against NRHS separate bq_solve calls (device buffers)")
     ap.add_argument("--only", default="", help="comma-separated kernel names to run (e.g. 'hop,hop x12'); default all")
     args = ap.parse_args()
     only = [v.strip() for v in args.only.split(",") if v.strip()]
@@ -58,20 +60,46 @@ def main():
         for pname in args.precs.split(","):
             prec = {"fp64": 0, "fp32": 1, "half": 2}[pname]
             for nrhs in [int(v) for v in args.nrhs.split(",") if v]:
-                for which, recon, csw in (("hop", 0, 0.0), ("hop", 1, 0.0), ("schur", 0, 0.0), ("schur", 0, 1.0)):
+                for which, recon, csw in (("hop", 0, 0.0), ("hop", 1, 0.0), ("schur", 0, 0.0), ("schur", 0, 1.0), ("bicg_iter", 0, 0.0),
+                                          ("bicg_iter", 0, 1.0)):
                     if only and f"{which} x{nrhs}" not in only:
                         continue
                     us, nb = bq.bq_bench_kernel_multi(lat.h, which, prec, nrhs, recon, csw, 0.1215, max(8, args.reps // nrhs), 2)
                     rows.append({"kernel": f"{which} x{nrhs}", "prec": pname, "recon": 12 if recon else 18, "csw": csw, "us": us,
                                  "bytes": nb, "gbs": nb / us / 1e3, "frac": nb / us / 1e3 / peak, "nrhs": nrhs, "us_per_rhs": us / nrhs})
+        solve = None
+        if args.solve > 0:
+            # the paper's propagator workload: point sources e_s (x) e_c at the origin, one gauge field
+            n = args.solve
+            Lx, Ly, Lz, Lt = L
+            b = torch.zeros((n, Lt, Lz, Ly, Lx, 4, 3), dtype=torch.complex128, device="cuda")
+            for k in range(n):
+                b[k, 0, 0, 0, 0, (k // 3) % 4, k % 3] = 1.0
+            x = torch.zeros_like(b)
+            solve = []
+            for pname, csw in (("fp32", 0.0), ("fp32", 1.0), ("half", 0.0)):
+                opts = bq.bq_solve_opts(inner_prec={"fp32": 1, "half": 2}[pname], csw=csw)
+                for rep in range(2):                       # first pass = warm-up (workspace, clover build)
+                    x.zero_()
+                    infos = bq.bq_solve_multi(lat.h, b, x, n, 0.1215, 1e-10, opts)
+                    t_multi = infos[0].seconds
+                    t_single = 0.0
+                    x.zero_()
+                    for k in range(n):
+                        t_single += bq.bq_solve(lat.h, b[k], x[k], 0.1215, 1e-10, opts).seconds
+                solve.append({"prec": pname, "csw": csw, "nrhs": n, "multi_s": t_multi, "single_s": t_single,
+                              "iters": [i.inner_iters for i in infos], "res": max(i.true_rel_residual for i in infos)})
     if args.json:
-        print(json.dumps({"lattice": L, "peak_gbs": peak, "rows": rows}))
+        print(json.dumps({"lattice": L, "peak_gbs": peak, "rows": rows, "solve": solve}))
         return
     print(f"# lattice {L}, reps {args.reps}, nsets {args.nsets}, peak {peak:.0f} GB/s (measured copy)")
     print(f"{'kernel':18s} {'prec':5s} {'links':5s} {'csw':>4s} {'us':>9s} {'MB':>9s} {'GB/s':>8s} {'frac':>6s}")
     for r in rows:
         tail = f"   {r['us_per_rhs']:7.1f} us/rhs" if "nrhs" in r else ""
         print(f"{r['kernel']:18s} {r['prec']:5s} {r['recon']:<5d} {r['csw']:4.1f} {r['us']:9.1f} {r['bytes'] / 1e6:9.1f} {r['gbs']:8.0f} {r['frac']:6.3f}{tail}")
+    for r in solve or []:
+        print(f"# solve x{r['nrhs']} {r['prec']} inner, csw {r['csw']}: bq_solve_multi {r['multi_s'] * 1e3:.1f} ms vs {r['nrhs']} x bq_solve "
+              f"{r['single_s'] * 1e3:.1f} ms (device time incl. layout conversion), inner iterations {r['iters']}, worst |r|/|b| {r['res']:.1e}")
 
 
 if __name__ == "__main__":
