@@ -21,6 +21,9 @@
  * eigenvalues in closed form, gamma5-hermiticity, gauge covariance, brute-force dense matrix on
  * 4^4 (assembled in numpy from Kronecker products: disjoint code path), abelian constant-flux
  * field strength, sign of the clover term, point-source pattern, even-odd Schur identities.
+ * D^dagger (bqo_dirac_apply_dag, the definition of the adjoint as a scatter) and the CGNR of bqo.py are pinned by
+ * tests/test_oracle_dagger_pins.py: conjugate transpose of the dense matrix, D^dag = g5 D g5, <x,Dy> = <D^dag x,y>,
+ * free-field eigenvalue conj(lambda), point-source stencil, numpy.linalg.solve.
  * Unpinned readings: S5 (trace part of F_mu_nu is NOT subtracted; `traceless` flag, default 0)
  * and S9 (meaning of nconv/diff) — "parity unpinned" for those two choices, see DESIGN.md §3.
  */
@@ -171,6 +174,56 @@ int bqo_dirac_apply_sites(const int* L, const double* bc, const double* U, doubl
 #pragma omp parallel for schedule(static)
     for (long k = 0; k < nsites; k++)
         dirac_site(L, (const cplx*)bc, (const cplx*)U, kappa, (const cplx*)A, (const cplx*)in, sites[k], (cplx*)out + 12 * k);
+    return 0;
+}
+
+/* out = D^dagger in on the whole lattice, by the DEFINITION of the adjoint, (D^dag)_{y,x} = (D_{x,y})^dag
+ * (the paper's set_mode("Ddag")): every 12x12 block D_{x,y} of Eq. 1 is
+ * taken exactly as dirac_site uses it and its conjugate transpose is scattered,  out(y) += (D_{x,y})^dag in(x).
+ *   D_{x,x}    = A(x)
+ *   D_{x,x+mu} = -kappa phi+_mu(x) (1 - gamma_mu) (x) U_mu(x)
+ *   D_{x,x-mu} = -kappa phi-_mu(x) (1 + gamma_mu) (x) U_mu(x-mu)^dag
+ * Block element: D[(sp,a),(sq,b)] = c * P[sp][sq] * W[a][b]  =>  (D^dag in)[(sq,b)] += conj(c P[sp][sq] W[a][b]) in[(sp,a)].
+ * Serial scatter (no derivation of a gather form, so that nothing but the definition is trusted).
+ * in and out must not alias. */
+int bqo_dirac_apply_dag(const int* L, const double* bc_, const double* U_, double kappa, const double* A_,
+                        const double* in_, double* out_) {
+    long V = volume(L);
+    const cplx *bc = (const cplx*)bc_, *U = (const cplx*)U_, *A = (const cplx*)A_, *in = (const cplx*)in_;
+    cplx* out = (cplx*)out_;
+    for (long i = 0; i < 12 * V; i++) out[i] = 0;
+    for (long s = 0; s < V; s++) {
+        int x[4];
+        coords(L, s, x);
+        const cplx* v = in + 12 * s;
+        /* diagonal block A(x) (identity for Wilson) */
+        for (int j = 0; j < 12; j++) {
+            if (A) {
+                cplx c = 0;
+                for (int i = 0; i < 12; i++) c += conj(A[144 * s + 12 * i + j]) * v[i];
+                out[12 * s + j] += c;
+            } else {
+                out[12 * s + j] += v[j];
+            }
+        }
+        for (int mu = 0; mu < 4; mu++) {
+            for (int dir = 0; dir < 2; dir++) {   /* 0: block D_{x,x+mu}, 1: block D_{x,x-mu} */
+                long y = shifted(L, x, mu, dir == 0 ? +1 : -1);
+                cplx c = -kappa * (dir == 0 ? ((x[mu] == L[mu] - 1) ? bc[mu] : 1.0) : ((x[mu] == 0) ? conj(bc[mu]) : 1.0));
+                const cplx* Um = U + 9 * (4 * (dir == 0 ? s : y) + mu);
+                for (int sp = 0; sp < 4; sp++)
+                    for (int sq = 0; sq < 4; sq++) {
+                        cplx P = (sp == sq ? 1.0 : 0.0) + (dir == 0 ? -1.0 : 1.0) * GAMMA[mu][sp][sq];
+                        if (P == 0) continue;
+                        for (int a = 0; a < 3; a++)
+                            for (int b = 0; b < 3; b++) {
+                                cplx W = dir == 0 ? Um[3 * a + b] : conj(Um[3 * b + a]);
+                                out[12 * y + 3 * sq + b] += conj(c * P * W) * v[3 * sp + a];
+                            }
+                    }
+            }
+        }
+    }
     return 0;
 }
 

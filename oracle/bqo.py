@@ -56,6 +56,7 @@ def _load():
         lib.bqo_gamma.argtypes = [ctypes.c_int, _dp]
         lib.bqo_gamma.restype = None
         lib.bqo_dirac_apply.argtypes = [_ip, _dp, _dp, ctypes.c_double, _dp, _dp, _dp]
+        lib.bqo_dirac_apply_dag.argtypes = [_ip, _dp, _dp, ctypes.c_double, _dp, _dp, _dp]
         lib.bqo_dirac_apply_sites.argtypes = [_ip, _dp, _dp, ctypes.c_double, _dp, _dp, ctypes.c_long, _lp, _dp]
         lib.bqo_field_strength.argtypes = [_ip, _dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp]
         lib.bqo_clover_build.argtypes = [_ip, _dp, ctypes.c_double, ctypes.c_double, ctypes.c_int, _dp]
@@ -110,6 +111,47 @@ def dirac_apply(U, psi, kappa, bc=None, A=None) -> np.ndarray:
     Ac = None if A is None else _c(A)
     _load().bqo_dirac_apply(_Larr(L), _p(bcv), _p(U), float(kappa), _p(Ac), _p(psi), _p(out))
     return out
+
+
+def dirac_apply_dag(U, psi, kappa, bc=None, A=None) -> np.ndarray:
+    """out = D^dagger psi, by the definition of the adjoint (scatter of the conjugate-transposed blocks of Eq. 1)."""
+    U, psi = _c(U), _c(psi)
+    L = lattice_of(psi)
+    out = np.empty_like(psi)
+    bcv = _bc(bc)
+    Ac = None if A is None else _c(A)
+    _load().bqo_dirac_apply_dag(_Larr(L), _p(bcv), _p(U), float(kappa), _p(Ac), _p(psi), _p(out))
+    return out
+
+
+def cgnr(U, b, kappa, tol=1e-12, max_iter=10000, bc=None, A=None):
+    """Solve D x = b by conjugate gradients on the normal equations D^dag D x = D^dag b (Hestenes-Stiefel CG,
+    textbook form).  Stops when the TRUE residual of the original system satisfies
+    |b - D x| / |b| <= tol (checked every iteration with its own operator apply: slow and obviously right).
+    Returns (x, info dict)."""
+    b = _c(b)
+    x = np.zeros_like(b)
+    bnorm = np.linalg.norm(b)
+    if bnorm == 0.0:
+        return x, {"status": 0, "iters": 0, "relres": 0.0}
+    r = dirac_apply_dag(U, b, kappa, bc=bc, A=A)        # normal-equation residual D^dag (b - D x), x = 0
+    p = r.copy()
+    rr = np.vdot(r, r).real
+    status, it, rel = 1, 0, 1.0
+    while it < max_iter:
+        q = dirac_apply(U, p, kappa, bc=bc, A=A)
+        alpha = rr / np.vdot(q, q).real                 # <p, D^dag D p> = |D p|^2
+        x = x + alpha * p
+        r = r - alpha * dirac_apply_dag(U, q, kappa, bc=bc, A=A)
+        it += 1
+        rel = np.linalg.norm(b - dirac_apply(U, x, kappa, bc=bc, A=A)) / bnorm
+        if rel <= tol:
+            status = 0
+            break
+        rr_new = np.vdot(r, r).real
+        p = r + (rr_new / rr) * p
+        rr = rr_new
+    return x, {"status": status, "iters": it, "relres": rel}
 
 
 def dirac_apply_sites(U, psi, kappa, sites, bc=None, A=None) -> np.ndarray:
