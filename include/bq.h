@@ -72,6 +72,8 @@ typedef enum { BQ_FP64 = 0, BQ_FP32 = 1, BQ_HALF = 2 } bq_prec;
 typedef enum { BQ_EVEN = 0, BQ_ODD = 1, BQ_FULL = 2 } bq_parity;
 /* 18 reals per link, or rows 0,1 only (12 reals) with row 2 = conj(row0 x row1) rebuilt in registers. */
 typedef enum { BQ_RECON18 = 0, BQ_RECON12 = 1 } bq_recon;
+/* Operator modes of the paper's interface, set_mode("D"), ("Ddag"), ("DdagD"). */
+typedef enum { BQ_MODE_D = 0, BQ_MODE_DDAG = 1, BQ_MODE_DDAGD = 2 } bq_mode;
 
 /* Lattice handle.  bc_phase = 4 x (re, im): psi(x + L_mu mu^) = phi_mu psi(x), |phi_mu| = 1
  * ("a boundary condition ... is imposed in each direction"; reading S3: the phase multiplies the
@@ -135,6 +137,18 @@ bq_status bq_dirac_apply(bq_lattice* lat, void* out, const void* in, double kapp
  * tmp: caller-provided scratch field of one parity (same precision).  in, out, tmp must not overlap. */
 bq_status bq_schur_apply(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw,
                          bq_prec prec, bq_recon recon, void* stream);
+
+/* The operator in the paper's three modes, full lattice, internal layout:
+ *   BQ_MODE_D: out = D in;   BQ_MODE_DDAG: out = D^dagger in;   BQ_MODE_DDAGD: out = D^dagger D in.
+ * D^dagger = g5 D g5: the same hop kernel with the projectors (1 -+ g_mu) exchanged (a compile-time variant that
+ * renames registers; links, phases and traffic are those of D); the clover term is Hermitian.
+ * tmp: scratch field of the full lattice, needed (and must be distinct) for BQ_MODE_DDAGD only. */
+bq_status bq_dirac_apply_mode(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw, bq_mode mode,
+                              bq_prec prec, bq_recon recon, void* stream);
+/* The even-odd Schur operator in the same modes: M^, M^^dagger = A_ee - kappa^2 H^dag_eo A_oo^-1 H^dag_oe, M^^dagger M^.
+ * tmp: one-parity scratch; tmp2: a second one, BQ_MODE_DDAGD only. */
+bq_status bq_schur_apply_mode(bq_lattice* lat, void* out, const void* in, void* tmp, void* tmp2, double kappa, double csw,
+                              bq_mode mode, bq_prec prec, bq_recon recon, void* stream);
 
 /* Multi-right-hand-side forms (the paper's use case is the 12 spin-colour sources of one
  * propagator on one gauge field): the same operators applied to nrhs fields in ONE launch per hop, so

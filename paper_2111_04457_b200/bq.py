@@ -21,13 +21,14 @@ BQ_OK, BQ_EINVAL, BQ_EODD_EXTENT, BQ_ENOGAUGE, BQ_ENOCLOVER, BQ_ESINGULAR_CLOVER
 BQ_FP64, BQ_FP32, BQ_HALF = 0, 1, 2
 BQ_EVEN, BQ_ODD, BQ_FULL = 0, 1, 2
 BQ_RECON18, BQ_RECON12 = 0, 1
+BQ_MODE_D, BQ_MODE_DDAG, BQ_MODE_DDAGD = 0, 1, 2
 
 EXPORTS = [
     "bq_lattice_create", "bq_lattice_destroy", "bq_status_string", "bq_last_error", "bq_gauge_load",
     "bq_field_bytes", "bq_field_import", "bq_field_export", "bq_wilson_apply", "bq_clover_apply",
     "bq_dirac_apply", "bq_schur_apply", "bq_solve", "bq_blas_norm2", "bq_blas_cdot", "bq_blas_caxpy",
     "bq_blas_bicg_update", "bq_get_counters", "bq_bench_kernel", "bq_schur_apply_dots",
-    "bq_wilson_apply_multi", "bq_schur_apply_multi", "bq_bench_kernel_multi", "bq_solve_multi",
+    "bq_wilson_apply_multi", "bq_schur_apply_multi", "bq_bench_kernel_multi", "bq_solve_multi", "bq_dirac_apply_mode", "bq_schur_apply_mode",
 ]
 
 
@@ -77,6 +78,8 @@ def lib():
         L.bq_schur_apply_dots.argtypes = [_vp, _vp, _vp, _vp, _d, _d, _i, _i, _vp, _dp]
         L.bq_solve.argtypes = [_vp, _vp, _vp, _d, _d, ctypes.POINTER(bq_solve_opts), ctypes.POINTER(bq_solve_info)]
         L.bq_solve_multi.argtypes = [_vp, _vp, _vp, _i, _d, _d, ctypes.POINTER(bq_solve_opts), ctypes.POINTER(bq_solve_info)]
+        L.bq_dirac_apply_mode.argtypes = [_vp, _vp, _vp, _vp, _d, _d, _i, _i, _i, _vp]
+        L.bq_schur_apply_mode.argtypes = [_vp, _vp, _vp, _vp, _vp, _d, _d, _i, _i, _i, _vp]
         L.bq_blas_norm2.argtypes = [_vp, _vp, _i, _dp]
         L.bq_blas_cdot.argtypes = [_vp, _vp, _vp, _i, _dp]
         L.bq_blas_caxpy.argtypes = [_vp, _dp, _vp, _vp, _i]
@@ -178,6 +181,15 @@ def bq_wilson_apply_multi(h, out, inp, nrhs, kappa, parity, prec=BQ_FP32, recon=
 def bq_schur_apply_multi(h, out, inp, tmp, nrhs, kappa, csw, prec, recon=BQ_RECON18, stream=None):
     _check(h, lib().bq_schur_apply_multi(h, _ptr(out), _ptr(inp), _ptr(tmp), nrhs, kappa, csw, prec, recon,
                                          _stream_ptr(stream)))
+
+
+def bq_dirac_apply_mode(h, out, inp, tmp, kappa, csw, mode, prec, recon=BQ_RECON18, stream=None):
+    _check(h, lib().bq_dirac_apply_mode(h, _ptr(out), _ptr(inp), _ptr(tmp), kappa, csw, mode, prec, recon, _stream_ptr(stream)))
+
+
+def bq_schur_apply_mode(h, out, inp, tmp, tmp2, kappa, csw, mode, prec, recon=BQ_RECON18, stream=None):
+    _check(h, lib().bq_schur_apply_mode(h, _ptr(out), _ptr(inp), _ptr(tmp), _ptr(tmp2), kappa, csw, mode, prec, recon,
+                                        _stream_ptr(stream)))
 
 
 def bq_schur_apply_dots(h, out, inp, tmp, kappa, csw, prec, recon=BQ_RECON18, w=None):

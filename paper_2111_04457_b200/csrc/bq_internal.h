@@ -106,10 +106,11 @@ struct HopMulti {
 };
 bq_status bq_hop(bq_lattice* lat, void* out, const void* in, const void* z, double scale, int out_parity, int prec,
                  int recon, const void* cl, int cl_mode, cudaStream_t stream, const HopRed* red = nullptr,
-                 const HopMulti* multi = nullptr);
+                 const HopMulti* multi = nullptr, bool dag = false /* hop of D^dagger: H^dag in place of H */);
 // out_e = M^ in_e (see bq_schur_apply) with an optional fused reduction on out in the second hop
 bq_status bq_schur_red(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw, int prec, int recon,
-                       cudaStream_t stream, const HopRed* red, int nrhs = 0 /* 0: single field; >= 1: arrays of nrhs fields */);
+                       cudaStream_t stream, const HopRed* red, int nrhs = 0 /* 0: single field; >= 1: arrays of nrhs fields */,
+                       bool dag = false /* M^^dagger = A_ee - kappa^2 H^dag_eo A_oo^-1 H^dag_oe */);
 // out = C in on one parity (site-diagonal clover multiply)
 bq_status bq_clover_mul(bq_lattice* lat, void* out, const void* in, const void* cl, int prec, cudaStream_t stream);
 

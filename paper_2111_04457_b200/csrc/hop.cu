@@ -105,7 +105,7 @@ template <int MODE> __global__ void __launch_bounds__(HOP_RED_FINAL_BLOCK) k_hop
 // storage precision), so that the solver needs no separate reduction pass over it:
 //   0: none;  1: <w, out> -> alpha = rho / <w, out>;  2 (EPI 1, 3 only): <out, z>, <out, out> -> omega
 // in / out / zp / wp: the operand fields of this thread's right-hand side; LSTREAM: see hop_dir.
-template <int PREC, int RECON, int EPI, bool CPLX, int RED, bool LSTREAM = true>
+template <int PREC, int RECON, int EPI, bool CPLX, int RED, bool LSTREAM = true, bool DAG = false>
 __device__ __forceinline__ void hop_site(const HopArgs<typename Prec<PREC>::comp>& a, const int h, const void* in, void* out,
                                          const void* zp, const void* wp, typename Prec<PREC>::comp* red) {
     using C = typename Prec<PREC>::comp;
@@ -130,39 +130,47 @@ __device__ __forceinline__ void hop_site(const HopArgs<typename Prec<PREC>::comp
     {
         const bool wf = r && (xh == a.Lxh - 1);
         const int nf = r ? (wf ? h - (a.Lxh - 1) : h + 1) : h;
-        hop_dir<PREC, RECON, 0, true, CPLX, LSTREAM>(acc, in, Vh, nf, gf, h, wf ? a.phr[0] : one, wf ? a.phi[0] : zero);
+        hop_dir<PREC, RECON, 0, true, CPLX, LSTREAM, DAG>(acc, in, Vh, nf, gf, h, wf ? a.phr[0] : one, wf ? a.phi[0] : zero);
         const bool wb = !r && (xh == 0);
         const int nb = r ? h : (wb ? h + (a.Lxh - 1) : h - 1);
-        hop_dir<PREC, RECON, 0, false, CPLX, LSTREAM>(acc, in, Vh, nb, gb, nb, wb ? a.phr[0] : one, wb ? -a.phi[0] : zero);
+        hop_dir<PREC, RECON, 0, false, CPLX, LSTREAM, DAG>(acc, in, Vh, nb, gb, nb, wb ? a.phr[0] : one, wb ? -a.phi[0] : zero);
     }
     // ---- y ----
     {
         const bool wf = (y == a.Ly - 1);
         const int nf = wf ? h - (a.Ly - 1) * sy : h + sy;
-        hop_dir<PREC, RECON, 1, true, CPLX, LSTREAM>(acc, in, Vh, nf, gf + a.ublk, h, wf ? a.phr[1] : one, wf ? a.phi[1] : zero);
+        hop_dir<PREC, RECON, 1, true, CPLX, LSTREAM, DAG>(acc, in, Vh, nf, gf + a.ublk, h, wf ? a.phr[1] : one, wf ? a.phi[1] : zero);
         const bool wb = (y == 0);
         const int nb = wb ? h + (a.Ly - 1) * sy : h - sy;
-        hop_dir<PREC, RECON, 1, false, CPLX, LSTREAM>(acc, in, Vh, nb, gb + a.ublk, nb, wb ? a.phr[1] : one, wb ? -a.phi[1] : zero);
+        hop_dir<PREC, RECON, 1, false, CPLX, LSTREAM, DAG>(acc, in, Vh, nb, gb + a.ublk, nb, wb ? a.phr[1] : one, wb ? -a.phi[1] : zero);
     }
     // ---- z ----
     {
         const bool wf = (z == a.Lz - 1);
         const int nf = wf ? h - (a.Lz - 1) * sz : h + sz;
-        hop_dir<PREC, RECON, 2, true, CPLX, LSTREAM>(acc, in, Vh, nf, gf + 2 * a.ublk, h, wf ? a.phr[2] : one, wf ? a.phi[2] : zero);
+        hop_dir<PREC, RECON, 2, true, CPLX, LSTREAM, DAG>(acc, in, Vh, nf, gf + 2 * a.ublk, h, wf ? a.phr[2] : one, wf ? a.phi[2] : zero);
         const bool wb = (z == 0);
         const int nb = wb ? h + (a.Lz - 1) * sz : h - sz;
-        hop_dir<PREC, RECON, 2, false, CPLX, LSTREAM>(acc, in, Vh, nb, gb + 2 * a.ublk, nb, wb ? a.phr[2] : one, wb ? -a.phi[2] : zero);
+        hop_dir<PREC, RECON, 2, false, CPLX, LSTREAM, DAG>(acc, in, Vh, nb, gb + 2 * a.ublk, nb, wb ? a.phr[2] : one, wb ? -a.phi[2] : zero);
     }
     // ---- t ----
     {
         const bool wf = (t == a.Lt - 1);
         const int nf = wf ? h - (a.Lt - 1) * st : h + st;
-        hop_dir<PREC, RECON, 3, true, CPLX, LSTREAM>(acc, in, Vh, nf, gf + 3 * a.ublk, h, wf ? a.phr[3] : one, wf ? a.phi[3] : zero);
+        hop_dir<PREC, RECON, 3, true, CPLX, LSTREAM, DAG>(acc, in, Vh, nf, gf + 3 * a.ublk, h, wf ? a.phr[3] : one, wf ? a.phi[3] : zero);
         const bool wb = (t == 0);
         const int nb = wb ? h + (a.Lt - 1) * st : h - st;
-        hop_dir<PREC, RECON, 3, false, CPLX, LSTREAM>(acc, in, Vh, nb, gb + 3 * a.ublk, nb, wb ? a.phr[3] : one, wb ? -a.phi[3] : zero);
+        hop_dir<PREC, RECON, 3, false, CPLX, LSTREAM, DAG>(acc, in, Vh, nb, gb + 3 * a.ublk, nb, wb ? a.phr[3] : one, wb ? -a.phi[3] : zero);
     }
 
+    if (DAG) {   // H^dag = S H S, S = exchange of the upper and lower spin pairs (hop_dir): the outer S
+#pragma unroll
+        for (int i = 0; i < 12; i++) {
+            const C tmp = acc[i];
+            acc[i] = acc[12 + i];
+            acc[12 + i] = tmp;
+        }
+    }
     // ---- epilogue ----
     if (EPI == 2) clover_site_mul<PREC, LSTREAM>(a.cl, Vh, h, acc);   // linear: the scale already inside acc commutes with it
     if (EPI == 1 || EPI == 3) {
@@ -200,17 +208,17 @@ __device__ __forceinline__ void hop_site(const HopArgs<typename Prec<PREC>::comp
     store_spinor<PREC, true>(out, Vh, h, acc);
 }
 
-template <int PREC, int RECON, int EPI, bool CPLX, int RED>
+template <int PREC, int RECON, int EPI, bool CPLX, int RED, bool DAG = false>
 __global__ void __launch_bounds__(HOP_BLOCK, PREC == BQ_FP64 ? HOP_MINB_64 : (PREC == BQ_FP32 ? HOP_MINB_LO : HOP_MINB_HALF))
 hop_kernel(const HopArgs<typename Prec<PREC>::comp> a) {
     using C = typename Prec<PREC>::comp;
     const int h = blockIdx.x * HOP_BLOCK + threadIdx.x;
     if (RED == 0) {
         if (h >= a.Vh) return;
-        hop_site<PREC, RECON, EPI, CPLX, 0>(a, h, a.in, a.out, a.z, a.w, nullptr);
+        hop_site<PREC, RECON, EPI, CPLX, 0, true, DAG>(a, h, a.in, a.out, a.z, a.w, nullptr);
     } else {
         C red[3] = {0, 0, 0};
-        if (h < a.Vh) hop_site<PREC, RECON, EPI, CPLX, RED>(a, h, a.in, a.out, a.z, a.w, red);
+        if (h < a.Vh) hop_site<PREC, RECON, EPI, CPLX, RED, true, DAG>(a, h, a.in, a.out, a.z, a.w, red);
         const double v[3] = {(double)red[0], (double)red[1], (double)red[2]};
         hop_block_partial<RED == 1 ? 2 : 3>(v, a.partials);
     }
@@ -248,7 +256,7 @@ template <int NRED> __device__ __forceinline__ void hop_block_partial_mrhs(const
     }
 }
 
-template <int PREC, int RECON, int EPI, bool CPLX, int RED>
+template <int PREC, int RECON, int EPI, bool CPLX, int RED, bool DAG = false>
 __global__ void __launch_bounds__(HOP_BLOCK, PREC == BQ_FP64 ? HOP_MINB_64 : (PREC == BQ_FP32 ? HOP_MINB_LO : HOP_MINB_HALF))
 hop_kernel_mrhs(const HopArgs<typename Prec<PREC>::comp> a) {
     using C = typename Prec<PREC>::comp;
@@ -261,10 +269,10 @@ hop_kernel_mrhs(const HopArgs<typename Prec<PREC>::comp> a) {
     const char* zp = a.z ? static_cast<const char*>(a.z) + (size_t)rhs * a.s_z : nullptr;
     const char* wp = a.w ? static_cast<const char*>(a.w) + (size_t)rhs * a.s_w : nullptr;
     if (RED == 0) {
-        if (live) hop_site<PREC, RECON, EPI, CPLX, 0, false>(a, h, in, out, zp, wp, nullptr);
+        if (live) hop_site<PREC, RECON, EPI, CPLX, 0, false, DAG>(a, h, in, out, zp, wp, nullptr);
     } else {
         C red[3] = {0, 0, 0};
-        if (live) hop_site<PREC, RECON, EPI, CPLX, RED, false>(a, h, in, out, zp, wp, red);
+        if (live) hop_site<PREC, RECON, EPI, CPLX, RED, false, DAG>(a, h, in, out, zp, wp, red);
         const double v[3] = {(double)red[0], (double)red[1], (double)red[2]};
         hop_block_partial_mrhs<RED == 1 ? 2 : 3>(v, a.partials, a.nrhs, a.T);
     }
@@ -272,7 +280,7 @@ hop_kernel_mrhs(const HopArgs<typename Prec<PREC>::comp> a) {
 
 template <int PREC, int RECON>
 static bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const void* z, double scale, int p, const void* gauge,
-                            const void* cl, int cl_mode, const HopRed* red, cudaStream_t stream, const HopMulti* m) {
+                            const void* cl, int cl_mode, const HopRed* red, cudaStream_t stream, const HopMulti* m, bool dag) {
     using C = typename Prec<PREC>::comp;
     const Geom& g = lat->g;
     HopArgs<C> a;
@@ -315,6 +323,18 @@ static bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const vo
     else if (cl_mode == 1 && !z) epi = 2;
     else if (cl_mode == 2 && z) epi = 3;
     else return bq_set_error(lat, BQ_EINVAL, "bq_hop: unsupported epilogue (cl_mode=%d, z=%p)", cl_mode, z);
+    // the dagger hop exists without fused reductions (the CG of the normal equations reduces on the plain hop)
+    if (dag && rmode) return bq_set_error(lat, BQ_EINVAL, "bq_hop: the dagger hop has no fused reduction");
+#define BQ_HOP_LAUNCH_DAG(E)                                                                        \
+    do {                                                                                            \
+        if (multi) {                                                                                \
+            if (cplx) hop_kernel_mrhs<PREC, RECON, E, true, 0, true><<<grid, block, 0, stream>>>(a);  \
+            else hop_kernel_mrhs<PREC, RECON, E, false, 0, true><<<grid, block, 0, stream>>>(a);      \
+        } else {                                                                                    \
+            if (cplx) hop_kernel<PREC, RECON, E, true, 0, true><<<grid, HOP_BLOCK, 0, stream>>>(a);   \
+            else hop_kernel<PREC, RECON, E, false, 0, true><<<grid, HOP_BLOCK, 0, stream>>>(a);       \
+        }                                                                                           \
+    } while (0)
 #define BQ_HOP_LAUNCH(E, R)                                                                         \
     do {                                                                                            \
         if (multi) {                                                                                \
@@ -326,6 +346,14 @@ static bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const vo
         }                                                                                           \
     } while (0)
     // fused reductions exist for the xpay epilogues only (the second hop of M^, which produces v and t)
+    if (dag) {
+        switch (epi) {
+            case 0: BQ_HOP_LAUNCH_DAG(0); break;
+            case 1: BQ_HOP_LAUNCH_DAG(1); break;
+            case 2: BQ_HOP_LAUNCH_DAG(2); break;
+            default: BQ_HOP_LAUNCH_DAG(3); break;
+        }
+    } else
     switch (epi * 3 + rmode) {
         case 0: BQ_HOP_LAUNCH(0, 0); break;
         case 3: BQ_HOP_LAUNCH(1, 0); break;
@@ -338,6 +366,7 @@ static bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const vo
         default: return bq_set_error(lat, BQ_EINVAL, "bq_hop: epilogue %d has no fused reduction %d", epi, rmode);
     }
 #undef BQ_HOP_LAUNCH
+#undef BQ_HOP_LAUNCH_DAG
     BQ_CHECK_LAUNCH(lat);
     lat->n_hop[PREC] += nrhs;     // counted per right-hand side: each is 1320 flop x Vh sites
     if (rmode) {
@@ -356,7 +385,7 @@ extern "C" bq_status bq_get_counters(const bq_lattice* lat, unsigned long long* 
 }
 
 bq_status bq_hop(bq_lattice* lat, void* out, const void* in, const void* z, double scale, int p, int prec, int recon,
-                 const void* cl, int cl_mode, cudaStream_t stream, const HopRed* red, const HopMulti* m) {
+                 const void* cl, int cl_mode, cudaStream_t stream, const HopRed* red, const HopMulti* m, bool dag) {
     const void* gauge = nullptr;
     BQ_TRY(bq_get_gauge(lat, prec, recon, &gauge));
     if (m && m->nrhs < 1) return bq_set_error(lat, BQ_EINVAL, "bq_hop: nrhs must be >= 1");
@@ -370,12 +399,12 @@ bq_status bq_hop(bq_lattice* lat, void* out, const void* in, const void* z, doub
             if (red) { rc = *red; rc.sc = red->sc + r0; if (rc.w) rc.w = static_cast<const char*>(red->w) + (size_t)r0 * m->s_w; }
             BQ_TRY(bq_hop(lat, static_cast<char*>(out) + (size_t)r0 * m->s_out, static_cast<const char*>(in) + (size_t)r0 * m->s_in,
                           z ? static_cast<const char*>(z) + (size_t)r0 * m->s_z : nullptr, scale, p, prec, recon, cl, cl_mode, stream,
-                          red ? &rc : nullptr, &c));
+                          red ? &rc : nullptr, &c, dag));
         }
         return BQ_OK;
     }
 #define BQ_HOP_CASE(P, R) \
-    if (prec == P && recon == R) return launch_hop<P, R>(lat, out, in, z, scale, p, gauge, cl, cl_mode, red, stream, m);
+    if (prec == P && recon == R) return launch_hop<P, R>(lat, out, in, z, scale, p, gauge, cl, cl_mode, red, stream, m, dag);
     BQ_HOP_CASE(BQ_FP64, BQ_RECON18)
     BQ_HOP_CASE(BQ_FP64, BQ_RECON12)
     BQ_HOP_CASE(BQ_FP32, BQ_RECON18)
@@ -431,7 +460,7 @@ extern "C" bq_status bq_schur_apply(bq_lattice* lat, void* out, const void* in, 
 }
 
 bq_status bq_schur_red(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw, int prec, int recon,
-                       cudaStream_t s, const HopRed* red, int nrhs) {
+                       cudaStream_t s, const HopRed* red, int nrhs, bool dag) {
     if (!lat) return BQ_EINVAL;
     if (!out || !in || !tmp || out == in || tmp == in || tmp == out)
         return bq_set_error(lat, BQ_EINVAL, "bq_schur_apply: NULL or aliased buffers");
@@ -442,8 +471,9 @@ bq_status bq_schur_red(bq_lattice* lat, void* out, const void* in, void* tmp, do
     const HopMulti* m = nrhs >= 1 ? &mm : nullptr;
     if (csw == 0.0) {
         // tmp_o = -kappa H_oe in_e ;  out_e = in_e + kappa H_eo tmp_o = in_e - kappa^2 H_eo H_oe in_e
-        BQ_TRY(bq_hop(lat, tmp, in, nullptr, -kappa, 1, prec, recon, nullptr, 0, s, nullptr, m));
-        return bq_hop(lat, out, tmp, in, kappa, 0, prec, recon, nullptr, 0, s, red, m);
+        // (dag: H^dag in place of H — M^^dag = 1 - kappa^2 H^dag_eo H^dag_oe)
+        BQ_TRY(bq_hop(lat, tmp, in, nullptr, -kappa, 1, prec, recon, nullptr, 0, s, nullptr, m, dag));
+        return bq_hop(lat, out, tmp, in, kappa, 0, prec, recon, nullptr, 0, s, red, m, dag);
     }
     BQ_TRY(bq_clover_build(lat, csw, kappa));
     const void *cl = nullptr, *cli = nullptr;
@@ -451,8 +481,64 @@ bq_status bq_schur_red(bq_lattice* lat, void* out, const void* in, void* tmp, do
     BQ_TRY(bq_get_clover(lat, prec, 1, &cli));
     const size_t cb = (size_t)lat->g.Vh * CLOVER_REALS * prec_real_bytes(prec);
     // tmp_o = -kappa A_oo^-1 H_oe in_e ;  out_e = A_ee in_e + kappa H_eo tmp_o
-    BQ_TRY(bq_hop(lat, tmp, in, nullptr, -kappa, 1, prec, recon, static_cast<const char*>(cli) + cb, 1, s, nullptr, m));
-    return bq_hop(lat, out, tmp, in, kappa, 0, prec, recon, cl, 2, s, red, m);
+    // (A is Hermitian, so the dagger only turns H into H^dag)
+    BQ_TRY(bq_hop(lat, tmp, in, nullptr, -kappa, 1, prec, recon, static_cast<const char*>(cli) + cb, 1, s, nullptr, m, dag));
+    return bq_hop(lat, out, tmp, in, kappa, 0, prec, recon, cl, 2, s, red, m, dag);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// operator modes of the paper's interface, set_mode("D" | "Ddag" | "DdagD")
+// ---------------------------------------------------------------------------------------------------
+static bq_status dirac_one(bq_lattice* lat, void* out, const void* in, double kappa, double csw, int prec, int recon,
+                           cudaStream_t s, bool dag) {
+    const size_t fb = field_bytes_one_parity(lat->g, prec);
+    char* o = static_cast<char*>(out);
+    const char* i = static_cast<const char*>(in);
+    // out_p = A_pp in_p - kappa H_{p,1-p} in_{1-p}   (dag: H^dag; A^dag = A)
+    if (csw == 0.0) {
+        BQ_TRY(bq_hop(lat, o, i + fb, i, -kappa, 0, prec, recon, nullptr, 0, s, nullptr, nullptr, dag));
+        return bq_hop(lat, o + fb, i, i + fb, -kappa, 1, prec, recon, nullptr, 0, s, nullptr, nullptr, dag);
+    }
+    BQ_TRY(bq_clover_build(lat, csw, kappa));
+    const void* cl = nullptr;
+    BQ_TRY(bq_get_clover(lat, prec, 0, &cl));
+    const size_t cb = (size_t)lat->g.Vh * CLOVER_REALS * prec_real_bytes(prec);
+    BQ_TRY(bq_hop(lat, o, i + fb, i, -kappa, 0, prec, recon, cl, 2, s, nullptr, nullptr, dag));
+    return bq_hop(lat, o + fb, i, i + fb, -kappa, 1, prec, recon, static_cast<const char*>(cl) + cb, 2, s, nullptr, nullptr, dag);
+}
+
+extern "C" bq_status bq_dirac_apply_mode(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw,
+                                         bq_mode mode, bq_prec prec, bq_recon recon, void* stream) {
+    if (!lat) return BQ_EINVAL;
+    if (!out || !in || out == in) return bq_set_error(lat, BQ_EINVAL, "bq_dirac_apply_mode: out/in NULL or aliased");
+    if (!valid_prec(prec) || !valid_recon(recon)) return bq_set_error(lat, BQ_EINVAL, "bq_dirac_apply_mode: bad prec/recon");
+    if (!lat->have_gauge) return bq_set_error(lat, BQ_ENOGAUGE, "bq_dirac_apply_mode: no gauge field loaded");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    switch (mode) {
+        case BQ_MODE_D: return dirac_one(lat, out, in, kappa, csw, prec, recon, s, false);
+        case BQ_MODE_DDAG: return dirac_one(lat, out, in, kappa, csw, prec, recon, s, true);
+        case BQ_MODE_DDAGD:
+            if (!tmp || tmp == in || tmp == out) return bq_set_error(lat, BQ_EINVAL, "bq_dirac_apply_mode: DdagD needs a distinct tmp field");
+            BQ_TRY(dirac_one(lat, tmp, in, kappa, csw, prec, recon, s, false));
+            return dirac_one(lat, out, tmp, kappa, csw, prec, recon, s, true);
+    }
+    return bq_set_error(lat, BQ_EINVAL, "bq_dirac_apply_mode: bad mode %d", (int)mode);
+}
+
+extern "C" bq_status bq_schur_apply_mode(bq_lattice* lat, void* out, const void* in, void* tmp, void* tmp2, double kappa, double csw,
+                                         bq_mode mode, bq_prec prec, bq_recon recon, void* stream) {
+    if (!lat) return BQ_EINVAL;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    switch (mode) {
+        case BQ_MODE_D: return bq_schur_red(lat, out, in, tmp, kappa, csw, prec, recon, s, nullptr, 0, false);
+        case BQ_MODE_DDAG: return bq_schur_red(lat, out, in, tmp, kappa, csw, prec, recon, s, nullptr, 0, true);
+        case BQ_MODE_DDAGD:
+            if (!tmp2 || tmp2 == in || tmp2 == out || tmp2 == tmp)
+                return bq_set_error(lat, BQ_EINVAL, "bq_schur_apply_mode: DdagD needs a second distinct scratch field");
+            BQ_TRY(bq_schur_red(lat, tmp2, in, tmp, kappa, csw, prec, recon, s, nullptr, 0, false));
+            return bq_schur_red(lat, out, tmp2, tmp, kappa, csw, prec, recon, s, nullptr, 0, true);
+    }
+    return bq_set_error(lat, BQ_EINVAL, "bq_schur_apply_mode: bad mode %d", (int)mode);
 }
 
 // ---------------------------------------------------------------------------------------------------

@@ -80,7 +80,13 @@ template <typename C> __device__ __forceinline__ void phase_mul(C* chi, C pr, C 
 //   mantissas are never rescaled on their own.
 //   LSTREAM: links read with the streaming (evict-first) policy — right when each link is used once (one right-hand
 //   side); the multi-rhs kernel reads them with the default policy so that the other right-hand sides hit in L1/L2.
-template <int PREC, int RECON, int MU, bool FWD, bool CPLX, bool LSTREAM = true>
+//   DAG: the hop of D^dagger = g5 D g5 (PAPER.md:44 set_mode).  In this basis g5 = -[[0,1],[1,0]]
+//   exchanges the upper and lower spin pairs (the two signs cancel), so the dagger hop is the same arithmetic on the
+//   gathered spinor with its halves exchanged (here) and on the accumulator with its halves exchanged (hop_site):
+//   register renaming only, no extra instruction.  Links and boundary phases are those of D (the adjoint of the
+//   forward hop from x+mu is the backward hop seen from there, with the conjugate phase — which is what D's backward
+//   hop carries already).
+template <int PREC, int RECON, int MU, bool FWD, bool CPLX, bool LSTREAM = true, bool DAG = false>
 __device__ __forceinline__ void hop_dir(typename Prec<PREC>::comp* acc, const void* in, int Vh, int nh, const void* ublock,
                                         int uidx, typename Prec<PREC>::comp pr, typename Prec<PREC>::comp pi) {
     using C = typename Prec<PREC>::comp;
@@ -88,12 +94,14 @@ __device__ __forceinline__ void hop_dir(typename Prec<PREC>::comp* acc, const vo
     if (MU < 3) {
         C psi[24];
         load_spinor_raw<PREC>(in, Vh, nh, psi, n);
+        const C* up = DAG ? psi + 12 : psi;
+        const C* lo = DAG ? psi : psi + 12;
 #pragma unroll
-        for (int i = 0; i < 12; i++) h[i] = psi[i];           // u
-        add_isigma<MU>(h, psi + 12, C(FWD ? 1 : -1));         // h = u +- i s_k l
+        for (int i = 0; i < 12; i++) h[i] = up[i];            // u
+        add_isigma<MU>(h, lo, C(FWD ? 1 : -1));               // h = u +- i s_k l
     } else {
         // (1 - g_t) psi = (0; 2l): forward needs l only; (1 + g_t) psi = (2u; 0): backward needs u only
-        load_spinor_half_raw<PREC, FWD ? 1 : 0>(in, Vh, nh, h, n);
+        load_spinor_half_raw<PREC, (FWD != DAG) ? 1 : 0>(in, Vh, nh, h, n);
     }
     load_link<PREC, RECON, LSTREAM>(ublock, Vh, uidx, u);
     su3_mul<!FWD>(u, h, chi);
