@@ -160,6 +160,10 @@ bq_status bq_wilson_apply_multi(bq_lattice* lat, void* out, const void* in, int 
 bq_status bq_schur_apply_multi(bq_lattice* lat, void* out, const void* in, void* tmp, int nrhs, double kappa, double csw,
                                bq_prec prec, bq_recon recon, void* stream);
 
+/* Krylov method of the (inner) solver: BiCGStab on M^ (reading O4), or conjugate gradients on the normal equations
+ * M^^dag M^ (uses the Ddag mode of the operator). */
+typedef enum { BQ_BICGSTAB = 0, BQ_CGNR = 1 } bq_method;
+
 typedef struct {
     int inner_prec;    /* bq_prec: BQ_FP64 = plain fp64 BiCGStab, no outer loop; BQ_FP32 / BQ_HALF = defect correction */
     int recon;         /* bq_recon used by the inner operator (the fp64 outer operator always uses 18 reals)          */
@@ -168,6 +172,7 @@ typedef struct {
     int max_inner;     /* cap on inner iterations per outer cycle; <= 0 = default (1000 fp32/fp64, 100 half)          */
     int max_outer;     /* cap on outer cycles; <= 0 = default (50)                                                    */
     int check_every;   /* inner iterations between host polls of the device-side convergence flag; <= 0 = default (8) */
+    int method;        /* bq_method: BQ_BICGSTAB (0, default) or BQ_CGNR = CG on the normal equations M^^dag M^ e = M^^dag r   */
     void* stream;      /* reserved, must be NULL (legacy default stream)                                               */
 } bq_solve_opts;
 

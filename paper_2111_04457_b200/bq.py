@@ -22,6 +22,7 @@ BQ_FP64, BQ_FP32, BQ_HALF = 0, 1, 2
 BQ_EVEN, BQ_ODD, BQ_FULL = 0, 1, 2
 BQ_RECON18, BQ_RECON12 = 0, 1
 BQ_MODE_D, BQ_MODE_DDAG, BQ_MODE_DDAGD = 0, 1, 2
+BQ_BICGSTAB, BQ_CGNR = 0, 1
 
 EXPORTS = [
     "bq_lattice_create", "bq_lattice_destroy", "bq_status_string", "bq_last_error", "bq_gauge_load",
@@ -35,7 +36,7 @@ EXPORTS = [
 class bq_solve_opts(ctypes.Structure):
     _fields_ = [("inner_prec", ctypes.c_int), ("recon", ctypes.c_int), ("csw", ctypes.c_double),
                 ("inner_tol", ctypes.c_double), ("max_inner", ctypes.c_int), ("max_outer", ctypes.c_int),
-                ("check_every", ctypes.c_int), ("stream", ctypes.c_void_p)]
+                ("check_every", ctypes.c_int), ("method", ctypes.c_int), ("stream", ctypes.c_void_p)]
 
 
 class bq_solve_info(ctypes.Structure):

@@ -128,8 +128,136 @@ template <int PREC> BLAS_KERNEL k_init(int Vh, const void* __restrict__ r, RedBu
         sc->alpha[0] = 1; sc->alpha[1] = 0;
         sc->omega[0] = 1; sc->omega[1] = 0;
         sc->iters = 0;
+        sc->cg = 0;
         sc->done = (r_[0] <= stop2) ? 1 : (r_[0] == 0.0 ? 1 : 0);
     });
+}
+
+// ---------------------------------------------------------------------------------------------------
+// CG on the normal equations M^dag M e = M^dag r, Hestenes-Stiefel form:
+//   r_N = M^dag r ; p = r_N ; rho = |r_N|^2
+//   q = M p ; alpha = rho / |q|^2 (hop epilogue, fin_omega) ; t = M^dag q
+//   x += alpha p ; r_N -= alpha t ; rho' = |r_N|^2 ; beta = rho'/rho ; rho = rho'      (k_cg_update)
+//   p = r_N + beta p                                                                    (k_cg_p)
+// stop when |r_N|^2 <= rel2 * |r_N(0)|^2 (rel2 per right-hand side from stop2s, or `rel2`).
+// ---------------------------------------------------------------------------------------------------
+template <int PREC> BLAS_KERNEL k_cg_init(int Vh, const void* __restrict__ rn, void* __restrict__ p, RedBuf rb, SolverScalars* sc,
+                                          double rel2, const double* __restrict__ rel2s, size_t stride) {
+    using I = Item<PREC>;
+    using C = typename I::C;
+    constexpr int UNR = UNR_UPDATE(I);
+    rn = rhs_field(rn, stride); p = rhs_field(p, stride); sc += blockIdx.y; rb = rhs_redbuf(rb);
+    if (rel2s) rel2 = rel2s[blockIdx.y];
+    C acc = 0;
+    const int n = I::count(Vh);
+    BLAS_TRIPS(I, n) {
+        C v[UNR][2 * I::NC];
+        BLAS_UNROLL(I) I::load_or_zero(rn, Vh, BLAS_IDX, n, v[u]);
+        BLAS_UNROLL(I) {
+#pragma unroll
+            for (int k = 0; k < 2 * I::NC; k++) acc = mad(v[u][k], v[u][k], acc);
+            if (BLAS_IDX < n) I::store(p, Vh, BLAS_IDX, v[u]);
+        }
+    }
+    double red[1] = {(double)acc};
+    grid_reduce<1>(red, rb, [sc, rel2](const double* r_) {
+        sc->r2 = r_[0];
+        sc->stop2 = rel2 * r_[0];
+        sc->rho[0] = r_[0]; sc->rho[1] = 0;
+        sc->beta[0] = 0; sc->beta[1] = 0;
+        sc->alpha[0] = 0; sc->alpha[1] = 0;
+        sc->omega[0] = 1; sc->omega[1] = 0;
+        sc->iters = 0;
+        sc->cg = 1;
+        sc->done = (r_[0] == 0.0 || !(rel2 < 1.0)) ? 1 : 0;   // rel2 >= 1 (or inf): nothing asked of this right-hand side
+    });
+}
+
+// x += alpha p ; r_N -= alpha t ; |r_N|^2 -> beta, rho.  x: fp32 accumulator when the storage is half.
+template <int PREC> BLAS_KERNEL k_cg_update(int Vh, const void* __restrict__ p, const void* __restrict__ t, void* __restrict__ x,
+                                            void* __restrict__ rn, RedBuf rb, SolverScalars* sc, size_t stride, size_t xstride) {
+    using I = Item<PREC>;
+    using C = typename I::C;
+    p = rhs_field(p, stride); t = rhs_field(t, stride); rn = rhs_field(rn, stride); x = rhs_field(x, xstride);
+    sc += blockIdx.y; rb = rhs_redbuf(rb);
+    if (sc->done) return;
+    const C a = (C)sc->alpha[0];
+    C r2 = 0;
+    const int n = I::count(Vh);
+    if constexpr (PREC == BQ_HALF) {
+        for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
+            C xv[24], w[24], rv[24];
+            load_spinor<BQ_FP32>(x, Vh, i, xv);
+            I::load(p, Vh, i, w);
+#pragma unroll
+            for (int k = 0; k < 24; k++) xv[k] = mad(a, w[k], xv[k]);
+            store_spinor<BQ_FP32>(x, Vh, i, xv);
+            I::load(rn, Vh, i, rv);
+            I::load(t, Vh, i, w);
+#pragma unroll
+            for (int k = 0; k < 24; k++) rv[k] = mad(-a, w[k], rv[k]);
+            I::store(rn, Vh, i, rv);
+            I::requantize(rv);       // the reduction sees r_N as stored
+#pragma unroll
+            for (int k = 0; k < 24; k++) r2 = mad(rv[k], rv[k], r2);
+        }
+    } else {
+        constexpr int UNR = 1;
+        BLAS_TRIPS(I, n) {
+            C xv[UNR][2 * I::NC], pv[UNR][2 * I::NC], rv[UNR][2 * I::NC], tv[UNR][2 * I::NC];
+            BLAS_UNROLL(I) {
+                I::load_or_zero(x, Vh, BLAS_IDX, n, xv[u]);
+                I::load_or_zero(p, Vh, BLAS_IDX, n, pv[u]);
+                I::load_or_zero(rn, Vh, BLAS_IDX, n, rv[u]);
+                I::load_or_zero(t, Vh, BLAS_IDX, n, tv[u]);
+            }
+            BLAS_UNROLL(I) {
+#pragma unroll
+                for (int k = 0; k < 2 * I::NC; k++) {
+                    xv[u][k] = mad(a, pv[u][k], xv[u][k]);
+                    rv[u][k] = mad(-a, tv[u][k], rv[u][k]);
+                    r2 = mad(rv[u][k], rv[u][k], r2);
+                }
+                if (BLAS_IDX < n) {
+                    I::store(x, Vh, BLAS_IDX, xv[u]);
+                    I::store(rn, Vh, BLAS_IDX, rv[u]);
+                }
+            }
+        }
+    }
+    double red[1] = {(double)r2};
+    grid_reduce<1>(red, rb, [sc](const double* q) {
+        sc->r2 = q[0];
+        sc->iters += 1;
+        if (q[0] <= sc->stop2) sc->done = 1;
+        else if (sc->rho[0] == 0.0) sc->done = 2;
+        else { sc->beta[0] = q[0] / sc->rho[0]; sc->beta[1] = 0; }
+        sc->rho[0] = q[0];
+    });
+}
+
+// p = r_N + beta p
+template <int PREC> BLAS_KERNEL k_cg_p(int Vh, const void* __restrict__ rn, void* __restrict__ p, const SolverScalars* __restrict__ sc,
+                                       size_t stride) {
+    using I = Item<PREC>;
+    using C = typename I::C;
+    constexpr int UNR = UNR_UPDATE(I);
+    rn = rhs_field(rn, stride); p = rhs_field(p, stride); sc += blockIdx.y;
+    if (sc->done) return;
+    const C b = (C)sc->beta[0];
+    const int n = I::count(Vh);
+    BLAS_TRIPS(I, n) {
+        C rv[UNR][2 * I::NC], pv[UNR][2 * I::NC];
+        BLAS_UNROLL(I) {
+            I::load_or_zero(rn, Vh, BLAS_IDX, n, rv[u]);
+            I::load_or_zero(p, Vh, BLAS_IDX, n, pv[u]);
+        }
+        BLAS_UNROLL(I) {
+#pragma unroll
+            for (int k = 0; k < 2 * I::NC; k++) rv[u][k] = mad(b, pv[u][k], rv[u][k]);
+            if (BLAS_IDX < n) I::store(p, Vh, BLAS_IDX, rv[u]);
+        }
+    }
 }
 
 // (i) p = r + beta (p - omega v)
@@ -433,6 +561,17 @@ bq_status blas_caxpy(bq_lattice* lat, const BlasCtx& c, int prec, double ar, dou
 bq_status bicg_init(bq_lattice* lat, const BlasCtx& c, int prec, const void* r, double stop2, bool per_rhs_stop2) {
     RedBuf rb{c.partials, c.ticket, c.pstride};
     DISPATCH_PREC(prec, k_init, c.Vh, r, rb, c.sc, stop2, per_rhs_stop2 ? c.stop2s : nullptr, c.stride);
+}
+bq_status cg_init(bq_lattice* lat, const BlasCtx& c, int prec, const void* rn, void* p, double rel2, bool per_rhs_rel2) {
+    RedBuf rb{c.partials, c.ticket, c.pstride};
+    DISPATCH_PREC(prec, k_cg_init, c.Vh, rn, p, rb, c.sc, rel2, per_rhs_rel2 ? c.stop2s : nullptr, c.stride);
+}
+bq_status cg_update(bq_lattice* lat, const BlasCtx& c, int prec, const void* p, const void* t, void* x, void* rn) {
+    RedBuf rb{c.partials, c.ticket, c.pstride};
+    DISPATCH_PREC(prec, k_cg_update, c.Vh, p, t, x, rn, rb, c.sc, c.stride, c.xstride);
+}
+bq_status cg_p_update(bq_lattice* lat, const BlasCtx& c, int prec, const void* rn, void* p) {
+    DISPATCH_PREC(prec, k_cg_p, c.Vh, rn, p, c.sc, c.stride);
 }
 bq_status bicg_p_update(bq_lattice* lat, const BlasCtx& c, int prec, const void* r, void* p, const void* v) {
     DISPATCH_PREC(prec, k_p_update, c.Vh, r, p, v, c.sc, c.stride);

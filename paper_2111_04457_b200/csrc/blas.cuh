@@ -90,7 +90,8 @@ struct SolverScalars {
     double scale;      // outer loop: 1/|r| of the fp64 residual (0 if r == 0)
     double rnorm;      // outer loop: |r| of the fp64 residual
     int done;          // 0 running, 1 converged, 2 breakdown
-    int iters;         // completed BiCGStab iterations
+    int iters;         // completed iterations
+    int cg;            // 1: the state belongs to a CG on the normal equations (rho = |r_N|^2, real alpha and beta)
 };
 
 struct RedBuf {
@@ -187,6 +188,10 @@ __device__ __forceinline__ void fin_omega(SolverScalars* sc, const double* r) {
     sc->ts[0] = r[0]; sc->ts[1] = r[1]; sc->tt = r[2];
     if (r[2] == 0.0) {
         if (!sc->done) sc->done = 2;
+    } else if (sc->cg) {
+        // CG on M^dag M (out = q = M p, z = p): alpha = |r_N|^2 / <p, M^dag M p> = rho / |q|^2
+        sc->alpha[0] = sc->rho[0] / r[2];
+        sc->alpha[1] = 0;
     } else {
         sc->omega[0] = r[0] / r[2];
         sc->omega[1] = r[1] / r[2];

@@ -44,6 +44,14 @@ bq_status bicg_omega(bq_lattice* lat, const BlasCtx& c, int prec, const void* t,
 bq_status bicg_final(bq_lattice* lat, const BlasCtx& c, int prec, const void* p, const void* s, const void* t, const void* rhat,
                      void* x, void* r);
 
+// --- CG on the normal equations M^dag M e = M^dag r; scalars in c.sc (rho = |r_N|^2) ---
+// p = r_N; rho = |r_N|^2; stop2 = rel2 * rho (rel2 from c.stop2s[rhs] when per_rhs_rel2); marks the state as CG
+bq_status cg_init(bq_lattice* lat, const BlasCtx& c, int prec, const void* rn, void* p, double rel2, bool per_rhs_rel2 = false);
+// x += alpha p ; r_N -= alpha t ; rho' = |r_N|^2 ; beta = rho'/rho ; iters++ ; convergence flag   (x: as in bicg_final)
+bq_status cg_update(bq_lattice* lat, const BlasCtx& c, int prec, const void* p, const void* t, void* x, void* rn);
+// p = r_N + beta p
+bq_status cg_p_update(bq_lattice* lat, const BlasCtx& c, int prec, const void* rn, void* p);
+
 // --- outer (fp64) loop ---
 // r = b - t (fp64); sc->r2 = red[0] = |r|^2; sc->scale = 1/|r| (0 if r == 0)
 // b: fields bstride bytes apart (the full-lattice b of the true-residual check, or b^_e); t, r: c.stride64 apart

@@ -1,0 +1,5 @@
+// hop_inst_fp32_18.cu — every hop-kernel variant for fp32 storage, 18-real links (see hop_kernels.cuh).
+#include "hop_kernels.cuh"
+
+template bq_status launch_hop<BQ_FP32, BQ_RECON18>(bq_lattice*, void*, const void*, const void*, double, int, const void*, const void*, int,
+                                                 const HopRed*, cudaStream_t, const HopMulti*, bool);

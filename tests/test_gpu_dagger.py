@@ -97,3 +97,50 @@ def test_dagger_adjointness_full_size(bq):
     assert relmax(Dy.reshape(-1, 4, 3)[sites], bqo.dirac_apply_sites(U, y, kappa, sites)) < 1e-12
     lhs, rhs = np.vdot(x, Dy), np.vdot(Ddx, y)
     assert abs(lhs - rhs) / abs(lhs) < 1e-12
+
+
+# ---------------------------------------------------------------------------------------------------
+# CG on the normal equations (bq_solve_opts.method = BQ_CGNR), judged with the ORACLE's operator
+# ---------------------------------------------------------------------------------------------------
+def oracle_residual(U, x, b, kappa, A=None):
+    return np.linalg.norm(b - bqo.dirac_apply(U, x, kappa, A=A)) / np.linalg.norm(b)
+
+
+@pytest.mark.parametrize("inner", [0, 1, 2])
+@pytest.mark.parametrize("csw", [0.0, 1.0])
+def test_cgnr_solve(bq, inner, csw):
+    L, kappa = (8, 4, 8, 8), 0.1215
+    U = inputs.gauge(L, 95, 0.5)
+    b = inputs.spinor(L, 95)
+    A = bqo.clover_build(U, csw, kappa) if csw else None
+    x = np.zeros_like(b)
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        opts = bq.bq_solve_opts(inner_prec=inner, csw=csw, method=bq.BQ_CGNR)
+        info = bq.bq_solve(lat.h, b, x, kappa, 1e-10, opts)
+        xb = np.zeros_like(b)
+        info_b = bq.bq_solve(lat.h, b, xb, kappa, 1e-10, bq.bq_solve_opts(inner_prec=inner, csw=csw))
+    res = oracle_residual(U, x, b, kappa, A=A)
+    print(f"cgnr inner={inner} csw={csw}: outer {info.outer_cycles} iters {info.inner_iters} res {res:.2e} (bicgstab iters {info_b.inner_iters})")
+    assert info.status == 0 and res <= 1e-10 and abs(res - info.true_rel_residual) < 1e-11
+    assert np.linalg.norm(x - xb) / np.linalg.norm(xb) < 1e-8          # both methods reach the same solution
+    x_ref, _ = bqo.cgnr(U, b, kappa, tol=1e-12, A=A)
+    assert np.linalg.norm(x - x_ref) / np.linalg.norm(x_ref) < 1e-8
+
+
+def test_cgnr_solve_multi(bq):
+    L, kappa, nrhs = (8, 4, 8, 8), 0.1215, 5
+    U = inputs.gauge(L, 96, 0.5)
+    b = np.stack([inputs.spinor(L, 96 + 100 * k) for k in range(nrhs)])
+    b[1] = 0
+    x = np.zeros_like(b)
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        opts = bq.bq_solve_opts(inner_prec=bq.BQ_FP32, method=bq.BQ_CGNR)
+        infos = bq.bq_solve_multi(lat.h, b, x, nrhs, kappa, 1e-10, opts)
+    for k in range(nrhs):
+        assert infos[k].status == 0
+        if k == 1:
+            assert not x[k].any()
+        else:
+            assert oracle_residual(U, x[k], b[k], kappa) <= 1e-10
