@@ -173,6 +173,8 @@ typedef struct {
     int max_outer;     /* cap on outer cycles; <= 0 = default (50)                                                    */
     int check_every;   /* inner iterations between host polls of the device-side convergence flag; <= 0 = default (8) */
     int method;        /* bq_method: BQ_BICGSTAB (0, default) or BQ_CGNR = CG on the normal equations M^^dag M^ e = M^^dag r   */
+    int lexical;       /* 0 (default): even-odd preconditioned Schur system; 1: BiCGStab on the full matrix D itself
+                          (the paper's `lex` operator); bq_solve only, BQ_BICGSTAB only       */
     void* stream;      /* reserved, must be NULL (legacy default stream)                                               */
 } bq_solve_opts;
 

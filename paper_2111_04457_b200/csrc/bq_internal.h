@@ -111,6 +111,9 @@ bq_status bq_hop(bq_lattice* lat, void* out, const void* in, const void* z, doub
 bq_status bq_schur_red(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw, int prec, int recon,
                        cudaStream_t stream, const HopRed* red, int nrhs = 0 /* 0: single field; >= 1: arrays of nrhs fields */,
                        bool dag = false /* M^^dagger = A_ee - kappa^2 H^dag_eo A_oo^-1 H^dag_oe */);
+// out = D in (dag: D^dagger in) on the whole lattice, [even | odd] buffers; csw = 0: Wilson
+bq_status bq_dirac_full(bq_lattice* lat, void* out, const void* in, double kappa, double csw, int prec, int recon,
+                        cudaStream_t stream, bool dag);
 // out = C in on one parity (site-diagonal clover multiply)
 bq_status bq_clover_mul(bq_lattice* lat, void* out, const void* in, const void* cl, int prec, cudaStream_t stream);
 

@@ -126,8 +126,8 @@ bq_status bq_schur_red(bq_lattice* lat, void* out, const void* in, void* tmp, do
 // ---------------------------------------------------------------------------------------------------
 // operator modes of the paper's interface, set_mode("D" | "Ddag" | "DdagD")
 // ---------------------------------------------------------------------------------------------------
-static bq_status dirac_one(bq_lattice* lat, void* out, const void* in, double kappa, double csw, int prec, int recon,
-                           cudaStream_t s, bool dag) {
+bq_status bq_dirac_full(bq_lattice* lat, void* out, const void* in, double kappa, double csw, int prec, int recon,
+                        cudaStream_t s, bool dag) {
     const size_t fb = field_bytes_one_parity(lat->g, prec);
     char* o = static_cast<char*>(out);
     const char* i = static_cast<const char*>(in);
@@ -152,12 +152,12 @@ extern "C" bq_status bq_dirac_apply_mode(bq_lattice* lat, void* out, const void*
     if (!lat->have_gauge) return bq_set_error(lat, BQ_ENOGAUGE, "bq_dirac_apply_mode: no gauge field loaded");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     switch (mode) {
-        case BQ_MODE_D: return dirac_one(lat, out, in, kappa, csw, prec, recon, s, false);
-        case BQ_MODE_DDAG: return dirac_one(lat, out, in, kappa, csw, prec, recon, s, true);
+        case BQ_MODE_D: return bq_dirac_full(lat, out, in, kappa, csw, prec, recon, s, false);
+        case BQ_MODE_DDAG: return bq_dirac_full(lat, out, in, kappa, csw, prec, recon, s, true);
         case BQ_MODE_DDAGD:
             if (!tmp || tmp == in || tmp == out) return bq_set_error(lat, BQ_EINVAL, "bq_dirac_apply_mode: DdagD needs a distinct tmp field");
-            BQ_TRY(dirac_one(lat, tmp, in, kappa, csw, prec, recon, s, false));
-            return dirac_one(lat, out, tmp, kappa, csw, prec, recon, s, true);
+            BQ_TRY(bq_dirac_full(lat, tmp, in, kappa, csw, prec, recon, s, false));
+            return bq_dirac_full(lat, out, tmp, kappa, csw, prec, recon, s, true);
     }
     return bq_set_error(lat, BQ_EINVAL, "bq_dirac_apply_mode: bad mode %d", (int)mode);
 }

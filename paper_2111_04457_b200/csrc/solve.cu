@@ -200,6 +200,28 @@ static bq_status inner_cgnr(bq_lattice* lat, SolverWork* w, double kappa, double
     return BQ_OK;
 }
 
+static bq_status solve_lex(bq_lattice* lat, SolverWork* w, const bq_solve_opts& o, double kappa, double tol, double inner_tol,
+                           int max_inner, int max_outer, int check_every, bq_solve_info* info, bq_status* result);
+
+// x (canonical, host or device) <- the n full-lattice fp64 fields of w->x; records w->ev1 and synchronises
+static bq_status export_solution(bq_lattice* lat, SolverWork* w, double* x, int n, const char* fn) {
+    const Geom& g = lat->g;
+    cudaStream_t s = w->blas.stream;
+    const size_t nb = (size_t)g.V * 24 * sizeof(double), fb64 = field_bytes_one_parity(g, BQ_FP64);
+    double* stage = nullptr;
+    cudaError_t e = cudaMalloc(&stage, nb);
+    bq_status st = BQ_OK;
+    for (int k = 0; k < n && e == cudaSuccess && st == BQ_OK; k++) {
+        st = bq_field_export(lat, stage, static_cast<char*>(w->x) + (size_t)k * 2 * fb64, BQ_FULL, BQ_FP64, s);
+        if (st == BQ_OK) e = cudaMemcpyAsync(reinterpret_cast<char*>(x) + (size_t)k * nb, stage, nb, cudaMemcpyDefault, s);
+    }
+    if (e == cudaSuccess) e = cudaEventRecord(w->ev1, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (stage) cudaFree(stage);
+    if (e != cudaSuccess) return bq_set_error(lat, BQ_ECUDA, "%s: export failed: %s", fn, cudaGetErrorString(e));
+    return st;
+}
+
 // bq_solve (nrhs = 1, single-field kernels) and bq_solve_multi (nrhs >= 1 right-hand sides solved together with the
 // multi-rhs kernels: one gauge-field read per hop for the whole batch).  b, x: nrhs canonical fields one after the other.
 static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrhs, bool multi, double kappa, double tol,
@@ -217,10 +239,11 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
     if (!lat->have_gauge) return bq_set_error(lat, BQ_ENOGAUGE, "%s: no gauge field loaded", fn);
     bq_solve_opts o;
     if (opts) o = *opts;
-    else { o.inner_prec = BQ_FP32; o.recon = BQ_RECON18; o.csw = 0; o.inner_tol = 0; o.max_inner = 0; o.max_outer = 0; o.check_every = 0; o.method = BQ_BICGSTAB; o.stream = nullptr; }
+    else { o.inner_prec = BQ_FP32; o.recon = BQ_RECON18; o.csw = 0; o.inner_tol = 0; o.max_inner = 0; o.max_outer = 0; o.check_every = 0; o.method = BQ_BICGSTAB; o.lexical = 0; o.stream = nullptr; }
     if (o.inner_prec != BQ_FP64 && o.inner_prec != BQ_FP32 && o.inner_prec != BQ_HALF) return bq_set_error(lat, BQ_EINVAL, "%s: bad inner_prec", fn);
     if (o.method != BQ_BICGSTAB && o.method != BQ_CGNR) return bq_set_error(lat, BQ_EINVAL, "%s: bad method %d", fn, o.method);
     const bool cgnr = o.method == BQ_CGNR;
+    if (o.lexical && (multi || cgnr)) return bq_set_error(lat, BQ_EINVAL, "%s: the lexical solve is BiCGStab on one right-hand side", fn);
     if (o.recon != BQ_RECON18 && o.recon != BQ_RECON12) return bq_set_error(lat, BQ_EINVAL, "%s: bad recon", fn);
     if (o.stream) return bq_set_error(lat, BQ_EINVAL, "%s: opts->stream must be NULL", fn);
     const int prec = o.inner_prec;
@@ -273,6 +296,18 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
         cudaFree(stage);
         if (e != cudaSuccess) return bq_set_error(lat, BQ_ECUDA, "%s: import failed: %s", fn, cudaGetErrorString(e));
         BQ_TRY(st);
+    }
+    if (o.lexical) {
+        // unpreconditioned solve on the full matrix (solve_lex); one right-hand side
+        bq_status result = BQ_OK;
+        bq_status st = solve_lex(lat, w, o, kappa, tol, inner_tol, max_inner, max_outer, check_every, info, &result);
+        if (st == BQ_OK) st = export_solution(lat, w, x, 1, fn);
+        w->blas.nrhs = 1;
+        if (st != BQ_OK) return st;
+        float ms = 0;
+        cudaEventElapsedTime(&ms, w->ev0, w->ev1);
+        if (info) { info->status = result; info->seconds = ms * 1e-3; }
+        return result;
     }
     // |b_k|^2 over the full lattice (two parities)
     double* bnorm = static_cast<double*>(calloc(5 * (size_t)n, sizeof(double)));
@@ -406,21 +441,7 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
         for (int k = 0; k < n; k++) true_rel[k] = bnorm[k] > 0.0 ? sqrt(true_rel[k]) / bnorm[k] : 0.0;
     }
     // ---- export x ----
-    {
-        const size_t nb = (size_t)g.V * 24 * sizeof(double);
-        double* stage = nullptr;
-        cudaError_t e = cudaMalloc(&stage, nb);
-        bq_status st = BQ_OK;
-        for (int k = 0; k < n && e == cudaSuccess && st == BQ_OK; k++) {
-            st = bq_field_export(lat, stage, xx + (size_t)k * 2 * fb64, BQ_FULL, BQ_FP64, s);
-            if (st == BQ_OK) e = cudaMemcpyAsync(reinterpret_cast<char*>(x) + (size_t)k * nb, stage, nb, cudaMemcpyDefault, s);
-        }
-        if (e == cudaSuccess) e = cudaEventRecord(w->ev1, s);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-        if (stage) cudaFree(stage);
-        if (e != cudaSuccess) { free(bnorm); free(ik); return bq_set_error(lat, BQ_ECUDA, "%s: export failed: %s", fn, cudaGetErrorString(e)); }
-        SOLVE_TRY(st);
-    }
+    SOLVE_TRY(export_solution(lat, w, x, n, fn));
 #undef SOLVE_TRY
     float ms = 0;
     cudaEventElapsedTime(&ms, w->ev0, w->ev1);
@@ -437,6 +458,105 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
     free(ik);
     w->blas.nrhs = 1;
     return result;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Lexical (not even-odd preconditioned) solve: BiCGStab on the full matrix D of Eq. 1 itself (the
+// paper's example instantiates the `lex` fermion operator) with the same defect-correction outer loop.
+// Vectors are full-lattice [even | odd] fields; the BLAS-1 kernels run on them as fields of V sites; D = two hop
+// launches with the site-diagonal term in their epilogue; the inner products are separate kernels (the two launches of
+// one apply cannot share a fused reduction).  One right-hand side.  Work vectors are allocated per call.
+// ---------------------------------------------------------------------------------------------------
+static bq_status solve_lex(bq_lattice* lat, SolverWork* w, const bq_solve_opts& o, double kappa, double tol, double inner_tol,
+                           int max_inner, int max_outer, int check_every, bq_solve_info* info, bq_status* result) {
+    const Geom& g = lat->g;
+    const int prec = o.inner_prec;
+    const double csw = o.csw;
+    BlasCtx c = w->blas;                 // the same scratch and scalars, fields of V = 2 Vh sites
+    c.Vh = g.V; c.nrhs = 1; c.stride = c.xstride = c.stride64 = 0;
+    cudaStream_t s = c.stream;
+    const size_t fb64 = 2 * field_bytes_one_parity(g, BQ_FP64), fb = 2 * field_bytes_one_parity(g, prec);
+    const size_t eb = 2 * field_bytes_one_parity(g, prec == BQ_HALF ? BQ_FP32 : prec);
+    char* pool = nullptr;
+    BQ_CUDA(lat, cudaMalloc(&pool, 2 * fb64 + 6 * fb + eb));
+    void *r64 = pool, *t64 = pool + fb64;
+    char* q = pool + 2 * fb64;
+    void *ir = q, *irhat = q + fb, *ip = q + 2 * fb, *iv = q + 3 * fb, *is = q + 4 * fb, *it = q + 5 * fb, *ie = q + 6 * fb;
+    bq_status st = BQ_OK;
+    double bnorm = 0, rnorm = 0, prev = INFINITY;
+    int outer = 0, inner_total = 0, restarts = 0, stalled = 0;
+#define LEX_TRY(expr)                                   \
+    do {                                                \
+        st = (expr);                                    \
+        if (st != BQ_OK) { cudaFree(pool); return st; } \
+    } while (0)
+    LEX_TRY(blas_norm2(lat, c, BQ_FP64, w->b));
+    LEX_TRY(poll(lat, w));
+    bnorm = sqrt(w->h_sc[0].red[0]);
+    if (bnorm == 0.0) {
+        cudaMemsetAsync(w->x, 0, fb64, s);
+    } else {
+        const double target = tol * bnorm;
+        for (;;) {
+            LEX_TRY(bq_dirac_full(lat, t64, w->x, kappa, csw, BQ_FP64, BQ_RECON18, s, false));
+            LEX_TRY(outer_residual(lat, c, w->b, 0, t64, r64));
+            LEX_TRY(poll(lat, w));
+            rnorm = sqrt(w->h_sc[0].r2);
+            if (!(rnorm == rnorm)) { *result = bq_set_error(lat, BQ_EBREAKDOWN, "bq_solve: residual is NaN"); break; }
+            if (rnorm <= target) break;
+            if (outer >= max_outer) { *result = bq_set_error(lat, BQ_ENOTCONVERGED, "bq_solve: max_outer reached, |r|/|b| = %.3e", rnorm / bnorm); break; }
+            if (rnorm > 0.5 * prev) {
+                if (++stalled >= 4) { *result = bq_set_error(lat, BQ_ENOTCONVERGED, "bq_solve: stalled at |r|/|b| = %.3e", rnorm / bnorm); break; }
+            } else stalled = 0;
+            prev = rnorm;
+            outer++;
+            LEX_TRY(outer_to_low(lat, c, prec, r64, ir));
+            const double rel = (prec == BQ_FP64) ? 0.9 * target / rnorm : fmax(inner_tol, 0.5 * target / rnorm);
+            // inner BiCGStab on D e = ir, e0 = 0 (reading O4)
+            cudaMemsetAsync(ie, 0, eb, s);
+            cudaMemsetAsync(ip, 0, fb, s);
+            cudaMemsetAsync(iv, 0, fb, s);
+            cudaMemcpyAsync(irhat, ir, fb, cudaMemcpyDeviceToDevice, s);
+            LEX_TRY(bicg_init(lat, c, prec, ir, rel * rel));
+            int launched = 0;
+            for (;;) {
+                const int batch = (max_inner - launched) < check_every ? (max_inner - launched) : check_every;
+                for (int k = 0; k < batch; k++) {
+                    LEX_TRY(bicg_p_update(lat, c, prec, ir, ip, iv));
+                    LEX_TRY(bq_dirac_full(lat, iv, ip, kappa, csw, prec, o.recon, s, false));     // v = D p
+                    LEX_TRY(bicg_alpha(lat, c, prec, irhat, iv));
+                    LEX_TRY(bicg_s_update(lat, c, prec, ir, iv, is));
+                    LEX_TRY(bq_dirac_full(lat, it, is, kappa, csw, prec, o.recon, s, false));     // t = D s
+                    LEX_TRY(bicg_omega(lat, c, prec, it, is));
+                    LEX_TRY(bicg_final(lat, c, prec, ip, is, it, irhat, ie, ir));
+                }
+                launched += batch;
+                LEX_TRY(poll(lat, w));
+                if (w->h_sc[0].done || launched >= max_inner) break;
+            }
+            inner_total += w->h_sc[0].iters;
+            if (w->h_sc[0].done == 2) {
+                restarts++;
+                if (w->h_sc[0].iters == 0 && restarts > 3) { *result = bq_set_error(lat, BQ_EBREAKDOWN, "bq_solve: BiCGStab breakdown"); break; }
+            }
+            LEX_TRY(outer_accumulate(lat, c, prec == BQ_HALF ? BQ_FP32 : prec, ie, w->x, 0));
+        }
+        // true residual of the returned x
+        LEX_TRY(bq_dirac_full(lat, t64, w->x, kappa, csw, BQ_FP64, BQ_RECON18, s, false));
+        LEX_TRY(outer_residual(lat, c, w->b, 0, t64, r64));
+        LEX_TRY(poll(lat, w));
+        rnorm = sqrt(w->h_sc[0].r2);
+    }
+#undef LEX_TRY
+    cudaStreamSynchronize(s);
+    cudaFree(pool);
+    if (info) {
+        info->outer_cycles = (prec == BQ_FP64) ? 0 : outer;
+        info->inner_iters = inner_total;
+        info->restarts = (prec == BQ_FP64) ? (outer > 0 ? outer - 1 : 0) + restarts : restarts;
+        info->true_rel_residual = bnorm > 0 ? rnorm / bnorm : 0.0;
+    }
+    return BQ_OK;
 }
 
 extern "C" bq_status bq_solve(bq_lattice* lat, const double* b, double* x, double kappa, double tol, const bq_solve_opts* opts,

@@ -32,7 +32,7 @@ def test_every_declared_symbol_is_exported(bq):
 
 
 def test_struct_layouts_match_header(bq):
-    assert ctypes.sizeof(bq.bq_solve_opts) == 48
+    assert ctypes.sizeof(bq.bq_solve_opts) == 56
     assert ctypes.sizeof(bq.bq_solve_info) == 32
 
 

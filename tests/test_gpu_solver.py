@@ -168,3 +168,30 @@ def test_solve_reports_non_convergence(bq, cfg1):
         assert abs(oracle_residual(U, x, b, kappa) - info.true_rel_residual) < 1e-9
         with pytest.raises(bq.BqError):
             bq.bq_solve(lat.h, b, x, kappa, -1.0)
+
+
+@pytest.mark.parametrize("inner", [0, 1, 2])
+@pytest.mark.parametrize("csw", [0.0, 1.0])
+def test_lexical_solve(bq, inner, csw):
+    """BiCGStab on the full matrix D (no even-odd preconditioning) — the oracle's own formulation."""
+    L, kappa = (8, 4, 8, 8), 0.1215
+    U = inputs.gauge(L, 63, 0.5)
+    b = inputs.spinor(L, 63)
+    A = bqo.clover_build(U, csw, kappa) if csw else None
+    x, xe = np.zeros_like(b), np.zeros_like(b)
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        info = bq.bq_solve(lat.h, b, x, kappa, 1e-10, bq.bq_solve_opts(inner_prec=inner, csw=csw, lexical=1))
+        info_eo = bq.bq_solve(lat.h, b, xe, kappa, 1e-10, bq.bq_solve_opts(inner_prec=inner, csw=csw))
+        with pytest.raises(bq.BqError):
+            bq.bq_solve(lat.h, b, x.copy(), kappa, 1e-10, bq.bq_solve_opts(lexical=1, method=bq.BQ_CGNR))
+        xz = inputs.spinor(L, 5)
+        infoz = bq.bq_solve(lat.h, np.zeros_like(b), xz, kappa, 1e-10, bq.bq_solve_opts(lexical=1))
+        assert infoz.status == 0 and np.all(xz == 0)
+    res = oracle_residual(U, x, b, kappa, A=A)
+    _, oinfo = bqo.bicgstab(U, b, kappa, tol=1e-10, A=A)
+    print(f"lexical inner={inner} csw={csw}: outer {info.outer_cycles} iters {info.inner_iters} (even-odd {info_eo.inner_iters}, "
+          f"oracle on full D {oinfo['iters']}) res {res:.2e}")
+    assert info.status == 0 and res <= 1e-10 and abs(res - info.true_rel_residual) < 1e-11
+    assert np.linalg.norm(x - xe) / np.linalg.norm(xe) < 1e-8
+    assert info.inner_iters > info_eo.inner_iters          # preconditioning helps (SURVEY P9: cond M^ < cond D)
