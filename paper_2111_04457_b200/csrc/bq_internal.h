@@ -47,6 +47,7 @@ struct bq_lattice {
     int* d_flag;             // device int scratch (singular-clover flag etc.)
     double* hop_partials;    // per-CTA partial sums of the hop kernel's fused reduction epilogues (lazily allocated)
     size_t hop_partials_cap; // doubles allocated there
+    int mrhs_patch;          // multi-rhs hop: 1 = patch mapping where the geometry allows (default), 0 = plain (env BQ_MRHS_PATCH)
     unsigned long long n_launch;      // kernels launched through this handle
     unsigned long long n_hop[3];      // hop-kernel launches per storage precision
     char err[512];

@@ -71,6 +71,10 @@ extern "C" bq_status bq_lattice_create(int Lx, int Ly, int Lz, int Lt, const dou
         free(lat);
         return BQ_ECUDA;
     }
+    {
+        const char* e = getenv("BQ_MRHS_PATCH");      // A/B switch of the multi-rhs hop's thread mapping (hop_kernels.cuh)
+        lat->mrhs_patch = e ? atoi(e) : 1;
+    }
     lat->err[0] = 0;
     *out = lat;
     return BQ_OK;

@@ -167,3 +167,52 @@ def test_solve_multi_device_buffers_and_errors(bq):
         xd.zero_()
         infos = bq.bq_solve_multi(lat.h, bd, xd, nrhs, kappa, 1e-12, opts, raise_on_fail=False)
         assert all(i.status == bq.BQ_ENOTCONVERGED for i in infos)
+
+
+# ---------------------------------------------------------------------------------------------------
+# patch mapping of the multi-rhs hop (4 rhs x 2 x 2 tiles per CTA; taken when the x-rows hold whole tiles, Lx % 16 == 0)
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("L", [(16, 4, 4, 4), (32, 6, 8, 2), (16, 2, 6, 4)])
+@pytest.mark.parametrize("prec", [0, 1, 2])
+@pytest.mark.parametrize("nrhs", [3, 5, 12, 16, 19])
+def test_hop_patch_parity(bq, L, prec, nrhs):
+    import torch
+    kappa = 0.125
+    U = inputs.gauge(L, 71, 0.5)
+    psis = rhs_set(L, nrhs, 72)
+    recon = nrhs % 2
+    for bc in (None, GENERAL_BC):
+        with bq.Lattice(L, bc) as lat:
+            bq.bq_gauge_load(lat.h, U)
+            for p in (0, 1):
+                src = import_multi(bq, lat, psis, prec, 1 - p)
+                fb = bq.bq_field_bytes(lat.h, prec, p)
+                out = torch.zeros(nrhs * fb, dtype=torch.uint8, device="cuda")
+                bq.bq_wilson_apply_multi(lat.h, out, src, nrhs, kappa, p, prec, recon)
+                got = export_multi(bq, lat, out, nrhs, prec, p)
+                one = lat.field(prec, p)
+                for k in range(nrhs):
+                    ref = bqo.hop_restricted(U, psis[k], kappa, p, bc=bc)
+                    assert relmax(got[k], ref) < TOL[prec], (L, prec, nrhs, k, p)
+                    bq.bq_wilson_apply(lat.h, one, src[k * fb:(k + 1) * fb], kappa, p, prec, recon)
+                    assert torch.equal(one, out[k * fb:(k + 1) * fb]), (L, prec, nrhs, k, p)
+
+
+@pytest.mark.parametrize("inner,csw,method", [(1, 0.0, 0), (1, 1.0, 0), (2, 0.0, 0), (0, 1.0, 0), (1, 1.0, 1)])
+def test_solve_multi_patch(bq, inner, csw, method):
+    """Batched solve through the patch-mapped kernels (fused reductions, dagger hops for CGNR)."""
+    L, kappa, nrhs = (16, 4, 4, 8), 0.1215, 6
+    U = inputs.gauge(L, 73, 0.5)
+    A = bqo.clover_build(U, csw, kappa) if csw else None
+    b = np.stack(rhs_set(L, nrhs, 74))
+    b[1] = 0
+    x = np.zeros_like(b)
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        infos = bq.bq_solve_multi(lat.h, b, x, nrhs, kappa, 1e-10, bq.bq_solve_opts(inner_prec=inner, csw=csw, method=method))
+    for k in range(nrhs):
+        assert infos[k].status == 0
+        if k == 1:
+            assert not x[k].any()
+        else:
+            assert oracle_residual(U, x[k], b[k], kappa, A=A) <= 1e-10, k
