@@ -256,10 +256,9 @@ def main():
         x_host = torch.zeros_like(b_host).pin_memory()
         lat4 = bq.Lattice(L)
         bq.bq_gauge_load(lat4.h, U4)
-        opts = bq.bq_solve_opts(inner_prec=bq.BQ_FP32, recon=bq.BQ_RECON18, csw=1.0)
+        opts = bq.bq_solve_opts(inner_prec=bq.BQ_FP32, recon=bq.BQ_RECON18, csw=1.0, x0_zero=1)   # x is output only
         times, infos, hops = [], [], []
         for it in range(1 + args.e2e_steps):      # first solve = warm-up (clover build, workspace allocation)
-            x_host.zero_()
             k0 = bq.bq_get_counters(lat4.h)
             barrier()
             t0 = time.perf_counter()
@@ -273,12 +272,28 @@ def main():
         dt = replicas.max_over_ranks(max(times))
         nbytes = b_host.numel() * 16
         e2e = {"value": world * FLOP_PER_SITE * Vh * hops[-1] / dt / 1e9, "unit": "GFlop/s",
-               "h2d_bytes_per_step": 2 * nbytes, "d2h_bytes_per_step": nbytes,
+               "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
                "what": "bq_solve host->host, BASELINE config 4 (32^3x64 Wilson-clover csw=1 kappa=0.1215, fp32 inner / fp64 outer "
-                       "BiCGStab to 1e-10): hop flops executed / wall time incl. H2D, layout conversion, solve, D2H",
+                       "BiCGStab to 1e-10, zero initial guess declared with opts.x0_zero): hop flops executed / wall time incl. H2D of b, "
+                       "layout conversion, solve, D2H of x",
                "time_to_solution_s": dt, "device_seconds": infos[-1].seconds, "inner_iters": infos[-1].inner_iters,
                "outer_cycles": infos[-1].outer_cycles, "hop_launches": hops[-1], "true_rel_residual": infos[-1].true_rel_residual}
         lat4.close()
+
+    # ---- the rest of the path, per kernel (bq_bench_kernel hooks; device times, operands rotated out of L2) ----
+    extras = None
+    if rank == 0 and world == 1 and not args.skip_e2e and L == (32, 32, 32, 64):
+        def gbs(us, nb):
+            return {"us": us, "gbs": nb / us / 1e3, "frac_of_peak": nb / us / 1e3 / peak}
+        extras = {"note": "device time per launch and algorithmic GB/s (every operand once) of other kernels of the path, same lattice"}
+        for name, which, pr, rc, csw in (("hop_fp32_12", "hop", 1, 1, 0.0), ("hop_fp64_18", "hop", 0, 0, 0.0), ("hop_half_18", "hop", 2, 0, 0.0),
+                                         ("bicg_iter_fp32_wilson", "bicg_iter", 1, 0, 0.0), ("bicg_iter_fp32_clover", "bicg_iter", 1, 0, 1.0),
+                                         ("bicg_iter_half_wilson", "bicg_iter", 2, 0, 0.0)):
+            extras[name] = gbs(*bq.bq_bench_kernel(lat.h, which, pr, rc, csw, 0.1215, 100, 3))
+        for name, which, csw in (("hop_fp32_18_x12", "hop", 0.0), ("bicg_iter_fp32_wilson_x12", "bicg_iter", 0.0)):
+            us, nb = bq.bq_bench_kernel_multi(lat.h, which, 1, 12, 0, csw, 0.1215, 16, 2)
+            extras[name] = dict(gbs(us, nb), us_per_rhs=us / 12, nrhs=12,
+                                gflops_hop=(FLOP_PER_SITE * Vh * 12 / us / 1e3 if which == "hop" else None))
 
     cpu = None
     if rank == 0 and world == 1 and not args.skip_cpu:
@@ -296,7 +311,7 @@ def main():
                    "l2": f"inputs larger than L2, no flush: {bps * Vh / 1e6:.0f} MB per apply (links streamed once) and {NSETS} (source, result) "
                          "pairs used round-robin, so no operand of a launch is left in the 126 MB L2 by the previous ones",
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
-        "hbm_gbs": achieved, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+        "hbm_gbs": achieved, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks, "extras": extras,
     }
     print(json.dumps(line))
 

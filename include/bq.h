@@ -175,6 +175,8 @@ typedef struct {
     int method;        /* bq_method: BQ_BICGSTAB (0, default) or BQ_CGNR = CG on the normal equations M^^dag M^ e = M^^dag r   */
     int lexical;       /* 0 (default): even-odd preconditioned Schur system; 1: BiCGStab on the full matrix D itself
                           (the paper's `lex` operator); bq_solve only, BQ_BICGSTAB only       */
+    int x0_zero;       /* 1: the initial guess is zero and x is output only — its contents on entry are neither read nor
+                          transferred (saves one host-to-device copy and one layout conversion per right-hand side)           */
     void* stream;      /* reserved, must be NULL (legacy default stream)                                               */
 } bq_solve_opts;
 
@@ -189,7 +191,7 @@ typedef struct {
 
 /* invert: solve D x = b on the whole lattice, D = Eq. 1 with the clover term for opts->csw != 0.
  * b, x: canonical fp64 layout, 24*V doubles each, HOST or DEVICE pointers (detected independently).  x is in/out:
- * initial guess on entry (zero it if none), solution on return.
+ * initial guess on entry (zero it if none, or set opts->x0_zero), solution on return.
  * Method (readings O3, O4, S10): even-odd Schur system M^ x_e = b^_e solved by BiCGStab; for inner_prec != FP64 by
  * defect correction — fp64 true residual, low-precision inner BiCGStab on the normalised residual, fp64 update —
  * then x_o = A_oo^-1 (b_o + kappa H_oe x_e).  Stops when |b^_e - M^ x_e| <= tol*|b| (fp64), then reports the true

@@ -36,7 +36,7 @@ EXPORTS = [
 class bq_solve_opts(ctypes.Structure):
     _fields_ = [("inner_prec", ctypes.c_int), ("recon", ctypes.c_int), ("csw", ctypes.c_double),
                 ("inner_tol", ctypes.c_double), ("max_inner", ctypes.c_int), ("max_outer", ctypes.c_int),
-                ("check_every", ctypes.c_int), ("method", ctypes.c_int), ("lexical", ctypes.c_int), ("stream", ctypes.c_void_p)]
+                ("check_every", ctypes.c_int), ("method", ctypes.c_int), ("lexical", ctypes.c_int), ("x0_zero", ctypes.c_int), ("stream", ctypes.c_void_p)]
 
 
 class bq_solve_info(ctypes.Structure):

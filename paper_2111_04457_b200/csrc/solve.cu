@@ -239,7 +239,7 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
     if (!lat->have_gauge) return bq_set_error(lat, BQ_ENOGAUGE, "%s: no gauge field loaded", fn);
     bq_solve_opts o;
     if (opts) o = *opts;
-    else { o.inner_prec = BQ_FP32; o.recon = BQ_RECON18; o.csw = 0; o.inner_tol = 0; o.max_inner = 0; o.max_outer = 0; o.check_every = 0; o.method = BQ_BICGSTAB; o.lexical = 0; o.stream = nullptr; }
+    else { o.inner_prec = BQ_FP32; o.recon = BQ_RECON18; o.csw = 0; o.inner_tol = 0; o.max_inner = 0; o.max_outer = 0; o.check_every = 0; o.method = BQ_BICGSTAB; o.lexical = 0; o.x0_zero = 0; o.stream = nullptr; }
     if (o.inner_prec != BQ_FP64 && o.inner_prec != BQ_FP32 && o.inner_prec != BQ_HALF) return bq_set_error(lat, BQ_EINVAL, "%s: bad inner_prec", fn);
     if (o.method != BQ_BICGSTAB && o.method != BQ_CGNR) return bq_set_error(lat, BQ_EINVAL, "%s: bad method %d", fn, o.method);
     const bool cgnr = o.method == BQ_CGNR;
@@ -289,6 +289,10 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
         for (int k = 0; k < n && e == cudaSuccess && st == BQ_OK; k++) {
             e = cudaMemcpyAsync(stage, reinterpret_cast<const char*>(b) + (size_t)k * nb, nb, cudaMemcpyDefault, s);
             if (e == cudaSuccess) st = bq_field_import(lat, bb + (size_t)k * 2 * fb64, stage, BQ_FULL, BQ_FP64, s);
+            if (o.x0_zero) {          // x is output only: no transfer, no conversion of an initial guess
+                if (e == cudaSuccess && st == BQ_OK) e = cudaMemsetAsync(xx + (size_t)k * 2 * fb64, 0, 2 * fb64, s);
+                continue;
+            }
             if (e == cudaSuccess && st == BQ_OK) e = cudaMemcpyAsync(stage, reinterpret_cast<const char*>(x) + (size_t)k * nb, nb, cudaMemcpyDefault, s);
             if (e == cudaSuccess && st == BQ_OK) st = bq_field_import(lat, xx + (size_t)k * 2 * fb64, stage, BQ_FULL, BQ_FP64, s);
         }

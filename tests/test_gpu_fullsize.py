@@ -126,3 +126,31 @@ def test_config5_half_solve_48x48x48x96(bq):
     print(f"config 5: {info.inner_iters} inner iters, {info.outer_cycles} outer, {info.seconds * 1e3:.1f} ms, "
           f"oracle residual {res:.2e}")
     assert info.status == 0 and res <= 1e-10
+
+
+def test_config3_multirhs_x12_sampled(bq):
+    """32^3 x 64 fp32 (BASELINE config 3 shape), 12 right-hand sides in one launch (the patch-mapped multi-rhs kernel, as
+    kbench times it): sampled output sites of every right-hand side against the oracle, and the first right-hand side
+    bit for bit against the single-rhs kernel."""
+    import torch
+    L, kappa, nrhs = (32, 32, 32, 64), 0.125, 12
+    seed = inputs.BASE_SEED + 3
+    U = inputs.gauge(L, seed, 0.5)
+    psis = [inputs.spinor(L, seed + 1000 * k) for k in range(nrhs)]
+    par = inputs.site_parity(L)
+    sites = sample_sites(L, 0, 256, 17)
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        fb = bq.bq_field_bytes(lat.h, bq.BQ_FP32, bq.BQ_EVEN)
+        src = torch.cat([lat.import_field(p, bq.BQ_FP32, bq.BQ_ODD) for p in psis])
+        out = torch.zeros(nrhs * fb, dtype=torch.uint8, device="cuda")
+        for recon in (bq.BQ_RECON18, bq.BQ_RECON12):
+            bq.bq_wilson_apply_multi(lat.h, out, src, nrhs, kappa, bq.BQ_EVEN, bq.BQ_FP32, recon)
+            one = lat.field(bq.BQ_FP32, bq.BQ_EVEN)
+            bq.bq_wilson_apply(lat.h, one, src[:fb], kappa, bq.BQ_EVEN, bq.BQ_FP32, recon)
+            assert torch.equal(one, out[:fb])
+            for k in range(nrhs):
+                got = lat.export_field(out[k * fb:(k + 1) * fb], bq.BQ_FP32, bq.BQ_EVEN).reshape(-1, 4, 3)[sites]
+                masked = np.where((par == 1)[..., None, None], psis[k], 0)
+                ref = bqo.dirac_apply_sites(U, masked, kappa, sites)
+                assert relmax(got, ref) < 1e-5, (recon, k)

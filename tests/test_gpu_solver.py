@@ -195,3 +195,19 @@ def test_lexical_solve(bq, inner, csw):
     assert info.status == 0 and res <= 1e-10 and abs(res - info.true_rel_residual) < 1e-11
     assert np.linalg.norm(x - xe) / np.linalg.norm(xe) < 1e-8
     assert info.inner_iters > info_eo.inner_iters          # preconditioning helps (cond M^ < cond D)
+
+
+def test_solve_x0_zero_ignores_x_on_entry(bq, cfg1):
+    """opts.x0_zero: x is output only — NaN garbage on entry must not matter, and the result equals the zero-guess solve."""
+    U, b, kappa, L = cfg1["U"], cfg1["b"], cfg1["kappa"], cfg1["L"]
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        x_ref = np.zeros_like(b)
+        bq.bq_solve(lat.h, b, x_ref, kappa, 1e-10)
+        x = np.full_like(b, np.nan)
+        info = bq.bq_solve(lat.h, b, x, kappa, 1e-10, bq.bq_solve_opts(inner_prec=bq.BQ_FP32, x0_zero=1))
+        assert info.status == 0 and np.array_equal(x, x_ref)
+        xm = np.full((2,) + b.shape, np.nan, dtype=np.complex128)
+        infos = bq.bq_solve_multi(lat.h, np.stack([b, 2 * b]), xm, 2, kappa, 1e-10, bq.bq_solve_opts(inner_prec=bq.BQ_FP32, x0_zero=1))
+        assert all(i.status == 0 for i in infos)
+        assert oracle_residual(U, xm[0], b, kappa) <= 1e-10 and oracle_residual(U, xm[1], 2 * b, kappa) <= 1e-10
