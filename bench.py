@@ -276,7 +276,8 @@ def main():
                "what": "bq_solve host->host, BASELINE config 4 (32^3x64 Wilson-clover csw=1 kappa=0.1215, fp32 inner / fp64 outer "
                        "BiCGStab to 1e-10, zero initial guess declared with opts.x0_zero): hop flops executed / wall time incl. H2D of b, "
                        "layout conversion, solve, D2H of x",
-               "time_to_solution_s": dt, "device_seconds": infos[-1].seconds, "inner_iters": infos[-1].inner_iters,
+               "time_to_solution_s": dt, "device_seconds": infos[-1].seconds,
+               "phase_seconds": dict(zip(("h2d+import", "prepare", "iterate", "reconstruct+residual", "export+d2h"), list(infos[-1].phase_seconds))), "inner_iters": infos[-1].inner_iters,
                "outer_cycles": infos[-1].outer_cycles, "hop_launches": hops[-1], "true_rel_residual": infos[-1].true_rel_residual}
         lat4.close()
 

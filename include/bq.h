@@ -187,6 +187,9 @@ typedef struct {
     int restarts;             /* BiCGStab restarts after a breakdown or a stalled inner solve                    */
     double true_rel_residual; /* |b - D x| / |b| recomputed in fp64 with the fp64 operator (= the paper's diff) */
     double seconds;           /* device time of the whole call (CUDA events), copies of b and x included       */
+    double phase_seconds[5];  /* the same, by phase: [0] transfer + layout conversion of b (and x0), [1] source
+                                 preparation b^_e (+ |b|), [2] the outer/inner iteration, [3] odd-site reconstruction +
+                                 true residual, [4] layout conversion + transfer of x                            */
 } bq_solve_info;
 
 /* invert: solve D x = b on the whole lattice, D = Eq. 1 with the clover term for opts->csw != 0.

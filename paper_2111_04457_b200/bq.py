@@ -41,7 +41,8 @@ class bq_solve_opts(ctypes.Structure):
 
 class bq_solve_info(ctypes.Structure):
     _fields_ = [("status", ctypes.c_int), ("outer_cycles", ctypes.c_int), ("inner_iters", ctypes.c_int),
-                ("restarts", ctypes.c_int), ("true_rel_residual", ctypes.c_double), ("seconds", ctypes.c_double)]
+                ("restarts", ctypes.c_int), ("true_rel_residual", ctypes.c_double), ("seconds", ctypes.c_double),
+                ("phase_seconds", ctypes.c_double * 5)]
 
 
 class BqError(RuntimeError):

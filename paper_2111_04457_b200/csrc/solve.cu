@@ -30,6 +30,8 @@ struct SolverWork {
     SolverScalars* h_sc;   // pinned host mirror, [rhs]
     double* h_stop2;       // pinned host staging of the per-rhs inner thresholds, [rhs]
     cudaEvent_t ev0, ev1;
+    cudaEvent_t evp[4];    // phase boundaries: import | prepare | iterate | finish | export (bq_solve_info.phase_seconds)
+    bool persistent_stage; double* stage;   // device staging buffer of one canonical field (import / export)
 };
 
 static void free_inner(SolverWork* w) {
@@ -61,6 +63,8 @@ void bq_solver_free(bq_lattice* lat) {
     if (w->blas_ok) blas_ctx_destroy(&w->blas);
     if (w->ev0) cudaEventDestroy(w->ev0);
     if (w->ev1) cudaEventDestroy(w->ev1);
+    for (cudaEvent_t& e : w->evp) if (e) cudaEventDestroy(e);
+    if (w->stage) cudaFree(w->stage);
     free(w);
     lat->work = nullptr;
 }
@@ -76,6 +80,8 @@ static bq_status get_work(bq_lattice* lat, int inner_prec, SolverWork** out, int
         w->blas_ok = true;
         BQ_CUDA(lat, cudaEventCreate(&w->ev0));
         BQ_CUDA(lat, cudaEventCreate(&w->ev1));
+        for (cudaEvent_t& e : w->evp) BQ_CUDA(lat, cudaEventCreate(&e));
+        BQ_CUDA(lat, cudaMalloc(&w->stage, (size_t)g.V * 24 * sizeof(double)));
     }
     SolverWork* w = lat->work;
     if (w->nrhs < nrhs) {
@@ -203,13 +209,24 @@ static bq_status inner_cgnr(bq_lattice* lat, SolverWork* w, double kappa, double
 static bq_status solve_lex(bq_lattice* lat, SolverWork* w, const bq_solve_opts& o, double kappa, double tol, double inner_tol,
                            int max_inner, int max_outer, int check_every, bq_solve_info* info, bq_status* result);
 
+// device time of the five phases of a solve from the events recorded along the way
+static void phase_times(SolverWork* w, bq_solve_info* info, int n) {
+    if (!info) return;
+    cudaEvent_t ev[6] = {w->ev0, w->evp[0], w->evp[1], w->evp[2], w->evp[3], w->ev1};
+    for (int p = 0; p < 5; p++) {
+        float ms = 0;
+        if (cudaEventElapsedTime(&ms, ev[p], ev[p + 1]) != cudaSuccess) ms = 0;
+        for (int k = 0; k < n; k++) info[k].phase_seconds[p] = ms * 1e-3;
+    }
+}
+
 // x (canonical, host or device) <- the n full-lattice fp64 fields of w->x; records w->ev1 and synchronises
 static bq_status export_solution(bq_lattice* lat, SolverWork* w, double* x, int n, const char* fn) {
     const Geom& g = lat->g;
     cudaStream_t s = w->blas.stream;
     const size_t nb = (size_t)g.V * 24 * sizeof(double), fb64 = field_bytes_one_parity(g, BQ_FP64);
-    double* stage = nullptr;
-    cudaError_t e = cudaMalloc(&stage, nb);
+    double* stage = w->stage;
+    cudaError_t e = cudaEventRecord(w->evp[3], s);
     bq_status st = BQ_OK;
     for (int k = 0; k < n && e == cudaSuccess && st == BQ_OK; k++) {
         st = bq_field_export(lat, stage, static_cast<char*>(w->x) + (size_t)k * 2 * fb64, BQ_FULL, BQ_FP64, s);
@@ -217,7 +234,6 @@ static bq_status export_solution(bq_lattice* lat, SolverWork* w, double* x, int 
     }
     if (e == cudaSuccess) e = cudaEventRecord(w->ev1, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-    if (stage) cudaFree(stage);
     if (e != cudaSuccess) return bq_set_error(lat, BQ_ECUDA, "%s: export failed: %s", fn, cudaGetErrorString(e));
     return st;
 }
@@ -232,6 +248,7 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
         for (int k = 0; k < (nrhs > 0 ? nrhs : 0); k++) {
             info[k].status = BQ_EINVAL; info[k].outer_cycles = 0; info[k].inner_iters = 0; info[k].restarts = 0;
             info[k].true_rel_residual = NAN; info[k].seconds = 0;
+            for (double& ps : info[k].phase_seconds) ps = 0;
         }
     if (nrhs < 1) return bq_set_error(lat, BQ_EINVAL, "%s: nrhs must be >= 1", fn);
     if (!b || !x) return bq_set_error(lat, BQ_EINVAL, "%s: b or x is NULL", fn);
@@ -282,8 +299,7 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
     // ---- import b and x0 (canonical, host or device) through a device staging buffer ----
     {
         const size_t nb = (size_t)g.V * 24 * sizeof(double);
-        double* stage = nullptr;
-        BQ_CUDA(lat, cudaMalloc(&stage, nb));
+        double* stage = w->stage;
         cudaError_t e = cudaSuccess;
         bq_status st = BQ_OK;
         for (int k = 0; k < n && e == cudaSuccess && st == BQ_OK; k++) {
@@ -296,21 +312,24 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
             if (e == cudaSuccess && st == BQ_OK) e = cudaMemcpyAsync(stage, reinterpret_cast<const char*>(x) + (size_t)k * nb, nb, cudaMemcpyDefault, s);
             if (e == cudaSuccess && st == BQ_OK) st = bq_field_import(lat, xx + (size_t)k * 2 * fb64, stage, BQ_FULL, BQ_FP64, s);
         }
+        if (e == cudaSuccess) e = cudaEventRecord(w->evp[0], s);
         if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-        cudaFree(stage);
         if (e != cudaSuccess) return bq_set_error(lat, BQ_ECUDA, "%s: import failed: %s", fn, cudaGetErrorString(e));
         BQ_TRY(st);
     }
     if (o.lexical) {
         // unpreconditioned solve on the full matrix (solve_lex); one right-hand side
         bq_status result = BQ_OK;
+        cudaEventRecord(w->evp[1], s);
         bq_status st = solve_lex(lat, w, o, kappa, tol, inner_tol, max_inner, max_outer, check_every, info, &result);
+        cudaEventRecord(w->evp[2], s);
         if (st == BQ_OK) st = export_solution(lat, w, x, 1, fn);
         w->blas.nrhs = 1;
         if (st != BQ_OK) return st;
         float ms = 0;
         cudaEventElapsedTime(&ms, w->ev0, w->ev1);
         if (info) { info->status = result; info->seconds = ms * 1e-3; }
+        phase_times(w, info, 1);
         return result;
     }
     // |b_k|^2 over the full lattice (two parities)
@@ -349,6 +368,8 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
             cudaError_t e = cudaMemsetAsync(xx + (size_t)k * 2 * fb64, 0, 2 * fb64, s);
             if (e != cudaSuccess) { free(bnorm); free(ik); return bq_set_error(lat, BQ_ECUDA, "%s: memset failed", fn); }
         }
+    cudaEventRecord(w->evp[1], s);
+    cudaEventRecord(w->evp[2], s);
     if (any_nonzero) {
         // ---- b^_e = b_e + kappa H_eo A_oo^-1 b_o ----
         const void* bo = bb + fb64;
@@ -364,6 +385,7 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
             const HopMulti m = hm(bo_stride, fb64, 2 * fb64);
             SOLVE_TRY(bq_hop(lat, w->bhat, bo, bb, kappa, 0, BQ_FP64, BQ_RECON18, nullptr, 0, s, nullptr, multi ? &m : none));
         }
+        cudaEventRecord(w->evp[1], s);
         for (;;) {
             // r = b^_e - M^ x_e in fp64
             {
@@ -423,6 +445,7 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
             // x_e += |r| e   (|r| = sc->rnorm, written by outer_residual; the inner loop does not touch it)
             SOLVE_TRY(outer_accumulate(lat, c, prec == BQ_HALF ? BQ_FP32 : prec, w->ie, xx, 2 * fb64));
         }
+        cudaEventRecord(w->evp[2], s);
         // ---- x_o = A_oo^-1 (b_o + kappa H_oe x_e) ----
         {
             const HopMulti m = hm(2 * fb64, 2 * fb64, 2 * fb64);
@@ -458,6 +481,7 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
             info[k].true_rel_residual = true_rel[k];
             info[k].seconds = ms * 1e-3;     // device time of the whole call (all right-hand sides together)
         }
+    phase_times(w, info, n);
     free(bnorm);
     free(ik);
     w->blas.nrhs = 1;

@@ -33,7 +33,7 @@ def test_every_declared_symbol_is_exported(bq):
 
 def test_struct_layouts_match_header(bq):
     assert ctypes.sizeof(bq.bq_solve_opts) == 56
-    assert ctypes.sizeof(bq.bq_solve_info) == 32
+    assert ctypes.sizeof(bq.bq_solve_info) == 72
 
 
 def test_status_strings(bq):
