@@ -28,16 +28,16 @@
 // ---------------------------------------------------------------------------------------------------
 // generic reductions
 // ---------------------------------------------------------------------------------------------------
-template <int PREC> BLAS_KERNEL k_norm2(int Vh, const void* __restrict__ a, RedBuf rb, SolverScalars* sc, size_t stride) {
+template <int PREC> BLAS_KERNEL k_norm2(int Vh, const void* __restrict__ a, RedBuf rb, SolverScalars* sc, int stride) {
     using I = Item<PREC>;
     using C = typename I::C;
     constexpr int UNR = UNR_REDUCE(I);
-    a = rhs_field(a, stride); sc += blockIdx.y; rb = rhs_redbuf(rb);
+    const int o = blockIdx.y * stride; sc += blockIdx.y; rb = rhs_redbuf(rb);
     C acc = 0;
     const int n = I::count(Vh);
     BLAS_TRIPS(I, n) {
         C v[UNR][2 * I::NC];
-        BLAS_UNROLL(I) I::load_or_zero(a, Vh, BLAS_IDX, n, v[u]);
+        BLAS_UNROLL(I) I::load_or_zero(a, Vh, BLAS_IDX, n, v[u], o);
         BLAS_UNROLL(I)
 #pragma unroll
         for (int k = 0; k < 2 * I::NC; k++) acc = mad(v[u][k], v[u][k], acc);
@@ -47,18 +47,18 @@ template <int PREC> BLAS_KERNEL k_norm2(int Vh, const void* __restrict__ a, RedB
 }
 
 template <int PREC> BLAS_KERNEL k_cdot(int Vh, const void* __restrict__ a, const void* __restrict__ b, RedBuf rb, SolverScalars* sc, int mode,
-                                       size_t stride) {
+                                       int stride) {
     using I = Item<PREC>;
     using C = typename I::C;
     constexpr int UNR = UNR_REDUCE(I);
-    a = rhs_field(a, stride); b = rhs_field(b, stride); sc += blockIdx.y; rb = rhs_redbuf(rb);
+    const int o = blockIdx.y * stride; sc += blockIdx.y; rb = rhs_redbuf(rb);
     C re = 0, im = 0;
     const int n = I::count(Vh);
     BLAS_TRIPS(I, n) {
         C x[UNR][2 * I::NC], y[UNR][2 * I::NC];
         BLAS_UNROLL(I) {
-            I::load_or_zero(a, Vh, BLAS_IDX, n, x[u]);
-            I::load_or_zero(b, Vh, BLAS_IDX, n, y[u]);
+            I::load_or_zero(a, Vh, BLAS_IDX, n, x[u], o);
+            I::load_or_zero(b, Vh, BLAS_IDX, n, y[u], o);
         }
         BLAS_UNROLL(I)
 #pragma unroll
@@ -104,17 +104,17 @@ template <int PREC> BLAS_KERNEL k_caxpy(int Vh, double ar_, double ai_, const vo
 // r2 = |r|^2; with rhat = r: rho = r2, beta = (rho/1)(1/1) = rho (p = v = 0 makes beta irrelevant), alpha = omega = 1
 // stop2s != nullptr: one stopping threshold per right-hand side (device array), else `stop2` for all
 template <int PREC> BLAS_KERNEL k_init(int Vh, const void* __restrict__ r, RedBuf rb, SolverScalars* sc, double stop2,
-                                       const double* __restrict__ stop2s, size_t stride) {
+                                       const double* __restrict__ stop2s, int stride) {
     using I = Item<PREC>;
     using C = typename I::C;
     constexpr int UNR = UNR_REDUCE(I);
-    r = rhs_field(r, stride); sc += blockIdx.y; rb = rhs_redbuf(rb);
+    const int o = blockIdx.y * stride; sc += blockIdx.y; rb = rhs_redbuf(rb);
     if (stop2s) stop2 = stop2s[blockIdx.y];
     C acc = 0;
     const int n = I::count(Vh);
     BLAS_TRIPS(I, n) {
         C v[UNR][2 * I::NC];
-        BLAS_UNROLL(I) I::load_or_zero(r, Vh, BLAS_IDX, n, v[u]);
+        BLAS_UNROLL(I) I::load_or_zero(r, Vh, BLAS_IDX, n, v[u], o);
         BLAS_UNROLL(I)
 #pragma unroll
         for (int k = 0; k < 2 * I::NC; k++) acc = mad(v[u][k], v[u][k], acc);
@@ -142,21 +142,21 @@ template <int PREC> BLAS_KERNEL k_init(int Vh, const void* __restrict__ r, RedBu
 // stop when |r_N|^2 <= rel2 * |r_N(0)|^2 (rel2 per right-hand side from stop2s, or `rel2`).
 // ---------------------------------------------------------------------------------------------------
 template <int PREC> BLAS_KERNEL k_cg_init(int Vh, const void* __restrict__ rn, void* __restrict__ p, RedBuf rb, SolverScalars* sc,
-                                          double rel2, const double* __restrict__ rel2s, size_t stride) {
+                                          double rel2, const double* __restrict__ rel2s, int stride) {
     using I = Item<PREC>;
     using C = typename I::C;
     constexpr int UNR = UNR_UPDATE(I);
-    rn = rhs_field(rn, stride); p = rhs_field(p, stride); sc += blockIdx.y; rb = rhs_redbuf(rb);
+    const int o = blockIdx.y * stride; sc += blockIdx.y; rb = rhs_redbuf(rb);
     if (rel2s) rel2 = rel2s[blockIdx.y];
     C acc = 0;
     const int n = I::count(Vh);
     BLAS_TRIPS(I, n) {
         C v[UNR][2 * I::NC];
-        BLAS_UNROLL(I) I::load_or_zero(rn, Vh, BLAS_IDX, n, v[u]);
+        BLAS_UNROLL(I) I::load_or_zero(rn, Vh, BLAS_IDX, n, v[u], o);
         BLAS_UNROLL(I) {
 #pragma unroll
             for (int k = 0; k < 2 * I::NC; k++) acc = mad(v[u][k], v[u][k], acc);
-            if (BLAS_IDX < n) I::store(p, Vh, BLAS_IDX, v[u]);
+            if (BLAS_IDX < n) I::store(p, Vh, BLAS_IDX + o, v[u]);
         }
     }
     double red[1] = {(double)acc};
@@ -175,10 +175,10 @@ template <int PREC> BLAS_KERNEL k_cg_init(int Vh, const void* __restrict__ rn, v
 
 // x += alpha p ; r_N -= alpha t ; |r_N|^2 -> beta, rho.  x: fp32 accumulator when the storage is half.
 template <int PREC> BLAS_KERNEL k_cg_update(int Vh, const void* __restrict__ p, const void* __restrict__ t, void* __restrict__ x,
-                                            void* __restrict__ rn, RedBuf rb, SolverScalars* sc, size_t stride, size_t xstride) {
+                                            void* __restrict__ rn, RedBuf rb, SolverScalars* sc, int stride, int xstride) {
     using I = Item<PREC>;
     using C = typename I::C;
-    p = rhs_field(p, stride); t = rhs_field(t, stride); rn = rhs_field(rn, stride); x = rhs_field(x, xstride);
+    const int o = blockIdx.y * stride, xo = blockIdx.y * xstride;
     sc += blockIdx.y; rb = rhs_redbuf(rb);
     if (sc->done) return;
     const C a = (C)sc->alpha[0];
@@ -187,16 +187,16 @@ template <int PREC> BLAS_KERNEL k_cg_update(int Vh, const void* __restrict__ p, 
     if constexpr (PREC == BQ_HALF) {
         for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
             C xv[24], w[24], rv[24];
-            load_spinor<BQ_FP32>(x, Vh, i, xv);
-            I::load(p, Vh, i, w);
+            load_spinor<BQ_FP32>(x, Vh, i + xo, xv);
+            I::load(p, Vh, i + o, w);
 #pragma unroll
             for (int k = 0; k < 24; k++) xv[k] = mad(a, w[k], xv[k]);
-            store_spinor<BQ_FP32>(x, Vh, i, xv);
-            I::load(rn, Vh, i, rv);
-            I::load(t, Vh, i, w);
+            store_spinor<BQ_FP32>(x, Vh, i + xo, xv);
+            I::load(rn, Vh, i + o, rv);
+            I::load(t, Vh, i + o, w);
 #pragma unroll
             for (int k = 0; k < 24; k++) rv[k] = mad(-a, w[k], rv[k]);
-            I::store(rn, Vh, i, rv);
+            I::store(rn, Vh, i + o, rv);
             I::requantize(rv);       // the reduction sees r_N as stored
 #pragma unroll
             for (int k = 0; k < 24; k++) r2 = mad(rv[k], rv[k], r2);
@@ -206,10 +206,10 @@ template <int PREC> BLAS_KERNEL k_cg_update(int Vh, const void* __restrict__ p, 
         BLAS_TRIPS(I, n) {
             C xv[UNR][2 * I::NC], pv[UNR][2 * I::NC], rv[UNR][2 * I::NC], tv[UNR][2 * I::NC];
             BLAS_UNROLL(I) {
-                I::load_or_zero(x, Vh, BLAS_IDX, n, xv[u]);
-                I::load_or_zero(p, Vh, BLAS_IDX, n, pv[u]);
-                I::load_or_zero(rn, Vh, BLAS_IDX, n, rv[u]);
-                I::load_or_zero(t, Vh, BLAS_IDX, n, tv[u]);
+                I::load_or_zero(x, Vh, BLAS_IDX, n, xv[u], xo);
+                I::load_or_zero(p, Vh, BLAS_IDX, n, pv[u], o);
+                I::load_or_zero(rn, Vh, BLAS_IDX, n, rv[u], o);
+                I::load_or_zero(t, Vh, BLAS_IDX, n, tv[u], o);
             }
             BLAS_UNROLL(I) {
 #pragma unroll
@@ -219,8 +219,8 @@ template <int PREC> BLAS_KERNEL k_cg_update(int Vh, const void* __restrict__ p, 
                     r2 = mad(rv[u][k], rv[u][k], r2);
                 }
                 if (BLAS_IDX < n) {
-                    I::store(x, Vh, BLAS_IDX, xv[u]);
-                    I::store(rn, Vh, BLAS_IDX, rv[u]);
+                    I::store(x, Vh, BLAS_IDX + xo, xv[u]);
+                    I::store(rn, Vh, BLAS_IDX + o, rv[u]);
                 }
             }
         }
@@ -238,44 +238,44 @@ template <int PREC> BLAS_KERNEL k_cg_update(int Vh, const void* __restrict__ p, 
 
 // p = r_N + beta p
 template <int PREC> BLAS_KERNEL k_cg_p(int Vh, const void* __restrict__ rn, void* __restrict__ p, const SolverScalars* __restrict__ sc,
-                                       size_t stride) {
+                                       int stride) {
     using I = Item<PREC>;
     using C = typename I::C;
     constexpr int UNR = UNR_UPDATE(I);
-    rn = rhs_field(rn, stride); p = rhs_field(p, stride); sc += blockIdx.y;
+    const int o = blockIdx.y * stride; sc += blockIdx.y;
     if (sc->done) return;
     const C b = (C)sc->beta[0];
     const int n = I::count(Vh);
     BLAS_TRIPS(I, n) {
         C rv[UNR][2 * I::NC], pv[UNR][2 * I::NC];
         BLAS_UNROLL(I) {
-            I::load_or_zero(rn, Vh, BLAS_IDX, n, rv[u]);
-            I::load_or_zero(p, Vh, BLAS_IDX, n, pv[u]);
+            I::load_or_zero(rn, Vh, BLAS_IDX, n, rv[u], o);
+            I::load_or_zero(p, Vh, BLAS_IDX, n, pv[u], o);
         }
         BLAS_UNROLL(I) {
 #pragma unroll
             for (int k = 0; k < 2 * I::NC; k++) rv[u][k] = mad(b, pv[u][k], rv[u][k]);
-            if (BLAS_IDX < n) I::store(p, Vh, BLAS_IDX, rv[u]);
+            if (BLAS_IDX < n) I::store(p, Vh, BLAS_IDX + o, rv[u]);
         }
     }
 }
 
 // (i) p = r + beta (p - omega v)
 template <int PREC> BLAS_KERNEL k_p_update(int Vh, const void* __restrict__ r, void* __restrict__ p, const void* __restrict__ v,
-                                           const SolverScalars* __restrict__ sc, size_t stride) {
+                                           const SolverScalars* __restrict__ sc, int stride) {
     using I = Item<PREC>;
     using C = typename I::C;
     constexpr int UNR = UNR_UPDATE(I);
-    r = rhs_field(r, stride); p = rhs_field(p, stride); v = rhs_field(v, stride); sc += blockIdx.y;
+    const int o = blockIdx.y * stride; sc += blockIdx.y;
     if (sc->done) return;
     const C br = (C)sc->beta[0], bi = (C)sc->beta[1], wr = (C)sc->omega[0], wi = (C)sc->omega[1];
     const int n = I::count(Vh);
     BLAS_TRIPS(I, n) {
         C rv[UNR][2 * I::NC], pv[UNR][2 * I::NC], vv[UNR][2 * I::NC];
         BLAS_UNROLL(I) {
-            I::load_or_zero(r, Vh, BLAS_IDX, n, rv[u]);
-            I::load_or_zero(p, Vh, BLAS_IDX, n, pv[u]);
-            I::load_or_zero(v, Vh, BLAS_IDX, n, vv[u]);
+            I::load_or_zero(r, Vh, BLAS_IDX, n, rv[u], o);
+            I::load_or_zero(p, Vh, BLAS_IDX, n, pv[u], o);
+            I::load_or_zero(v, Vh, BLAS_IDX, n, vv[u], o);
         }
         BLAS_UNROLL(I) {
 #pragma unroll
@@ -283,49 +283,49 @@ template <int PREC> BLAS_KERNEL k_p_update(int Vh, const void* __restrict__ r, v
                 cfma(pv[u] + 2 * k, -wr, -wi, vv[u] + 2 * k);    // p - omega v
                 cfma(rv[u] + 2 * k, br, bi, pv[u] + 2 * k);      // r + beta (.)
             }
-            if (BLAS_IDX < n) I::store(p, Vh, BLAS_IDX, rv[u]);
+            if (BLAS_IDX < n) I::store(p, Vh, BLAS_IDX + o, rv[u]);
         }
     }
 }
 
 // (ii) s = r - alpha v
 template <int PREC> BLAS_KERNEL k_s_update(int Vh, const void* __restrict__ r, const void* __restrict__ v, void* __restrict__ s,
-                                           const SolverScalars* __restrict__ sc, size_t stride) {
+                                           const SolverScalars* __restrict__ sc, int stride) {
     using I = Item<PREC>;
     using C = typename I::C;
     constexpr int UNR = UNR_UPDATE(I);
-    r = rhs_field(r, stride); v = rhs_field(v, stride); s = rhs_field(s, stride); sc += blockIdx.y;
+    const int o = blockIdx.y * stride; sc += blockIdx.y;
     if (sc->done) return;
     const C ar = (C)sc->alpha[0], ai = (C)sc->alpha[1];
     const int n = I::count(Vh);
     BLAS_TRIPS(I, n) {
         C rv[UNR][2 * I::NC], vv[UNR][2 * I::NC];
         BLAS_UNROLL(I) {
-            I::load_or_zero(r, Vh, BLAS_IDX, n, rv[u]);
-            I::load_or_zero(v, Vh, BLAS_IDX, n, vv[u]);
+            I::load_or_zero(r, Vh, BLAS_IDX, n, rv[u], o);
+            I::load_or_zero(v, Vh, BLAS_IDX, n, vv[u], o);
         }
         BLAS_UNROLL(I) {
 #pragma unroll
             for (int k = 0; k < I::NC; k++) cfma(rv[u] + 2 * k, -ar, -ai, vv[u] + 2 * k);
-            if (BLAS_IDX < n) I::store(s, Vh, BLAS_IDX, rv[u]);
+            if (BLAS_IDX < n) I::store(s, Vh, BLAS_IDX + o, rv[u]);
         }
     }
 }
 
 // (iii) <t,s>, <t,t> in one pass; omega = <t,s>/<t,t>
 template <int PREC> BLAS_KERNEL k_omega(int Vh, const void* __restrict__ t, const void* __restrict__ s, RedBuf rb, SolverScalars* sc,
-                                        size_t stride) {
+                                        int stride) {
     using I = Item<PREC>;
     using C = typename I::C;
     constexpr int UNR = UNR_REDUCE(I);
-    t = rhs_field(t, stride); s = rhs_field(s, stride); sc += blockIdx.y; rb = rhs_redbuf(rb);
+    const int o = blockIdx.y * stride; sc += blockIdx.y; rb = rhs_redbuf(rb);
     C re = 0, im = 0, tt = 0;
     const int n = I::count(Vh);
     BLAS_TRIPS(I, n) {
         C x[UNR][2 * I::NC], y[UNR][2 * I::NC];
         BLAS_UNROLL(I) {
-            I::load_or_zero(t, Vh, BLAS_IDX, n, x[u]);
-            I::load_or_zero(s, Vh, BLAS_IDX, n, y[u]);
+            I::load_or_zero(t, Vh, BLAS_IDX, n, x[u], o);
+            I::load_or_zero(s, Vh, BLAS_IDX, n, y[u], o);
         }
         BLAS_UNROLL(I)
 #pragma unroll
@@ -343,11 +343,11 @@ template <int PREC> BLAS_KERNEL k_omega(int Vh, const void* __restrict__ t, cons
 // The finaliser prepares the next iteration: rho' = <rhat,r>, beta = (rho'/rho)(alpha/omega), rho = rho'.
 template <int PREC> BLAS_KERNEL k_final(int Vh, const void* __restrict__ p, const void* __restrict__ s, const void* __restrict__ t,
                                         const void* __restrict__ rhat, void* __restrict__ x, void* __restrict__ r, RedBuf rb,
-                                        SolverScalars* sc, size_t stride, size_t xstride) {
+                                        SolverScalars* sc, int stride, int xstride) {
     using I = Item<PREC>;
     using C = typename I::C;
-    p = rhs_field(p, stride); s = rhs_field(s, stride); t = rhs_field(t, stride); rhat = rhs_field(rhat, stride);
-    r = rhs_field(r, stride); x = rhs_field(x, xstride); sc += blockIdx.y; rb = rhs_redbuf(rb);
+    const int o = blockIdx.y * stride, xo = blockIdx.y * xstride;
+    sc += blockIdx.y; rb = rhs_redbuf(rb);
     if (sc->done) return;   // converged or broken down in an earlier iteration of this batch: x stays frozen
     const C ar = (C)sc->alpha[0], ai = (C)sc->alpha[1], wr = (C)sc->omega[0], wi = (C)sc->omega[1];
     C r2 = 0, re = 0, im = 0;
@@ -355,20 +355,20 @@ template <int PREC> BLAS_KERNEL k_final(int Vh, const void* __restrict__ p, cons
     if constexpr (PREC == BQ_HALF) {
         for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
             C xv[24], sv[24], w[24];
-            load_spinor<BQ_FP32>(x, Vh, i, xv);   // fp32 solution accumulator
-            I::load(p, Vh, i, w);
+            load_spinor<BQ_FP32>(x, Vh, i + xo, xv);   // fp32 solution accumulator
+            I::load(p, Vh, i + o, w);
 #pragma unroll
             for (int k = 0; k < 12; k++) cfma(xv + 2 * k, ar, ai, w + 2 * k);
-            I::load(s, Vh, i, sv);
+            I::load(s, Vh, i + o, sv);
 #pragma unroll
             for (int k = 0; k < 12; k++) cfma(xv + 2 * k, wr, wi, sv + 2 * k);
-            store_spinor<BQ_FP32>(x, Vh, i, xv);
-            I::load(t, Vh, i, w);
+            store_spinor<BQ_FP32>(x, Vh, i + xo, xv);
+            I::load(t, Vh, i + o, w);
 #pragma unroll
             for (int k = 0; k < 12; k++) cfma(sv + 2 * k, -wr, -wi, w + 2 * k);   // r = s - omega t
-            I::store(r, Vh, i, sv);
+            I::store(r, Vh, i + o, sv);
             I::requantize(sv);       // reductions see r as stored (rounded to half storage)
-            I::load(rhat, Vh, i, w);
+            I::load(rhat, Vh, i + o, w);
 #pragma unroll
             for (int k = 0; k < 12; k++) {
                 r2 = mad(sv[2 * k + 1], sv[2 * k + 1], mad(sv[2 * k], sv[2 * k], r2));
@@ -382,11 +382,11 @@ template <int PREC> BLAS_KERNEL k_final(int Vh, const void* __restrict__ p, cons
             C xv[U2][2 * I::NC], pv[U2][2 * I::NC], sv[U2][2 * I::NC], tv[U2][2 * I::NC], hv[U2][2 * I::NC];
 #pragma unroll
             for (int u = 0; u < U2; u++) {
-                I::load_or_zero(x, Vh, BLAS_IDX, n, xv[u]);
-                I::load_or_zero(p, Vh, BLAS_IDX, n, pv[u]);
-                I::load_or_zero(s, Vh, BLAS_IDX, n, sv[u]);
-                I::load_or_zero(t, Vh, BLAS_IDX, n, tv[u]);
-                I::load_or_zero(rhat, Vh, BLAS_IDX, n, hv[u]);
+                I::load_or_zero(x, Vh, BLAS_IDX, n, xv[u], xo);
+                I::load_or_zero(p, Vh, BLAS_IDX, n, pv[u], o);
+                I::load_or_zero(s, Vh, BLAS_IDX, n, sv[u], o);
+                I::load_or_zero(t, Vh, BLAS_IDX, n, tv[u], o);
+                I::load_or_zero(rhat, Vh, BLAS_IDX, n, hv[u], o);
             }
 #pragma unroll
             for (int u = 0; u < U2; u++) {
@@ -400,8 +400,8 @@ template <int PREC> BLAS_KERNEL k_final(int Vh, const void* __restrict__ p, cons
                     im = mad(-hv[u][2 * k + 1], sv[u][2 * k], mad(hv[u][2 * k], sv[u][2 * k + 1], im));
                 }
                 if (BLAS_IDX < n) {
-                    I::store(x, Vh, BLAS_IDX, xv[u]);
-                    I::store(r, Vh, BLAS_IDX, sv[u]);
+                    I::store(x, Vh, BLAS_IDX + xo, xv[u]);
+                    I::store(r, Vh, BLAS_IDX + o, sv[u]);
                 }
             }
         }
@@ -430,22 +430,22 @@ template <int PREC> BLAS_KERNEL k_final(int Vh, const void* __restrict__ p, cons
 // outer loop (fp64)
 // ---------------------------------------------------------------------------------------------------
 BLAS_KERNEL k_outer_residual(int Vh, const void* __restrict__ b, const void* __restrict__ t, void* __restrict__ r, RedBuf rb,
-                             SolverScalars* sc, size_t bstride, size_t stride) {
+                             SolverScalars* sc, int bstride, int stride) {
     using I = Item<BQ_FP64>;
     constexpr int UNR = UNR_UPDATE(I);
-    b = rhs_field(b, bstride); t = rhs_field(t, stride); r = rhs_field(r, stride); sc += blockIdx.y; rb = rhs_redbuf(rb);
+    const int bo = blockIdx.y * bstride, o = blockIdx.y * stride; sc += blockIdx.y; rb = rhs_redbuf(rb);
     double acc = 0;
     const int n = I::count(Vh);
     BLAS_TRIPS(I, n) {
         double bv[UNR][2], tv[UNR][2];
         BLAS_UNROLL(I) {
-            I::load_or_zero(b, Vh, BLAS_IDX, n, bv[u]);
-            I::load_or_zero(t, Vh, BLAS_IDX, n, tv[u]);
+            I::load_or_zero(b, Vh, BLAS_IDX, n, bv[u], bo);
+            I::load_or_zero(t, Vh, BLAS_IDX, n, tv[u], o);
         }
         BLAS_UNROLL(I) {
             bv[u][0] -= tv[u][0];
             bv[u][1] -= tv[u][1];
-            if (BLAS_IDX < n) I::store(r, Vh, BLAS_IDX, bv[u]);
+            if (BLAS_IDX < n) I::store(r, Vh, BLAS_IDX + o, bv[u]);
             acc += bv[u][0] * bv[u][0] + bv[u][1] * bv[u][1];
         }
     }
@@ -459,32 +459,33 @@ BLAS_KERNEL k_outer_residual(int Vh, const void* __restrict__ b, const void* __r
 }
 
 template <int PREC_LO> __global__ void __launch_bounds__(128) k_to_low(int Vh, const void* __restrict__ r64, void* __restrict__ lo,
-                                                                      const SolverScalars* __restrict__ sc, size_t stride64, size_t stride_lo) {
+                                                                      const SolverScalars* __restrict__ sc, int stride64, int stride_lo) {
     const int h = blockIdx.x * blockDim.x + threadIdx.x;
     if (h >= Vh) return;
-    r64 = rhs_field(r64, stride64); lo = rhs_field(lo, stride_lo); sc += blockIdx.y;
+    sc += blockIdx.y;
     const double sca = sc->scale;
     double v[24];
-    load_spinor<BQ_FP64, true>(r64, Vh, h, v);
+    load_spinor<BQ_FP64, true>(r64, Vh, h + blockIdx.y * stride64, v);     // strides in sites
     typename Prec<PREC_LO>::comp w[24];
 #pragma unroll
     for (int i = 0; i < 24; i++) w[i] = (typename Prec<PREC_LO>::comp)(v[i] * sca);
-    store_spinor<PREC_LO>(lo, Vh, h, w);
+    store_spinor<PREC_LO>(lo, Vh, h + blockIdx.y * stride_lo, w);
 }
 
 template <int EPREC> __global__ void __launch_bounds__(128) k_accumulate(int Vh, const void* __restrict__ e, void* __restrict__ x64,
-                                                                        const SolverScalars* __restrict__ sc, size_t estride, size_t xstride) {
+                                                                        const SolverScalars* __restrict__ sc, int estride, int xstride) {
     const int h = blockIdx.x * blockDim.x + threadIdx.x;
     if (h >= Vh) return;
-    e = rhs_field(e, estride); x64 = rhs_field(x64, xstride); sc += blockIdx.y;
+    sc += blockIdx.y;
+    const int he = h + blockIdx.y * estride, hx = h + blockIdx.y * xstride;     // strides in sites
     const double rn = sc->rnorm;
     typename Prec<EPREC>::comp ev[24];
-    load_spinor<EPREC, true>(e, Vh, h, ev);
+    load_spinor<EPREC, true>(e, Vh, he, ev);
     double xv[24];
-    load_spinor<BQ_FP64, true>(x64, Vh, h, xv);
+    load_spinor<BQ_FP64, true>(x64, Vh, hx, xv);
 #pragma unroll
     for (int i = 0; i < 24; i++) xv[i] += rn * (double)ev[i];
-    store_spinor<BQ_FP64>(x64, Vh, h, xv);
+    store_spinor<BQ_FP64>(x64, Vh, hx, xv);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -531,7 +532,12 @@ void blas_ctx_destroy(BlasCtx* c) {
     c->partials = nullptr; c->ticket = nullptr; c->sc = nullptr; c->stop2s = nullptr; c->cap = 0;
 }
 
-// c.nrhs right-hand sides per launch (gridDim.y), operand fields c.stride bytes apart (storage precision of the call)
+// c.nrhs right-hand sides per launch (gridDim.y).  The context holds the distances between the fields of one operand in
+// BYTES; the kernels want them in items (blas.cuh): 16-byte chunks for fp64 / fp32 vectors, sites for half storage.
+static int items_of(int prec, size_t bytes) { return (int)(bytes / (prec == BQ_HALF ? spinor_site_bytes(BQ_HALF) : 16)); }
+// the solution accumulator of k_final / k_cg_update: an fp32 field read site-wise when the storage is half
+static int x_items_of(int prec, size_t bytes) { return (int)(bytes / (prec == BQ_HALF ? spinor_site_bytes(BQ_FP32) : 16)); }
+static int sites_of(int prec, size_t bytes) { return (int)(bytes / spinor_site_bytes(prec)); }
 #define DISPATCH_PREC(prec, KERNEL, ...)                                                          \
     do {                                                                                          \
         const dim3 g_(c.grid, c.nrhs);                                                            \
@@ -544,11 +550,11 @@ void blas_ctx_destroy(BlasCtx* c) {
 
 bq_status blas_norm2(bq_lattice* lat, const BlasCtx& c, int prec, const void* a) {
     RedBuf rb{c.partials, c.ticket, c.pstride};
-    DISPATCH_PREC(prec, k_norm2, c.Vh, a, rb, c.sc, c.stride);
+    DISPATCH_PREC(prec, k_norm2, c.Vh, a, rb, c.sc, items_of(prec, c.stride));
 }
 bq_status blas_cdot(bq_lattice* lat, const BlasCtx& c, int prec, const void* a, const void* b) {
     RedBuf rb{c.partials, c.ticket, c.pstride};
-    DISPATCH_PREC(prec, k_cdot, c.Vh, a, b, rb, c.sc, 0, c.stride);
+    DISPATCH_PREC(prec, k_cdot, c.Vh, a, b, rb, c.sc, 0, items_of(prec, c.stride));
 }
 bq_status blas_caxpy(bq_lattice* lat, const BlasCtx& c, int prec, double ar, double ai, const void* x, void* y) {
     const BlasCtx one = blas_single(c);
@@ -560,57 +566,57 @@ bq_status blas_caxpy(bq_lattice* lat, const BlasCtx& c, int prec, double ar, dou
 }
 bq_status bicg_init(bq_lattice* lat, const BlasCtx& c, int prec, const void* r, double stop2, bool per_rhs_stop2) {
     RedBuf rb{c.partials, c.ticket, c.pstride};
-    DISPATCH_PREC(prec, k_init, c.Vh, r, rb, c.sc, stop2, per_rhs_stop2 ? c.stop2s : nullptr, c.stride);
+    DISPATCH_PREC(prec, k_init, c.Vh, r, rb, c.sc, stop2, per_rhs_stop2 ? c.stop2s : nullptr, items_of(prec, c.stride));
 }
 bq_status cg_init(bq_lattice* lat, const BlasCtx& c, int prec, const void* rn, void* p, double rel2, bool per_rhs_rel2) {
     RedBuf rb{c.partials, c.ticket, c.pstride};
-    DISPATCH_PREC(prec, k_cg_init, c.Vh, rn, p, rb, c.sc, rel2, per_rhs_rel2 ? c.stop2s : nullptr, c.stride);
+    DISPATCH_PREC(prec, k_cg_init, c.Vh, rn, p, rb, c.sc, rel2, per_rhs_rel2 ? c.stop2s : nullptr, items_of(prec, c.stride));
 }
 bq_status cg_update(bq_lattice* lat, const BlasCtx& c, int prec, const void* p, const void* t, void* x, void* rn) {
     RedBuf rb{c.partials, c.ticket, c.pstride};
-    DISPATCH_PREC(prec, k_cg_update, c.Vh, p, t, x, rn, rb, c.sc, c.stride, c.xstride);
+    DISPATCH_PREC(prec, k_cg_update, c.Vh, p, t, x, rn, rb, c.sc, items_of(prec, c.stride), x_items_of(prec, c.xstride));
 }
 bq_status cg_p_update(bq_lattice* lat, const BlasCtx& c, int prec, const void* rn, void* p) {
-    DISPATCH_PREC(prec, k_cg_p, c.Vh, rn, p, c.sc, c.stride);
+    DISPATCH_PREC(prec, k_cg_p, c.Vh, rn, p, c.sc, items_of(prec, c.stride));
 }
 bq_status bicg_p_update(bq_lattice* lat, const BlasCtx& c, int prec, const void* r, void* p, const void* v) {
-    DISPATCH_PREC(prec, k_p_update, c.Vh, r, p, v, c.sc, c.stride);
+    DISPATCH_PREC(prec, k_p_update, c.Vh, r, p, v, c.sc, items_of(prec, c.stride));
 }
 bq_status bicg_alpha(bq_lattice* lat, const BlasCtx& c, int prec, const void* rhat, const void* v) {
     RedBuf rb{c.partials, c.ticket, c.pstride};
-    DISPATCH_PREC(prec, k_cdot, c.Vh, rhat, v, rb, c.sc, 1, c.stride);
+    DISPATCH_PREC(prec, k_cdot, c.Vh, rhat, v, rb, c.sc, 1, items_of(prec, c.stride));
 }
 bq_status bicg_s_update(bq_lattice* lat, const BlasCtx& c, int prec, const void* r, const void* v, void* s) {
-    DISPATCH_PREC(prec, k_s_update, c.Vh, r, v, s, c.sc, c.stride);
+    DISPATCH_PREC(prec, k_s_update, c.Vh, r, v, s, c.sc, items_of(prec, c.stride));
 }
 bq_status bicg_omega(bq_lattice* lat, const BlasCtx& c, int prec, const void* t, const void* s) {
     RedBuf rb{c.partials, c.ticket, c.pstride};
-    DISPATCH_PREC(prec, k_omega, c.Vh, t, s, rb, c.sc, c.stride);
+    DISPATCH_PREC(prec, k_omega, c.Vh, t, s, rb, c.sc, items_of(prec, c.stride));
 }
 bq_status bicg_final(bq_lattice* lat, const BlasCtx& c, int prec, const void* p, const void* s, const void* t, const void* rhat,
                      void* x, void* r) {
     RedBuf rb{c.partials, c.ticket, c.pstride};
-    DISPATCH_PREC(prec, k_final, c.Vh, p, s, t, rhat, x, r, rb, c.sc, c.stride, c.xstride);
+    DISPATCH_PREC(prec, k_final, c.Vh, p, s, t, rhat, x, r, rb, c.sc, items_of(prec, c.stride), x_items_of(prec, c.xstride));
 }
 
 bq_status outer_residual(bq_lattice* lat, const BlasCtx& c, const void* b, size_t bstride, const void* t, void* r) {
     RedBuf rb{c.partials, c.ticket, c.pstride};
-    k_outer_residual<<<dim3(c.grid, c.nrhs), BLAS_BLOCK, 0, c.stream>>>(c.Vh, b, t, r, rb, c.sc, bstride, c.stride64);
+    k_outer_residual<<<dim3(c.grid, c.nrhs), BLAS_BLOCK, 0, c.stream>>>(c.Vh, b, t, r, rb, c.sc, items_of(BQ_FP64, bstride), items_of(BQ_FP64, c.stride64));
     BQ_CHECK_LAUNCH(lat);
     return BQ_OK;
 }
 bq_status outer_to_low(bq_lattice* lat, const BlasCtx& c, int prec_lo, const void* r64, void* lo) {
     const dim3 grid((c.Vh + 127) / 128, c.nrhs);
-    if (prec_lo == BQ_FP64) k_to_low<BQ_FP64><<<grid, 128, 0, c.stream>>>(c.Vh, r64, lo, c.sc, c.stride64, c.stride);
-    else if (prec_lo == BQ_FP32) k_to_low<BQ_FP32><<<grid, 128, 0, c.stream>>>(c.Vh, r64, lo, c.sc, c.stride64, c.stride);
-    else k_to_low<BQ_HALF><<<grid, 128, 0, c.stream>>>(c.Vh, r64, lo, c.sc, c.stride64, c.stride);
+    if (prec_lo == BQ_FP64) k_to_low<BQ_FP64><<<grid, 128, 0, c.stream>>>(c.Vh, r64, lo, c.sc, sites_of(BQ_FP64, c.stride64), sites_of(prec_lo, c.stride));
+    else if (prec_lo == BQ_FP32) k_to_low<BQ_FP32><<<grid, 128, 0, c.stream>>>(c.Vh, r64, lo, c.sc, sites_of(BQ_FP64, c.stride64), sites_of(prec_lo, c.stride));
+    else k_to_low<BQ_HALF><<<grid, 128, 0, c.stream>>>(c.Vh, r64, lo, c.sc, sites_of(BQ_FP64, c.stride64), sites_of(prec_lo, c.stride));
     BQ_CHECK_LAUNCH(lat);
     return BQ_OK;
 }
 bq_status outer_accumulate(bq_lattice* lat, const BlasCtx& c, int e_prec, const void* e, void* x64, size_t x64stride) {
     const dim3 grid((c.Vh + 127) / 128, c.nrhs);
-    if (e_prec == BQ_FP64) k_accumulate<BQ_FP64><<<grid, 128, 0, c.stream>>>(c.Vh, e, x64, c.sc, c.xstride, x64stride);
-    else if (e_prec == BQ_FP32) k_accumulate<BQ_FP32><<<grid, 128, 0, c.stream>>>(c.Vh, e, x64, c.sc, c.xstride, x64stride);
+    if (e_prec == BQ_FP64) k_accumulate<BQ_FP64><<<grid, 128, 0, c.stream>>>(c.Vh, e, x64, c.sc, sites_of(e_prec, c.xstride), sites_of(BQ_FP64, x64stride));
+    else if (e_prec == BQ_FP32) k_accumulate<BQ_FP32><<<grid, 128, 0, c.stream>>>(c.Vh, e, x64, c.sc, sites_of(e_prec, c.xstride), sites_of(BQ_FP64, x64stride));
     else return bq_set_error(lat, BQ_EINVAL, "outer_accumulate: accumulator cannot be half");
     BQ_CHECK_LAUNCH(lat);
     return BQ_OK;

@@ -30,8 +30,8 @@ template <> struct Item<BQ_FP64> {
     static constexpr int NC = 1;
     static constexpr bool FLAT = true;   // items are independent 16-byte chunks: several per thread per trip (blas.cu)
     __host__ __device__ static int count(int Vh) { return 12 * Vh; }
-    __device__ static void load_or_zero(const void* b, int Vh, int i, int n, C* v) {
-        if (i < n) load(b, Vh, i, v);
+    __device__ static void load_or_zero(const void* b, int Vh, int i, int n, C* v, int off = 0) {
+        if (i < n) load(b, Vh, i + off, v);
         else v[0] = v[1] = 0;
     }
     __device__ static void load(const void* b, int, int i, C* v) {
@@ -45,8 +45,8 @@ template <> struct Item<BQ_FP32> {
     static constexpr int NC = 2;
     static constexpr bool FLAT = true;
     __host__ __device__ static int count(int Vh) { return 6 * Vh; }
-    __device__ static void load_or_zero(const void* b, int Vh, int i, int n, C* v) {
-        if (i < n) load(b, Vh, i, v);
+    __device__ static void load_or_zero(const void* b, int Vh, int i, int n, C* v, int off = 0) {
+        if (i < n) load(b, Vh, i + off, v);
         else v[0] = v[1] = v[2] = v[3] = 0;
     }
     __device__ static void load(const void* b, int, int i, C* v) {
@@ -60,8 +60,8 @@ template <> struct Item<BQ_HALF> {
     static constexpr int NC = 12;
     static constexpr bool FLAT = false;  // a site is already 52 bytes in 4 requests
     __host__ __device__ static int count(int Vh) { return Vh; }
-    __device__ static void load_or_zero(const void* b, int Vh, int i, int n, C* v) {
-        if (i < n) load(b, Vh, i, v);
+    __device__ static void load_or_zero(const void* b, int Vh, int i, int n, C* v, int off = 0) {
+        if (i < n) load(b, Vh, i + off, v);
         else {
 #pragma unroll
             for (int k = 0; k < 24; k++) v[k] = 0;
@@ -100,10 +100,12 @@ struct RedBuf {
     int pstride;             // doubles of partials per right-hand side
 };
 
-// Batched (multi-rhs) launches: gridDim.y = right-hand sides; blockIdx.y selects the operand fields (`stride` bytes
-// apart), the BiCGStab state sc[rhs] and the reduction scratch of that right-hand side.  gridDim.y = 1 is the plain case.
-__device__ __forceinline__ const void* rhs_field(const void* p, size_t stride) { return static_cast<const char*>(p) + blockIdx.y * stride; }
-__device__ __forceinline__ void* rhs_field(void* p, size_t stride) { return static_cast<char*>(p) + blockIdx.y * stride; }
+// Batched (multi-rhs) launches: gridDim.y = right-hand sides; blockIdx.y selects the operand fields, the BiCGStab state
+// sc[rhs] and the reduction scratch of that right-hand side.  gridDim.y = 1 is the plain case.  The fields of one operand
+// are `stride` ITEMS apart (16-byte chunks for fp64 / fp32 vectors, sites for half-storage vectors and for the site-wise
+// conversion kernels) and are reached through the item index, i + blockIdx.y * stride, NOT by offsetting the pointer
+// parameters: with offset pointers ptxas no longer issued the 5 loads of k_final ahead of the arithmetic (2 instead of 5
+// requests in flight per thread: 115 -> 211 us).  Item indices stay below 2^31 (checked by the callers).
 __device__ __forceinline__ RedBuf rhs_redbuf(RedBuf rb) {
     rb.partials += (size_t)blockIdx.y * rb.pstride;
     rb.ticket += blockIdx.y;

@@ -271,6 +271,9 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
     const double csw = o.csw;
     const bool clover = csw != 0.0;
     const int n = nrhs, mrhs = multi ? n : 0;      // mrhs = 0 selects the single-field kernels
+    // the batched BLAS-1 kernels index all right-hand sides of an operand with one int (blas.cuh)
+    if ((double)n * 2.0 * 12.0 * lat->g.Vh >= 2147483648.0)
+        return bq_set_error(lat, BQ_EINVAL, "%s: nrhs * 24 * Vh must stay below 2^31 — split the batch", fn);
 
     SolverWork* w = nullptr;
     BQ_TRY(get_work(lat, prec, &w, n));
@@ -826,6 +829,7 @@ extern "C" bq_status bq_bench_kernel_multi(bq_lattice* lat, int which, bq_prec p
     if (prec != BQ_FP64 && prec != BQ_FP32 && prec != BQ_HALF) return bq_set_error(lat, BQ_EINVAL, "bq_bench_kernel_multi: bad precision");
     if (recon != BQ_RECON18 && recon != BQ_RECON12) return bq_set_error(lat, BQ_EINVAL, "bq_bench_kernel_multi: bad recon");
     if (!lat->have_gauge) return bq_set_error(lat, BQ_ENOGAUGE, "bq_bench_kernel_multi: no gauge field loaded");
+    if ((double)nrhs * 2.0 * 12.0 * lat->g.Vh >= 2147483648.0) return bq_set_error(lat, BQ_EINVAL, "bq_bench_kernel_multi: batch too large");
     const Geom& g = lat->g;
     cudaStream_t s = 0;
     const size_t fb = field_bytes_one_parity(g, prec);
