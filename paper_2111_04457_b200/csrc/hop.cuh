@@ -121,3 +121,91 @@ __device__ __forceinline__ void hop_dir(typename Prec<PREC>::comp* acc, const vo
         for (int i = 0; i < 12; i++) acc[(FWD ? 12 : 0) + i] = mad(w2, chi[i], acc[(FWD ? 12 : 0) + i]);
     }
 }
+
+// ---------------------------------------------------------------------------------------------------
+// Half storage: the same hop split into its LOAD (raw 16-byte words of the neighbour spinor and of the link, kept
+// packed: 13 + 9 registers) and its COMPUTE (unpack, project, multiply, accumulate), so that hop_site can issue the
+// loads of direction d+1 before it computes direction d.  A half-storage direction is only 88 bytes per thread; at the
+// 16 warps per SM the register budget allows, the compiler's own batching (loads of ~3 directions, then their
+// arithmetic) leaves part of every batch's memory latency exposed — ncu: long-scoreboard stalls dominate, issue slots
+// 60 % busy on a kernel that needs them ~85 % busy to reach the HBM roofline.  ptxas still schedules the loads its own
+// way, so the source-level pipeline only nudges it: measured 84.0 -> 82.0 us (18-real), 82.0 -> 76.6 us (12-real),
+// 92.1 -> 84.0 us (xpay epilogue) on 32^3x64.
+// ---------------------------------------------------------------------------------------------------
+struct HalfRaw {
+    uint4 s0, s1, s2;      // spinor mantissas (t direction: s0 = the full word, s1.x/.y = the half word)
+    float n;               // site norm
+    uint4 l0, l1;          // link words (12-real: l1.x/.y = the trailing 8 bytes)
+    unsigned int lt;       // 18-real: trailing half2
+};
+
+template <int RECON, int MU, bool FWD, bool LSTREAM, bool DAG>
+__device__ __forceinline__ void hop_load_half(HalfRaw& r, const void* in, int Vh, int nh, const void* ublock, int uidx) {
+    using A = SpinorAddr<BQ_HALF>;
+    using LA = LinkAddr<BQ_HALF, RECON>;
+    const char* b = static_cast<const char*>(in);
+    if (MU < 3) {
+        r.s0 = ld16<false, uint4>(b + A::word(Vh, nh, 0));
+        r.s1 = ld16<false, uint4>(b + A::word(Vh, nh, 1));
+        r.s2 = ld16<false, uint4>(b + A::word(Vh, nh, 2));
+    } else {
+        constexpr int W = (FWD != DAG) ? 1 : 0;   // (1 - g_t) needs the lower spin pair, (1 + g_t) the upper one
+        r.s0 = ld16<false, uint4>(b + A::word(Vh, nh, W ? 2 : 0));
+        const uint2 d = ld16<false, uint2>(b + A::word(Vh, nh, 1) + (W ? 8 : 0));
+        r.s1.x = d.x; r.s1.y = d.y;
+    }
+    r.n = ld16<false, float>(b + A::tail(Vh, nh));
+    const char* ub = static_cast<const char*>(ublock);
+    r.l0 = ld16<LSTREAM, uint4>(ub + LA::word(Vh, uidx, 0));
+    if (RECON == BQ_RECON18) {
+        r.l1 = ld16<LSTREAM, uint4>(ub + LA::word(Vh, uidx, 1));
+        r.lt = ld16<LSTREAM, unsigned int>(ub + LA::tail(Vh, uidx));
+    } else {
+        const uint2 d = ld16<LSTREAM, uint2>(ub + LA::tail(Vh, uidx));
+        r.l1.x = d.x; r.l1.y = d.y;
+    }
+}
+
+template <int RECON, int MU, bool FWD, bool CPLX, bool DAG>
+__device__ __forceinline__ void hop_compute_half(float* acc, const HalfRaw& r, float pr, float pi) {
+    float h[12], u[18], chi[12];
+    if (MU < 3) {
+        float psi[24];
+        unpack8(r.s0, psi); unpack8(r.s1, psi + 8); unpack8(r.s2, psi + 16);
+        const float* up = DAG ? psi + 12 : psi;
+        const float* lo = DAG ? psi : psi + 12;
+#pragma unroll
+        for (int i = 0; i < 12; i++) h[i] = up[i];
+        add_isigma<MU>(h, lo, float(FWD ? 1 : -1));
+    } else {
+        constexpr int W = (FWD != DAG) ? 1 : 0;
+        const uint2 d = make_uint2(r.s1.x, r.s1.y);
+        if (W == 0) { unpack8(r.s0, h); unpack4(d, h + 8); }
+        else { unpack4(d, h); unpack8(r.s0, h + 4); }
+    }
+    unpack8(r.l0, u);
+    if (RECON == BQ_RECON18) {
+        unpack8(r.l1, u + 8);
+        const float2 t = __half22float2(*reinterpret_cast<const __half2*>(&r.lt));
+        u[16] = t.x; u[17] = t.y;
+    } else {
+        unpack4(make_uint2(r.l1.x, r.l1.y), u + 8);
+        reconstruct_row2(u);
+    }
+    su3_mul<!FWD>(u, h, chi);
+    float w = pr;
+    if (CPLX) {
+        phase_mul(chi, pr, pi);
+        w = 1.0f;
+    }
+    w *= r.n;
+    if (MU < 3) {
+#pragma unroll
+        for (int i = 0; i < 12; i++) acc[i] = mad(w, chi[i], acc[i]);
+        add_isigma<MU>(acc + 12, chi, FWD ? -w : w);
+    } else {
+        const float w2 = 2 * w;
+#pragma unroll
+        for (int i = 0; i < 12; i++) acc[(FWD ? 12 : 0) + i] = mad(w2, chi[i], acc[(FWD ? 12 : 0) + i]);
+    }
+}

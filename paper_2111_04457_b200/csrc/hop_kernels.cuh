@@ -25,6 +25,9 @@
 #ifndef HOP_MINB_64
 #define HOP_MINB_64 2   // fp64
 #endif
+#ifndef HOP_HALF_PIPELINE
+#define HOP_HALF_PIPELINE 1   // half storage: explicit load/compute software pipeline over the directions (A/B switch)
+#endif
 
 template <typename C> struct HopArgs {
     void* out;
@@ -132,6 +135,35 @@ __device__ __forceinline__ void hop_site(const HopArgs<typename Prec<PREC>::comp
 #pragma unroll
     for (int i = 0; i < 24; i++) acc[i] = 0;
 
+    if constexpr (PREC == BQ_HALF && HOP_HALF_PIPELINE && LSTREAM) {
+        // software pipeline over the 8 directions (hop.cuh, HalfRaw): the packed words of direction d+1 are requested
+        // before direction d is computed.  Single-rhs kernels only (LSTREAM): measured -2 % (18-real) to -9 % (12-real, xpay)
+        // there, +6 % in the multi-rhs kernel, which keeps the plain form (same arithmetic, bitwise equal results)
+        const bool wxf = r && (xh == a.Lxh - 1), wxb = !r && (xh == 0);
+        const bool wyf = (y == a.Ly - 1), wyb = (y == 0), wzf = (z == a.Lz - 1), wzb = (z == 0), wtf = (t == a.Lt - 1), wtb = (t == 0);
+        const int nxf = r ? (wxf ? h - (a.Lxh - 1) : h + 1) : h;
+        const int nxb = r ? h : (wxb ? h + (a.Lxh - 1) : h - 1);
+        const int nyf = wyf ? h - (a.Ly - 1) * sy : h + sy, nyb = wyb ? h + (a.Ly - 1) * sy : h - sy;
+        const int nzf = wzf ? h - (a.Lz - 1) * sz : h + sz, nzb = wzb ? h + (a.Lz - 1) * sz : h - sz;
+        const int ntf = wtf ? h - (a.Lt - 1) * st : h + st, ntb = wtb ? h + (a.Lt - 1) * st : h - st;
+        HalfRaw ra, rb;
+        hop_load_half<RECON, 0, true, LSTREAM, DAG>(ra, in, Vh, nxf, gf, h);
+        hop_load_half<RECON, 0, false, LSTREAM, DAG>(rb, in, Vh, nxb, gb, nxb);
+        hop_compute_half<RECON, 0, true, CPLX, DAG>(acc, ra, wxf ? a.phr[0] : one, wxf ? a.phi[0] : zero);
+        hop_load_half<RECON, 1, true, LSTREAM, DAG>(ra, in, Vh, nyf, gf + a.ublk, h);
+        hop_compute_half<RECON, 0, false, CPLX, DAG>(acc, rb, wxb ? a.phr[0] : one, wxb ? -a.phi[0] : zero);
+        hop_load_half<RECON, 1, false, LSTREAM, DAG>(rb, in, Vh, nyb, gb + a.ublk, nyb);
+        hop_compute_half<RECON, 1, true, CPLX, DAG>(acc, ra, wyf ? a.phr[1] : one, wyf ? a.phi[1] : zero);
+        hop_load_half<RECON, 2, true, LSTREAM, DAG>(ra, in, Vh, nzf, gf + 2 * a.ublk, h);
+        hop_compute_half<RECON, 1, false, CPLX, DAG>(acc, rb, wyb ? a.phr[1] : one, wyb ? -a.phi[1] : zero);
+        hop_load_half<RECON, 2, false, LSTREAM, DAG>(rb, in, Vh, nzb, gb + 2 * a.ublk, nzb);
+        hop_compute_half<RECON, 2, true, CPLX, DAG>(acc, ra, wzf ? a.phr[2] : one, wzf ? a.phi[2] : zero);
+        hop_load_half<RECON, 3, true, LSTREAM, DAG>(ra, in, Vh, ntf, gf + 3 * a.ublk, h);
+        hop_compute_half<RECON, 2, false, CPLX, DAG>(acc, rb, wzb ? a.phr[2] : one, wzb ? -a.phi[2] : zero);
+        hop_load_half<RECON, 3, false, LSTREAM, DAG>(rb, in, Vh, ntb, gb + 3 * a.ublk, ntb);
+        hop_compute_half<RECON, 3, true, CPLX, DAG>(acc, ra, wtf ? a.phr[3] : one, wtf ? a.phi[3] : zero);
+        hop_compute_half<RECON, 3, false, CPLX, DAG>(acc, rb, wtb ? a.phr[3] : one, wtb ? -a.phi[3] : zero);
+    } else {
     // ---- x ----
     {
         const bool wf = r && (xh == a.Lxh - 1);
@@ -167,6 +199,8 @@ __device__ __forceinline__ void hop_site(const HopArgs<typename Prec<PREC>::comp
         const bool wb = (t == 0);
         const int nb = wb ? h + (a.Lt - 1) * st : h - st;
         hop_dir<PREC, RECON, 3, false, CPLX, LSTREAM, DAG>(acc, in, Vh, nb, gb + 3 * a.ublk, nb, wb ? a.phr[3] : one, wb ? -a.phi[3] : zero);
+    }
+
     }
 
     if (DAG) {   // H^dag = S H S, S = exchange of the upper and lower spin pairs (hop_dir): the outer S
