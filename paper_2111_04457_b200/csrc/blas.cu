@@ -187,13 +187,17 @@ template <int PREC> BLAS_KERNEL k_cg_update(int Vh, const void* __restrict__ p, 
     if constexpr (PREC == BQ_HALF) {
         for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
             C xv[24], w[24], rv[24];
+            typename I::Raw rp, rr, rt;              // all requests of the site in flight before the first conversion
+            I::load_raw(p, Vh, i + o, rp);
+            I::load_raw(rn, Vh, i + o, rr);
+            I::load_raw(t, Vh, i + o, rt);
             load_spinor<BQ_FP32>(x, Vh, i + xo, xv);
-            I::load(p, Vh, i + o, w);
+            I::unpack(rp, w);
 #pragma unroll
             for (int k = 0; k < 24; k++) xv[k] = mad(a, w[k], xv[k]);
             store_spinor<BQ_FP32>(x, Vh, i + xo, xv);
-            I::load(rn, Vh, i + o, rv);
-            I::load(t, Vh, i + o, w);
+            I::unpack(rr, rv);
+            I::unpack(rt, w);
 #pragma unroll
             for (int k = 0; k < 24; k++) rv[k] = mad(-a, w[k], rv[k]);
             I::store(rn, Vh, i + o, rv);
@@ -355,20 +359,25 @@ template <int PREC> BLAS_KERNEL k_final(int Vh, const void* __restrict__ p, cons
     if constexpr (PREC == BQ_HALF) {
         for (int i = blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += gridDim.x * BLAS_BLOCK) {
             C xv[24], sv[24], w[24];
+            typename I::Raw rp, rs, rt, rh;          // all 22 requests of the site in flight before the first conversion
+            I::load_raw(p, Vh, i + o, rp);
+            I::load_raw(s, Vh, i + o, rs);
+            I::load_raw(t, Vh, i + o, rt);
+            I::load_raw(rhat, Vh, i + o, rh);
             load_spinor<BQ_FP32>(x, Vh, i + xo, xv);   // fp32 solution accumulator
-            I::load(p, Vh, i + o, w);
+            I::unpack(rp, w);
 #pragma unroll
             for (int k = 0; k < 12; k++) cfma(xv + 2 * k, ar, ai, w + 2 * k);
-            I::load(s, Vh, i + o, sv);
+            I::unpack(rs, sv);
 #pragma unroll
             for (int k = 0; k < 12; k++) cfma(xv + 2 * k, wr, wi, sv + 2 * k);
             store_spinor<BQ_FP32>(x, Vh, i + xo, xv);
-            I::load(t, Vh, i + o, w);
+            I::unpack(rt, w);
 #pragma unroll
             for (int k = 0; k < 12; k++) cfma(sv + 2 * k, -wr, -wi, w + 2 * k);   // r = s - omega t
             I::store(r, Vh, i + o, sv);
             I::requantize(sv);       // reductions see r as stored (rounded to half storage)
-            I::load(rhat, Vh, i + o, w);
+            I::unpack(rh, w);
 #pragma unroll
             for (int k = 0; k < 12; k++) {
                 r2 = mad(sv[2 * k + 1], sv[2 * k + 1], mad(sv[2 * k], sv[2 * k], r2));

@@ -69,6 +69,22 @@ template <> struct Item<BQ_HALF> {
     }
     __device__ static void load(const void* b, int Vh, int i, C* v) { load_spinor<BQ_HALF>(b, Vh, i, v); }
     __device__ static void store(void* b, int Vh, int i, const C* v) { store_spinor<BQ_HALF>(b, Vh, i, v); }
+    // The same load in two steps — request the packed words, unpack later — so that a kernel with several operands can
+    // put all its requests in flight before the first conversion (k_final: 5 operands, 22 requests per site).
+    struct Raw { uint4 q[3]; float n; };
+    __device__ static void load_raw(const void* b, int Vh, int i, Raw& r) {
+        using A = SpinorAddr<BQ_HALF>;
+        const char* c = static_cast<const char*>(b);
+#pragma unroll
+        for (int k = 0; k < 3; k++) r.q[k] = *reinterpret_cast<const uint4*>(c + A::word(Vh, i, k));
+        r.n = *reinterpret_cast<const float*>(c + A::tail(Vh, i));
+    }
+    __device__ static void unpack(const Raw& r, C* v) {
+#pragma unroll
+        for (int k = 0; k < 3; k++) unpack8(r.q[k], v + 8 * k);
+#pragma unroll
+        for (int k = 0; k < 24; k++) v[k] *= r.n;
+    }
     // what a load of the just-stored item would return: v -> fp16(v/n) * n, n = max|v|
     __device__ static void requantize(C* v) {
         float n = 0.f;
