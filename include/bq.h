@@ -40,7 +40,10 @@
  * DEVICE pointers; the library never keeps them after the call returns.  The handle owns its gauge
  * copies, clover blocks and solver workspace.  Calls on one handle must not run concurrently.
  * Unless a `stream` argument says otherwise, work is enqueued on the CUDA legacy default stream and
- * the call returns without synchronising (bq_solve and bq_gauge_load synchronise before returning).
+ * the call returns without synchronising (bq_solve and bq_gauge_load synchronise before returning).  The solver and
+ * the bq_blas_* / bq_bench_* hooks run on a stream the handle owns — a blocking stream, i.e. ordered with the legacy
+ * default stream exactly as the legacy stream is with itself — because batches of solver iterations are replayed as
+ * CUDA graphs and the legacy stream cannot be captured.
  * ---------------------------------------------------------------------------------------------
  */
 #ifndef BQ_H

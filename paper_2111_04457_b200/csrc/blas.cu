@@ -512,7 +512,10 @@ bq_status blas_ctx_create(bq_lattice* lat, BlasCtx* c) {
     if (grid > need) grid = need;
     grid = ((grid + BLAS_CLUSTER - 1) / BLAS_CLUSTER) * BLAS_CLUSTER;
     c->grid = grid;
-    c->stream = 0;
+    // a stream of its own (blocking: ordered with the legacy default stream exactly like the legacy stream itself), because
+    // the legacy stream cannot be captured into a CUDA graph (solve.cu replays batches of iterations as graphs)
+    c->stream = nullptr;
+    BQ_CUDA(lat, cudaStreamCreateWithFlags(&c->stream, cudaStreamDefault));
     c->nrhs = 1; c->stride = 0; c->xstride = 0; c->stride64 = 0;
     c->cap = 0; c->partials = nullptr; c->ticket = nullptr; c->sc = nullptr; c->stop2s = nullptr;
     return blas_ctx_reserve(lat, c, 1);

@@ -47,6 +47,8 @@ struct bq_lattice {
     int* d_flag;             // device int scratch (singular-clover flag etc.)
     double* hop_partials;    // per-CTA partial sums of the hop kernel's fused reduction epilogues (lazily allocated)
     size_t hop_partials_cap; // doubles allocated there
+    unsigned long long epoch;  // bumped whenever gauge or clover stores are freed: cached CUDA graphs of the solver hold their addresses
+    int use_graphs;          // solver: replay the batches of inner iterations as CUDA graphs (default 1; env BQ_GRAPH=0 disables)
     int mrhs_patch;          // multi-rhs hop: 1 = patch mapping where the geometry allows (default), 0 = plain (env BQ_MRHS_PATCH)
     unsigned long long n_launch;      // kernels launched through this handle
     unsigned long long n_hop[3];      // hop-kernel launches per storage precision

@@ -236,6 +236,7 @@ bq_status bq_clover_build(bq_lattice* lat, double csw, double kappa) {
             lat->clover[p][i] = nullptr;
         }
     lat->have_clover = false;
+    lat->epoch++;
     const Geom& g = lat->g;
     const size_t nb = (size_t)2 * CLOVER_REALS * g.Vh * sizeof(double);
     BQ_CUDA(lat, cudaMalloc(&lat->clover[BQ_FP64][0], nb));

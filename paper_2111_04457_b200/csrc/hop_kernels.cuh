@@ -403,6 +403,7 @@ bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const void* z, 
         if (lat->hop_partials_cap < need) {
             if (lat->hop_partials) BQ_CUDA(lat, cudaFree(lat->hop_partials));
             lat->hop_partials = nullptr; lat->hop_partials_cap = 0;
+            lat->epoch++;     // cached solver graphs hold the old address
             BQ_CUDA(lat, cudaMalloc(&lat->hop_partials, sizeof(double) * need));
             lat->hop_partials_cap = need;
         }

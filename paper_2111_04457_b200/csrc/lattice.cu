@@ -74,6 +74,8 @@ extern "C" bq_status bq_lattice_create(int Lx, int Ly, int Lz, int Lt, const dou
     {
         const char* e = getenv("BQ_MRHS_PATCH");      // A/B switch of the multi-rhs hop's thread mapping (hop_kernels.cuh)
         lat->mrhs_patch = e ? atoi(e) : 1;
+        const char* gph = getenv("BQ_GRAPH");         // A/B switch: CUDA-graph replay of the solver's iteration batches (solve.cu)
+        lat->use_graphs = gph ? atoi(gph) : 1;
     }
     lat->err[0] = 0;
     *out = lat;
@@ -81,6 +83,7 @@ extern "C" bq_status bq_lattice_create(int Lx, int Ly, int Lz, int Lt, const dou
 }
 
 static void free_gauge(bq_lattice* lat) {
+    lat->epoch++;
     for (int p = 0; p < 3; p++)
         for (int r = 0; r < 2; r++) {
             if (lat->gauge[p][r]) cudaFree(lat->gauge[p][r]);
@@ -91,6 +94,7 @@ static void free_gauge(bq_lattice* lat) {
     lat->have_gauge = false;
 }
 static void free_clover(bq_lattice* lat) {
+    lat->epoch++;
     for (int p = 0; p < 3; p++)
         for (int i = 0; i < 2; i++) {
             if (lat->clover[p][i]) cudaFree(lat->clover[p][i]);

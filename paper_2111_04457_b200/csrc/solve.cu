@@ -16,8 +16,21 @@
 #include "blas.cuh"
 #include "blas_api.h"
 
+// One batch of `batch` inner iterations captured as a CUDA graph.  Every kernel argument of an iteration is fixed for a
+// given (method, precision, link form, kappa, csw, batch shape) — the vectors are the handle's workspace and all scalars
+// live in device memory — so the graph is instantiated once and replayed for every later batch, inner solve and call.
+struct IterGraph {
+    cudaGraphExec_t exec;
+    int method, prec, recon, nrhs, batch;
+    double kappa, csw;
+    unsigned long long epoch;
+    bool warm;                               // a batch with this key has run eagerly (lazy stores and scratch exist)
+    unsigned long long d_launch, d_hop[3];   // what one replay adds to the handle's launch counters
+};
+
 struct SolverWork {
     BlasCtx blas;
+    IterGraph graph;
     bool blas_ok;
     int nrhs;              // right-hand sides the buffers below are sized for
     // fp64, full lattice, [rhs][even | odd]
@@ -34,7 +47,14 @@ struct SolverWork {
     bool persistent_stage; double* stage;   // device staging buffer of one canonical field (import / export)
 };
 
+static void drop_graph(SolverWork* w) {
+    if (w->graph.exec) cudaGraphExecDestroy(w->graph.exec);
+    w->graph.exec = nullptr;
+    w->graph.warm = false;
+}
+
 static void free_inner(SolverWork* w) {
+    drop_graph(w);
     void** v[] = {&w->irhat, &w->ir, &w->ip, &w->iv, &w->is, &w->it, &w->itmp, &w->ie};
     for (void** p : v) {
         if (*p) cudaFree(*p);
@@ -60,7 +80,10 @@ void bq_solver_free(bq_lattice* lat) {
     if (!w) return;
     free_inner(w);
     free_outer(w);
-    if (w->blas_ok) blas_ctx_destroy(&w->blas);
+    if (w->blas_ok) {
+        blas_ctx_destroy(&w->blas);
+        if (w->blas.stream) cudaStreamDestroy(w->blas.stream);
+    }
     if (w->ev0) cudaEventDestroy(w->ev0);
     if (w->ev1) cudaEventDestroy(w->ev1);
     for (cudaEvent_t& e : w->evp) if (e) cudaEventDestroy(e);
@@ -134,6 +157,60 @@ static bq_status poll(bq_lattice* lat, SolverWork* w) {
     return BQ_OK;
 }
 
+// Run `batch` iterations, enqueued one at a time by `one()`: eagerly the first time a key is seen (that run also creates
+// whatever is made on first use: low-precision gauge / clover copies, reduction scratch), as a replay of the cached
+// graph afterwards; full batches only.  Any failure of the capture falls back to eager launches.
+template <class F>
+static bq_status run_batch(bq_lattice* lat, SolverWork* w, int method, int prec, int recon, double kappa, double csw, int batch,
+                           int full_batch, F one) {
+    IterGraph& g = w->graph;
+    cudaStream_t s = w->blas.stream;
+    const bool same = g.method == method && g.prec == prec && g.recon == recon && g.nrhs == w->blas.nrhs && g.batch == batch &&
+                      g.kappa == kappa && g.csw == csw && g.epoch == lat->epoch;
+    auto eager = [&]() -> bq_status {
+        for (int k = 0; k < batch; k++) BQ_TRY(one());
+        return BQ_OK;
+    };
+    if (!lat->use_graphs || batch != full_batch) return eager();
+    if (same && g.exec) {
+        BQ_CUDA(lat, cudaGraphLaunch(g.exec, s));
+        lat->n_launch += g.d_launch;
+        for (int p = 0; p < 3; p++) lat->n_hop[p] += g.d_hop[p];
+        return BQ_OK;
+    }
+    if (!same || !g.warm) {
+        drop_graph(w);
+        g.method = method; g.prec = prec; g.recon = recon; g.nrhs = w->blas.nrhs; g.batch = batch; g.kappa = kappa; g.csw = csw;
+        g.epoch = lat->epoch;
+        BQ_TRY(eager());
+        g.warm = true;
+        return BQ_OK;
+    }
+    // second batch with this key: capture it, then launch what was captured
+    const unsigned long long l0 = lat->n_launch, h0[3] = {lat->n_hop[0], lat->n_hop[1], lat->n_hop[2]};
+    if (cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+        cudaGetLastError();
+        return eager();
+    }
+    bq_status st = eager();
+    cudaGraph_t graph = nullptr;
+    cudaError_t e = cudaStreamEndCapture(s, &graph);
+    if (st == BQ_OK && e == cudaSuccess && graph) e = cudaGraphInstantiate(&g.exec, graph, 0);
+    if (graph) cudaGraphDestroy(graph);
+    if (st != BQ_OK || e != cudaSuccess || !g.exec) {
+        cudaGetLastError();
+        g.exec = nullptr;
+        lat->use_graphs = 0;              // do not try again on this handle
+        lat->n_launch = l0;
+        for (int p = 0; p < 3; p++) lat->n_hop[p] = h0[p];
+        return eager();
+    }
+    g.d_launch = lat->n_launch - l0;
+    for (int p = 0; p < 3; p++) g.d_hop[p] = lat->n_hop[p] - h0[p];
+    BQ_CUDA(lat, cudaGraphLaunch(g.exec, s));
+    return BQ_OK;
+}
+
 // Inner BiCGStab on M^ e = ir (e0 = 0) for every right-hand side of the batch (w->blas.nrhs), each with its own
 // device-resident scalars; rhs k stops when |r_k|^2 <= w->h_stop2[k] or after max_iter iterations.  A right-hand
 // side that has stopped keeps its iterate frozen (its update kernels exit early) while the others go on; the hop
@@ -157,13 +234,13 @@ static bq_status inner_bicgstab(bq_lattice* lat, SolverWork* w, double kappa, do
     const HopRed red_alpha{1, w->irhat, c.sc}, red_omega{2, nullptr, c.sc};
     for (;;) {
         const int batch = (max_iter - launched) < check_every ? (max_iter - launched) : check_every;
-        for (int k = 0; k < batch; k++) {
+        BQ_TRY(run_batch(lat, w, BQ_BICGSTAB, prec, recon, kappa, csw, batch, check_every, [&]() -> bq_status {
             BQ_TRY(bicg_p_update(lat, c, prec, w->ir, w->ip, w->iv));                                // p = r + beta (p - omega v)
             BQ_TRY(schur(lat, w->iv, w->ip, w->itmp, kappa, csw, prec, recon, s, &red_alpha, mrhs)); // v = M^ p; alpha = rho/<rhat,v>
             BQ_TRY(bicg_s_update(lat, c, prec, w->ir, w->iv, w->is));                                // s = r - alpha v
             BQ_TRY(schur(lat, w->it, w->is, w->itmp, kappa, csw, prec, recon, s, &red_omega, mrhs)); // t = M^ s; omega = <t,s>/<t,t>
-            BQ_TRY(bicg_final(lat, c, prec, w->ip, w->is, w->it, w->irhat, w->ie, w->ir));
-        }
+            return bicg_final(lat, c, prec, w->ip, w->is, w->it, w->irhat, w->ie, w->ir);
+        }));
         launched += batch;
         BQ_TRY(poll(lat, w));
         bool all_done = true;
@@ -191,12 +268,12 @@ static bq_status inner_cgnr(bq_lattice* lat, SolverWork* w, double kappa, double
     const HopRed red_qq{2, nullptr, c.sc};
     for (;;) {
         const int batch = (max_iter - launched) < check_every ? (max_iter - launched) : check_every;
-        for (int k = 0; k < batch; k++) {
+        BQ_TRY(run_batch(lat, w, BQ_CGNR, prec, recon, kappa, csw, batch, check_every, [&]() -> bq_status {
             BQ_TRY(bq_schur_red(lat, w->iv, w->ip, w->itmp, kappa, csw, prec, recon, s, &red_qq, mrhs, false));  // q = M^ p; alpha = rho/|q|^2
             BQ_TRY(bq_schur_red(lat, w->it, w->iv, w->itmp, kappa, csw, prec, recon, s, nullptr, mrhs, true));   // t = M^^dag q
             BQ_TRY(cg_update(lat, c, prec, w->ip, w->it, w->ie, w->irhat));                                       // e, r_N, beta
-            BQ_TRY(cg_p_update(lat, c, prec, w->irhat, w->ip));                                                   // p = r_N + beta p
-        }
+            return cg_p_update(lat, c, prec, w->irhat, w->ip);                                                    // p = r_N + beta p
+        }));
         launched += batch;
         BQ_TRY(poll(lat, w));
         bool all_done = true;
@@ -849,6 +926,7 @@ extern "C" bq_status bq_bench_kernel_multi(bq_lattice* lat, int which, bq_prec p
     SolverWork* w = nullptr;
     if (iter) {
         BQ_TRY(get_work(lat, lat->work && lat->work->inner_prec >= 0 ? lat->work->inner_prec : BQ_FP32, &w));
+        drop_graph(w);
         BQ_TRY(blas_ctx_reserve(lat, &w->blas, nrhs));
         w->blas.nrhs = nrhs; w->blas.stride = fb; w->blas.xstride = xb; w->blas.stride64 = field_bytes_one_parity(g, BQ_FP64);
         s = w->blas.stream;

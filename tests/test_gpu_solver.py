@@ -211,3 +211,48 @@ def test_solve_x0_zero_ignores_x_on_entry(bq, cfg1):
         infos = bq.bq_solve_multi(lat.h, np.stack([b, 2 * b]), xm, 2, kappa, 1e-10, bq.bq_solve_opts(inner_prec=bq.BQ_FP32, x0_zero=1))
         assert all(i.status == 0 for i in infos)
         assert oracle_residual(U, xm[0], b, kappa) <= 1e-10 and oracle_residual(U, xm[1], 2 * b, kappa) <= 1e-10
+
+
+def test_graph_replay_matches_eager_and_survives_reconfiguration(bq, monkeypatch):
+    """The batches of inner iterations are replayed as CUDA graphs from their third occurrence on (eager, capture, replay).
+    The solution must be bitwise that of eager launches (BQ_GRAPH=0), and a cached graph must not outlive what it points
+    at: another batch shape, another precision, a multi-rhs solve in between (reduction scratch regrows), a new gauge field."""
+    L, kappa = (8, 8, 8, 8), 0.124
+    U, U2 = inputs.gauge(L, 81, 0.6), inputs.gauge(L, 82, 0.6)
+    b = inputs.spinor(L, 81)
+    opts = bq.bq_solve_opts(inner_prec=bq.BQ_FP32, check_every=2, x0_zero=1)       # many full batches per solve
+
+    def solve(lat, rhs=b, o=opts):
+        x = np.empty_like(rhs)
+        info = bq.bq_solve(lat.h, rhs, x, kappa, 1e-10, o)
+        return x, info
+
+    monkeypatch.setenv("BQ_GRAPH", "0")
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        x_eager, info_eager = solve(lat)
+        c_eager = bq.bq_get_counters(lat.h)
+        bq.bq_gauge_load(lat.h, U2)
+        x2_eager, _ = solve(lat)
+    monkeypatch.setenv("BQ_GRAPH", "1")
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        x1, info1 = solve(lat)
+        c1 = bq.bq_get_counters(lat.h)
+        assert np.array_equal(x1, x_eager) and info1.inner_iters == info_eager.inner_iters
+        assert c1 == c_eager                                   # replays are counted like the launches they stand for
+        for _ in range(3):
+            x, _ = solve(lat)
+            assert np.array_equal(x, x_eager)
+        xh, ih = solve(lat, o=bq.bq_solve_opts(inner_prec=bq.BQ_HALF, check_every=2, x0_zero=1))
+        assert ih.status == 0 and oracle_residual(U, xh, b, kappa) <= 1e-10
+        xm = np.empty((3,) + b.shape, dtype=np.complex128)
+        infos = bq.bq_solve_multi(lat.h, np.stack([b, 2 * b, -b]), xm, 3, kappa, 1e-10, opts)
+        assert all(i.status == 0 for i in infos) and oracle_residual(U, xm[2], -b, kappa) <= 1e-10
+        x, _ = solve(lat)
+        assert np.array_equal(x, x_eager)
+        xc, ic = solve(lat, o=bq.bq_solve_opts(inner_prec=bq.BQ_FP32, check_every=2, x0_zero=1, method=bq.BQ_CGNR))
+        assert ic.status == 0 and oracle_residual(U, xc, b, kappa) <= 1e-10
+        bq.bq_gauge_load(lat.h, U2)
+        x2, _ = solve(lat)
+        assert np.array_equal(x2, x2_eager) and oracle_residual(U2, x2, b, kappa) <= 1e-10
