@@ -73,3 +73,23 @@ def test_product_does_not_import_oracle():
                     src = fh.read()
                 assert "oracle" not in src.replace("the oracle", "").replace("oracle/", "").replace("CPU oracle", "").replace(
                     "oracle's", ""), f"{f} mentions the oracle module"
+
+
+def test_header_is_plain_c_and_links(bq, tmp_path):
+    """include/bq.h must be usable from plain C (the boundary is a C ABI): a C99 translation unit that includes it, takes
+    the address of every declared function and fills the option / info structs compiles with gcc and links against libbq.so."""
+    import subprocess
+    names = declared_symbols()
+    src = tmp_path / "abi_check.c"
+    lines = ['#include "bq.h"', "#include <stddef.h>", "typedef void (*fn_t)(void);", "int main(void) {", "    fn_t fns[] = {"]
+    lines += [f"        (fn_t){n}," for n in names]
+    lines += ["    };", "    bq_solve_opts o = {0};", "    bq_solve_info info;", "    o.inner_prec = BQ_HALF; o.method = BQ_CGNR; o.lexical = 0; o.x0_zero = 1;",
+              "    info.phase_seconds[4] = 0.0; info.inner_iters = (int)BQ_MODE_DDAGD;",
+              "    return (fns[0] != NULL && o.x0_zero && info.inner_iters == 2) ? 0 : 1;", "}"]
+    src.write_text("\n".join(lines) + "\n")
+    libdir = os.path.join(ROOT, "paper_2111_04457_b200")
+    exe = tmp_path / "abi_check"
+    cmd = ["gcc", "-std=c99", "-Wall", "-Werror", "-pedantic", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe),
+           "-L", libdir, "-l:libbq.so", f"-Wl,-rpath,{libdir}", "-Wl,--allow-shlib-undefined"]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
