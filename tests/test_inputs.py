@@ -52,3 +52,25 @@ def test_independent_of_thread_count():
         outs.append(subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True,
                                    check=True).stdout.strip())
     assert outs[0] == outs[1]
+
+
+def test_golden_config1():
+    """Drift guard (tests/golden/README.md): the seeded inputs and the oracle reproduce the stored numbers of config 1."""
+    import importlib.util
+    import json
+    import os
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(here, "make_golden.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    now = mod.compute()
+    with open(os.path.join(here, "config1_oracle.json")) as f:
+        ref = json.load(f)
+    assert set(now) == set(ref)
+    for k, v in ref.items():
+        if k.startswith("_"):
+            continue
+        if k.startswith("bicgstab_iters"):
+            assert abs(now[k] - v) <= 2, k
+        else:
+            assert np.allclose(now[k], v, rtol=1e-11, atol=1e-11), (k, now[k], v)
