@@ -467,8 +467,11 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
         }
         cudaEventRecord(w->evp[1], s);
         for (;;) {
-            // r = b^_e - M^ x_e in fp64
-            {
+            // r = b^_e - M^ x_e in fp64  (declared zero guess, first cycle: M^ x_e = 0 without applying the operator)
+            if (o.x0_zero && outer == 0) {
+                cudaError_t e = cudaMemsetAsync(w->t, 0, fb64 * n, s);
+                if (e != cudaSuccess) { free(bnorm); free(ik); return bq_set_error(lat, BQ_ECUDA, "%s: memset failed", fn); }
+            } else {
                 // x_e of rhs k lives at xx + k*2*fb64: Schur with input stride 2*fb64 = two hops by hand
                 const HopMulti m1 = hm(2 * fb64, fb64, 0), m2 = hm(fb64, fb64, 2 * fb64);
                 if (!clover) {
