@@ -256,3 +256,20 @@ def test_graph_replay_matches_eager_and_survives_reconfiguration(bq, monkeypatch
         bq.bq_gauge_load(lat.h, U2)
         x2, _ = solve(lat)
         assert np.array_equal(x2, x2_eager) and oracle_residual(U2, x2, b, kappa) <= 1e-10
+
+
+@pytest.mark.parametrize("inner,method", [(1, 0), (2, 0), (0, 0), (1, 1)])
+def test_near_free_field_long_solve(bq, inner, method):
+    """A smooth field (eps = 0.05) close to the free critical point (kappa = 0.1245): ~90 iterations instead of ~12, i.e.
+    many batches (graph replays), several half-precision outer cycles — all judged with the oracle's operator."""
+    L, kappa = (8, 8, 8, 16), 0.1245
+    U = inputs.gauge(L, 777, 0.05)
+    b = inputs.spinor(L, 777)
+    x = np.zeros_like(b)
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        info = bq.bq_solve(lat.h, b, x, kappa, 1e-10, bq.bq_solve_opts(inner_prec=inner, method=method, max_inner=2000, max_outer=100))
+    res = oracle_residual(U, x, b, kappa)
+    print(f"near-free inner={inner} method={method}: outer {info.outer_cycles} iters {info.inner_iters} res {res:.2e}")
+    assert info.status == 0 and res <= 1e-10 and abs(res - info.true_rel_residual) < 1e-11
+    assert info.inner_iters > 40
