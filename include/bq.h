@@ -217,6 +217,13 @@ bq_status bq_solve(bq_lattice* lat, const double* b, double* x, double kappa, do
 bq_status bq_solve_multi(bq_lattice* lat, const double* b, double* x, int nrhs, double kappa, double tol,
                          const bq_solve_opts* opts, bq_solve_info* info /*[nrhs]*/);
 
+/* The program of the paper's Fig. 1: "for each spin id and colour ic: set a point source, invert" — the quark
+ * propagator from one site — as ONE batched solve (bq_solve_multi with nrhs = 12).  src_site = {x, y, z, t} (0-based).
+ * The 12 sources delta_{x,src} e_id (x) e_ic are made on the device; S (HOST or DEVICE, 12 * 24*V doubles, output only)
+ * receives the 12 solutions in the canonical layout, solution k = 3*id + ic first index.  info: 12 entries or NULL. */
+bq_status bq_propagator(bq_lattice* lat, const int* src_site /*[4]*/, double* S, double kappa, double tol,
+                        const bq_solve_opts* opts, bq_solve_info* info /*[12]*/);
+
 /* The same operator with the BiCGStab inner products fused into the epilogue of its second hop kernel (SURVEY A6
  * (iii), (v): no separate reduction pass over the result), exposed for tests:
  *   w != NULL: dots[0..1] = <w, out>;      w == NULL: dots[0..1] = <out, in>, dots[2] = <out, out>

@@ -29,7 +29,7 @@ EXPORTS = [
     "bq_field_bytes", "bq_field_import", "bq_field_export", "bq_wilson_apply", "bq_clover_apply",
     "bq_dirac_apply", "bq_schur_apply", "bq_solve", "bq_blas_norm2", "bq_blas_cdot", "bq_blas_caxpy",
     "bq_blas_bicg_update", "bq_get_counters", "bq_bench_kernel", "bq_schur_apply_dots",
-    "bq_wilson_apply_multi", "bq_schur_apply_multi", "bq_bench_kernel_multi", "bq_solve_multi", "bq_dirac_apply_mode", "bq_schur_apply_mode",
+    "bq_wilson_apply_multi", "bq_schur_apply_multi", "bq_bench_kernel_multi", "bq_solve_multi", "bq_dirac_apply_mode", "bq_schur_apply_mode", "bq_propagator",
 ]
 
 
@@ -80,6 +80,7 @@ def lib():
         L.bq_schur_apply_dots.argtypes = [_vp, _vp, _vp, _vp, _d, _d, _i, _i, _vp, _dp]
         L.bq_solve.argtypes = [_vp, _vp, _vp, _d, _d, ctypes.POINTER(bq_solve_opts), ctypes.POINTER(bq_solve_info)]
         L.bq_solve_multi.argtypes = [_vp, _vp, _vp, _i, _d, _d, ctypes.POINTER(bq_solve_opts), ctypes.POINTER(bq_solve_info)]
+        L.bq_propagator.argtypes = [_vp, ctypes.POINTER(_i), _vp, _d, _d, ctypes.POINTER(bq_solve_opts), ctypes.POINTER(bq_solve_info)]
         L.bq_dirac_apply_mode.argtypes = [_vp, _vp, _vp, _vp, _d, _d, _i, _i, _i, _vp]
         L.bq_schur_apply_mode.argtypes = [_vp, _vp, _vp, _vp, _vp, _d, _d, _i, _i, _i, _vp]
         L.bq_blas_norm2.argtypes = [_vp, _vp, _i, _dp]
@@ -216,6 +217,15 @@ def bq_solve_multi(h, b, x, nrhs, kappa, tol, opts: bq_solve_opts | None = None,
     """b, x: [nrhs, Lt,Lz,Ly,Lx,4,3] complex128 (numpy host arrays or torch CUDA tensors); x is in/out.  Returns [bq_solve_info]."""
     infos = (bq_solve_info * nrhs)()
     st = lib().bq_solve_multi(h, _ptr(b), _ptr(x), nrhs, kappa, tol, ctypes.byref(opts) if opts is not None else None, infos)
+    _check(h, st, allow=() if raise_on_fail else (BQ_ENOTCONVERGED, BQ_EBREAKDOWN))
+    return list(infos)
+
+
+def bq_propagator(h, src_site, S, kappa, tol, opts: bq_solve_opts | None = None, raise_on_fail=True):
+    """S: [12, Lt,Lz,Ly,Lx,4,3] complex128 output (numpy host array or torch CUDA tensor); src_site = (x, y, z, t)."""
+    infos = (bq_solve_info * 12)()
+    site = (_i * 4)(*[int(v) for v in src_site])
+    st = lib().bq_propagator(h, site, _ptr(S), kappa, tol, ctypes.byref(opts) if opts is not None else None, infos)
     _check(h, st, allow=() if raise_on_fail else (BQ_ENOTCONVERGED, BQ_EBREAKDOWN))
     return list(infos)
 

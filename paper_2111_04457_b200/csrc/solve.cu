@@ -681,6 +681,46 @@ extern "C" bq_status bq_solve_multi(bq_lattice* lat, const double* b, double* x,
 }
 
 // ---------------------------------------------------------------------------------------------------
+// bq_propagator: the program of the paper's Fig. 1 — for each of the 12 spin-colour components (id, ic)
+// set a point source at one site and invert — as ONE batched solve.  The sources are made on the device (no host
+// transfer of 12 mostly-zero fields); S receives the 12 solutions, canonical layout, source index 3*id + ic.
+// ---------------------------------------------------------------------------------------------------
+__global__ void k_point_sources(double* b, size_t field_doubles, size_t site) {
+    const int k = threadIdx.x;                       // source index 3*spin + colour
+    if (k < 12) b[(size_t)k * field_doubles + site * 24 + 2 * k] = 1.0;
+}
+
+extern "C" bq_status bq_propagator(bq_lattice* lat, const int* src_site, double* S, double kappa, double tol, const bq_solve_opts* opts,
+                                   bq_solve_info* info) {
+    if (!lat) return BQ_EINVAL;
+    if (!src_site || !S) return bq_set_error(lat, BQ_EINVAL, "bq_propagator: src_site or S is NULL");
+    const Geom& g = lat->g;
+    for (int mu = 0; mu < 4; mu++)
+        if (src_site[mu] < 0 || src_site[mu] >= g.L[mu]) return bq_set_error(lat, BQ_EINVAL, "bq_propagator: source site outside the lattice");
+    const size_t site = src_site[0] + (size_t)g.L[0] * (src_site[1] + (size_t)g.L[1] * (src_site[2] + (size_t)g.L[2] * src_site[3]));
+    const size_t fd = (size_t)g.V * 24;
+    double* b = nullptr;
+    BQ_CUDA(lat, cudaMalloc(&b, 12 * fd * sizeof(double)));
+    cudaError_t e = cudaMemset(b, 0, 12 * fd * sizeof(double));
+    if (e == cudaSuccess) {
+        k_point_sources<<<1, 32>>>(b, fd, site);
+        e = cudaGetLastError();
+    }
+    if (e != cudaSuccess) {
+        cudaFree(b);
+        return bq_set_error(lat, BQ_ECUDA, "bq_propagator: %s", cudaGetErrorString(e));
+    }
+    lat->n_launch++;
+    bq_solve_opts o;
+    if (opts) o = *opts;
+    else { o.inner_prec = BQ_FP32; o.recon = BQ_RECON18; o.csw = 0; o.inner_tol = 0; o.max_inner = 0; o.max_outer = 0; o.check_every = 0; o.method = BQ_BICGSTAB; o.lexical = 0; o.x0_zero = 0; o.stream = nullptr; }
+    o.x0_zero = 1;                                   // S is output only
+    const bq_status st = solve_impl(lat, b, S, 12, true, kappa, tol, &o, info);
+    cudaFree(b);
+    return st;
+}
+
+// ---------------------------------------------------------------------------------------------------
 // BLAS-1 test / benchmark entry points
 // ---------------------------------------------------------------------------------------------------
 static bq_status blas_entry(bq_lattice* lat, int prec, SolverWork** w) {

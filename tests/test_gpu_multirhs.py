@@ -216,3 +216,28 @@ def test_solve_multi_patch(bq, inner, csw, method):
             assert not x[k].any()
         else:
             assert oracle_residual(U, x[k], b[k], kappa, A=A) <= 1e-10, k
+
+
+def test_propagator_is_fig1_of_the_paper(bq):
+    """bq_propagator = the loop of the paper's Fig. 1: 12 point sources at one site, one inversion each.
+    Every column against the oracle's operator, and against the oracle's own BiCGStab solution."""
+    L, kappa, csw = (4, 4, 4, 8), 0.12, 1.0
+    U = inputs.gauge(L, 75, 0.4)
+    A = bqo.clover_build(U, csw, kappa)
+    src = (1, 2, 3, 5)
+    S = np.full((12, L[3], L[2], L[1], L[0], 4, 3), np.nan, dtype=np.complex128)
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        infos = bq.bq_propagator(lat.h, src, S, kappa, 1e-10, bq.bq_solve_opts(inner_prec=bq.BQ_FP32, csw=csw))
+        with pytest.raises(bq.BqError):
+            bq.bq_propagator(lat.h, (4, 0, 0, 0), S.copy(), kappa, 1e-10)
+    assert len(infos) == 12 and all(i.status == 0 for i in infos)
+    for s in range(4):
+        for c in range(3):
+            b = np.zeros(S.shape[1:], dtype=np.complex128)
+            b[src[3], src[2], src[1], src[0], s, c] = 1.0
+            k = 3 * s + c
+            assert oracle_residual(U, S[k], b, kappa, A=A) <= 1e-10, k
+            if k in (0, 7):
+                x_ref, _ = bqo.bicgstab(U, b, kappa, tol=1e-12, A=A)
+                assert np.linalg.norm(S[k] - x_ref) / np.linalg.norm(x_ref) < 1e-8
