@@ -279,6 +279,29 @@ def main():
                "time_to_solution_s": dt, "device_seconds": infos[-1].seconds,
                "phase_seconds": dict(zip(("h2d+import", "prepare", "iterate", "reconstruct+residual", "export+d2h"), list(infos[-1].phase_seconds))), "inner_iters": infos[-1].inner_iters,
                "outer_cycles": infos[-1].outer_cycles, "hop_launches": hops[-1], "true_rel_residual": infos[-1].true_rel_residual}
+        # the plain operator through host buffers, for completeness: canonical fp64 field on the (pinned) host -> H2D -> layout
+        # conversion -> ONE hop -> conversion back -> D2H.  PCIe moves 2 x 402 MB for 1.38 GFlop: transfer-bound by construction.
+        psi_host = torch.from_numpy(psi).pin_memory()
+        out_host = torch.zeros_like(psi_host).pin_memory()
+        dev_in = torch.empty_like(psi_host, device="cuda")
+        dev_out = torch.zeros_like(dev_in)
+        buf_in, buf_out = lat.field(prec, bq.BQ_ODD), lat.field(prec, bq.BQ_EVEN)
+        ts = []
+        for it in range(3):
+            barrier()
+            t0 = time.perf_counter()
+            dev_in.copy_(psi_host, non_blocking=True)
+            bq.bq_field_import(lat.h, buf_in, dev_in, bq.BQ_ODD, prec)
+            bq.bq_wilson_apply(lat.h, buf_out, buf_in, kappa, bq.BQ_EVEN, prec, recon)
+            bq.bq_field_export(lat.h, dev_out, buf_out, bq.BQ_EVEN, prec)
+            out_host.copy_(dev_out, non_blocking=True)
+            torch.cuda.synchronize()
+            ts.append(time.perf_counter() - t0)
+        ta = replicas.max_over_ranks(min(ts[1:]))
+        e2e["host_apply"] = {"value": world * FLOP_PER_SITE * Vh / ta / 1e9, "unit": "GFlop/s", "seconds": ta,
+                             "h2d_bytes_per_step": psi_host.numel() * 16, "d2h_bytes_per_step": out_host.numel() * 16,
+                             "what": "one bq_wilson_apply(EVEN) from a pinned host canonical field to a pinned host canonical field "
+                                     "(H2D, bq_field_import, hop, bq_field_export, D2H)"}
         lat4.close()
 
     # ---- the rest of the path, per kernel (bq_bench_kernel hooks; device times, operands rotated out of L2) ----
