@@ -347,7 +347,7 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
     const int check_every = o.check_every > 0 ? o.check_every : 8;
     const double csw = o.csw;
     const bool clover = csw != 0.0;
-    const int n = nrhs, mrhs = multi ? n : 0;      // mrhs = 0 selects the single-field kernels
+    const int n = nrhs;
     // the batched BLAS-1 kernels index all right-hand sides of an operand with one int (blas.cuh)
     if ((double)n * 2.0 * 12.0 * lat->g.Vh >= 2147483648.0)
         return bq_set_error(lat, BQ_EINVAL, "%s: nrhs * 24 * Vh must stay below 2^31 — split the batch", fn);
