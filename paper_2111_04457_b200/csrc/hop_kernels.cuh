@@ -303,7 +303,7 @@ __device__ __forceinline__ void hop_block_partial_mrhs(const double* v, double* 
 }
 
 // Thread -> (site, rhs).  Plain mapping: T consecutive tiles x all nrhs right-hand sides per CTA.  Patch mapping
-// (a.patch; needs tiles that are pieces of x-rows, Lxh % 8 == 0): 4 right-hand sides x the 2 x 2 tiles (y, y+1) x (z, z+1)
+// (a.patch; needs tiles that are pieces of x-rows, Lxh % 8 == 0): by default 4 right-hand sides x the 2 x 2 tiles (y, y+1) x (z, z+1)
 // per CTA, the CTAs of the other rhs groups of the same patch next in blockIdx (they run at the same time, so the links
 // still come from HBM once and from L2 for the other groups).  Every input spinor is gathered by its 8 neighbours and L1
 // only catches what a CTA's own warps share; the patch keeps half of the y and z gathers inside the SM.  Measured
@@ -326,18 +326,21 @@ hop_kernel_mrhs(const HopArgs<typename Prec<PREC>::comp> a) {
     int rhs, h, R, T, rhs0, slot, nslots;
     bool live;
     if (a.patch) {
-        R = 4; T = 4;
-        const int rl = q & 3, tl = q >> 2, dy = tl & 1, dz = tl >> 1;
+        // a.patch packs the CTA shape: log2 of (rhs per CTA, tiles in y, in z, in t), 4 bits each; their product is 16
+        const int lR = a.patch & 15, ly = (a.patch >> 4) & 15, lz = (a.patch >> 8) & 15, lt = (a.patch >> 12) & 15;
+        R = 1 << lR; T = 16 >> lR;
+        const int rl = q & (R - 1), tl = q >> lR;
+        const int dy = tl & ((1 << ly) - 1), dz = (tl >> ly) & ((1 << lz) - 1), dt = tl >> (ly + lz);
         const int g = blockIdx.x % a.ngroups;
         int pb = blockIdx.x / a.ngroups;
         slot = pb; nslots = gridDim.x / a.ngroups;
         const int xt = pb % a.nxt; pb /= a.nxt;
-        const int yp = pb % (a.Ly >> 1); pb /= (a.Ly >> 1);
-        const int zp = pb % (a.Lz >> 1);
-        const int t = pb / (a.Lz >> 1);
-        const int tile = xt + a.nxt * ((2 * yp + dy) + a.Ly * ((2 * zp + dz) + a.Lz * t));
+        const int yp = pb % (a.Ly >> ly); pb /= (a.Ly >> ly);
+        const int zp = pb % (a.Lz >> lz);
+        const int tp = pb / (a.Lz >> lz);
+        const int tile = xt + a.nxt * (((yp << ly) + dy) + a.Ly * (((zp << lz) + dz) + a.Lz * ((tp << lt) + dt)));
         h = tile * 8 + s8;
-        rhs0 = g * 4; rhs = rhs0 + rl;
+        rhs0 = g * R; rhs = rhs0 + rl;
         live = rhs < a.nrhs;
     } else {
         R = a.nrhs; T = a.T; rhs0 = 0; slot = blockIdx.x; nslots = gridDim.x;
@@ -389,10 +392,16 @@ bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const void* z, 
     int nslots = grid;                    // partial sums per right-hand side of the fused reductions
     a.patch = 0; a.nxt = 0; a.ngroups = 1;
     if (multi && nrhs >= 3 && g.Lxh % 8 == 0 && lat->mrhs_patch) {
-        a.patch = 1; a.nxt = g.Lxh / 8; a.ngroups = (nrhs + 3) / 4;
-        nslots = g.Vh / 8 / 4;            // patches of 4 tiles (Ly, Lz are even)
-        grid = nslots * a.ngroups;
-        block = HOP_BLOCK;
+        // CTA shape (log2): rhs per CTA, tiles in y, z, t.  Default 4 rhs x 2 x 2 x 1; lat->mrhs_patch > 1 carries another
+        // packed shape (env BQ_MRHS_PATCH=0xtzyR, tuning switch).  Falls back to the plain mapping if the extents do not divide.
+        const int shape = lat->mrhs_patch > 1 ? lat->mrhs_patch : 0x0112;
+        const int lR = shape & 15, ly = (shape >> 4) & 15, lz = (shape >> 8) & 15, lt = (shape >> 12) & 15;
+        if (lR + ly + lz + lt == 4 && g.L[1] % (1 << ly) == 0 && g.L[2] % (1 << lz) == 0 && g.L[3] % (1 << lt) == 0) {
+            a.patch = shape; a.nxt = g.Lxh / 8; a.ngroups = (nrhs + (1 << lR) - 1) >> lR;
+            nslots = g.Vh / 8 / (16 >> lR);            // patches
+            grid = nslots * a.ngroups;
+            block = HOP_BLOCK;
+        }
     }
     const int rmode = red ? red->mode : 0;
     a.w = nullptr; a.partials = nullptr;
