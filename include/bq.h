@@ -40,8 +40,8 @@
  * DEVICE pointers; the library never keeps them after the call returns.  The handle owns its gauge
  * copies, clover blocks and solver workspace.  Calls on one handle must not run concurrently.
  * Unless a `stream` argument says otherwise, work is enqueued on the CUDA legacy default stream and
- * the call returns without synchronising (bq_solve and bq_gauge_load synchronise before returning).  The solver and
- * the bq_blas_* / bq_bench_* hooks run on a stream the handle owns — a blocking stream, i.e. ordered with the legacy
+ * the call returns without synchronising (bq_solve and bq_gauge_load synchronise before returning).  The solver (and
+ * the test / benchmark hooks of bq_test.h) run on a stream the handle owns — a blocking stream, i.e. ordered with the legacy
  * default stream exactly as the legacy stream is with itself — because batches of solver iterations are replayed as
  * CUDA graphs and the legacy stream cannot be captured.
  * ---------------------------------------------------------------------------------------------
@@ -62,7 +62,7 @@ typedef enum {
     BQ_EINVAL = 1,           /* NULL pointer, bad enum, |phase| != 1, non-positive tolerance ...            */
     BQ_EODD_EXTENT = 2,      /* an extent is odd or < 2 (checkerboard needs even L_mu)                    */
     BQ_ENOGAUGE = 3,         /* apply / solve before bq_gauge_load                                        */
-    BQ_ENOCLOVER = 4,        /* reserved                                                                  */
+    BQ_ENOCLOVER = 4,        /* a clover kernel was asked for but no clover term exists (csw = 0 / not built) */
     BQ_ESINGULAR_CLOVER = 5, /* a 6x6 clover block is not positive definite (Cholesky failed)             */
     BQ_ECUDA = 6,            /* CUDA runtime error or no device; text in bq_last_error                    */
     BQ_ENOMEM = 7,           /* device allocation failed                                                  */
@@ -125,10 +125,11 @@ bq_status bq_wilson_apply(bq_lattice* lat, void* out, const void* in, double kap
  * The first call for a given (csw, kappa) after bq_gauge_load builds the blocks and their inverses (Cholesky in
  * fp64) and caches them; out == NULL && in == NULL means "build only".
  *   out(x) = A(x) in(x)   (inverse = 0)   or   A(x)^-1 in(x)   (inverse = 1),   x of `parity` (BQ_FULL: all sites).
- * in/out: internal-layout DEVICE buffers of precision `prec`; out may equal in.  Legacy default stream.
+ * in/out: internal-layout DEVICE buffers of precision `prec`; out may equal in.  The apply is one kernel launch on `stream`
+ * (a cudaStream_t, NULL = legacy default stream), no host synchronisation; a build synchronises.
  * Errors: BQ_ENOGAUGE, BQ_ESINGULAR_CLOVER (build), BQ_EINVAL, BQ_ECUDA. */
 bq_status bq_clover_apply(bq_lattice* lat, double csw, double kappa, void* out, const void* in, bq_parity parity,
-                          int inverse, bq_prec prec);
+                          int inverse, bq_prec prec, void* stream);
 
 /* Full Wilson-clover matrix of Eq. 1 on the whole lattice, internal layout ([even | odd] buffers):
  *   out = D in = A in - kappa H in;   csw = 0 gives the Wilson matrix. */
@@ -223,65 +224,6 @@ bq_status bq_solve_multi(bq_lattice* lat, const double* b, double* x, int nrhs, 
  * receives the 12 solutions in the canonical layout, solution k = 3*id + ic first index.  info: 12 entries or NULL. */
 bq_status bq_propagator(bq_lattice* lat, const int* src_site /*[4]*/, double* S, double kappa, double tol,
                         const bq_solve_opts* opts, bq_solve_info* info /*[12]*/);
-
-/* The same operator with the BiCGStab inner products fused into the epilogue of its second hop kernel (SURVEY A6
- * (iii), (v): no separate reduction pass over the result), exposed for tests:
- *   w != NULL: dots[0..1] = <w, out>;      w == NULL: dots[0..1] = <out, in>, dots[2] = <out, out>
- * (<a,b> = sum conj(a_i) b_i).  The sums are taken over the values of out BEFORE they are rounded to the storage
- * precision (BQ_HALF: before the per-site renormalisation), per thread in the compute type, in fp64 across threads,
- * in a fixed order.  w: internal-layout even-site field of precision prec.  dots: HOST doubles.  Synchronises. */
-bq_status bq_schur_apply_dots(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw,
-                              bq_prec prec, bq_recon recon, const void* w, double* dots /*[3]*/);
-
-/* Launch accounting for benchmarks: out[0] = kernels launched through this handle since creation,
- * out[1..3] = hop-kernel launches with fp64 / fp32 / half storage (each is 1320 flop x Vh sites). */
-bq_status bq_get_counters(const bq_lattice* lat, unsigned long long* out /*[4]*/);
-
-/* Fused BLAS-1 on one-parity internal-layout fields, exposed for tests and benchmarks.
- * All complex scalars are (re, im) pairs of doubles on the HOST; results are written to HOST doubles after a
- * stream synchronise.  <a,b> = sum conj(a_i) b_i.  Reductions are accumulated in fp64 for BQ_FP64 and in fp32
- * per thread, fp64 across threads, for BQ_FP32 / BQ_HALF; the summation order is fixed (bitwise reproducible). */
-bq_status bq_blas_norm2(bq_lattice* lat, const void* a, bq_prec prec, double* result);
-bq_status bq_blas_cdot(bq_lattice* lat, const void* a, const void* b, bq_prec prec, double* result /*[2]*/);
-/* y <- y + alpha x */
-bq_status bq_blas_caxpy(bq_lattice* lat, const double* alpha /*[2]*/, const void* x, void* y, bq_prec prec);
-/* BiCGStab update (iv): x += alpha p + omega s;  r = s - omega t;  returns |r|^2 and <rhat, r>. */
-bq_status bq_blas_bicg_update(bq_lattice* lat, const double* alpha, const double* omega, const void* p, const void* s,
-                              const void* t, const void* rhat, void* x, void* r, bq_prec prec,
-                              double* r_norm2, double* rhat_r /*[2]*/);
-
-/* Benchmark hook: device time (CUDA events on the library's stream, after one warm-up launch per set) of ONE
- * internal kernel of the hot path, averaged over `reps` back-to-back launches that rotate over `nsets` (1..16) sets
- * of scratch vectors allocated inside the call, so that a launch does not find its operands in L2.
- * bytes_per_launch = the kernel's ALGORITHMIC bytes (every operand read once, every result written
- * once).  BQ_K_HOP* launch on even output sites; the clover variants need csw != 0.  Synchronises. */
-typedef enum {
-    BQ_K_HOP = 0,            /* out = -kappa H in                                   (A3, epilogue 0)                 */
-    BQ_K_HOP_XPAY = 1,       /* out = z + kappa H in                                (A3, epilogue 1; Wilson M^ step 2) */
-    BQ_K_HOP_CLOVINV = 2,    /* out = -kappa A^-1 H in                              (A3+A5, clover M^ step 1)        */
-    BQ_K_HOP_CLOV_XPAY = 3,  /* out = A z + kappa H in                              (A3+A5, clover M^ step 2)        */
-    BQ_K_SCHUR = 4,          /* out = M^ in (two hop launches)                      (A7)                             */
-    BQ_K_NORM2 = 5,          /* |a|^2                                               (A6)                             */
-    BQ_K_P_UPDATE = 6,       /* p = r + beta (p - omega v)                          (A6 i)                           */
-    BQ_K_ALPHA = 7,          /* <rhat, v> -> alpha                                  (A6 v)                           */
-    BQ_K_S_UPDATE = 8,       /* s = r - alpha v                                     (A6 ii)                          */
-    BQ_K_OMEGA = 9,          /* <t,s>, <t,t> -> omega                               (A6 iii)                         */
-    BQ_K_FINAL = 10,         /* x += alpha p + omega s; r = s - omega t; |r|^2; <rhat,r>   (A6 iv)                   */
-    BQ_K_BICG_ITER = 11,     /* one whole inner BiCGStab iteration as bq_solve runs it: 4 hops (two of them with
-                                fused inner products) + 3 BLAS-1 kernels                    (A8)                     */
-    BQ_K_HOP_XPAY_ALPHA = 12,   /* out = [A] z + kappa H in and <w, out> -> alpha           (A3 [+A5] + A6 v)        */
-    BQ_K_HOP_XPAY_OMEGA = 13,   /* out = [A] z + kappa H in and <out,z>, <out,out> -> omega  (A3 [+A5] + A6 iii)     */
-    BQ_K_BICG_ITER_UNFUSED = 14 /* the same iteration with the two inner products as separate kernels (4 + 5)        */
-} bq_kernel_id;
-bq_status bq_bench_kernel(bq_lattice* lat, int which, bq_prec prec, bq_recon recon, double csw, double kappa, int reps,
-                          int nsets, double* us_per_launch, double* bytes_per_launch);
-
-/* The same for the multi-rhs kernels (BQ_K_HOP, BQ_K_HOP_XPAY, BQ_K_HOP_CLOVINV, BQ_K_HOP_CLOV_XPAY, BQ_K_SCHUR,
- * BQ_K_BICG_ITER = one batched inner iteration of bq_solve_multi):
- * one launch processes nrhs right-hand sides; bytes_per_launch counts links and clover blocks once and the spinors
- * once per right-hand side. */
-bq_status bq_bench_kernel_multi(bq_lattice* lat, int which, bq_prec prec, bq_recon recon, double csw, double kappa,
-                                int nrhs, int reps, int nsets, double* us_per_launch, double* bytes_per_launch);
 
 #ifdef __cplusplus
 }

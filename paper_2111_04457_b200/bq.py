@@ -1,4 +1,4 @@
-"""Thin ctypes binding of libbq.so (include/bq.h) — argument marshalling only.
+"""Thin ctypes binding of libbq.so (include/bq.h; test and benchmark hooks: include/bq_test.h) — argument marshalling only.
 
 Every function has the name and argument order of its C counterpart; every step of the path runs in the
 library's CUDA kernels.  torch is used only to own device memory (tensors -> raw pointers) and streams.
@@ -74,7 +74,7 @@ def lib():
         L.bq_field_import.argtypes = [_vp, _vp, _vp, _i, _i, _vp]
         L.bq_field_export.argtypes = [_vp, _vp, _vp, _i, _i, _vp]
         L.bq_wilson_apply.argtypes = [_vp, _vp, _vp, _d, _i, _i, _i, _vp]
-        L.bq_clover_apply.argtypes = [_vp, _d, _d, _vp, _vp, _i, _i, _i]
+        L.bq_clover_apply.argtypes = [_vp, _d, _d, _vp, _vp, _i, _i, _i, _vp]
         L.bq_dirac_apply.argtypes = [_vp, _vp, _vp, _d, _d, _i, _i, _vp]
         L.bq_schur_apply.argtypes = [_vp, _vp, _vp, _vp, _d, _d, _i, _i, _vp]
         L.bq_schur_apply_dots.argtypes = [_vp, _vp, _vp, _vp, _d, _d, _i, _i, _vp, _dp]
@@ -165,8 +165,8 @@ def bq_wilson_apply(h, out, inp, kappa, parity, prec=BQ_FP32, recon=BQ_RECON18, 
     _check(h, lib().bq_wilson_apply(h, _ptr(out), _ptr(inp), kappa, parity, prec, recon, _stream_ptr(stream)))
 
 
-def bq_clover_apply(h, csw, kappa, out, inp, parity, inverse, prec):
-    _check(h, lib().bq_clover_apply(h, csw, kappa, _ptr(out), _ptr(inp), parity, int(inverse), prec))
+def bq_clover_apply(h, csw, kappa, out, inp, parity, inverse, prec, stream=None):
+    _check(h, lib().bq_clover_apply(h, csw, kappa, _ptr(out), _ptr(inp), parity, int(inverse), prec, stream))
 
 
 def bq_dirac_apply(h, out, inp, kappa, csw, prec, recon=BQ_RECON18, stream=None):
@@ -231,10 +231,11 @@ def bq_propagator(h, src_site, S, kappa, tol, opts: bq_solve_opts | None = None,
 
 
 def bq_get_counters(h):
-    """{'launches': all kernels, 'hop_fp64' / 'hop_fp32' / 'hop_half': hop-kernel launches} since handle creation."""
-    out = (ctypes.c_ulonglong * 4)()
+    """{'launches': all kernels, 'hop_fp64' / 'hop_fp32' / 'hop_half': hop applications per right-hand side,
+    'ls': launches of the link-stationary multi-rhs kernel} since handle creation."""
+    out = (ctypes.c_ulonglong * 5)()
     _check(h, lib().bq_get_counters(h, out))
-    return {"launches": out[0], "hop_fp64": out[1], "hop_fp32": out[2], "hop_half": out[3]}
+    return {"launches": out[0], "hop_fp64": out[1], "hop_fp32": out[2], "hop_half": out[3], "ls": out[4]}
 
 
 BQ_K = {"hop": 0, "hop_xpay": 1, "hop_clovinv": 2, "hop_clov_xpay": 3, "schur": 4, "norm2": 5, "p_update": 6, "alpha": 7,

@@ -39,7 +39,7 @@ def _nvcc() -> str:
 
 def _source_hash() -> str:
     h = hashlib.sha256()
-    names = sorted(os.listdir(CSRC)) + ["../../include/bq.h"]
+    names = sorted(os.listdir(CSRC)) + ["../../include/bq.h", "../../include/bq_test.h"]
     for n in names:
         p = os.path.join(CSRC, n)
         if os.path.isfile(p):

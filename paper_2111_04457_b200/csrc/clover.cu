@@ -278,7 +278,7 @@ bq_status bq_get_clover(bq_lattice* lat, int prec, int inverse, const void** out
 }
 
 template <int PREC>
-__global__ void __launch_bounds__(128) clover_mul_kernel(int Vh, void* __restrict__ out, const void* in, const void* __restrict__ cl) {
+__global__ void __launch_bounds__(128) clover_mul_kernel(int Vh, void* out, const void* in, const void* __restrict__ cl) {   // out may be in (in-place apply)
     const int h = blockIdx.x * blockDim.x + threadIdx.x;
     if (h >= Vh) return;
     typename Prec<PREC>::comp v[24];
@@ -297,7 +297,7 @@ bq_status bq_clover_mul(bq_lattice* lat, void* out, const void* in, const void* 
 }
 
 extern "C" bq_status bq_clover_apply(bq_lattice* lat, double csw, double kappa, void* out, const void* in, bq_parity parity,
-                                     int inverse, bq_prec prec) {
+                                     int inverse, bq_prec prec, void* stream) {
     if (!lat) return BQ_EINVAL;
     if (!lat->have_gauge) return bq_set_error(lat, BQ_ENOGAUGE, "bq_clover_apply: no gauge field loaded");
     if ((out == nullptr) != (in == nullptr)) return bq_set_error(lat, BQ_EINVAL, "bq_clover_apply: only one of out/in is NULL");
@@ -313,7 +313,7 @@ extern "C" bq_status bq_clover_apply(bq_lattice* lat, double csw, double kappa, 
         if (parity != BQ_FULL && p != (int)parity) continue;
         const size_t off = (parity == BQ_FULL) ? p * fb : 0;
         BQ_TRY(bq_clover_mul(lat, static_cast<char*>(out) + off, static_cast<const char*>(in) + off,
-                             static_cast<const char*>(cl) + p * cb, prec, 0));
+                             static_cast<const char*>(cl) + p * cb, prec, static_cast<cudaStream_t>(stream)));
     }
     return BQ_OK;
 }

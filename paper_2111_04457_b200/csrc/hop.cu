@@ -14,10 +14,27 @@ BQ_HOP_EXTERN(BQ_HALF, BQ_RECON18)
 BQ_HOP_EXTERN(BQ_HALF, BQ_RECON12)
 #undef BQ_HOP_EXTERN
 
+// cuTensorMapEncodeTiled, looked up in the driver at run time (the library does not link against libcuda)
+ls_encode_fn ls_get_encoder() {
+    static ls_encode_fn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) == cudaSuccess && qr == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<ls_encode_fn>(p);
+        else
+            cudaGetLastError();
+    }
+    return fn;
+}
+
 extern "C" bq_status bq_get_counters(const bq_lattice* lat, unsigned long long* out) {
     if (!lat || !out) return BQ_EINVAL;
     out[0] = lat->n_launch;
     for (int p = 0; p < 3; p++) out[1 + p] = lat->n_hop[p];
+    out[4] = lat->n_ls;
     return BQ_OK;
 }
 

@@ -48,6 +48,10 @@ template <typename C> struct HopArgs {
     size_t s_in, s_out, s_z, s_w;
     // patch mapping of the multi-rhs kernel (patch != 0): a CTA = 4 right-hand sides x a 2 x 2 patch of tiles in (y, z)
     int patch, nxt, ngroups;
+    // solver: device-resident state(s) of the right-hand side(s); a set `done` flag (converged / broken down) turns the
+    // launch (single field) or that right-hand side (multi-rhs) into a no-op, as in the BLAS-1 kernels, so that the rest of
+    // a batch of iterations costs nothing once the solve is over (nullptr: always run)
+    const SolverScalars* done;
 };
 
 // Grid-wide sum for the hop kernel's reduction epilogues (no clusters here: the hop grid is one CTA per 128 sites).
@@ -81,6 +85,7 @@ template <int MODE> __global__ void __launch_bounds__(HOP_RED_FINAL_BLOCK) k_hop
     constexpr int NRED = MODE == 1 ? 2 : 3;
     partials += (size_t)blockIdx.x * n * NRED;
     sc += blockIdx.x;
+    if (sc->done) return;      // the hop that feeds this reduction did not run (HopArgs::done)
     __shared__ double s_w[NRED][HOP_RED_FINAL_BLOCK / 32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double acc[NRED];
@@ -252,6 +257,7 @@ template <int PREC, int RECON, int EPI, bool CPLX, int RED, bool DAG = false>
 __global__ void __launch_bounds__(HOP_BLOCK, PREC == BQ_FP64 ? HOP_MINB_64 : (PREC == BQ_FP32 ? HOP_MINB_LO : HOP_MINB_HALF))
 hop_kernel(const HopArgs<typename Prec<PREC>::comp> a) {
     using C = typename Prec<PREC>::comp;
+    if (a.done && a.done->done) return;     // uniform over the grid
     const int h = blockIdx.x * HOP_BLOCK + threadIdx.x;
     if (RED == 0) {
         if (h >= a.Vh) return;
@@ -349,6 +355,7 @@ hop_kernel_mrhs(const HopArgs<typename Prec<PREC>::comp> a) {
         h = (blockIdx.x * a.T + tl) * 8 + s8;
         live = tl < a.T && h < a.Vh;     // the CTA is padded to whole warps
     }
+    if (a.done && live && a.done[rhs].done) live = false;     // this right-hand side has stopped: its output is left alone
     const char* in = static_cast<const char*>(a.in) + (size_t)rhs * a.s_in;
     char* out = static_cast<char*>(a.out) + (size_t)rhs * a.s_out;
     const char* zp_ = a.z ? static_cast<const char*>(a.z) + (size_t)rhs * a.s_z : nullptr;
@@ -362,6 +369,8 @@ hop_kernel_mrhs(const HopArgs<typename Prec<PREC>::comp> a) {
         hop_block_partial_mrhs<RED == 1 ? 2 : 3>(v, a.partials, R, T, rhs0, a.nrhs, slot, nslots);
     }
 }
+
+#include "hop_ls.cuh"
 
 template <int PREC, int RECON>
 bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const void* z, double scale, int p, const void* gauge,
@@ -404,6 +413,10 @@ bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const void* z, 
         }
     }
     const int rmode = red ? red->mode : 0;
+    a.done = lat->hop_done;
+    // link-stationary kernel (hop_ls.cuh) where the geometry, the operand strides and the epilogue allow
+    const bool use_ls = multi && !(dag && rmode) && ls_eligible<PREC>(lat, m, in, z, rmode == 1 ? red->w : nullptr, cl_mode);
+    if (use_ls) nslots = (g.Lxh / 8) * (g.L[1] / LS_BY) * (g.L[2] / LS_BZ) * (g.L[3] / LS_BT);
     a.w = nullptr; a.partials = nullptr;
     if (rmode) {
         if ((rmode != 1 && rmode != 2) || !red->sc || (rmode == 1 && !red->w) || !z)
@@ -425,6 +438,20 @@ bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const void* z, 
     else return bq_set_error(lat, BQ_EINVAL, "bq_hop: unsupported epilogue (cl_mode=%d, z=%p)", cl_mode, z);
     // the dagger hop exists without fused reductions (the CG of the normal equations reduces on the plain hop)
     if (dag && rmode) return bq_set_error(lat, BQ_EINVAL, "bq_hop: the dagger hop has no fused reduction");
+    if (use_ls) {
+        if constexpr (PREC != BQ_FP64) {
+            BQ_TRY((ls_launch<PREC, RECON>(lat, a, cplx, rmode, dag, m, lat->hop_done, stream)));
+            BQ_CHECK_LAUNCH(lat);
+            lat->n_hop[PREC] += nrhs;
+            lat->n_ls++;
+            if (rmode) {
+                if (rmode == 1) k_hop_red_final<1><<<nrhs, HOP_RED_FINAL_BLOCK, 0, stream>>>(lat->hop_partials, nslots, red->sc);
+                else k_hop_red_final<2><<<nrhs, HOP_RED_FINAL_BLOCK, 0, stream>>>(lat->hop_partials, nslots, red->sc);
+                BQ_CHECK_LAUNCH(lat);
+            }
+            return BQ_OK;
+        }
+    }
 #define BQ_HOP_LAUNCH_DAG(E)                                                                        \
     do {                                                                                            \
         if (multi) {                                                                                \

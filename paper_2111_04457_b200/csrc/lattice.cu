@@ -74,6 +74,8 @@ extern "C" bq_status bq_lattice_create(int Lx, int Ly, int Lz, int Lt, const dou
     {
         const char* e = getenv("BQ_MRHS_PATCH");      // A/B switch of the multi-rhs hop's thread mapping (hop_kernels.cuh)
         lat->mrhs_patch = e ? (int)strtol(e, nullptr, 0) : 1;
+        const char* ls = getenv("BQ_MRHS_LS");        // A/B switch: link-stationary multi-rhs hop (hop_ls.cuh)
+        lat->mrhs_ls = ls ? atoi(ls) : 1;
         const char* gph = getenv("BQ_GRAPH");         // A/B switch: CUDA-graph replay of the solver's iteration batches (solve.cu)
         lat->use_graphs = gph ? atoi(gph) : 1;
     }

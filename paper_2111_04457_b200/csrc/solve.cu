@@ -211,10 +211,19 @@ static bq_status run_batch(bq_lattice* lat, SolverWork* w, int method, int prec,
     return BQ_OK;
 }
 
+// While one of these lives, every hop launched through the handle tests the `done` flag of its right-hand side's solver
+// state at entry (HopArgs::done) exactly as the BLAS-1 kernels do: once a right-hand side has converged (or broken
+// down) the rest of the batch of iterations already enqueued for it — hops included — costs a launch and nothing else.
+struct HopDoneScope {
+    bq_lattice* lat;
+    HopDoneScope(bq_lattice* l, const SolverScalars* sc) : lat(l) { lat->hop_done = sc; }
+    ~HopDoneScope() { lat->hop_done = nullptr; }
+};
+
 // Inner BiCGStab on M^ e = ir (e0 = 0) for every right-hand side of the batch (w->blas.nrhs), each with its own
 // device-resident scalars; rhs k stops when |r_k|^2 <= w->h_stop2[k] or after max_iter iterations.  A right-hand
-// side that has stopped keeps its iterate frozen (its update kernels exit early) while the others go on; the hop
-// kernels always process the whole batch.  On return w->h_sc holds the final device states.
+// side that has stopped keeps its iterate frozen (its update kernels and its share of the hop kernels exit early) while
+// the others go on.  On return w->h_sc holds the final device states.
 // Textbook van der Vorst recurrences (reading O4).
 static bq_status inner_bicgstab(bq_lattice* lat, SolverWork* w, double kappa, double csw, int prec, int recon, int max_iter,
                                 int check_every) {
@@ -230,6 +239,7 @@ static bq_status inner_bicgstab(bq_lattice* lat, SolverWork* w, double kappa, do
     BQ_CUDA(lat, cudaMemcpyAsync(c.stop2s, w->h_stop2, sizeof(double) * n, cudaMemcpyHostToDevice, s));
     BQ_TRY(bicg_init(lat, c, prec, w->ir, 0.0, true));
     int launched = 0;
+    const HopDoneScope done_scope(lat, c.sc);
     // the two inner products on v and t ride on the second hop of M^ (hop.cu, RED epilogues): 7 kernels per iteration
     const HopRed red_alpha{1, w->irhat, c.sc}, red_omega{2, nullptr, c.sc};
     for (;;) {
@@ -265,6 +275,7 @@ static bq_status inner_cgnr(bq_lattice* lat, SolverWork* w, double kappa, double
     BQ_TRY(bq_schur_red(lat, w->irhat, w->ir, w->itmp, kappa, csw, prec, recon, s, nullptr, mrhs, true));   // r_N = M^^dag r
     BQ_TRY(cg_init(lat, c, prec, w->irhat, w->ip, 0.0, true));
     int launched = 0;
+    const HopDoneScope done_scope(lat, c.sc);
     const HopRed red_qq{2, nullptr, c.sc};
     for (;;) {
         const int batch = (max_iter - launched) < check_every ? (max_iter - launched) : check_every;
@@ -630,6 +641,7 @@ static bq_status solve_lex(bq_lattice* lat, SolverWork* w, const bq_solve_opts& 
             cudaMemcpyAsync(irhat, ir, fb, cudaMemcpyDeviceToDevice, s);
             LEX_TRY(bicg_init(lat, c, prec, ir, rel * rel));
             int launched = 0;
+            const HopDoneScope done_scope(lat, c.sc);
             for (;;) {
                 const int batch = (max_inner - launched) < check_every ? (max_inner - launched) : check_every;
                 for (int k = 0; k < batch; k++) {
@@ -869,11 +881,11 @@ extern "C" bq_status bq_bench_kernel(bq_lattice* lat, int which, bq_prec prec, b
             case BQ_K_HOP: bytes = 8 * link_b + 2 * spin_b; return bq_hop(lat, v0, v1, nullptr, -kappa, 0, prec, recon, nullptr, 0, s);
             case BQ_K_HOP_XPAY: bytes = 8 * link_b + 3 * spin_b; return bq_hop(lat, v0, v1, v2, kappa, 0, prec, recon, nullptr, 0, s);
             case BQ_K_HOP_CLOVINV:
-                if (!clover) return bq_set_error(lat, BQ_EINVAL, "bq_bench_kernel: clover kernels need csw != 0");
+                if (!clover) return bq_set_error(lat, BQ_ENOCLOVER, "bq_bench_kernel: clover kernels need csw != 0");
                 bytes = 8 * link_b + 2 * spin_b + clov_b;
                 return bq_hop(lat, v0, v1, nullptr, -kappa, 1, prec, recon, static_cast<const char*>(cli) + cb, 1, s);
             case BQ_K_HOP_CLOV_XPAY:
-                if (!clover) return bq_set_error(lat, BQ_EINVAL, "bq_bench_kernel: clover kernels need csw != 0");
+                if (!clover) return bq_set_error(lat, BQ_ENOCLOVER, "bq_bench_kernel: clover kernels need csw != 0");
                 bytes = 8 * link_b + 3 * spin_b + clov_b;
                 return bq_hop(lat, v0, v1, v2, kappa, 0, prec, recon, cl, 2, s);
             case BQ_K_SCHUR:
@@ -997,11 +1009,11 @@ extern "C" bq_status bq_bench_kernel_multi(bq_lattice* lat, int which, bq_prec p
             case BQ_K_HOP: bytes = 8 * link_b + nrhs * 2 * spin_b; return bq_hop(lat, v0, v1, nullptr, -kappa, 0, prec, recon, nullptr, 0, s, nullptr, &m);
             case BQ_K_HOP_XPAY: bytes = 8 * link_b + nrhs * 3 * spin_b; return bq_hop(lat, v0, v1, v2, kappa, 0, prec, recon, nullptr, 0, s, nullptr, &m);
             case BQ_K_HOP_CLOVINV:
-                if (!clover) return bq_set_error(lat, BQ_EINVAL, "bq_bench_kernel_multi: clover kernels need csw != 0");
+                if (!clover) return bq_set_error(lat, BQ_ENOCLOVER, "bq_bench_kernel_multi: clover kernels need csw != 0");
                 bytes = 8 * link_b + clov_b + nrhs * 2 * spin_b;
                 return bq_hop(lat, v0, v1, nullptr, -kappa, 1, prec, recon, static_cast<const char*>(cli) + cb, 1, s, nullptr, &m);
             case BQ_K_HOP_CLOV_XPAY:
-                if (!clover) return bq_set_error(lat, BQ_EINVAL, "bq_bench_kernel_multi: clover kernels need csw != 0");
+                if (!clover) return bq_set_error(lat, BQ_ENOCLOVER, "bq_bench_kernel_multi: clover kernels need csw != 0");
                 bytes = 8 * link_b + clov_b + nrhs * 3 * spin_b;
                 return bq_hop(lat, v0, v1, v2, kappa, 0, prec, recon, cl, 2, s, nullptr, &m);
             case BQ_K_SCHUR:

@@ -1,4 +1,4 @@
-"""C-ABI library checks that need no GPU: libbq.so builds, loads and exports every symbol include/bq.h declares;
+"""C-ABI library checks that need no GPU: libbq.so builds, loads and exports every symbol include/*.h declares;
 argument validation that happens before any device work; no silent CPU fallback."""
 import ctypes
 import os
@@ -17,10 +17,24 @@ def bq():
     return _bq
 
 
-def declared_symbols():
-    with open(os.path.join(ROOT, "include", "bq.h")) as f:
-        text = re.sub(r"/\*.*?\*/", "", f.read(), flags=re.S)
-    return sorted(set(re.findall(r"\b(bq_[a-z0-9_]+)\s*\(", text)))
+HEADERS = ("bq.h", "bq_test.h")     # the product boundary, and the test / benchmark hooks
+
+
+def declared_symbols(headers=HEADERS):
+    names = set()
+    for hname in headers:
+        with open(os.path.join(ROOT, "include", hname)) as f:
+            text = re.sub(r"/\*.*?\*/", "", f.read(), flags=re.S)
+        names |= set(re.findall(r"\b(bq_[a-z0-9_]+)\s*\(", text))
+    return sorted(names)
+
+
+def test_product_header_holds_only_the_boundary():
+    """include/bq.h is SURVEY §8(b)'s boundary; the bq_blas_* / bq_bench_* / counter hooks live in bq_test.h."""
+    prod = declared_symbols(("bq.h",))
+    assert not [n for n in prod if n.startswith(("bq_blas_", "bq_bench_")) or n in ("bq_get_counters", "bq_schur_apply_dots")]
+    for n in ("bq_lattice_create", "bq_gauge_load", "bq_wilson_apply", "bq_clover_apply", "bq_solve"):
+        assert n in prod
 
 
 def test_every_declared_symbol_is_exported(bq):
@@ -81,7 +95,7 @@ def test_header_is_plain_c_and_links(bq, tmp_path):
     import subprocess
     names = declared_symbols()
     src = tmp_path / "abi_check.c"
-    lines = ['#include "bq.h"', "#include <stddef.h>", "typedef void (*fn_t)(void);", "int main(void) {", "    fn_t fns[] = {"]
+    lines = ['#include "bq.h"', '#include "bq_test.h"', "#include <stddef.h>", "typedef void (*fn_t)(void);", "int main(void) {", "    fn_t fns[] = {"]
     lines += [f"        (fn_t){n}," for n in names]
     lines += ["    };", "    bq_solve_opts o = {0};", "    bq_solve_info info;", "    o.inner_prec = BQ_HALF; o.method = BQ_CGNR; o.lexical = 0; o.x0_zero = 1;",
               "    info.phase_seconds[4] = 0.0; info.inner_iters = (int)BQ_MODE_DDAGD;",

@@ -241,3 +241,93 @@ def test_propagator_is_fig1_of_the_paper(bq):
             if k in (0, 7):
                 x_ref, _ = bqo.bicgstab(U, b, kappa, tol=1e-12, A=A)
                 assert np.linalg.norm(S[k] - x_ref) / np.linalg.norm(x_ref) < 1e-8
+
+
+# ---------------------------------------------------------------------------------------------------
+# link-stationary multi-rhs hop (hop_ls.cuh): links in registers for all right-hand sides of a 8 x 4 x 4 x 2 block of
+# sites, spinor blocks + halos through shared memory by TMA.  Taken for fp32 / half storage when Lx % 16 == 0 and
+# Ly % 4 == Lz % 4 == Lt % 2 == 0.  Lattices: one block in y, z, t (every halo wraps onto the block itself); several
+# blocks per direction; three x tiles per row; wrap-around blocks in every direction with general boundary phases.
+# ---------------------------------------------------------------------------------------------------
+LS_LATTICES = [(16, 4, 4, 2), (16, 8, 4, 4), (32, 4, 8, 2), (48, 4, 4, 4)]
+
+
+@pytest.mark.parametrize("L", LS_LATTICES)
+@pytest.mark.parametrize("prec", [1, 2])
+@pytest.mark.parametrize("nrhs", [2, 3, 12])
+def test_hop_ls_parity(bq, L, prec, nrhs):
+    import torch
+    kappa = 0.125
+    U = inputs.gauge(L, 81, 0.5)
+    psis = rhs_set(L, nrhs, 82)
+    recon = nrhs % 2
+    for bc in (None, GENERAL_BC):
+        with bq.Lattice(L, bc) as lat:
+            bq.bq_gauge_load(lat.h, U)
+            for p in (0, 1):
+                src = import_multi(bq, lat, psis, prec, 1 - p)
+                fb = bq.bq_field_bytes(lat.h, prec, p)
+                out = torch.zeros(nrhs * fb, dtype=torch.uint8, device="cuda")
+                n0 = bq.bq_get_counters(lat.h)["ls"]
+                bq.bq_wilson_apply_multi(lat.h, out, src, nrhs, kappa, p, prec, recon)
+                assert bq.bq_get_counters(lat.h)["ls"] == n0 + 1, "the link-stationary kernel did not take this launch"
+                got = export_multi(bq, lat, out, nrhs, prec, p)
+                one = lat.field(prec, p)
+                for k in range(nrhs):
+                    ref = bqo.hop_restricted(U, psis[k], kappa, p, bc=bc)
+                    assert relmax(got[k], ref) < TOL[prec], (L, prec, nrhs, k, p)
+                    bq.bq_wilson_apply(lat.h, one, src[k * fb:(k + 1) * fb], kappa, p, prec, recon)
+                    assert torch.equal(one, out[k * fb:(k + 1) * fb]), (L, prec, nrhs, k, p)
+
+
+@pytest.mark.parametrize("prec", [1, 2])
+def test_ls_full_apply_and_schur(bq, prec):
+    """[even | odd] buffers (operand stride = two fields), the xpay epilogue, and the Schur operator through the
+    link-stationary kernel, every right-hand side against the oracle."""
+    import torch
+    L, kappa, nrhs = (16, 4, 8, 4), 0.12, 5
+    U = inputs.gauge(L, 83, 0.4)
+    psis = rhs_set(L, nrhs, 84)
+    par = (inputs.site_parity(L) == 0)[..., None, None]
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        src = import_multi(bq, lat, psis, prec, bq.BQ_FULL)
+        out = torch.zeros_like(src)
+        n0 = bq.bq_get_counters(lat.h)["ls"]
+        bq.bq_wilson_apply_multi(lat.h, out, src, nrhs, kappa, bq.BQ_FULL, prec, bq.BQ_RECON18)
+        assert bq.bq_get_counters(lat.h)["ls"] == n0 + 2
+        for k, got in enumerate(export_multi(bq, lat, out, nrhs, prec, bq.BQ_FULL)):
+            assert relmax(got, bqo.dirac_apply(U, psis[k], kappa)) < TOL[prec], k
+        src_e = import_multi(bq, lat, psis, prec, bq.BQ_EVEN)
+        out_e, tmp = torch.zeros_like(src_e), torch.zeros_like(src_e)
+        bq.bq_schur_apply_multi(lat.h, out_e, src_e, tmp, nrhs, kappa, 0.0, prec)
+        assert bq.bq_get_counters(lat.h)["ls"] == n0 + 4
+        for k, got in enumerate(export_multi(bq, lat, out_e, nrhs, prec, bq.BQ_EVEN)):
+            ref = bqo.schur_apply(U, np.where(par, psis[k], 0), kappa)
+            assert relmax(got, ref) < 2 * TOL[prec], (prec, k)
+
+
+@pytest.mark.parametrize("inner,method", [(1, 0), (2, 0), (1, 1)])
+def test_solve_multi_ls(bq, inner, method):
+    """Batched Wilson solve whose inner hops all run through the link-stationary kernel (fused inner products, per-rhs
+    done flags, dagger hops for CGNR); one zero and one tiny right-hand side stop early while the others go on."""
+    L, kappa, nrhs = (16, 4, 4, 8), 0.1215, 6
+    U = inputs.gauge(L, 85, 0.5)
+    b = np.stack(rhs_set(L, nrhs, 86))
+    b[1] = 0
+    b[2] *= 1e-6
+    x = np.zeros_like(b)
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        infos = bq.bq_solve_multi(lat.h, b, x, nrhs, kappa, 1e-10, bq.bq_solve_opts(inner_prec=inner, method=method, check_every=3))
+        assert bq.bq_get_counters(lat.h)["ls"] > 0
+        x1 = np.zeros_like(b[0])
+        info1 = bq.bq_solve(lat.h, b[0], x1, kappa, 1e-10, bq.bq_solve_opts(inner_prec=inner, method=method, check_every=3))
+    for k in range(nrhs):
+        assert infos[k].status == 0
+        if k == 1:
+            assert not x[k].any()
+        else:
+            assert oracle_residual(U, x[k], b[k], kappa) <= 1e-10, k
+    assert np.linalg.norm(x[0] - x1) / np.linalg.norm(x1) < 1e-9
+    assert abs(infos[0].inner_iters - info1.inner_iters) <= 1      # the fused inner products are summed in another order
