@@ -36,12 +36,15 @@
 #define LS_BZ 4
 #endif
 #ifndef LS_BT
-#define LS_BT 2
+#define LS_BT 1
 #endif
 
 constexpr int LS_NT = LS_BY * LS_BZ * LS_BT;      // tiles (rows of 8 sites) per block
 constexpr int LS_THREADS = 8 * LS_NT;             // one thread per output site
 constexpr int LS_MAX_RHS = 32;                    // right-hand sides per launch (active list = one ballot)
+// 255 registers per thread either way: one CTA of 256 threads per SM, or two of 128 — two CTAs overlap one's prologue (its
+// 8 x 18 link loads per thread, 147 KB per 256 sites, nothing to compute yet) with the other's arithmetic
+constexpr int LS_MINB = LS_THREADS <= 128 ? 2 : 1;
 static_assert(LS_NT % 8 == 0 && LS_THREADS % 32 == 0 && LS_THREADS <= 1024, "block shape");
 static_assert((LS_BY * LS_BZ) % 4 == 0 && (LS_BZ * LS_BT) % 4 == 0 && (LS_BY * LS_BT) % 4 == 0,
               "every halo region must be a multiple of 4 tiles (128-byte alignment of the TMA destinations in half storage)");
@@ -58,7 +61,7 @@ template <int PREC> struct LsGeom {
     static constexpr int ZM = YP + LS_BZ * LS_BT * TS, ZP = ZM + LS_BY * LS_BT * TS;
     static constexpr int TM = ZP + LS_BY * LS_BT * TS, TP = TM + LS_BY * LS_BZ * HT;
     static constexpr int X = TP + LS_BY * LS_BZ * HT;     // x halo sites, 8 to a pseudo tile
-    static constexpr int STAGE = X + (LS_NT / 8) * TS;
+    static constexpr int STAGE = (X + (LS_NT / 8) * TS + 127) / 128 * 128;
     static constexpr int TX = X;                          // bytes a stage receives through TMA (everything but the x halo)
     static constexpr int OPER = LS_NT * TS;               // one interior-only operand buffer (z or w)
     static constexpr int NXC = (PREC == BQ_HALF ? 4 : NW) * LS_NT;   // cp.async copies of the x halo per stage
@@ -224,14 +227,14 @@ template <int PREC> __device__ __forceinline__ void ls_load_site(const char* til
     }
 }
 
-template <int EPI, int RED> __host__ __device__ constexpr int ls_stages() { return EPI == 0 ? 3 : 2; }
+template <int EPI, int RED> __host__ __device__ constexpr int ls_stages() { return (EPI == 0 && LS_MINB == 1) ? 3 : 2; }
 template <int PREC, int EPI, int RED> __host__ __device__ constexpr size_t ls_smem_bytes() {
     return (size_t)ls_stages<EPI, RED>() * LsGeom<PREC>::STAGE + (EPI == 1 ? LsGeom<PREC>::OPER : 0) + (RED == 1 ? LsGeom<PREC>::OPER : 0) +
-           128 /* mbarriers, active list */ + (RED ? 2 * 3 * (LS_THREADS / 32) * sizeof(double) : 0);
+           256 /* mbarriers, active list */ + (RED ? 2 * 3 * (LS_THREADS / 32) * sizeof(double) : 0);
 }
 
 template <int PREC, int RECON, int EPI, bool CPLX, int RED, bool DAG>
-__global__ void __launch_bounds__(LS_THREADS, 1) hop_ls_kernel(const __grid_constant__ LsParams<typename Prec<PREC>::comp> P) {
+__global__ void __launch_bounds__(LS_THREADS, LS_MINB) hop_ls_kernel(const __grid_constant__ LsParams<typename Prec<PREC>::comp> P) {
     using C = typename Prec<PREC>::comp;
     using G = LsGeom<PREC>;
     constexpr int NS = ls_stages<EPI, RED>();
@@ -242,8 +245,8 @@ __global__ void __launch_bounds__(LS_THREADS, 1) hop_ls_kernel(const __grid_cons
     unsigned char* const wbuf = zbuf + (EPI == 1 ? G::OPER : 0);
     unsigned char* const ctl = wbuf + (RED == 1 ? G::OPER : 0);
     unsigned long long* const bars = reinterpret_cast<unsigned long long*>(ctl);     // full[NS], fullz
-    int* const act = reinterpret_cast<int*>(ctl + 64);                              // [0] = count, [1] = mask of active rhs
-    double* const s_red = reinterpret_cast<double*>(ctl + 128);                     // [2][NRED][warps]
+    int* const act = reinterpret_cast<int*>(ctl + 64);                              // [0] = count, [1] = mask, [2..] = list of active rhs
+    double* const s_red = reinterpret_cast<double*>(ctl + 256);                     // [2][NRED][warps]
     const HopArgs<C>& a = P.a;
 
     const int tid = threadIdx.x, s8 = tid & 7, tl = tid >> 3;
@@ -269,6 +272,7 @@ __global__ void __launch_bounds__(LS_THREADS, 1) hop_ls_kernel(const __grid_cons
         } else {
             mask = a.nrhs >= 32 ? 0xffffffffu : ((1u << a.nrhs) - 1u);
         }
+        if (mask & (1u << tid)) act[2 + __popc(mask & ((1u << tid) - 1u))] = tid;    // act[2 + i] = i-th active right-hand side
         if (tid == 0) {
             act[0] = __popc(mask);
             act[1] = (int)mask;
@@ -279,10 +283,8 @@ __global__ void __launch_bounds__(LS_THREADS, 1) hop_ls_kernel(const __grid_cons
     }
     __syncthreads();
     const int nact = act[0];
-    const unsigned int amask = (unsigned int)act[1];
     if (nact == 0) return;
-    // i-th active right-hand side
-    auto rhs_of = [&](int i) { return (int)__fns(amask, 0, i + 1); };
+    auto rhs_of = [&](int i) { return act[2 + i]; };
 
     // ---- this thread's x-halo copy (cp.async): row jr of the block, 16-byte word jk (half storage: jk == 3 is the norm) ----
     const bool xcopy = tid < G::NXC;

@@ -28,7 +28,7 @@ def main():
                     help="also time bq_solve_multi on NRHS point sources against NRHS separate bq_solve calls (device buffers)")
     ap.add_argument("--only", default="", help="comma-separated kernel names to run (e.g. 'hop,hop x12'); default all")
     args = ap.parse_args()
-    only = [v.strip() for v in args.only.split(",") if v.strip()]
+    only = [v.strip().replace("_x", " x") for v in args.only.split(",") if v.strip()]     # "hop_x12" = "hop x12"
     import torch
     from . import bq, build, inputs
     assert torch.cuda.is_available(), "kbench needs a CUDA device"
