@@ -315,17 +315,28 @@ __global__ void __launch_bounds__(LS_THREADS, LS_MINB) hop_ls_kernel(const __gri
     auto fill = [&](int i) {       // input tiles of the i-th active right-hand side -> stage i % NS   (all threads)
         const int k = rhs_of(i), s = i % NS;
         const unsigned int sb = ls_smem_u32(stage0 + s * G::STAGE), bar = ls_smem_u32(bars + s);
-        if (tid == 0) {
-            ls_mbar_expect_tx(bar, G::TX);
-            const int tk = k * P.tk_in;
-            ls_tma5(sb + G::C, &P.m.in_c, bar, 0, xt, y0, z0, t0 + tk);
-            ls_tma5(sb + G::YM, &P.m.in_y, bar, 0, xt, ym, z0, t0 + tk);
-            ls_tma5(sb + G::YP, &P.m.in_y, bar, 0, xt, yp, z0, t0 + tk);
-            ls_tma5(sb + G::ZM, &P.m.in_z, bar, 0, xt, y0, zm, t0 + tk);
-            ls_tma5(sb + G::ZP, &P.m.in_z, bar, 0, xt, y0, zp, t0 + tk);
-            // backward t hop: (1 + g_t) keeps the upper spin pair, forward: (1 - g_t) the lower one (exchanged for DAG)
-            ls_tma5(sb + G::TM, &P.m.in_t, bar, DAG ? EH : 0, xt, y0, z0, tm + tk);
-            ls_tma5(sb + G::TP, &P.m.in_t, bar, DAG ? 0 : EH, xt, y0, z0, tp + tk);
+        // the 7 tensor copies are issued by lane 0 of 4 different warps (a transfer may complete before the expect_tx of
+        // thread 0 is counted: the phase cannot end before all 1 + LS_THREADS arrivals are in)
+        if ((tid & 31) == 0) {
+            const int tk = k * P.tk_in, wq = (tid >> 5) & 3;
+            if (wq == 0) {
+                if (tid == 0) {
+                    ls_mbar_expect_tx(bar, G::TX);
+                    ls_tma5(sb + G::C, &P.m.in_c, bar, 0, xt, y0, z0, t0 + tk);
+                }
+            } else if (tid < 128) {
+                if (wq == 1) {
+                    ls_tma5(sb + G::YM, &P.m.in_y, bar, 0, xt, ym, z0, t0 + tk);
+                    ls_tma5(sb + G::YP, &P.m.in_y, bar, 0, xt, yp, z0, t0 + tk);
+                } else if (wq == 2) {
+                    ls_tma5(sb + G::ZM, &P.m.in_z, bar, 0, xt, y0, zm, t0 + tk);
+                    ls_tma5(sb + G::ZP, &P.m.in_z, bar, 0, xt, y0, zp, t0 + tk);
+                } else {
+                    // backward t hop: (1 + g_t) keeps the upper spin pair, forward: (1 - g_t) the lower one (exchanged for DAG)
+                    ls_tma5(sb + G::TM, &P.m.in_t, bar, DAG ? EH : 0, xt, y0, z0, tm + tk);
+                    ls_tma5(sb + G::TP, &P.m.in_t, bar, DAG ? 0 : EH, xt, y0, z0, tp + tk);
+                }
+            }
         }
         if (xcopy) {
             const char* src = static_cast<const char*>(a.in) + (size_t)k * a.s_in + xsrc;
