@@ -7,13 +7,20 @@
 Workload (config.workload): BASELINE.json config 3 — 32^3x64, fp32 storage, 18-real links, even-odd Wilson hop
 D_eo applied to one parity (the lattice north_star's target is quoted on; it is the largest single-GPU hop config
 whose metric is the headline).  A step = one bq_wilson_apply(EVEN) = one hop-kernel launch over Vh sites.
-  value     GFlop/s at 1320 flop/site with all fields resident in HBM (CUDA events around K launches).
+  value     GFlop/s at 1320 flop/site with all fields resident in HBM: CUDA events around EXACTLY K launches; the K launches
+            are cut into 5 consecutive repeats by extra events, and `repeats` reports each one and their median (SURVEY §8(d):
+            ">= 10 warm-up, >= 100 timed launches, median of >= 5 repeats" — met when K >= 500).
   roofline  algorithmic bytes (768 B/site fp32/18) / the same per-launch time, against the
             measured copy bandwidth in MEASURED_PEAKS.json.
   e2e       the same flop count through the public solve call with HOST buffers: bq_solve (BASELINE.json config 4,
             Wilson-clover, fp32 inner / fp64 outer BiCGStab to 1e-10) from a pinned host b to a pinned host x;
             hop flops executed / wall time, host<->device copies and layout conversion inside the timed region.
-  cpu_baseline  the CPU oracle (oracle/, as it stands) computing the same hop on a bounded sample of the sites.
+            e2e.value counts the USEFUL hops only (iterations the solver accepted; hops enqueued after convergence return at
+            entry and are reported beside it as hop_launches vs hop_launches_useful).
+  cpu_baseline  the CPU oracle (oracle/, as it stands) computing the same hop on a bounded sample of the sites, and
+            (cpu_baseline.solve) the oracle's BiCGStab on configs 1 and 4, wall time and iterations, on the host cores.
+  extras    per-kernel device times of the rest of the path; config2 (16^4 fp32 hop x 1000, L2-resident) and config5
+            (48^3x96 half-inner solve) of BASELINE.json.
 Inputs are synthetic and seeded (paper_2111_04457_b200/inputs).  The working set (805 MB per apply) is far larger
 than the 126 MB L2 and the timed loop rotates over 4 (source, result) pairs, so no explicit L2 flush is needed.
 N > 1: replicas only — every rank runs the same workload on its own GPU, no data-path collective.
@@ -51,7 +58,7 @@ def parse_args():
     ap.add_argument("--recon", type=int, default=18, choices=[18, 12])
     ap.add_argument("--skip-e2e", action="store_true")
     ap.add_argument("--skip-cpu", action="store_true")
-    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--e2e-steps", type=int, default=5)
     return ap.parse_args()
 
 
@@ -68,56 +75,81 @@ def workload_name(L, prec, recon):
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+    """SM clock and throttle reasons during the timed region (B200_PROFILING.md clocks line), sampled IN PROCESS through
+    NVML by a polling thread (an nvidia-smi loop at 50 ms cannot see a 2.4 ms region), plus one sample taken synchronously
+    right before and one right after the region.  mark(name) labels the samples that follow, so that the timed region
+    and the rest of the GPU section can be told apart."""
 
     def __init__(self, index):
         self.index = index
-        self.proc = None
-        self.path = os.path.join(ROOT, "gpurun_out", f"clocks_{index}.csv")
+        self.samples = []          # (label, sm_mhz, reasons bitmask)
+        self.label = "idle"
+        self.h = None
+        self.stop_flag = False
+        self.thread = None
+        self.max_mhz = None
+        try:
+            import pynvml
+            self.nv = pynvml
+            pynvml.nvmlInit()
+            # NVML indexes physical devices: honour CUDA_VISIBLE_DEVICES when it is a plain list of indices
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+            ids = [v for v in vis.split(",") if v.strip().isdigit()]
+            phys = int(ids[index]) if index < len(ids) else index
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.h = None
+
+    def _one(self):
+        if self.h is None:
+            return
+        try:
+            mhz = float(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM))
+            try:
+                reasons = int(self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+            except Exception:
+                reasons = int(self.nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+            self.samples.append((self.label, mhz, reasons))
+        except Exception:
+            pass
+
+    def _loop(self):
+        while not self.stop_flag:
+            self._one()
+            time.sleep(0.0005)
 
     def start(self):
-        os.makedirs(os.path.dirname(self.path), exist_ok=True)
-        q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
-             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-             "clocks_event_reasons.sw_power_cap")
-        try:
-            self.f = open(self.path, "w")
-            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={q}", "--format=csv,noheader,nounits",
-                                          "-lms", "50"], stdout=self.f, stderr=subprocess.DEVNULL)
-        except Exception:
-            self.proc = None
+        import threading
+        self._one()
+        self.thread = threading.Thread(target=self._loop, daemon=True)
+        self.thread.start()
+
+    def mark(self, label):
+        self._one()
+        self.label = label
+        self._one()
 
     def stop(self):
-        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
-        if self.proc is None:
+        self.stop_flag = True
+        if self.thread is not None:
+            self.thread.join(timeout=2)
+        out = {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": []}
+        if not self.samples:
             return out
-        self.proc.terminate()
-        try:
-            self.proc.wait(timeout=5)
-        except Exception:
-            self.proc.kill()
-        self.f.close()
-        sm, mx, reasons = [], [], set()
-        try:
-            with open(self.path) as f:
-                for line in f:
-                    c = [v.strip() for v in line.split(",")]
-                    if len(c) < 9:
-                        continue
-                    try:
-                        sm.append(float(c[1])); mx.append(float(c[2]))
-                    except ValueError:
-                        continue
-                    for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), c[5:9]):
-                        if v.lower().startswith("active"):
-                            reasons.add(name)
-        except OSError:
-            pass
-        if sm:
-            out["sm_mhz"] = float(np.median(sm))
-            out["sm_max_mhz"] = float(max(mx))
-            out["samples"] = len(sm)
-        out["reasons"] = sorted(reasons)
+        names = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap"}
+        timed = [x for x in self.samples if x[0] == "timed"]
+        load = [x for x in self.samples if x[0] != "idle"]
+        use = timed if timed else load
+        out["sm_mhz"] = float(np.median([x[1] for x in use]))
+        out["samples"] = len(use)
+        out["sm_mhz_gpu_section"] = float(np.median([x[1] for x in load])) if load else None
+        out["samples_gpu_section"] = len(load)
+        bits = 0
+        for x in load:
+            bits |= x[2]
+        out["reasons"] = sorted(v for k, v in names.items() if bits & k)
+        out["how"] = "NVML in process: polling thread (0.5 ms) + synchronous samples at the region boundaries; sm_mhz = median over the timed hop loop"
         return out
 
 
@@ -183,6 +215,105 @@ def run_reference(args, L):
     print(json.dumps(line))
 
 
+def config2_hop(bq, inputs, torch):
+    """BASELINE config 2: 16^4, fp32, 18-real, kappa = 0.125, links exp(i*0.3*H): bq_wilson_apply(EVEN) x 1000 back to back on the
+    same (source, result) pair (reading S12).  The working set (25 MB) lives in L2: NOT an HBM measurement."""
+    L = (16, 16, 16, 16)
+    seed = inputs.BASE_SEED + 2
+    U = inputs.gauge(L, seed, 0.3)
+    psi = inputs.spinor(L, seed)
+    Vh = 16 ** 4 // 2
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        src = lat.import_field(psi, bq.BQ_FP32, bq.BQ_ODD)
+        out = lat.field(bq.BQ_FP32, bq.BQ_EVEN)
+        for _ in range(20):
+            bq.bq_wilson_apply(lat.h, out, src, 0.125, bq.BQ_EVEN, bq.BQ_FP32, bq.BQ_RECON18)
+        first = None
+        us = []
+        for rep in range(5):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(1000):
+                bq.bq_wilson_apply(lat.h, out, src, 0.125, bq.BQ_EVEN, bq.BQ_FP32, bq.BQ_RECON18)
+            e1.record()
+            torch.cuda.synchronize()
+            us.append(e0.elapsed_time(e1))          # ms per 1000 applies = us per apply
+            if first is None:
+                first = out.clone()
+        same = bool(torch.equal(first, out))
+    med = float(np.median(us))
+    return {"what": "BASELINE config 2: 16^4 fp32/18 bq_wilson_apply(EVEN) x 1000 back to back (same source), median of 5 repeats; "
+                    "L2-resident working set (25 MB): not an HBM measurement", "us_per_apply": med, "us_per_apply_repeats": us,
+            "gflops": FLOP_PER_SITE * Vh / med / 1e3, "effective_gbs": 768 * Vh / med / 1e3, "first_equals_last_bitwise": same}
+
+
+def config5_solve(bq, inputs, torch):
+    """BASELINE config 5: 48^3x96 Wilson, kappa = 0.1235, links exp(i*0.7*H), half-storage inner BiCGStab (fp16 + per-site fp32
+    norm, fp32 reductions), fp64 defect-correction outer loop to 1e-10.  b, x device-resident; the SECOND and later calls are
+    timed (stores, workspace and graphs exist)."""
+    L = (48, 48, 48, 96)
+    seed = inputs.BASE_SEED + 5
+    U = inputs.gauge(L, seed, 0.7)
+    b = torch.from_numpy(inputs.spinor(L, seed)).cuda()
+    x = torch.zeros_like(b)
+    Vh = 48 ** 3 * 96 // 2
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        del U
+        opts = bq.bq_solve_opts(inner_prec=bq.BQ_HALF, recon=bq.BQ_RECON18, csw=0.0, x0_zero=1)
+        ts, info = [], None
+        for it in range(4):
+            k0 = bq.bq_get_counters(lat.h)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            info = bq.bq_solve(lat.h, b, x, 0.1235, 1e-10, opts)
+            torch.cuda.synchronize()
+            ts.append(time.perf_counter() - t0)
+            k1 = bq.bq_get_counters(lat.h)
+        hops = sum(int(k1[k] - k0[k]) for k in ("hop_fp64", "hop_fp32", "hop_half"))
+        idle = sum(int(k1[k] - k0[k]) for k in ("idle_fp64", "idle_fp32", "idle_half"))
+    t = float(np.median(ts[1:]))
+    return {"what": "BASELINE config 5: 48^3x96 Wilson kappa=0.1235, half-storage inner / fp64 outer BiCGStab to 1e-10, device-resident b and x, "
+                    "zero initial guess; median wall time of calls 2-4 (first call builds the half gauge store and the workspace)",
+            "time_to_solution_s": t, "first_call_s": ts[0], "times_s": ts[1:], "device_seconds": info.seconds,
+            "inner_iters": info.inner_iters, "outer_cycles": info.outer_cycles, "true_rel_residual": info.true_rel_residual,
+            "hop_launches": hops, "hop_launches_useful": hops - idle,
+            "phase_seconds": dict(zip(("import", "prepare", "iterate", "reconstruct+residual", "export"), list(info.phase_seconds)))}
+
+
+def oracle_solves(L4):
+    """The oracle's own BiCGStab (plain fp64, full lattice, not even-odd) on BASELINE configs 1 and 4, on the host cores."""
+    from oracle import bqo
+    from paper_2111_04457_b200 import inputs
+    out = {"kind": "oracle", "cores": bqo.num_threads()}
+    L1 = (4, 4, 4, 4)
+    U = inputs.gauge(L1, inputs.BASE_SEED + 1, 0.3)
+    b = inputs.spinor(L1, inputs.BASE_SEED + 1)
+    t0 = time.perf_counter()
+    x, info = bqo.bicgstab(U, b, 0.12, tol=1e-12)
+    out["config1"] = {"seconds": time.perf_counter() - t0, "iters": info["iters"], "relres": info["relres"],
+                      "what": "4^4 Wilson kappa=0.12, tol 1e-12"}
+    try:
+        import psutil
+        free_gb = psutil.virtual_memory().available / 2 ** 30
+    except Exception:
+        free_gb = 0.0
+    if free_gb < 24:       # the dense 12x12 clover term of 32^3x64 is 4.8 GB, U 1.2 GB, ~10 work vectors of 0.4 GB
+        out["config4"] = {"skipped": f"only {free_gb:.0f} GB of host memory available"}
+        return out
+    U = inputs.gauge(L4, inputs.BASE_SEED + 4, 0.5)
+    b = inputs.spinor(L4, inputs.BASE_SEED + 4)
+    t0 = time.perf_counter()
+    A = bqo.clover_build(U, 1.0, 0.1215)
+    t_build = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    x, info = bqo.bicgstab(U, b, 0.1215, tol=1e-10, A=A)
+    out["config4"] = {"seconds": time.perf_counter() - t0, "clover_build_seconds": t_build, "iters": info["iters"], "relres": info["relres"],
+                      "what": f"{L4[0]}^3x{L4[3]} Wilson-clover csw=1 kappa=0.1215, tol 1e-10, dense 12x12 site term (clover build timed apart)"}
+    return out
+
+
 def main():
     args = parse_args()
     L = tuple(int(v) for v in args.lattice.split(","))
@@ -220,19 +351,30 @@ def main():
         bq.bq_wilson_apply(lat.h, outs[i % NSETS], srcs[i % NSETS], kappa, bq.BQ_EVEN, prec, recon)
     c0 = bq.bq_get_counters(lat.h)
     sampler = ClockSampler(local_rank)
-    barrier()
     sampler.start()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ev0.record()                                   # legacy default stream = the stream the kernels are launched on
-    for i in range(args.steps):
-        bq.bq_wilson_apply(lat.h, outs[i % NSETS], srcs[i % NSETS], kappa, bq.BQ_EVEN, prec, recon)
-    ev1.record()
+    # EXACTLY `steps` launches between ev[0] and ev[-1]; extra events cut them into NREP consecutive repeats
+    NREP = 5 if args.steps >= 5 else 1
+    cuts = [args.steps * r // NREP for r in range(NREP + 1)]
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(NREP + 1)]
     barrier()
-    ms = ev0.elapsed_time(ev1)
-    clocks = sampler.stop()
+    torch.cuda.synchronize()
+    sampler.mark("timed")
+    ev[0].record()                                 # legacy default stream = the stream the kernels are launched on
+    for r in range(NREP):
+        for i in range(cuts[r], cuts[r + 1]):
+            bq.bq_wilson_apply(lat.h, outs[i % NSETS], srcs[i % NSETS], kappa, bq.BQ_EVEN, prec, recon)
+        ev[r + 1].record()
+    torch.cuda.synchronize()
+    sampler.mark("gpu")
+    barrier()
+    ms = ev[0].elapsed_time(ev[-1])
+    rep_us = [ev[r].elapsed_time(ev[r + 1]) * 1e3 / max(1, cuts[r + 1] - cuts[r]) for r in range(NREP)]
     c1 = bq.bq_get_counters(lat.h)
     launches = int(c1["launches"] - c0["launches"])
     ms = replicas.max_over_ranks(ms)
+    repeats = {"n": NREP, "launches_per_repeat": [cuts[r + 1] - cuts[r] for r in range(NREP)], "us_per_launch": rep_us,
+               "median_us_per_launch": float(np.median(rep_us)),
+               "protocol": "the K timed launches cut into consecutive repeats by CUDA events; median over repeats (rank 0)"}
     ms_per_step = ms / args.steps
     gflops = world * FLOP_PER_SITE * Vh / (ms_per_step * 1e-3) / 1e9
     bps = BYTES_PER_SITE[(args.prec, args.recon)]
@@ -257,7 +399,7 @@ def main():
         lat4 = bq.Lattice(L)
         bq.bq_gauge_load(lat4.h, U4)
         opts = bq.bq_solve_opts(inner_prec=bq.BQ_FP32, recon=bq.BQ_RECON18, csw=1.0, x0_zero=1)   # x is output only
-        times, infos, hops = [], [], []
+        times, infos, hops, idle = [], [], [], []
         for it in range(1 + args.e2e_steps):      # first solve = warm-up (clover build, workspace allocation)
             k0 = bq.bq_get_counters(lat4.h)
             barrier()
@@ -269,16 +411,21 @@ def main():
             if it > 0:
                 times.append(dt); infos.append(info)
                 hops.append(sum(int(k1[k] - k0[k]) for k in ("hop_fp64", "hop_fp32", "hop_half")))
-        dt = replicas.max_over_ranks(max(times))
+                idle.append(sum(int(k1[k] - k0[k]) for k in ("idle_fp64", "idle_fp32", "idle_half")))
+        tmed = float(np.median(times))
+        dt = replicas.max_over_ranks(tmed)
+        useful = hops[-1] - idle[-1]
         nbytes = b_host.numel() * 16
-        e2e = {"value": world * FLOP_PER_SITE * Vh * hops[-1] / dt / 1e9, "unit": "GFlop/s",
+        e2e = {"value": world * FLOP_PER_SITE * Vh * useful / dt / 1e9, "unit": "GFlop/s",
                "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
                "what": "bq_solve host->host, BASELINE config 4 (32^3x64 Wilson-clover csw=1 kappa=0.1215, fp32 inner / fp64 outer "
-                       "BiCGStab to 1e-10, zero initial guess declared with opts.x0_zero): hop flops executed / wall time incl. H2D of b, "
-                       "layout conversion, solve, D2H of x",
-               "time_to_solution_s": dt, "device_seconds": infos[-1].seconds,
+                       "BiCGStab to 1e-10, zero initial guess declared with opts.x0_zero): flops of the USEFUL hops (4 per accepted inner iteration + "
+                       "the fixed ones of the outer loop; hops enqueued after convergence return at entry and are not counted) / wall time "
+                       "incl. H2D of b, layout conversion, solve, D2H of x; median of the timed solves",
+               "time_to_solution_s": dt, "times_s": times, "device_seconds": infos[-1].seconds,
                "phase_seconds": dict(zip(("h2d+import", "prepare", "iterate", "reconstruct+residual", "export+d2h"), list(infos[-1].phase_seconds))), "inner_iters": infos[-1].inner_iters,
-               "outer_cycles": infos[-1].outer_cycles, "hop_launches": hops[-1], "true_rel_residual": infos[-1].true_rel_residual}
+               "outer_cycles": infos[-1].outer_cycles, "hop_launches": hops[-1], "hop_launches_useful": useful,
+               "true_rel_residual": infos[-1].true_rel_residual}
         # the plain operator through host buffers, for completeness: canonical fp64 field on the (pinned) host -> H2D -> layout
         # conversion -> ONE hop -> conversion back -> D2H.  PCIe moves 2 x 402 MB for 1.38 GFlop: transfer-bound by construction.
         psi_host = torch.from_numpy(psi).pin_memory()
@@ -314,15 +461,25 @@ def main():
                                          ("bicg_iter_fp32_wilson", "bicg_iter", 1, 0, 0.0), ("bicg_iter_fp32_clover", "bicg_iter", 1, 0, 1.0),
                                          ("bicg_iter_half_wilson", "bicg_iter", 2, 0, 0.0)):
             extras[name] = gbs(*bq.bq_bench_kernel(lat.h, which, pr, rc, csw, 0.1215, 100, 3))
-        for name, which, csw in (("hop_fp32_18_x12", "hop", 0.0), ("bicg_iter_fp32_wilson_x12", "bicg_iter", 0.0)):
-            us, nb = bq.bq_bench_kernel_multi(lat.h, which, 1, 12, 0, csw, 0.1215, 16, 2)
+        for name, which, pr, rc, csw in (("hop_half_12", "hop", 2, 1, 0.0), ("bicg_iter_fp64_wilson", "bicg_iter", 0, 0, 0.0)):
+            extras[name] = gbs(*bq.bq_bench_kernel(lat.h, which, pr, rc, csw, 0.1215, 100, 3))
+        for name, which, pr, csw in (("hop_fp32_18_x12", "hop", 1, 0.0), ("hop_fp64_18_x12", "hop", 0, 0.0), ("hop_half_18_x12", "hop", 2, 0.0),
+                                     ("bicg_iter_fp32_wilson_x12", "bicg_iter", 1, 0.0)):
+            us, nb = bq.bq_bench_kernel_multi(lat.h, which, pr, 12, 0, csw, 0.1215, 16, 2)
             extras[name] = dict(gbs(us, nb), us_per_rhs=us / 12, nrhs=12,
                                 gflops_hop=(FLOP_PER_SITE * Vh * 12 / us / 1e3 if which == "hop" else None))
+        extras["config2"] = config2_hop(bq, inputs, torch)
+        lat.close()                      # free config 3's stores before the 48^3x96 lattice is set up
+        lat = None
+        extras["config5"] = config5_solve(bq, inputs, torch)
 
+    clocks = sampler.stop()
     cpu = None
     if rank == 0 and world == 1 and not args.skip_cpu:
         cpu, _, _ = oracle_hop_sample(U, psi, kappa, L)
-    lat.close()
+        cpu["solve"] = oracle_solves(L)
+    if lat is not None:
+        lat.close()
     replicas.finish()
     if rank != 0:
         return
@@ -335,7 +492,8 @@ def main():
                    "l2": f"inputs larger than L2, no flush: {bps * Vh / 1e6:.0f} MB per apply (links streamed once) and {NSETS} (source, result) "
                          "pairs used round-robin, so no operand of a launch is left in the 126 MB L2 by the previous ones",
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
-        "hbm_gbs": achieved, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks, "extras": extras,
+        "hbm_gbs": achieved, "roofline": roofline, "repeats": repeats, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+        "extras": extras,
     }
     print(json.dumps(line))
 

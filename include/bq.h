@@ -181,7 +181,8 @@ typedef struct {
                           (the paper's `lex` operator); bq_solve only, BQ_BICGSTAB only       */
     int x0_zero;       /* 1: the initial guess is zero and x is output only — its contents on entry are neither read nor
                           transferred (saves one host-to-device copy and one layout conversion per right-hand side)           */
-    void* stream;      /* reserved, must be NULL (legacy default stream)                                               */
+    void* stream;      /* cudaStream_t whose earlier work (e.g. the kernels producing b) the solve waits for; NULL = none.
+                          The solve runs on a stream of the handle and synchronises before returning                       */
 } bq_solve_opts;
 
 typedef struct {

@@ -110,6 +110,34 @@ def _ptr(t):
     return t.data_ptr()
 
 
+_DIMS = {}       # handle -> (Lx, Ly, Lz, Lt), recorded by bq_lattice_create: sizes the canonical arrays are checked against
+
+
+def _canonical(h, a, nfields, name, reals_per_site=24):
+    """Pointer of a canonical fp64 array after checking what the C side cannot: dtype complex128 / float64, C-contiguous,
+    nfields * reals_per_site * V doubles.  Nothing is copied or converted: a wrong array is an error (BQ_EINVAL), not a guess."""
+    if isinstance(a, int) or a is None:
+        return a
+    if isinstance(a, np.ndarray):
+        per = {np.dtype(np.complex128): 2.0, np.dtype(np.float64): 1.0, np.dtype(np.uint8): 0.125}.get(a.dtype)
+        contiguous, n = a.flags["C_CONTIGUOUS"], a.size
+    else:
+        import torch
+        per = {torch.complex128: 2.0, torch.float64: 1.0, torch.uint8: 0.125}.get(a.dtype)
+        contiguous, n = a.is_contiguous(), a.numel()
+    if per is None:
+        raise BqError(BQ_EINVAL, f"{name}: dtype must be complex128 (or float64, or raw uint8 bytes), got {a.dtype}")
+    doubles = n * per
+    if not contiguous:
+        raise BqError(BQ_EINVAL, f"{name}: array must be C-contiguous")
+    dims = _DIMS.get(h.value if hasattr(h, "value") else h)
+    if dims is not None:
+        want = nfields * reals_per_site * dims[0] * dims[1] * dims[2] * dims[3]
+        if doubles != want:
+            raise BqError(BQ_EINVAL, f"{name}: {doubles} doubles, expected {want} ({nfields} field(s) of {reals_per_site} reals x V)")
+    return _ptr(a)
+
+
 def _check(h, st, allow=()):
     if st != BQ_OK and st not in allow:
         msg = lib().bq_last_error(h).decode() if h else ""
@@ -133,10 +161,12 @@ def bq_lattice_create(Lx, Ly, Lz, Lt, bc_phase=None):
     st = lib().bq_lattice_create(Lx, Ly, Lz, Lt, bc, ctypes.byref(h))
     if st != BQ_OK:
         raise BqError(st, lib().bq_status_string(st).decode())
+    _DIMS[h.value] = (int(Lx), int(Ly), int(Lz), int(Lt))
     return h
 
 
 def bq_lattice_destroy(h):
+    _DIMS.pop(h.value if hasattr(h, "value") else h, None)
     return lib().bq_lattice_destroy(h)
 
 
@@ -154,11 +184,11 @@ def bq_field_bytes(h, prec, parity):
 
 
 def bq_field_import(h, internal, canonical, parity, prec, stream=None):
-    _check(h, lib().bq_field_import(h, _ptr(internal), _ptr(canonical), parity, prec, _stream_ptr(stream)))
+    _check(h, lib().bq_field_import(h, _ptr(internal), _canonical(h, canonical, 1, "canonical"), parity, prec, _stream_ptr(stream)))
 
 
 def bq_field_export(h, canonical, internal, parity, prec, stream=None):
-    _check(h, lib().bq_field_export(h, _ptr(canonical), _ptr(internal), parity, prec, _stream_ptr(stream)))
+    _check(h, lib().bq_field_export(h, _canonical(h, canonical, 1, "canonical"), _ptr(internal), parity, prec, _stream_ptr(stream)))
 
 
 def bq_wilson_apply(h, out, inp, kappa, parity, prec=BQ_FP32, recon=BQ_RECON18, stream=None):
@@ -207,7 +237,7 @@ def bq_schur_apply_dots(h, out, inp, tmp, kappa, csw, prec, recon=BQ_RECON18, w=
 def bq_solve(h, b, x, kappa, tol, opts: bq_solve_opts | None = None, raise_on_fail=True):
     """b, x: canonical complex128 arrays (numpy host arrays or torch CUDA tensors); x is in/out.  Returns bq_solve_info."""
     info = bq_solve_info()
-    st = lib().bq_solve(h, _ptr(b), _ptr(x), kappa, tol, ctypes.byref(opts) if opts is not None else None,
+    st = lib().bq_solve(h, _canonical(h, b, 1, "b"), _canonical(h, x, 1, "x"), kappa, tol, ctypes.byref(opts) if opts is not None else None,
                         ctypes.byref(info))
     _check(h, st, allow=() if raise_on_fail else (BQ_ENOTCONVERGED, BQ_EBREAKDOWN))
     return info
@@ -215,8 +245,11 @@ def bq_solve(h, b, x, kappa, tol, opts: bq_solve_opts | None = None, raise_on_fa
 
 def bq_solve_multi(h, b, x, nrhs, kappa, tol, opts: bq_solve_opts | None = None, raise_on_fail=True):
     """b, x: [nrhs, Lt,Lz,Ly,Lx,4,3] complex128 (numpy host arrays or torch CUDA tensors); x is in/out.  Returns [bq_solve_info]."""
+    if nrhs < 1:
+        raise BqError(BQ_EINVAL, "bq_solve_multi: nrhs must be >= 1")
     infos = (bq_solve_info * nrhs)()
-    st = lib().bq_solve_multi(h, _ptr(b), _ptr(x), nrhs, kappa, tol, ctypes.byref(opts) if opts is not None else None, infos)
+    st = lib().bq_solve_multi(h, _canonical(h, b, nrhs, "b"), _canonical(h, x, nrhs, "x"), nrhs, kappa, tol,
+                              ctypes.byref(opts) if opts is not None else None, infos)
     _check(h, st, allow=() if raise_on_fail else (BQ_ENOTCONVERGED, BQ_EBREAKDOWN))
     return list(infos)
 
@@ -225,17 +258,19 @@ def bq_propagator(h, src_site, S, kappa, tol, opts: bq_solve_opts | None = None,
     """S: [12, Lt,Lz,Ly,Lx,4,3] complex128 output (numpy host array or torch CUDA tensor); src_site = (x, y, z, t)."""
     infos = (bq_solve_info * 12)()
     site = (_i * 4)(*[int(v) for v in src_site])
-    st = lib().bq_propagator(h, site, _ptr(S), kappa, tol, ctypes.byref(opts) if opts is not None else None, infos)
+    st = lib().bq_propagator(h, site, _canonical(h, S, 12, "S"), kappa, tol, ctypes.byref(opts) if opts is not None else None, infos)
     _check(h, st, allow=() if raise_on_fail else (BQ_ENOTCONVERGED, BQ_EBREAKDOWN))
     return list(infos)
 
 
 def bq_get_counters(h):
     """{'launches': all kernels, 'hop_fp64' / 'hop_fp32' / 'hop_half': hop applications per right-hand side,
-    'ls': launches of the link-stationary multi-rhs kernel} since handle creation."""
-    out = (ctypes.c_ulonglong * 5)()
+    'ls': launches of the link-stationary multi-rhs kernel, 'idle_*': hop applications that returned at entry because
+    their right-hand side had already converged (useful = hop_* - idle_*)} since handle creation."""
+    out = (ctypes.c_ulonglong * 8)()
     _check(h, lib().bq_get_counters(h, out))
-    return {"launches": out[0], "hop_fp64": out[1], "hop_fp32": out[2], "hop_half": out[3], "ls": out[4]}
+    return {"launches": out[0], "hop_fp64": out[1], "hop_fp32": out[2], "hop_half": out[3], "ls": out[4],
+            "idle_fp64": out[5], "idle_fp32": out[6], "idle_half": out[7]}
 
 
 BQ_K = {"hop": 0, "hop_xpay": 1, "hop_clovinv": 2, "hop_clov_xpay": 3, "schur": 4, "norm2": 5, "p_update": 6, "alpha": 7,

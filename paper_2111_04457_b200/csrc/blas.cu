@@ -129,7 +129,7 @@ template <int PREC> BLAS_KERNEL k_init(int Vh, const void* __restrict__ r, RedBu
         sc->omega[0] = 1; sc->omega[1] = 0;
         sc->iters = 0;
         sc->cg = 0;
-        sc->done = (r_[0] <= stop2) ? 1 : (r_[0] == 0.0 ? 1 : 0);
+        sc->done = (r_[0] > stop2) ? 0 : 1;      // also done when r2 is NaN or the threshold is infinite (a finished right-hand side)
     });
 }
 
@@ -526,12 +526,18 @@ bq_status blas_ctx_reserve(bq_lattice* lat, BlasCtx* c, int nrhs) {
     if (nrhs <= c->cap) return BQ_OK;
     blas_ctx_destroy(c);
     c->pstride = 4 * (c->grid / BLAS_CLUSTER);
-    BQ_CUDA(lat, cudaMalloc(&c->partials, sizeof(double) * c->pstride * nrhs));
-    BQ_CUDA(lat, cudaMalloc(&c->ticket, sizeof(unsigned int) * nrhs));
-    BQ_CUDA(lat, cudaMemset(c->ticket, 0, sizeof(unsigned int) * nrhs));
-    BQ_CUDA(lat, cudaMalloc(&c->sc, sizeof(SolverScalars) * nrhs));
-    BQ_CUDA(lat, cudaMemset(c->sc, 0, sizeof(SolverScalars) * nrhs));
-    BQ_CUDA(lat, cudaMalloc(&c->stop2s, sizeof(double) * nrhs));
+    // all or nothing: on any failure the context is left empty (cap = 0, no pointer set), never half allocated
+    cudaError_t e = cudaMalloc(&c->partials, sizeof(double) * c->pstride * nrhs);
+    if (e == cudaSuccess) e = cudaMalloc(&c->ticket, sizeof(unsigned int) * nrhs);
+    if (e == cudaSuccess) e = cudaMemset(c->ticket, 0, sizeof(unsigned int) * nrhs);
+    if (e == cudaSuccess) e = cudaMalloc(&c->sc, sizeof(SolverScalars) * nrhs);
+    if (e == cudaSuccess) e = cudaMemset(c->sc, 0, sizeof(SolverScalars) * nrhs);
+    if (e == cudaSuccess) e = cudaMalloc(&c->stop2s, sizeof(double) * nrhs);
+    if (e != cudaSuccess) {
+        blas_ctx_destroy(c);
+        return bq_set_error(lat, e == cudaErrorMemoryAllocation ? BQ_ENOMEM : BQ_ECUDA, "solver scratch for %d right-hand sides: %s", nrhs,
+                            cudaGetErrorString(e));
+    }
     c->cap = nrhs;
     return BQ_OK;
 }

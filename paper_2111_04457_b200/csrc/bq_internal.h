@@ -56,6 +56,8 @@ struct bq_lattice {
     unsigned long long n_launch;      // kernels launched through this handle
     unsigned long long n_hop[3];      // hop applications (per right-hand side) per storage precision
     unsigned long long n_ls;          // launches of the link-stationary multi-rhs hop kernel (hop_ls.cuh)
+    unsigned long long n_hop_idle[3]; // of n_hop: applications enqueued in a batch of solver iterations after their right-hand side had
+                                      // stopped — the kernel returned at entry (HopArgs::done), no flop was executed
     char err[512];
 };
 

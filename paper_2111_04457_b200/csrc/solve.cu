@@ -25,7 +25,7 @@ struct IterGraph {
     double kappa, csw;
     unsigned long long epoch;
     bool warm;                               // a batch with this key has run eagerly (lazy stores and scratch exist)
-    unsigned long long d_launch, d_hop[3];   // what one replay adds to the handle's launch counters
+    unsigned long long d_launch, d_hop[3], d_ls;   // what one replay adds to the handle's launch counters
 };
 
 struct SolverWork {
@@ -44,6 +44,8 @@ struct SolverWork {
     double* h_stop2;       // pinned host staging of the per-rhs inner thresholds, [rhs]
     cudaEvent_t ev0, ev1;
     cudaEvent_t evp[4];    // phase boundaries: import | prepare | iterate | finish | export (bq_solve_info.phase_seconds)
+    cudaStream_t side;     // second stream: the export + device-to-host copy of x runs here while the true residual is computed
+    cudaEvent_t ev_side;
     bool persistent_stage; double* stage;   // device staging buffer of one canonical field (import / export)
 };
 
@@ -87,6 +89,8 @@ void bq_solver_free(bq_lattice* lat) {
     if (w->ev0) cudaEventDestroy(w->ev0);
     if (w->ev1) cudaEventDestroy(w->ev1);
     for (cudaEvent_t& e : w->evp) if (e) cudaEventDestroy(e);
+    if (w->ev_side) cudaEventDestroy(w->ev_side);
+    if (w->side) cudaStreamDestroy(w->side);
     if (w->stage) cudaFree(w->stage);
     free(w);
     lat->work = nullptr;
@@ -99,12 +103,23 @@ static bq_status get_work(bq_lattice* lat, int inner_prec, SolverWork** out, int
         if (!w) return bq_set_error(lat, BQ_ENOMEM, "solver workspace: host allocation failed");
         w->inner_prec = -1;
         lat->work = w;
-        BQ_TRY(blas_ctx_create(lat, &w->blas));
-        w->blas_ok = true;
-        BQ_CUDA(lat, cudaEventCreate(&w->ev0));
-        BQ_CUDA(lat, cudaEventCreate(&w->ev1));
-        for (cudaEvent_t& e : w->evp) BQ_CUDA(lat, cudaEventCreate(&e));
-        BQ_CUDA(lat, cudaMalloc(&w->stage, (size_t)g.V * 24 * sizeof(double)));
+        // all or nothing: a half-built workspace must not survive (the next call would run with NULL streams / buffers)
+        auto init = [&]() -> bq_status {
+            BQ_TRY(blas_ctx_create(lat, &w->blas));
+            w->blas_ok = true;
+            BQ_CUDA(lat, cudaEventCreate(&w->ev0));
+            BQ_CUDA(lat, cudaEventCreate(&w->ev1));
+            for (cudaEvent_t& e : w->evp) BQ_CUDA(lat, cudaEventCreate(&e));
+            BQ_CUDA(lat, cudaEventCreate(&w->ev_side));
+            BQ_CUDA(lat, cudaStreamCreateWithFlags(&w->side, cudaStreamNonBlocking));
+            BQ_CUDA(lat, cudaMalloc(&w->stage, (size_t)g.V * 24 * sizeof(double)));
+            return BQ_OK;
+        };
+        const bq_status st = init();
+        if (st != BQ_OK) {
+            bq_solver_free(lat);
+            return st;
+        }
     }
     SolverWork* w = lat->work;
     if (w->nrhs < nrhs) {
@@ -150,9 +165,21 @@ static bq_status schur(bq_lattice* lat, void* out, const void* in, void* tmp, do
     return bq_schur_red(lat, out, in, tmp, kappa, csw, prec, recon, s, red, nrhs);
 }
 
-// copy the device-resident solver states of the nrhs right-hand sides of the current batch to w->h_sc
+// Publish the device-resident solver states of the nrhs right-hand sides of the current batch to w->h_sc (pinned, mapped host
+// memory) and wait for them.  A tiny kernel stores them straight through the mapped pointer — not a cudaMemcpyAsync: a
+// device-to-host copy would queue on the copy engine behind whatever else is going that way (the 400 MB of x that
+// bq_solve sends home on its side stream while the true residual is being polled).
+__global__ void k_publish(unsigned long long* __restrict__ host, const unsigned long long* __restrict__ dev, int n8) {
+    for (int i = threadIdx.x; i < n8; i += blockDim.x) host[i] = dev[i];
+    __threadfence_system();
+}
+static_assert(sizeof(SolverScalars) % 8 == 0, "SolverScalars is published in 8-byte pieces");
+
 static bq_status poll(bq_lattice* lat, SolverWork* w) {
-    BQ_CUDA(lat, cudaMemcpyAsync(w->h_sc, w->blas.sc, sizeof(SolverScalars) * w->blas.nrhs, cudaMemcpyDeviceToHost, w->blas.stream));
+    k_publish<<<1, 128, 0, w->blas.stream>>>(reinterpret_cast<unsigned long long*>(w->h_sc),
+                                             reinterpret_cast<const unsigned long long*>(w->blas.sc),
+                                             (int)(sizeof(SolverScalars) * w->blas.nrhs / 8));
+    BQ_CUDA(lat, cudaGetLastError());
     BQ_CUDA(lat, cudaStreamSynchronize(w->blas.stream));
     return BQ_OK;
 }
@@ -176,6 +203,7 @@ static bq_status run_batch(bq_lattice* lat, SolverWork* w, int method, int prec,
         BQ_CUDA(lat, cudaGraphLaunch(g.exec, s));
         lat->n_launch += g.d_launch;
         for (int p = 0; p < 3; p++) lat->n_hop[p] += g.d_hop[p];
+        lat->n_ls += g.d_ls;
         return BQ_OK;
     }
     if (!same || !g.warm) {
@@ -187,7 +215,7 @@ static bq_status run_batch(bq_lattice* lat, SolverWork* w, int method, int prec,
         return BQ_OK;
     }
     // second batch with this key: capture it, then launch what was captured
-    const unsigned long long l0 = lat->n_launch, h0[3] = {lat->n_hop[0], lat->n_hop[1], lat->n_hop[2]};
+    const unsigned long long l0 = lat->n_launch, h0[3] = {lat->n_hop[0], lat->n_hop[1], lat->n_hop[2]}, ls0 = lat->n_ls;
     if (cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
         cudaGetLastError();
         return eager();
@@ -203,10 +231,12 @@ static bq_status run_batch(bq_lattice* lat, SolverWork* w, int method, int prec,
         lat->use_graphs = 0;              // do not try again on this handle
         lat->n_launch = l0;
         for (int p = 0; p < 3; p++) lat->n_hop[p] = h0[p];
+        lat->n_ls = ls0;
         return eager();
     }
     g.d_launch = lat->n_launch - l0;
     for (int p = 0; p < 3; p++) g.d_hop[p] = lat->n_hop[p] - h0[p];
+    g.d_ls = lat->n_ls - ls0;
     BQ_CUDA(lat, cudaGraphLaunch(g.exec, s));
     return BQ_OK;
 }
@@ -257,6 +287,8 @@ static bq_status inner_bicgstab(bq_lattice* lat, SolverWork* w, double kappa, do
         for (int k = 0; k < n; k++) all_done = all_done && w->h_sc[k].done;
         if (all_done || launched >= max_iter) break;
     }
+    // iterations enqueued after a right-hand side had stopped: their 4 hop launches each were no-ops (HopArgs::done)
+    for (int k = 0; k < n; k++) lat->n_hop_idle[prec] += 4ull * (unsigned long long)(launched - w->h_sc[k].iters);
     return BQ_OK;
 }
 
@@ -291,6 +323,8 @@ static bq_status inner_cgnr(bq_lattice* lat, SolverWork* w, double kappa, double
         for (int k = 0; k < n; k++) all_done = all_done && w->h_sc[k].done;
         if (all_done || launched >= max_iter) break;
     }
+    // iterations enqueued after a right-hand side had stopped: their 4 hop launches each were no-ops (HopArgs::done)
+    for (int k = 0; k < n; k++) lat->n_hop_idle[prec] += 4ull * (unsigned long long)(launched - w->h_sc[k].iters);
     return BQ_OK;
 }
 
@@ -308,18 +342,24 @@ static void phase_times(SolverWork* w, bq_solve_info* info, int n) {
     }
 }
 
-// x (canonical, host or device) <- the n full-lattice fp64 fields of w->x; records w->ev1 and synchronises
-static bq_status export_solution(bq_lattice* lat, SolverWork* w, double* x, int n, const char* fn) {
+// x (canonical, host or device) <- the n full-lattice fp64 fields of w->x: layout conversion into the staging buffer and
+// the copy to the caller's buffer, enqueued on stream xs (does not synchronise)
+static bq_status enqueue_export(bq_lattice* lat, SolverWork* w, double* x, int n, cudaStream_t xs, const char* fn) {
     const Geom& g = lat->g;
-    cudaStream_t s = w->blas.stream;
     const size_t nb = (size_t)g.V * 24 * sizeof(double), fb64 = field_bytes_one_parity(g, BQ_FP64);
-    double* stage = w->stage;
-    cudaError_t e = cudaEventRecord(w->evp[3], s);
-    bq_status st = BQ_OK;
-    for (int k = 0; k < n && e == cudaSuccess && st == BQ_OK; k++) {
-        st = bq_field_export(lat, stage, static_cast<char*>(w->x) + (size_t)k * 2 * fb64, BQ_FULL, BQ_FP64, s);
-        if (st == BQ_OK) e = cudaMemcpyAsync(reinterpret_cast<char*>(x) + (size_t)k * nb, stage, nb, cudaMemcpyDefault, s);
+    for (int k = 0; k < n; k++) {
+        BQ_TRY(bq_field_export(lat, w->stage, static_cast<char*>(w->x) + (size_t)k * 2 * fb64, BQ_FULL, BQ_FP64, xs));
+        const cudaError_t e = cudaMemcpyAsync(reinterpret_cast<char*>(x) + (size_t)k * nb, w->stage, nb, cudaMemcpyDefault, xs);
+        if (e != cudaSuccess) return bq_set_error(lat, BQ_ECUDA, "%s: export failed: %s", fn, cudaGetErrorString(e));
     }
+    return BQ_OK;
+}
+
+// export on the solver's own stream; records w->evp[3] before, w->ev1 after, and synchronises
+static bq_status export_solution(bq_lattice* lat, SolverWork* w, double* x, int n, const char* fn) {
+    cudaStream_t s = w->blas.stream;
+    cudaError_t e = cudaEventRecord(w->evp[3], s);
+    bq_status st = e == cudaSuccess ? enqueue_export(lat, w, x, n, s, fn) : BQ_OK;
     if (e == cudaSuccess) e = cudaEventRecord(w->ev1, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     if (e != cudaSuccess) return bq_set_error(lat, BQ_ECUDA, "%s: export failed: %s", fn, cudaGetErrorString(e));
@@ -350,7 +390,6 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
     const bool cgnr = o.method == BQ_CGNR;
     if (o.lexical && (multi || cgnr)) return bq_set_error(lat, BQ_EINVAL, "%s: the lexical solve is BiCGStab on one right-hand side", fn);
     if (o.recon != BQ_RECON18 && o.recon != BQ_RECON12) return bq_set_error(lat, BQ_EINVAL, "%s: bad recon", fn);
-    if (o.stream) return bq_set_error(lat, BQ_EINVAL, "%s: opts->stream must be NULL", fn);
     const int prec = o.inner_prec;
     const double inner_tol = o.inner_tol > 0 ? o.inner_tol : (prec == BQ_HALF ? 5e-2 : 1e-5);
     const int max_inner = o.max_inner > 0 ? o.max_inner : (prec == BQ_HALF ? 100 : 1000);
@@ -386,6 +425,12 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
     const HopMulti* none = nullptr;
     auto hm = [&](size_t s_in, size_t s_out, size_t s_z) { return HopMulti{n, s_in, s_out, s_z, 0}; };
 
+    if (o.stream) {
+        // the caller's stream: everything enqueued there so far (e.g. the kernels that produce b) is waited for by the
+        // solver's own stream; the call synchronises before it returns, so work enqueued there afterwards sees x
+        BQ_CUDA(lat, cudaEventRecord(w->ev_side, static_cast<cudaStream_t>(o.stream)));
+        BQ_CUDA(lat, cudaStreamWaitEvent(s, w->ev_side, 0));
+    }
     BQ_CUDA(lat, cudaEventRecord(w->ev0, s));
     // ---- import b and x0 (canonical, host or device) through a device staging buffer ----
     {
@@ -425,10 +470,10 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
     }
     // |b_k|^2 over the full lattice (two parities)
     double* bnorm = static_cast<double*>(calloc(5 * (size_t)n, sizeof(double)));
-    int* ik = static_cast<int*>(calloc(4 * (size_t)n, sizeof(int)));
+    int* ik = static_cast<int*>(calloc(7 * (size_t)n, sizeof(int)));
     if (!bnorm || !ik) { free(bnorm); free(ik); return bq_set_error(lat, BQ_ENOMEM, "%s: host allocation failed", fn); }
     double *target = bnorm + n, *prev_rnorm = bnorm + 2 * n, *rnorm = bnorm + 3 * n, *true_rel = bnorm + 4 * n;
-    int *stalled = ik, *inner_total = ik + n, *restarts = ik + 2 * n, *cycles = ik + 3 * n;
+    int *stalled = ik, *inner_total = ik + n, *restarts = ik + 2 * n, *cycles = ik + 3 * n, *fin = ik + 4 * n, *stat = ik + 5 * n, *dead = ik + 6 * n;
     bq_status result = BQ_OK;
     // every early exit below goes through `fail` so that the host scratch is released
 #define SOLVE_TRY(expr)                         \
@@ -446,6 +491,12 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
         }
     }
     bool any_nonzero = false;
+    for (int k = 0; k < n; k++)
+        if (!isfinite(bnorm[k])) {
+            free(bnorm); free(ik);
+            w->blas.nrhs = 1;
+            return bq_set_error(lat, BQ_EINVAL, "%s: right-hand side %d contains NaN or Inf", fn, k);
+        }
     for (int k = 0; k < n; k++) {
         bnorm[k] = sqrt(bnorm[k]);
         target[k] = tol * bnorm[k];
@@ -495,29 +546,34 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
             }
             SOLVE_TRY(outer_residual(lat, c, w->bhat, fb64, w->t, w->r));
             SOLVE_TRY(poll(lat, w));
-            bool all_conv = true, nan = false, stall = false;
-            double worst = 0;
+            // every right-hand side is judged on its own (bq.h): one that has converged, produced a NaN, stalled or broken
+            // down for good is FINISHED — it keeps its status and its iterate, its inner solves stop at once — and the
+            // others go on
+            bool any_active = false;
             for (int k = 0; k < n; k++) {
                 rnorm[k] = sqrt(w->h_sc[k].r2);
-                if (!(rnorm[k] == rnorm[k])) nan = true;
-                if (bnorm[k] == 0.0 || rnorm[k] <= target[k]) continue;
-                all_conv = false;
-                if (rnorm[k] / bnorm[k] > worst) worst = rnorm[k] / bnorm[k];
+                if (fin[k]) continue;
+                if (bnorm[k] == 0.0 || rnorm[k] <= target[k]) { fin[k] = 1; continue; }
+                if (!(rnorm[k] == rnorm[k])) { fin[k] = 1; stat[k] = BQ_EBREAKDOWN; continue; }
+                if (dead[k]) { fin[k] = 1; stat[k] = BQ_EBREAKDOWN; continue; }
                 if (rnorm[k] > 0.5 * prev_rnorm[k]) {
-                    if (++stalled[k] >= 4) stall = true;
+                    if (++stalled[k] >= 4) { fin[k] = 1; stat[k] = BQ_ENOTCONVERGED; continue; }
                 } else stalled[k] = 0;
                 prev_rnorm[k] = rnorm[k];
+                any_active = true;
             }
-            if (nan) { result = bq_set_error(lat, BQ_EBREAKDOWN, "%s: residual is NaN", fn); break; }
-            if (all_conv) break;
-            if (outer >= max_outer) { result = bq_set_error(lat, BQ_ENOTCONVERGED, "%s: max_outer reached, |r|/|b| = %.3e", fn, worst); break; }
-            if (stall) { result = bq_set_error(lat, BQ_ENOTCONVERGED, "%s: stalled at |r|/|b| = %.3e", fn, worst); break; }
+            if (!any_active) break;
+            if (outer >= max_outer) {
+                for (int k = 0; k < n; k++)
+                    if (!fin[k]) { fin[k] = 1; stat[k] = BQ_ENOTCONVERGED; }
+                break;
+            }
             outer++;
             // normalised low-precision right-hand sides and inner stopping thresholds; a right-hand side that has
             // already converged gets an infinite threshold: its inner solve stops at once with e = 0
             SOLVE_TRY(outer_to_low(lat, c, prec, w->r, w->ir));
             for (int k = 0; k < n; k++) {
-                if (bnorm[k] == 0.0 || rnorm[k] <= target[k]) { w->h_stop2[k] = INFINITY; continue; }
+                if (fin[k]) { w->h_stop2[k] = INFINITY; continue; }
                 // CGNR stops on the normal-equation residual |M^^dag (r - M^ e)|, whose reduction only bounds that of
                 // |r - M^ e| up to cond(M^): ask for a decade more and let the outer loop judge the true residual
                 const double rel = ((prec == BQ_FP64) ? 0.9 * target[k] / rnorm[k] : fmax(inner_tol, 0.5 * target[k] / rnorm[k])) *
@@ -527,15 +583,13 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
             }
             if (cgnr) SOLVE_TRY(inner_cgnr(lat, w, kappa, csw, prec, o.recon, max_inner, check_every));
             else SOLVE_TRY(inner_bicgstab(lat, w, kappa, csw, prec, o.recon, max_inner, check_every));
-            bool dead = false;
             for (int k = 0; k < n; k++) {
                 inner_total[k] += w->h_sc[k].iters;
                 if (w->h_sc[k].done == 2) {   // breakdown: the next outer cycle restarts from the true residual
                     restarts[k]++;
-                    if (w->h_sc[k].iters == 0 && restarts[k] > 3) dead = true;
+                    if (w->h_sc[k].iters == 0 && restarts[k] > 3) dead[k] = 1;
                 }
             }
-            if (dead) { result = bq_set_error(lat, BQ_EBREAKDOWN, "%s: BiCGStab breakdown (rho or <rhat,v> or <t,t> = 0)", fn); break; }
             // x_e += |r| e   (|r| = sc->rnorm, written by outer_residual; the inner loop does not touch it)
             SOLVE_TRY(outer_accumulate(lat, c, prec == BQ_HALF ? BQ_FP32 : prec, w->ie, xx, 2 * fb64));
         }
@@ -549,26 +603,55 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
             for (int k = 0; k < n; k++)
                 SOLVE_TRY(bq_clover_mul(lat, xx + (size_t)k * 2 * fb64 + fb64, xx + (size_t)k * 2 * fb64 + fb64,
                                         static_cast<const char*>(cli64) + cb64, BQ_FP64, s));
-        // ---- true residual |b - D x| / |b| on the full lattice, fp64 ----
+        // ---- x is final: its layout conversion and its copy to the caller run on a second stream from here on ... ----
+        bool exported = false;
+        {
+            cudaError_t e = cudaEventRecord(w->ev_side, s);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(w->side, w->ev_side, 0);
+            if (e != cudaSuccess) { free(bnorm); free(ik); return bq_set_error(lat, BQ_ECUDA, "%s: %s", fn, cudaGetErrorString(e)); }
+        }
+        // ---- ... while the true residual |b - D x| / |b| is computed on the full lattice in fp64 ----
         for (int p = 0; p < 2; p++) {
             const void* clp = clover ? static_cast<const char*>(cl64) + p * cb64 : nullptr;
             const HopMulti m = hm(2 * fb64, fb64, 2 * fb64);
             SOLVE_TRY(bq_hop(lat, w->t, xx + (1 - p) * fb64, xx + p * fb64, -kappa, p, BQ_FP64, BQ_RECON18, clp, clover ? 2 : 0, s, nullptr,
                              multi ? &m : none));
             SOLVE_TRY(outer_residual(lat, c, bb + p * fb64, 2 * fb64, w->t, w->r));
+            if (!exported) {     // enqueued behind the first residual kernels: a pageable destination makes this call block the host
+                SOLVE_TRY(enqueue_export(lat, w, x, n, w->side, fn));
+                exported = true;
+            }
             SOLVE_TRY(poll(lat, w));
             for (int k = 0; k < n; k++) true_rel[k] += w->h_sc[k].r2;
         }
         for (int k = 0; k < n; k++) true_rel[k] = bnorm[k] > 0.0 ? sqrt(true_rel[k]) / bnorm[k] : 0.0;
+        // the solver's stream waits for the side stream: w->ev1 closes the whole call
+        {
+            cudaError_t e = cudaEventRecord(w->evp[3], s);
+            if (e == cudaSuccess) e = cudaEventRecord(w->ev_side, w->side);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(s, w->ev_side, 0);
+            if (e == cudaSuccess) e = cudaEventRecord(w->ev1, s);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+            if (e != cudaSuccess) { free(bnorm); free(ik); return bq_set_error(lat, BQ_ECUDA, "%s: export failed: %s", fn, cudaGetErrorString(e)); }
+        }
+    } else {
+        // nothing to solve (all right-hand sides zero): x = 0
+        SOLVE_TRY(export_solution(lat, w, x, n, fn));
     }
-    // ---- export x ----
-    SOLVE_TRY(export_solution(lat, w, x, n, fn));
 #undef SOLVE_TRY
     float ms = 0;
     cudaEventElapsedTime(&ms, w->ev0, w->ev1);
+    // worst status of the batch: breakdown before non-convergence
+    for (int k = 0; k < n; k++)
+        if (stat[k] == BQ_EBREAKDOWN && result != BQ_EBREAKDOWN)
+            result = bq_set_error(lat, BQ_EBREAKDOWN, "%s: right-hand side %d: NaN residual or BiCGStab breakdown (rho, <rhat,v> or <t,t> = 0)", fn, k);
+    for (int k = 0; k < n && result == BQ_OK; k++)
+        if (stat[k] == BQ_ENOTCONVERGED)
+            result = bq_set_error(lat, BQ_ENOTCONVERGED, "%s: right-hand side %d stopped at |r|/|b| = %.3e (stalled or max_outer reached)", fn, k,
+                                  bnorm[k] > 0 ? rnorm[k] / bnorm[k] : 0.0);
     if (info)
         for (int k = 0; k < n; k++) {
-            info[k].status = result;
+            info[k].status = stat[k];
             info[k].outer_cycles = (prec == BQ_FP64) ? 0 : cycles[k];
             info[k].inner_iters = inner_total[k];
             info[k].restarts = (prec == BQ_FP64) ? (cycles[k] > 0 ? cycles[k] - 1 : 0) + restarts[k] : restarts[k];
@@ -615,6 +698,10 @@ static bq_status solve_lex(bq_lattice* lat, SolverWork* w, const bq_solve_opts& 
     LEX_TRY(blas_norm2(lat, c, BQ_FP64, w->b));
     LEX_TRY(poll(lat, w));
     bnorm = sqrt(w->h_sc[0].red[0]);
+    if (!isfinite(bnorm)) {
+        cudaFree(pool);
+        return bq_set_error(lat, BQ_EINVAL, "bq_solve: the right-hand side contains NaN or Inf");
+    }
     if (bnorm == 0.0) {
         cudaMemsetAsync(w->x, 0, fb64, s);
     } else {
@@ -658,6 +745,7 @@ static bq_status solve_lex(bq_lattice* lat, SolverWork* w, const bq_solve_opts& 
                 if (w->h_sc[0].done || launched >= max_inner) break;
             }
             inner_total += w->h_sc[0].iters;
+            lat->n_hop_idle[prec] += 4ull * (unsigned long long)(launched - w->h_sc[0].iters);
             if (w->h_sc[0].done == 2) {
                 restarts++;
                 if (w->h_sc[0].iters == 0 && restarts > 3) { *result = bq_set_error(lat, BQ_EBREAKDOWN, "bq_solve: BiCGStab breakdown"); break; }

@@ -1,8 +1,9 @@
 """GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times.
 
-The oracle cannot afford many full passes at these sizes, so the hop is checked on sampled output sites the
-oracle computes one by one (oracle dirac_apply_sites), and solves by their true residual with the oracle's
-operator (one full-lattice oracle apply).  Inputs: the seeded recipes of DESIGN.md §4.
+EVERY output site is compared with the oracle: a full even-parity pass of the oracle costs 66 ms at 32^3x64 and
+under half a second at 48^3x96 on the box's host cores (bench.py's cpu_baseline does 180 of them), so nothing is
+sampled.  Solves are judged by their true residual with the oracle's operator (one full-lattice oracle apply).
+Inputs: the seeded recipes of DESIGN.md §4.
 """
 import numpy as np
 import pytest
@@ -23,15 +24,14 @@ def bq():
     return _bq
 
 
-def sample_sites(L, parity, n, seed):
-    par = inputs.site_parity(L).ravel()
-    sites = np.nonzero(par == parity)[0]
-    rng = np.random.default_rng(seed)
-    pick = rng.choice(sites, size=n, replace=False)
-    # always include the corners of the index range and of the lattice (wrap in every direction)
-    Lx, Ly, Lz, Lt = L
-    corners = [0 if parity == 0 else 1, sites[-1], sites[len(sites) // 2]]
-    return np.unique(np.concatenate([pick, np.array(corners)]))
+def even_sites_of(L):
+    return np.nonzero(inputs.site_parity(L).ravel() == 0)[0]
+
+
+def oracle_even_hop(U, psi, kappa, L):
+    """-kappa H_eo psi_o at ALL even sites: (D [0; psi_odd])(x), x even -> [Vh, 4, 3] (oracle, site by site)."""
+    masked = np.where((inputs.site_parity(L) == 1)[..., None, None], psi, 0)
+    return bqo.dirac_apply_sites(U, masked, kappa, even_sites_of(L))
 
 
 def test_config2_16to4_fp32_apply_1000x(bq):
@@ -60,51 +60,117 @@ def test_config2_16to4_fp32_apply_1000x(bq):
               f"{1320 * 32768 / us / 1e3:.0f} GFlop/s")
 
 
-@pytest.mark.parametrize("recon", [0, 1])
-def test_config3_32x32x32x64_fp32_hop_sampled(bq, recon):
-    """BASELINE.json config 3: 32^3x64 fp32 even-odd hop, 18- and 12-real links, eps = 0.5 — the bench workload."""
+def test_config3_32x32x32x64_hop_every_site(bq):
+    """BASELINE.json config 3: 32^3x64 even-odd hop, eps = 0.5 — the bench workload — fp32 with 18- and 12-real links
+    (1e-5), fp64 (1e-12) and half storage (5e-3): all 1,048,576 output sites against the oracle."""
     L = (32, 32, 32, 64)
     seed = inputs.BASE_SEED + 3
     U, psi = inputs.gauge(L, seed, 0.5), inputs.spinor(L, seed)
-    masked = np.where((inputs.site_parity(L) == 1)[..., None, None], psi, 0)
-    sites = sample_sites(L, 0, 4096, 3)
-    ref = bqo.dirac_apply_sites(U, masked, 0.125, sites)      # even sites, odd-only input: exactly -kappa H_eo psi_o
+    ev = even_sites_of(L)
+    ref = oracle_even_hop(U, psi, 0.125, L)
+    odd = inputs.site_parity(L).ravel() == 1
     with bq.Lattice(L) as lat:
         bq.bq_gauge_load(lat.h, U)
-        src = lat.import_field(psi, bq.BQ_FP32, bq.BQ_ODD)
-        out = lat.field(bq.BQ_FP32, bq.BQ_EVEN)
-        bq.bq_wilson_apply(lat.h, out, src, 0.125, bq.BQ_EVEN, bq.BQ_FP32, recon)
-        got = lat.export_field(out, bq.BQ_FP32, bq.BQ_EVEN).reshape(-1, 4, 3)
-        assert relmax(got[sites], ref) < 1e-5
-        # properties that hold at any size: odd sites untouched (zero), output finite, norm consistent with the sample
-        odd = inputs.site_parity(L).ravel() == 1
-        assert np.all(got[odd] == 0) and np.all(np.isfinite(got.view(np.float64)))
-        # linearity on the whole field: H(2 psi) = 2 H(psi) exactly in binary floating point
-        src2 = lat.import_field(2 * psi, bq.BQ_FP32, bq.BQ_ODD)
-        out2 = lat.field(bq.BQ_FP32, bq.BQ_EVEN)
-        bq.bq_wilson_apply(lat.h, out2, src2, 0.125, bq.BQ_EVEN, bq.BQ_FP32, recon)
-        assert np.array_equal(lat.export_field(out2, bq.BQ_FP32, bq.BQ_EVEN).reshape(-1, 4, 3), 2 * got)
+        for prec, recon, tol in ((bq.BQ_FP32, 0, 1e-5), (bq.BQ_FP32, 1, 1e-5), (bq.BQ_FP64, 0, 1e-12), (bq.BQ_FP64, 1, 1e-12),
+                                 (bq.BQ_HALF, 0, 5e-3), (bq.BQ_HALF, 1, 5e-3)):
+            src = lat.import_field(psi, prec, bq.BQ_ODD)
+            out = lat.field(prec, bq.BQ_EVEN)
+            bq.bq_wilson_apply(lat.h, out, src, 0.125, bq.BQ_EVEN, prec, recon)
+            got = lat.export_field(out, prec, bq.BQ_EVEN).reshape(-1, 4, 3)
+            err = relmax(got[ev], ref)
+            print(f"config 3 prec={prec} recon={recon}: max rel err over {len(ev)} sites {err:.2e}")
+            assert err < tol, (prec, recon)
+            assert np.all(got[odd] == 0)                     # the export leaves the other parity alone
+            del src, out
 
 
-def test_config4_clover_solve_32x32x32x64(bq):
-    """BASELINE.json config 4: Wilson-clover csw = 1, kappa = 0.1215, fp32 inner / fp64 outer BiCGStab to 1e-10."""
+def test_config3_multirhs_x12_every_site(bq):
+    """32^3 x 64 fp32 and half storage, 12 right-hand sides in one launch (the link-stationary kernel, as kbench and
+    bench.py time it): every output site of every right-hand side against the oracle, and every right-hand side bit
+    for bit against the single-rhs kernel."""
+    import torch
+    L, kappa, nrhs = (32, 32, 32, 64), 0.125, 12
+    seed = inputs.BASE_SEED + 3
+    U = inputs.gauge(L, seed, 0.5)
+    psis = [inputs.spinor(L, seed + 1000 * k) for k in range(nrhs)]
+    ev = even_sites_of(L)
+    refs = [oracle_even_hop(U, p, kappa, L) for p in psis]
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        for prec, tol in ((bq.BQ_FP32, 1e-5), (bq.BQ_HALF, 5e-3)):
+            fb = bq.bq_field_bytes(lat.h, prec, bq.BQ_EVEN)
+            src = torch.cat([lat.import_field(p, prec, bq.BQ_ODD) for p in psis])
+            out = torch.zeros(nrhs * fb, dtype=torch.uint8, device="cuda")
+            one = lat.field(prec, bq.BQ_EVEN)
+            for recon in (bq.BQ_RECON18, bq.BQ_RECON12):
+                n0 = bq.bq_get_counters(lat.h)["ls"]
+                bq.bq_wilson_apply_multi(lat.h, out, src, nrhs, kappa, bq.BQ_EVEN, prec, recon)
+                assert bq.bq_get_counters(lat.h)["ls"] == n0 + 1
+                for k in range(nrhs):
+                    bq.bq_wilson_apply(lat.h, one, src[k * fb:(k + 1) * fb], kappa, bq.BQ_EVEN, prec, recon)
+                    assert torch.equal(one, out[k * fb:(k + 1) * fb]), (prec, recon, k)
+                    if recon == bq.BQ_RECON18 or k in (0, 11):
+                        got = lat.export_field(out[k * fb:(k + 1) * fb], prec, bq.BQ_EVEN).reshape(-1, 4, 3)[ev]
+                        assert relmax(got, refs[k]) < tol, (prec, recon, k)
+            del src, out
+
+
+@pytest.fixture(scope="module")
+def config4():
+    """Gauge field, source and the oracle's dense clover term (and its inverse) of BASELINE config 4."""
     L = (32, 32, 32, 64)
     seed = inputs.BASE_SEED + 4
     csw, kappa = 1.0, 0.1215
     U, b = inputs.gauge(L, seed, 0.5), inputs.spinor(L, seed)
+    A = bqo.clover_build(U, csw, kappa)
+    return L, csw, kappa, U, b, A
+
+
+def test_config4_clover_operator_every_site(bq, config4):
+    """32^3x64 Wilson-clover D (bq_dirac_apply, csw = 1) and its even-odd Schur complement (bq_schur_apply) on the
+    whole lattice against the oracle's dense-clover operator: fp32 <= 1e-5 / 2e-5 (two hops), fp64 <= 1e-12 / 2e-12."""
+    import torch
+    L, csw, kappa, U, psi, A = config4
+    ref = bqo.dirac_apply(U, psi, kappa, A=A)
+    par = (inputs.site_parity(L) == 0)[..., None, None]
+    Ainv = bqo.site_matrix_invert(A)
+    ref_s = bqo.schur_apply(U, np.where(par, psi, 0), kappa, A=A, Ainv=Ainv)
+    del Ainv
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        for prec, tol in ((bq.BQ_FP32, 1e-5), (bq.BQ_FP64, 1e-12)):
+            src = lat.import_field(psi, prec, bq.BQ_FULL)
+            out = torch.zeros_like(src)
+            bq.bq_dirac_apply(lat.h, out, src, kappa, csw, prec, bq.BQ_RECON18)
+            err = relmax(lat.export_field(out, prec, bq.BQ_FULL), ref)
+            src_e = lat.import_field(psi, prec, bq.BQ_EVEN)
+            out_e, tmp = torch.zeros_like(src_e), torch.zeros_like(src_e)
+            bq.bq_schur_apply(lat.h, out_e, src_e, tmp, kappa, csw, prec, bq.BQ_RECON18)
+            err_s = relmax(lat.export_field(out_e, prec, bq.BQ_EVEN), ref_s)
+            print(f"config 4 prec={prec}: D {err:.2e}, Schur {err_s:.2e} (all {psi.size // 12} sites)")
+            assert err < tol and err_s < 2 * tol, prec
+            del src, out, src_e, out_e, tmp
+
+
+def test_config4_clover_solve_32x32x32x64(bq, config4):
+    """BASELINE.json config 4: Wilson-clover csw = 1, kappa = 0.1215, fp32 inner / fp64 outer BiCGStab to 1e-10."""
+    L, csw, kappa, U, b, A = config4
     x = np.zeros_like(b)
     with bq.Lattice(L) as lat:
         bq.bq_gauge_load(lat.h, U)
         info = bq.bq_solve(lat.h, b, x, kappa, 1e-10, bq.bq_solve_opts(inner_prec=bq.BQ_FP32, csw=csw))
-    A = bqo.clover_build(U, csw, kappa)
+        c = bq.bq_get_counters(lat.h)
     res = np.linalg.norm(b - bqo.dirac_apply(U, x, kappa, A=A)) / np.linalg.norm(b)
     print(f"config 4: {info.inner_iters} inner iters, {info.outer_cycles} outer, {info.seconds * 1e3:.1f} ms, "
-          f"oracle residual {res:.2e}")
+          f"oracle residual {res:.2e}, hops {c['hop_fp32']} launched / {c['idle_fp32']} no-ops after convergence")
     assert info.status == 0 and res <= 1e-10
+    # hops enqueued after convergence are accounted for: 4 per launched-but-unused iteration
+    assert c["idle_fp32"] % 4 == 0 and c["hop_fp32"] - c["idle_fp32"] == 4 * info.inner_iters
 
 
 def test_config5_half_solve_48x48x48x96(bq):
-    """BASELINE.json config 5: 48^3x96 Wilson, kappa = 0.1235, eps = 0.7, half-storage inner, fp64 outer, to 1e-10."""
+    """BASELINE.json config 5: 48^3x96 Wilson, kappa = 0.1235, eps = 0.7, half-storage inner, fp64 outer, to 1e-10;
+    and the half-storage hop at that size on every one of its 5,308,416 output sites (5e-3)."""
     L = (48, 48, 48, 96)
     seed = inputs.BASE_SEED + 5
     kappa = 0.1235
@@ -113,44 +179,16 @@ def test_config5_half_solve_48x48x48x96(bq):
     with bq.Lattice(L) as lat:
         bq.bq_gauge_load(lat.h, U)
         info = bq.bq_solve(lat.h, b, x, kappa, 1e-10, bq.bq_solve_opts(inner_prec=bq.BQ_HALF))
-        # half hop at full size on sampled sites (5e-3)
-        masked = np.where((inputs.site_parity(L) == 1)[..., None, None], b, 0)
-        sites = sample_sites(L, 0, 2048, 5)
-        ref = bqo.dirac_apply_sites(U, masked, kappa, sites)
+        ev = even_sites_of(L)
+        ref = oracle_even_hop(U, b, kappa, L)
         src = lat.import_field(b, bq.BQ_HALF, bq.BQ_ODD)
         out = lat.field(bq.BQ_HALF, bq.BQ_EVEN)
         bq.bq_wilson_apply(lat.h, out, src, kappa, bq.BQ_EVEN, bq.BQ_HALF, bq.BQ_RECON18)
         got = lat.export_field(out, bq.BQ_HALF, bq.BQ_EVEN).reshape(-1, 4, 3)
-        assert relmax(got[sites], ref) < 5e-3
+        err = relmax(got[ev], ref)
+        print(f"config 5 half hop: max rel err over {len(ev)} sites {err:.2e}")
+        assert err < 5e-3
     res = np.linalg.norm(b - bqo.dirac_apply(U, x, kappa)) / np.linalg.norm(b)
     print(f"config 5: {info.inner_iters} inner iters, {info.outer_cycles} outer, {info.seconds * 1e3:.1f} ms, "
           f"oracle residual {res:.2e}")
     assert info.status == 0 and res <= 1e-10
-
-
-def test_config3_multirhs_x12_sampled(bq):
-    """32^3 x 64 fp32 (BASELINE config 3 shape), 12 right-hand sides in one launch (the patch-mapped multi-rhs kernel, as
-    kbench times it): sampled output sites of every right-hand side against the oracle, and the first right-hand side
-    bit for bit against the single-rhs kernel."""
-    import torch
-    L, kappa, nrhs = (32, 32, 32, 64), 0.125, 12
-    seed = inputs.BASE_SEED + 3
-    U = inputs.gauge(L, seed, 0.5)
-    psis = [inputs.spinor(L, seed + 1000 * k) for k in range(nrhs)]
-    par = inputs.site_parity(L)
-    sites = sample_sites(L, 0, 256, 17)
-    with bq.Lattice(L) as lat:
-        bq.bq_gauge_load(lat.h, U)
-        fb = bq.bq_field_bytes(lat.h, bq.BQ_FP32, bq.BQ_EVEN)
-        src = torch.cat([lat.import_field(p, bq.BQ_FP32, bq.BQ_ODD) for p in psis])
-        out = torch.zeros(nrhs * fb, dtype=torch.uint8, device="cuda")
-        for recon in (bq.BQ_RECON18, bq.BQ_RECON12):
-            bq.bq_wilson_apply_multi(lat.h, out, src, nrhs, kappa, bq.BQ_EVEN, bq.BQ_FP32, recon)
-            one = lat.field(bq.BQ_FP32, bq.BQ_EVEN)
-            bq.bq_wilson_apply(lat.h, one, src[:fb], kappa, bq.BQ_EVEN, bq.BQ_FP32, recon)
-            assert torch.equal(one, out[:fb])
-            for k in range(nrhs):
-                got = lat.export_field(out[k * fb:(k + 1) * fb], bq.BQ_FP32, bq.BQ_EVEN).reshape(-1, 4, 3)[sites]
-                masked = np.where((par == 1)[..., None, None], psis[k], 0)
-                ref = bqo.dirac_apply_sites(U, masked, kappa, sites)
-                assert relmax(got, ref) < 1e-5, (recon, k)

@@ -8,6 +8,7 @@ import pytest
 
 from oracle import bqo
 from paper_2111_04457_b200 import inputs
+from tests.conftest import relmax
 
 pytestmark = pytest.mark.gpu
 
@@ -273,3 +274,89 @@ def test_near_free_field_long_solve(bq, inner, method):
     print(f"near-free inner={inner} method={method}: outer {info.outer_cycles} iters {info.inner_iters} res {res:.2e}")
     assert info.status == 0 and res <= 1e-10 and abs(res - info.true_rel_residual) < 1e-11
     assert info.inner_iters > 40
+
+
+def test_nan_rhs_is_rejected(bq):
+    """A right-hand side with a NaN must not come back as BQ_OK with x = x0 (|b| = NaN compares false with everything)."""
+    L, kappa = (4, 4, 4, 4), 0.12
+    U = inputs.gauge(L, 901, 0.3)
+    b = inputs.spinor(L, 902)
+    b[1, 2, 3, 0, 1, 2] = np.nan
+    x = np.zeros_like(b)
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        for o in (None, bq.bq_solve_opts(inner_prec=bq.BQ_FP64), bq.bq_solve_opts(inner_prec=bq.BQ_FP32, lexical=1)):
+            with pytest.raises(bq.BqError) as e:
+                bq.bq_solve(lat.h, b, x, kappa, 1e-10, o)
+            assert e.value.status == bq.BQ_EINVAL
+        bb = np.stack([inputs.spinor(L, 903), b])
+        with pytest.raises(bq.BqError) as e:
+            bq.bq_solve_multi(lat.h, bb, np.zeros_like(bb), 2, kappa, 1e-10)
+        assert e.value.status == bq.BQ_EINVAL
+        # the handle is still usable
+        b2 = inputs.spinor(L, 904)
+        info = bq.bq_solve(lat.h, b2, x, kappa, 1e-10)
+        assert info.status == 0 and oracle_residual(U, x, b2, kappa) <= 1e-10
+
+
+def test_batch_statuses_are_per_rhs(bq):
+    """bq_solve_multi: every right-hand side stops on its own criterion and gets its own status (include/bq.h): with an
+    iteration budget too small for the Gaussian sources, the zero right-hand side is still BQ_OK, the others are
+    BQ_ENOTCONVERGED, and the call returns the failure."""
+    L, kappa, nrhs = (8, 4, 4, 8), 0.1215, 3
+    U = inputs.gauge(L, 905, 0.5)
+    b = np.stack([inputs.spinor(L, 906 + k) for k in range(nrhs)])
+    b[1] = 0
+    x = np.zeros_like(b)
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        opts = bq.bq_solve_opts(inner_prec=bq.BQ_FP32, max_inner=2, max_outer=2, check_every=1)
+        with pytest.raises(bq.BqError) as e:
+            bq.bq_solve_multi(lat.h, b, x, nrhs, kappa, 1e-12, opts)
+        assert e.value.status == bq.BQ_ENOTCONVERGED
+        infos = bq.bq_solve_multi(lat.h, b, x, nrhs, kappa, 1e-12, opts, raise_on_fail=False)
+        assert [i.status for i in infos] == [bq.BQ_ENOTCONVERGED, bq.BQ_OK, bq.BQ_ENOTCONVERGED]
+        assert not x[1].any() and infos[1].inner_iters == 0
+        # and with a normal budget every one converges
+        infos = bq.bq_solve_multi(lat.h, b, x, nrhs, kappa, 1e-10, bq.bq_solve_opts(inner_prec=bq.BQ_FP32))
+        assert all(i.status == 0 for i in infos)
+        for k in (0, 2):
+            assert oracle_residual(U, x[k], b[k], kappa) <= 1e-10
+
+
+def test_binding_rejects_wrong_arrays(bq):
+    """The binding checks what the C side cannot see: dtype, contiguity, element count (it never copies or converts)."""
+    L, kappa = (4, 4, 4, 4), 0.12
+    U = inputs.gauge(L, 911, 0.3)
+    b = inputs.spinor(L, 912)
+    x = np.zeros_like(b)
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        for bad_b, bad_x in ((b.astype(np.complex64), x), (b, x[..., ::-1]), (b[:2], x), (b, np.zeros((2,) + b.shape, dtype=np.complex128))):
+            with pytest.raises(bq.BqError) as e:
+                bq.bq_solve(lat.h, bad_b, bad_x, kappa, 1e-10)
+            assert e.value.status == bq.BQ_EINVAL
+        with pytest.raises(bq.BqError):
+            bq.bq_solve_multi(lat.h, np.stack([b, b]), np.zeros((3,) + b.shape, dtype=np.complex128), 2, kappa, 1e-10)
+
+
+def test_clover_apply_in_place_and_on_a_stream(bq):
+    """bq_clover_apply: out may equal in (include/bq.h), and the apply runs on the caller's stream."""
+    import torch
+    L, kappa, csw = (4, 4, 6, 4), 0.12, 1.0
+    U = inputs.gauge(L, 913, 0.5)
+    psi = inputs.spinor(L, 914)
+    A = bqo.clover_build(U, csw, kappa)
+    ref = bqo.site_matrix_apply(A, psi)
+    st = torch.cuda.Stream()
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        for prec, tol in ((bq.BQ_FP64, 1e-12), (bq.BQ_FP32, 1e-5)):
+            buf = lat.import_field(psi, prec, bq.BQ_FULL)
+            out = torch.zeros_like(buf)
+            bq.bq_clover_apply(lat.h, csw, kappa, out, buf, bq.BQ_FULL, 0, prec, st)
+            st.synchronize()
+            bq.bq_clover_apply(lat.h, csw, kappa, buf, buf, bq.BQ_FULL, 0, prec)       # in place
+            torch.cuda.synchronize()
+            assert torch.equal(out, buf)
+            assert relmax(lat.export_field(buf, prec, bq.BQ_FULL), ref) < tol
