@@ -51,6 +51,7 @@ struct bq_lattice {
     unsigned long long epoch;  // bumped whenever gauge or clover stores are freed: cached CUDA graphs of the solver hold their addresses
     int use_graphs;          // solver: replay the batches of inner iterations as CUDA graphs (default 1; env BQ_GRAPH=0 disables)
     int mrhs_patch;          // multi-rhs hop: 1 = patch mapping where the geometry allows (default), 0 = plain (env BQ_MRHS_PATCH)
+    int hop_pdl;             // single-rhs hop: programmatic dependent launch when Vh <= this (default 262144; env BQ_PDL = 0 off, or a bound)
     int mrhs_ls;             // multi-rhs hop: 1 = link-stationary kernel (hop_ls.cuh) where it applies (default), 0 = off (env BQ_MRHS_LS)
     const SolverScalars* hop_done;   // set by the solver around its inner iterations: hop launches test these `done` flags (HopArgs::done)
     unsigned long long n_launch;      // kernels launched through this handle

@@ -257,6 +257,11 @@ template <int PREC, int RECON, int EPI, bool CPLX, int RED, bool DAG = false>
 __global__ void __launch_bounds__(HOP_BLOCK, PREC == BQ_FP64 ? HOP_MINB_64 : (PREC == BQ_FP32 ? HOP_MINB_LO : HOP_MINB_HALF))
 hop_kernel(const HopArgs<typename Prec<PREC>::comp> a) {
     using C = typename Prec<PREC>::comp;
+    // Programmatic dependent launch (small lattices, where a hop lasts a few microseconds and the launch latency between two
+    // kernels of a stream is a third of it): the NEXT kernel of the stream may be launched and scheduled now; this one waits
+    // here until the kernel before it has completed and its writes are visible.  Both are no-ops in an ordinary launch.
+    asm volatile("griddepcontrol.launch_dependents;");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     if (a.done && a.done->done) return;     // uniform over the grid
     const int h = blockIdx.x * HOP_BLOCK + threadIdx.x;
     if (RED == 0) {
@@ -372,6 +377,17 @@ hop_kernel_mrhs(const HopArgs<typename Prec<PREC>::comp> a) {
 
 #include "hop_ls.cuh"
 
+// <<<grid, block, 0, stream>>> with the programmatic-stream-serialization attribute when `pdl` (see hop_kernel)
+template <class K, class A> static void hop_launch_pdl(K kern, int grid, int block, cudaStream_t stream, const A& a, bool pdl) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = 0; cfg.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+    cudaLaunchKernelEx(&cfg, kern, a);
+}
+
 template <int PREC, int RECON>
 bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const void* z, double scale, int p, const void* gauge,
                             const void* cl, int cl_mode, const HopRed* red, cudaStream_t stream, const HopMulti* m, bool dag) {
@@ -413,6 +429,7 @@ bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const void* z, 
         }
     }
     const int rmode = red ? red->mode : 0;
+    const bool pdl = !multi && lat->hop_pdl && g.Vh <= lat->hop_pdl;     // programmatic dependent launch on small lattices
     a.done = lat->hop_done;
     // link-stationary kernel (hop_ls.cuh) where the geometry, the operand strides and the epilogue allow
     const bool use_ls = multi && !(dag && rmode) && ls_eligible<PREC>(lat, m, in, z, rmode == 1 ? red->w : nullptr, cl_mode);
@@ -458,8 +475,8 @@ bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const void* z, 
             if (cplx) hop_kernel_mrhs<PREC, RECON, E, true, 0, true><<<grid, block, 0, stream>>>(a);  \
             else hop_kernel_mrhs<PREC, RECON, E, false, 0, true><<<grid, block, 0, stream>>>(a);      \
         } else {                                                                                    \
-            if (cplx) hop_kernel<PREC, RECON, E, true, 0, true><<<grid, HOP_BLOCK, 0, stream>>>(a);   \
-            else hop_kernel<PREC, RECON, E, false, 0, true><<<grid, HOP_BLOCK, 0, stream>>>(a);       \
+            if (cplx) hop_launch_pdl(hop_kernel<PREC, RECON, E, true, 0, true>, grid, HOP_BLOCK, stream, a, pdl);   \
+            else hop_launch_pdl(hop_kernel<PREC, RECON, E, false, 0, true>, grid, HOP_BLOCK, stream, a, pdl);       \
         }                                                                                           \
     } while (0)
 #define BQ_HOP_LAUNCH(E, R)                                                                         \
@@ -468,8 +485,8 @@ bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const void* z, 
             if (cplx) hop_kernel_mrhs<PREC, RECON, E, true, R><<<grid, block, 0, stream>>>(a);       \
             else hop_kernel_mrhs<PREC, RECON, E, false, R><<<grid, block, 0, stream>>>(a);           \
         } else {                                                                                    \
-            if (cplx) hop_kernel<PREC, RECON, E, true, R><<<grid, HOP_BLOCK, 0, stream>>>(a);        \
-            else hop_kernel<PREC, RECON, E, false, R><<<grid, HOP_BLOCK, 0, stream>>>(a);            \
+            if (cplx) hop_launch_pdl(hop_kernel<PREC, RECON, E, true, R>, grid, HOP_BLOCK, stream, a, pdl);        \
+            else hop_launch_pdl(hop_kernel<PREC, RECON, E, false, R>, grid, HOP_BLOCK, stream, a, pdl);            \
         }                                                                                           \
     } while (0)
     // fused reductions exist for the xpay epilogues only (the second hop of M^, which produces v and t)
