@@ -226,6 +226,43 @@ bq_status bq_solve_multi(bq_lattice* lat, const double* b, double* x, int nrhs, 
 bq_status bq_propagator(bq_lattice* lat, const int* src_site /*[4]*/, double* S, double kappa, double tol,
                         const bq_solve_opts* opts, bq_solve_info* info /*[12]*/);
 
+/* ---------------------------------------------------------------------------------------------
+ * Domain decomposition — OPT-IN; the calls above never use it.  The paper's code is "parallelized with
+ * MPI": a 4-D process grid, one halo exchange per matrix application overlapped with the bulk
+ * (PAPER.md:95), weak scaling as its experiment.  Here: Wilson operator (csw = 0), fp64 / fp32 storage.
+ *
+ * bq_lattice_create_sub: the sub-lattice of one rank.  lx..lt = LOCAL extents (even), grid[4] = ranks per direction,
+ * coords[4] = this rank's position (rank number = coords[0] + grid[0]*(coords[1] + ...)); bc_phase = the GLOBAL boundary
+ * phases.  bq_gauge_load takes the rank's LOCAL block of the link field (no ghost links are needed).  On such a handle
+ * bq_wilson_apply computes the INTERIOR part of the hop (hops that leave the rank in a partitioned direction contribute
+ * nothing); the rest arrives through the faces:
+ *   bq_dd_pack    send[2*mu + side], partitioned directions only: 12 reals per boundary site of the input parity, in the
+ *                 storage type (bq_dd_face_bytes): side 0 = slice x_mu = 0, spin-projected with (1 - g_mu), for the rank
+ *                 BELOW; side 1 = slice x_mu = l_mu - 1, projected with (1 + g_mu) and multiplied by U_mu^dag, for the rank ABOVE.
+ *   bq_dd_unpack  recv[2*mu + side]: side 1 = what the rank above packed as its side 0 (added to our slice x_mu = l_mu - 1
+ *                 after multiplication by our U_mu), side 0 = what the rank below packed as its side 1 (added to our slice
+ *                 x_mu = 0).  out += scale * (...), scale = the factor the interior call used (-kappa for bq_wilson_apply);
+ *                 the global boundary phase is applied here on the ranks at the edge of the grid.
+ * A process per GPU moves send -> recv with peer copies or NCCL send/recv between pack and unpack while the interior
+ * call runs (paper_2111_04457_b200/dd.py).  UNMEASURED on hardware: no multi-GPU node was available to this build.
+ *
+ * bq_dd_wilson_apply / bq_dd_solve: the same with VIRTUAL RANKS — all nranks = prod(grid) handles in this process on one
+ * device (ranks[r] at rank number r), faces moved by device copies: what the tests compare with the oracle on the global
+ * lattice.  out / in / b / x: one pointer per rank (internal-layout fields; b, x: the rank's local canonical block, HOST or
+ * DEVICE).  bq_dd_solve: fp64 even-odd BiCGStab to |b^_e - M^ x_e| <= tol |b|, every inner product a sum over ranks;
+ * info->inner_iters, ->true_rel_residual (of the Schur system) and ->status are filled. */
+bq_status bq_lattice_create_sub(int lx, int ly, int lz, int lt, const double* bc_phase, const int* grid /*[4]*/,
+                                const int* coords /*[4]*/, bq_lattice** out);
+bq_status bq_dd_face_bytes(const bq_lattice* lat, int mu, bq_prec prec, size_t* bytes);
+bq_status bq_dd_pack(bq_lattice* lat, void* const* send /*[8]*/, const void* in, bq_parity out_parity, bq_prec prec, bq_recon recon,
+                     void* stream);
+bq_status bq_dd_unpack(bq_lattice* lat, void* out, void* const* recv /*[8]*/, double scale, bq_parity out_parity, bq_prec prec,
+                       bq_recon recon, void* stream);
+bq_status bq_dd_wilson_apply(bq_lattice* const* ranks, int nranks, void* const* out, const void* const* in, double kappa,
+                             bq_parity parity, bq_prec prec, bq_recon recon, void* stream);
+bq_status bq_dd_solve(bq_lattice* const* ranks, int nranks, const double* const* b, double* const* x, double kappa, double tol,
+                      int max_iter, bq_solve_info* info);
+
 #ifdef __cplusplus
 }
 #endif

@@ -30,6 +30,7 @@ EXPORTS = [
     "bq_dirac_apply", "bq_schur_apply", "bq_solve", "bq_blas_norm2", "bq_blas_cdot", "bq_blas_caxpy",
     "bq_blas_bicg_update", "bq_get_counters", "bq_bench_kernel", "bq_schur_apply_dots",
     "bq_wilson_apply_multi", "bq_schur_apply_multi", "bq_bench_kernel_multi", "bq_solve_multi", "bq_dirac_apply_mode", "bq_schur_apply_mode", "bq_propagator",
+    "bq_lattice_create_sub", "bq_dd_face_bytes", "bq_dd_pack", "bq_dd_unpack", "bq_dd_wilson_apply", "bq_dd_solve",
 ]
 
 
@@ -92,6 +93,13 @@ def lib():
         L.bq_wilson_apply_multi.argtypes = [_vp, _vp, _vp, _i, _d, _i, _i, _i, _vp]
         L.bq_schur_apply_multi.argtypes = [_vp, _vp, _vp, _vp, _i, _d, _d, _i, _i, _vp]
         L.bq_bench_kernel_multi.argtypes = [_vp, _i, _i, _i, _d, _d, _i, _i, _i, _dp, _dp]
+        _pp = ctypes.POINTER(_vp)
+        L.bq_lattice_create_sub.argtypes = [_i, _i, _i, _i, _dp, ctypes.POINTER(_i), ctypes.POINTER(_i), ctypes.POINTER(_vp)]
+        L.bq_dd_face_bytes.argtypes = [_vp, _i, _i, ctypes.POINTER(ctypes.c_size_t)]
+        L.bq_dd_pack.argtypes = [_vp, _pp, _vp, _i, _i, _i, _vp]
+        L.bq_dd_unpack.argtypes = [_vp, _vp, _pp, _d, _i, _i, _i, _vp]
+        L.bq_dd_wilson_apply.argtypes = [_pp, _i, _pp, _pp, _d, _i, _i, _i, _vp]
+        L.bq_dd_solve.argtypes = [_pp, _i, _pp, _pp, _d, _d, _i, ctypes.POINTER(bq_solve_info)]
         for name in EXPORTS:
             if name not in ("bq_status_string", "bq_last_error"):
                 getattr(L, name).restype = _i
@@ -321,13 +329,66 @@ def bq_blas_bicg_update(h, alpha, omega, p, s, t, rhat, x, r, prec):
     return r2.value, complex(rr[0], rr[1])
 
 
+# ---- domain decomposition (opt-in; include/bq.h) -------------------------------------------
+def _ptr_array(items):
+    arr = (_vp * len(items))()
+    for k, it in enumerate(items):
+        arr[k] = it.value if hasattr(it, "value") else _ptr(it)
+    return arr
+
+
+def bq_lattice_create_sub(lx, ly, lz, lt, grid, coords, bc_phase=None):
+    h = _vp()
+    bc = None
+    if bc_phase is not None:
+        arr = np.asarray(bc_phase, dtype=np.complex128).view(np.float64)
+        bc = (ctypes.c_double * 8)(*arr)
+    st = lib().bq_lattice_create_sub(lx, ly, lz, lt, bc, (_i * 4)(*[int(v) for v in grid]), (_i * 4)(*[int(v) for v in coords]),
+                                     ctypes.byref(h))
+    if st != BQ_OK:
+        raise BqError(st, lib().bq_status_string(st).decode())
+    _DIMS[h.value] = (int(lx), int(ly), int(lz), int(lt))
+    return h
+
+
+def bq_dd_face_bytes(h, mu, prec):
+    n = ctypes.c_size_t(0)
+    _check(h, lib().bq_dd_face_bytes(h, mu, prec, ctypes.byref(n)))
+    return n.value
+
+
+def bq_dd_pack(h, send, inp, out_parity, prec, recon=BQ_RECON18, stream=None):
+    """send: 8 buffers (or None for unpartitioned directions), index 2*mu + side."""
+    _check(h, lib().bq_dd_pack(h, _ptr_array(send), _ptr(inp), out_parity, prec, recon, _stream_ptr(stream)))
+
+
+def bq_dd_unpack(h, out, recv, scale, out_parity, prec, recon=BQ_RECON18, stream=None):
+    _check(h, lib().bq_dd_unpack(h, _ptr(out), _ptr_array(recv), scale, out_parity, prec, recon, _stream_ptr(stream)))
+
+
+def bq_dd_wilson_apply(handles, outs, ins, kappa, parity, prec, recon=BQ_RECON18, stream=None):
+    """Virtual ranks: handles[r], outs[r], ins[r] for every rank r of the grid (rank number: x fastest)."""
+    _check(handles[0], lib().bq_dd_wilson_apply(_ptr_array(handles), len(handles), _ptr_array(outs), _ptr_array(ins), kappa, parity, prec,
+                                                recon, _stream_ptr(stream)))
+
+
+def bq_dd_solve(handles, bs, xs, kappa, tol, max_iter=0, raise_on_fail=True):
+    """bs[r], xs[r]: the local canonical complex128 blocks of rank r (numpy host arrays or torch CUDA tensors); xs is in/out."""
+    info = bq_solve_info()
+    st = lib().bq_dd_solve(_ptr_array(handles), len(handles), _ptr_array([_canonical(h, b, 1, "b") for h, b in zip(handles, bs)]),
+                           _ptr_array([_canonical(h, x, 1, "x") for h, x in zip(handles, xs)]), kappa, tol, max_iter, ctypes.byref(info))
+    _check(handles[0], st, allow=() if raise_on_fail else (BQ_ENOTCONVERGED, BQ_EBREAKDOWN))
+    return info
+
+
 # ---- convenience wrapper: owns the handle and allocates internal-layout buffers with torch --------------
 class Lattice:
     """RAII handle + torch-allocated internal-layout fields.  Pure marshalling; no arithmetic."""
 
-    def __init__(self, L, bc_phase=None):
+    def __init__(self, L, bc_phase=None, grid=None, coords=None):
+        """grid / coords given: the sub-lattice of one rank of a process grid (L = local extents; opt-in domain decomposition)."""
         self.L = tuple(int(v) for v in L)
-        self.h = bq_lattice_create(*self.L, bc_phase)
+        self.h = bq_lattice_create(*self.L, bc_phase) if grid is None else bq_lattice_create_sub(*self.L, grid, coords, bc_phase)
 
     def close(self):
         if self.h is not None:

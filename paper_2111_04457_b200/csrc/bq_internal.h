@@ -44,6 +44,9 @@ struct bq_lattice {
     void* clover[3][2];
     bool have_clover;
     double clover_csw, clover_kappa;
+    // domain decomposition (dd.cu; opt-in): a sub-lattice of a process grid.  sub == 0 for ordinary handles.
+    int sub, grid[4], coords[4];
+    void* dd;                // DdBufs: face buffers, side stream
     SolverWork* work;
     int* d_flag;             // device int scratch (singular-clover flag etc.)
     double* hop_partials;    // per-CTA partial sums of the hop kernel's fused reduction epilogues (lazily allocated)
@@ -128,5 +131,6 @@ bq_status bq_dirac_full(bq_lattice* lat, void* out, const void* in, double kappa
 bq_status bq_clover_mul(bq_lattice* lat, void* out, const void* in, const void* cl, int prec, cudaStream_t stream);
 
 void bq_solver_free(bq_lattice* lat);
+void bq_dd_free(bq_lattice* lat);
 
 static inline size_t field_bytes_one_parity(const Geom& g, int prec) { return (size_t)g.Vh * spinor_site_bytes(prec); }

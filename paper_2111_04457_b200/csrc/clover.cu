@@ -229,6 +229,7 @@ template <int PREC> __global__ void clover_convert_kernel(int Vh, const double* 
 
 bq_status bq_clover_build(bq_lattice* lat, double csw, double kappa) {
     if (!lat->have_gauge) return bq_set_error(lat, BQ_ENOGAUGE, "clover build: no gauge field loaded");
+    if (lat->sub) return bq_set_error(lat, BQ_EINVAL, "clover term on a sub-lattice: not built (the field strength needs the neighbours' links)");
     if (lat->have_clover && lat->clover_csw == csw && lat->clover_kappa == kappa) return BQ_OK;
     for (int p = 0; p < 3; p++)
         for (int i = 0; i < 2; i++) {

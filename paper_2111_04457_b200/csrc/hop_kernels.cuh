@@ -402,9 +402,12 @@ bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const void* z, 
     a.scale = (C)scale;
     bool cplx = false;
     for (int mu = 0; mu < 4; mu++) {
-        a.phr[mu] = (C)(scale * lat->bc[2 * mu]);
-        a.phi[mu] = (C)(scale * lat->bc[2 * mu + 1]);
-        if (lat->bc[2 * mu + 1] != 0.0) cplx = true;
+        // sub-lattice of a process grid (dd.cu): a hop that wraps in a partitioned direction leaves the rank — weight 0 here,
+        // its contribution arrives with the neighbour's face (bq_dd_unpack)
+        const bool off_rank = lat->sub && lat->grid[mu] > 1;
+        a.phr[mu] = off_rank ? (C)0 : (C)(scale * lat->bc[2 * mu]);
+        a.phi[mu] = off_rank ? (C)0 : (C)(scale * lat->bc[2 * mu + 1]);
+        if (!off_rank && lat->bc[2 * mu + 1] != 0.0) cplx = true;
     }
     // launch shape: one thread per site (128 per CTA), or — multi-rhs — T tiles x nrhs x 8 sites per CTA, padded to warps
     const bool multi = m != nullptr;

@@ -113,6 +113,7 @@ extern "C" bq_status bq_lattice_destroy(bq_lattice* lat) {
     free_gauge(lat);
     free_clover(lat);
     bq_solver_free(lat);
+    bq_dd_free(lat);
     if (lat->d_flag) cudaFree(lat->d_flag);
     if (lat->hop_partials) cudaFree(lat->hop_partials);
     free(lat);

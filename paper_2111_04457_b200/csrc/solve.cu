@@ -152,6 +152,15 @@ static bq_status get_work(bq_lattice* lat, int inner_prec, SolverWork** out, int
     return BQ_OK;
 }
 
+// dd.cu: the BLAS-1 context (reduction scratch, device scalars, stream) and the pinned host mirror of a handle
+bq_status bq_solver_blas(bq_lattice* lat, BlasCtx** ctx, SolverScalars** host_mirror) {
+    SolverWork* w = nullptr;
+    BQ_TRY(get_work(lat, lat->work && lat->work->inner_prec >= 0 ? lat->work->inner_prec : BQ_FP32, &w));
+    *ctx = &w->blas;
+    *host_mirror = w->h_sc;
+    return BQ_OK;
+}
+
 __global__ void k_set_bicg_scalars(SolverScalars* sc, double ar, double ai, double wr, double wi) {
     sc->alpha[0] = ar; sc->alpha[1] = ai;
     sc->omega[0] = wr; sc->omega[1] = wi;
@@ -382,6 +391,7 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
     if (!b || !x) return bq_set_error(lat, BQ_EINVAL, "%s: b or x is NULL", fn);
     if (!(tol > 0.0) || !isfinite(tol)) return bq_set_error(lat, BQ_EINVAL, "%s: tol must be positive", fn);
     if (!lat->have_gauge) return bq_set_error(lat, BQ_ENOGAUGE, "%s: no gauge field loaded", fn);
+    if (lat->sub) return bq_set_error(lat, BQ_EINVAL, "%s: a sub-lattice handle solves through bq_dd_solve", fn);
     bq_solve_opts o;
     if (opts) o = *opts;
     else { o.inner_prec = BQ_FP32; o.recon = BQ_RECON18; o.csw = 0; o.inner_tol = 0; o.max_inner = 0; o.max_outer = 0; o.check_every = 0; o.method = BQ_BICGSTAB; o.lexical = 0; o.x0_zero = 0; o.stream = nullptr; }
