@@ -83,7 +83,7 @@ template <> struct Item<BQ_HALF> {
 #pragma unroll
         for (int k = 0; k < 3; k++) unpack8(r.q[k], v + 8 * k);
 #pragma unroll
-        for (int k = 0; k < 24; k++) v[k] *= r.n;
+        for (int k = 0; k < 24; k++) v[k] = __fmul_rn(v[k], r.n);   // as load_spinor
     }
     // what a load of the just-stored item would return: v -> fp16(v/n) * n, n = max|v|
     __device__ static void requantize(C* v) {

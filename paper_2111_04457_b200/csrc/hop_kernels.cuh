@@ -460,7 +460,7 @@ bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const void* z, 
     if (dag && rmode) return bq_set_error(lat, BQ_EINVAL, "bq_hop: the dagger hop has no fused reduction");
     if (use_ls) {
         if constexpr (PREC != BQ_FP64) {
-            BQ_TRY((ls_launch<PREC, RECON>(lat, a, cplx, rmode, dag, m, lat->hop_done, stream)));
+            BQ_TRY((ls_launch<PREC, RECON>(lat, a, cplx, rmode, dag, m, lat->hop_done, stream, cl_mode)));
             BQ_CHECK_LAUNCH(lat);
             lat->n_hop[PREC] += nrhs;
             lat->n_ls++;

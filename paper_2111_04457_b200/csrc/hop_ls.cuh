@@ -20,7 +20,8 @@
 //     (BY, BZ, BT) = (4, 4, 2): 88 tile loads per 32 output tiles = 264 B per (site, rhs) in fp32.
 //   * The xpay operand z and the left operand w of a fused inner product come the same way (one stage each).
 // Per (site, rhs) the arithmetic is hop.cuh's, direction by direction in the same order, so results are bit for bit
-// those of hop_kernel / hop_kernel_mrhs.  fp32 and half storage; Wilson epilogues (EPI 0, 1) with the fused reductions.
+// those of hop_kernel / hop_kernel_mrhs.  fp32 and half storage; all four epilogues (Wilson and clover) with the fused reductions:
+// for the clover ones the block's clover tiles sit in shared memory for all right-hand sides (one more TMA copy per block).
 // Needs Lx % 16 == 0 (tiles are pieces of x-rows) and extents divisible by the block; anything else (and fp64, clover
 // epilogues) takes hop_kernel_mrhs.
 #pragma once
@@ -64,6 +65,8 @@ template <int PREC> struct LsGeom {
     static constexpr int STAGE = (X + (LS_NT / 8) * TS + 127) / 128 * 128;
     static constexpr int TX = X;                          // bytes a stage receives through TMA (everything but the x halo)
     static constexpr int OPER = LS_NT * TS;               // one interior-only operand buffer (z or w)
+    static constexpr int CLS = 72 * (PREC == BQ_FP64 ? 8 : (PREC == BQ_FP32 ? 4 : 2));   // clover blocks: bytes per site = 3 spinor-fp-tiles' worth per 8 sites
+    static constexpr int CLOV = LS_NT * 8 * CLS;          // the block's clover tiles (site-diagonal epilogues EPI 2, 3)
     static constexpr int NXC = (PREC == BQ_HALF ? 4 : NW) * LS_NT;   // cp.async copies of the x halo per stage
     static_assert(STAGE % 128 == 0 && OPER % 128 == 0, "alignment");
     static_assert(PREC == BQ_FP64 || NXC <= LS_THREADS, "one x-halo copy per thread");
@@ -72,6 +75,7 @@ template <int PREC> struct LsGeom {
 struct LsMaps {
     alignas(64) CUtensorMap in_c, in_y, in_z, in_t;   // input field: interior box, y-halo box, z-halo box, t-halo box
     alignas(64) CUtensorMap z_c, w_c;                 // interior boxes of the xpay operand and of the inner-product operand
+    alignas(64) CUtensorMap cl_c;                     // interior box of the clover store (EPI 2, 3)
 };
 
 template <typename C> struct LsParams {
@@ -211,7 +215,7 @@ template <int PREC> __device__ __forceinline__ void ls_load_site(const char* til
         for (int k = 0; k < 3; k++) unpack8(*reinterpret_cast<const uint4*>(tile + k * 128 + pos * 16), v + 8 * k);
         const float n = *reinterpret_cast<const float*>(tile + 384 + pos * 4);
 #pragma unroll
-        for (int i = 0; i < 24; i++) v[i] *= n;
+        for (int i = 0; i < 24; i++) v[i] = __fmul_rn(v[i], n);      // as load_spinor: never contracted
     } else if constexpr (PREC == BQ_FP32) {
 #pragma unroll
         for (int k = 0; k < 6; k++) {
@@ -229,8 +233,8 @@ template <int PREC> __device__ __forceinline__ void ls_load_site(const char* til
 
 template <int EPI, int RED> __host__ __device__ constexpr int ls_stages() { return (EPI == 0 && LS_MINB == 1) ? 3 : 2; }
 template <int PREC, int EPI, int RED> __host__ __device__ constexpr size_t ls_smem_bytes() {
-    return (size_t)ls_stages<EPI, RED>() * LsGeom<PREC>::STAGE + (EPI == 1 ? LsGeom<PREC>::OPER : 0) + (RED == 1 ? LsGeom<PREC>::OPER : 0) +
-           256 /* mbarriers, active list */ + (RED ? 2 * 3 * (LS_THREADS / 32) * sizeof(double) : 0);
+    return (size_t)ls_stages<EPI, RED>() * LsGeom<PREC>::STAGE + (EPI == 1 ? LsGeom<PREC>::OPER : 0) + (EPI == 1 && RED == 1 ? LsGeom<PREC>::OPER : 0) +
+           (EPI >= 2 ? LsGeom<PREC>::CLOV : 0) + 256 /* mbarriers, active list */ + (RED ? 2 * 3 * (LS_THREADS / 32) * sizeof(double) : 0);
 }
 
 template <int PREC, int RECON, int EPI, bool CPLX, int RED, bool DAG>
@@ -243,8 +247,9 @@ __global__ void __launch_bounds__(LS_THREADS, LS_MINB) hop_ls_kernel(const __gri
     unsigned char* const stage0 = ls_smem;
     unsigned char* const zbuf = ls_smem + NS * G::STAGE;
     unsigned char* const wbuf = zbuf + (EPI == 1 ? G::OPER : 0);
-    unsigned char* const ctl = wbuf + (RED == 1 ? G::OPER : 0);
-    unsigned long long* const bars = reinterpret_cast<unsigned long long*>(ctl);     // full[NS], fullz
+    unsigned char* const cbuf = wbuf + (EPI == 1 && RED == 1 ? G::OPER : 0);         // clover tiles of the block (EPI 2, 3)
+    unsigned char* const ctl = cbuf + (EPI >= 2 ? G::CLOV : 0);
+    unsigned long long* const bars = reinterpret_cast<unsigned long long*>(ctl);     // full[NS], fullz, clover
     int* const act = reinterpret_cast<int*>(ctl + 64);                              // [0] = count, [1] = mask, [2..] = list of active rhs
     double* const s_red = reinterpret_cast<double*>(ctl + 256);                     // [2][NRED][warps]
     const HopArgs<C>& a = P.a;
@@ -278,6 +283,7 @@ __global__ void __launch_bounds__(LS_THREADS, LS_MINB) hop_ls_kernel(const __gri
             act[1] = (int)mask;
             for (int s = 0; s < NS; s++) ls_mbar_init(ls_smem_u32(bars + s), 1 + LS_THREADS);
             ls_mbar_init(ls_smem_u32(bars + NS), 1);
+            ls_mbar_init(ls_smem_u32(bars + NS + 1), 1);
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         }
     }
@@ -357,6 +363,11 @@ __global__ void __launch_bounds__(LS_THREADS, LS_MINB) hop_ls_kernel(const __gri
     };
     for (int i = 0; i < NS && i < nact; i++) fill(i);
     if (tid == 0) fill_oper(0);
+    if (EPI >= 2 && tid == 32) {     // the clover blocks of the block's sites: once, for all right-hand sides (a clover tile = 3 x 192 reals)
+        const unsigned int bar = ls_smem_u32(bars + NS + 1);
+        ls_mbar_expect_tx(bar, G::CLOV);
+        ls_tma5(ls_smem_u32(cbuf), &P.m.cl_c, bar, 0, 3 * xt, y0, z0, t0);
+    }
 
     // ---- neighbour addresses inside a stage (bytes from its base) ----
     const bool wxf = r && (xh == a.Lxh - 1), wxb = !r && (xh == 0);
@@ -417,6 +428,16 @@ __global__ void __launch_bounds__(LS_THREADS, LS_MINB) hop_ls_kernel(const __gri
     for (int i = 0; i < nact; i++) {
         const int k = rhs_of(i), s = i % NS;
         const char* sb = reinterpret_cast<const char*>(stage0 + s * G::STAGE);
+        if (EPI == 3 && s8 == 0) {   // the tile's 768 / 416 bytes of z (and w): asked into L2 now, read in the epilogue
+            const char* zt = static_cast<const char*>(a.z) + (size_t)k * a.s_z + (size_t)(h >> 3) * G::TS;
+#pragma unroll
+            for (int q = 0; q < (G::TS + 127) / 128; q++) asm volatile("prefetch.global.L2 [%0];" ::"l"(zt + q * 128));
+            if (RED == 1) {
+                const char* wt = static_cast<const char*>(a.w) + (size_t)k * a.s_w + (size_t)(h >> 3) * G::TS;
+#pragma unroll
+                for (int q = 0; q < (G::TS + 127) / 128; q++) asm volatile("prefetch.global.L2 [%0];" ::"l"(wt + q * 128));
+            }
+        }
         ls_mbar_wait(ls_smem_u32(bars + s), (unsigned int)(i / NS) & 1u);
         C acc[24];
 #pragma unroll
@@ -439,12 +460,27 @@ __global__ void __launch_bounds__(LS_THREADS, LS_MINB) hop_ls_kernel(const __gri
             }
         }
         C red[3] = {0, 0, 0};
-        if (EPI == 1) {
-            ls_mbar_wait(ls_smem_u32(bars + NS), (unsigned int)i & 1u);
+        if (EPI == 2) {      // out = scale * Cl(H in): the scale already inside acc commutes with the site-diagonal multiply
+            ls_mbar_wait(ls_smem_u32(bars + NS + 1), 0u);
+            clover_site_mul<PREC, false>(cbuf, Vh, tl * 8 + s8, acc);
+        }
+        if (EPI == 1 || EPI == 3) {
             C zz[24];
-            ls_load_site<PREC>(reinterpret_cast<const char*>(zbuf) + tl * G::TS, s8, zz);
+            if (EPI == 1) {
+                ls_mbar_wait(ls_smem_u32(bars + NS), (unsigned int)i & 1u);
+                ls_load_site<PREC>(reinterpret_cast<const char*>(zbuf) + tl * G::TS, s8, zz);
 #pragma unroll
-            for (int q = 0; q < 24; q++) acc[q] += zz[q];
+                for (int q = 0; q < 24; q++) acc[q] += zz[q];
+            } else {         // out = Cl(z) + scale * H in; z (and w below) straight from global memory: requested into L2 before the hops
+                load_spinor<PREC, true>(static_cast<const char*>(a.z) + (size_t)k * a.s_z, Vh, h, zz);
+                C az[24];
+#pragma unroll
+                for (int q = 0; q < 24; q++) az[q] = zz[q];
+                ls_mbar_wait(ls_smem_u32(bars + NS + 1), 0u);
+                clover_site_mul<PREC, false>(cbuf, Vh, tl * 8 + s8, az);
+#pragma unroll
+                for (int q = 0; q < 24; q++) acc[q] += az[q];
+            }
             if (RED == 2) {
 #pragma unroll
                 for (int q = 0; q < 12; q++) {
@@ -455,7 +491,8 @@ __global__ void __launch_bounds__(LS_THREADS, LS_MINB) hop_ls_kernel(const __gri
             }
             if (RED == 1) {
                 C wv[24];
-                ls_load_site<PREC>(reinterpret_cast<const char*>(wbuf) + tl * G::TS, s8, wv);
+                if (EPI == 1) ls_load_site<PREC>(reinterpret_cast<const char*>(wbuf) + tl * G::TS, s8, wv);
+                else load_spinor<PREC, true>(static_cast<const char*>(a.w) + (size_t)k * a.s_w, Vh, h, wv);
 #pragma unroll
                 for (int q = 0; q < 12; q++) {
                     red[0] = mad(wv[2 * q + 1], acc[2 * q + 1], mad(wv[2 * q], acc[2 * q], red[0]));
@@ -517,12 +554,13 @@ static bool ls_make_map(CUtensorMap* m, const void* base, const Geom& g, int nf,
 // Can this launch take the link-stationary kernel?  (geometry, operand strides, epilogue)
 template <int PREC> static bool ls_eligible(const bq_lattice* lat, const HopMulti* m, const void* in, const void* z, const void* w, int cl_mode) {
     if constexpr (PREC == BQ_FP64) return false;
-    if (!m || !lat->mrhs_ls || cl_mode != 0) return false;
+    if (!m || !lat->mrhs_ls || cl_mode < 0 || cl_mode > 2) return false;
     const Geom& g = lat->g;
     if (m->nrhs < 2 || m->nrhs > LS_MAX_RHS) return false;
     if (g.Lxh % 8 || g.L[1] % LS_BY || g.L[2] % LS_BZ || g.L[3] % LS_BT) return false;
     const size_t slice = (size_t)(g.Lxh / 8) * g.L[1] * g.L[2] * LsGeom<PREC>::TS;
-    if (m->s_in % slice || (z && m->s_z % slice) || (w && m->s_w % slice)) return false;
+    // z and w come through TMA for the Wilson xpay epilogue (their strides must be whole t slices), by plain loads for the clover ones
+    if (m->s_in % slice || (cl_mode == 0 && ((z && m->s_z % slice) || (w && m->s_w % slice)))) return false;
     if (((uintptr_t)in & 15) || ((uintptr_t)z & 15) || ((uintptr_t)w & 15)) return false;
     return ls_get_encoder() != nullptr;
 }
@@ -543,7 +581,7 @@ static bq_status ls_launch_one(bq_lattice* lat, const LsParams<typename Prec<PRE
 // a: the HopArgs launch_hop has filled (operands, links, geometry, weights, partials); nslots_out: partial sums per rhs
 template <int PREC, int RECON>
 static bq_status ls_launch(bq_lattice* lat, const HopArgs<typename Prec<PREC>::comp>& a, bool cplx, int rmode, bool dag, const HopMulti* m,
-                           const SolverScalars* done, cudaStream_t stream) {
+                           const SolverScalars* done, cudaStream_t stream, int cl_mode) {
     using C = typename Prec<PREC>::comp;
     using G = LsGeom<PREC>;
     const Geom& g = lat->g;
@@ -558,11 +596,25 @@ static bq_status ls_launch(bq_lattice* lat, const HopArgs<typename Prec<PREC>::c
               ls_make_map<PREC>(&P.m.in_y, a.in, g, m->nrhs, P.tk_in, E, 1, LS_BZ, LS_BT) &&
               ls_make_map<PREC>(&P.m.in_z, a.in, g, m->nrhs, P.tk_in, E, LS_BY, 1, LS_BT) &&
               ls_make_map<PREC>(&P.m.in_t, a.in, g, m->nrhs, P.tk_in, G::SPLIT_T ? E / 2 : E, LS_BY, LS_BZ, 1);
-    ok = ok && ls_make_map<PREC>(&P.m.z_c, a.z ? a.z : a.in, g, m->nrhs, a.z ? P.tk_z : P.tk_in, E, LS_BY, LS_BZ, LS_BT);
-    ok = ok && ls_make_map<PREC>(&P.m.w_c, a.w ? a.w : a.in, g, m->nrhs, a.w ? P.tk_w : P.tk_in, E, LS_BY, LS_BZ, LS_BT);
+    const bool tma_zw = cl_mode == 0;
+    ok = ok && ls_make_map<PREC>(&P.m.z_c, tma_zw && a.z ? a.z : a.in, g, m->nrhs, tma_zw && a.z ? P.tk_z : P.tk_in, E, LS_BY, LS_BZ, LS_BT);
+    ok = ok && ls_make_map<PREC>(&P.m.w_c, tma_zw && a.w ? a.w : a.in, g, m->nrhs, tma_zw && a.w ? P.tk_w : P.tk_in, E, LS_BY, LS_BZ, LS_BT);
+    if (cl_mode) {
+        // the clover store of one parity as a 5-D tensor of 192-real pieces: a tile of 8 sites x 72 reals is 3 of them
+        ls_encode_fn enc = ls_get_encoder();
+        const cuuint64_t es = prec_real_bytes(PREC), piece = 192 * es;
+        const cuuint64_t dims[5] = {192, (cuuint64_t)3 * P.nxt, (cuuint64_t)g.L[1], (cuuint64_t)g.L[2], (cuuint64_t)g.L[3]};
+        const cuuint64_t strides[4] = {piece, piece * 3 * P.nxt, piece * 3 * P.nxt * g.L[1], piece * 3 * P.nxt * g.L[1] * g.L[2]};
+        const cuuint32_t box[5] = {192, 3, LS_BY, LS_BZ, LS_BT}, estr[5] = {1, 1, 1, 1, 1};
+        ok = ok && enc && enc(&P.m.cl_c, PREC == BQ_FP32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_UINT16, 5, const_cast<void*>(a.cl), dims,
+                              strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+    } else {
+        P.m.cl_c = P.m.in_c;
+    }
     if (!ok) return bq_set_error(lat, BQ_ECUDA, "bq_hop: cuTensorMapEncodeTiled failed");
     const int grid = P.nxt * P.nyb * P.nzb * (g.L[3] / LS_BT);
-    const int epi = a.z ? 1 : 0;
+    const int epi = cl_mode == 0 ? (a.z ? 1 : 0) : (cl_mode == 1 ? 2 : 3);
 #define LS_GO(E_, R_)                                                                                                   \
     do {                                                                                                                \
         if (dag) return cplx ? ls_launch_one<PREC, RECON, E_, true, 0, true>(lat, P, grid, stream)                      \
@@ -571,8 +623,14 @@ static bq_status ls_launch(bq_lattice* lat, const HopArgs<typename Prec<PREC>::c
                     : ls_launch_one<PREC, RECON, E_, false, R_, false>(lat, P, grid, stream);                           \
     } while (0)
     if (epi == 0) LS_GO(0, 0);
-    if (rmode == 0) LS_GO(1, 0);
-    if (rmode == 1) LS_GO(1, 1);
-    LS_GO(1, 2);
+    if (epi == 2) LS_GO(2, 0);
+    if (epi == 1) {
+        if (rmode == 0) LS_GO(1, 0);
+        if (rmode == 1) LS_GO(1, 1);
+        LS_GO(1, 2);
+    }
+    if (rmode == 0) LS_GO(3, 0);
+    if (rmode == 1) LS_GO(3, 1);
+    LS_GO(3, 2);
 #undef LS_GO
 }

@@ -125,8 +125,10 @@ __device__ __forceinline__ void load_spinor(const void* base, int Vh, int h, typ
     typename Prec<PREC>::comp n;
     load_spinor_raw<PREC, STREAM>(base, Vh, h, v, n);
     if constexpr (PREC == BQ_HALF) {
+        // __fmul_rn: a product of its own, never contracted into an FMA with whatever the caller adds to it — so that every
+        // kernel that loads this site sees the same 24 values bit for bit, whatever ptxas fuses around the load
 #pragma unroll
-        for (int i = 0; i < 24; i++) v[i] *= n;
+        for (int i = 0; i < 24; i++) v[i] = __fmul_rn(v[i], n);
     }
 }
 

@@ -331,3 +331,40 @@ def test_solve_multi_ls(bq, inner, method):
             assert oracle_residual(U, x[k], b[k], kappa) <= 1e-10, k
     assert np.linalg.norm(x[0] - x1) / np.linalg.norm(x1) < 1e-9
     assert abs(infos[0].inner_iters - info1.inner_iters) <= 1      # the fused inner products are summed in another order
+
+
+@pytest.mark.parametrize("prec", [1, 2])
+def test_ls_clover_schur_and_solve(bq, prec):
+    """Clover epilogues of the link-stationary kernel (clover tiles of the block in shared memory): the batched clover Schur
+    operator against the oracle and against the single-field kernels bit for bit, then a batched clover solve."""
+    import torch
+    L, kappa, csw, nrhs = (16, 4, 8, 4), 0.1215, 1.0, 5
+    U = inputs.gauge(L, 87, 0.5)
+    psis = rhs_set(L, nrhs, 88)
+    A = bqo.clover_build(U, csw, kappa)
+    Ainv = bqo.site_matrix_invert(A)
+    par = (inputs.site_parity(L) == 0)[..., None, None]
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        src = import_multi(bq, lat, psis, prec, bq.BQ_EVEN)
+        out, tmp = torch.zeros_like(src), torch.zeros_like(src)
+        n0 = bq.bq_get_counters(lat.h)["ls"]
+        bq.bq_schur_apply_multi(lat.h, out, src, tmp, nrhs, kappa, csw, prec)
+        assert bq.bq_get_counters(lat.h)["ls"] == n0 + 2, "the clover hops did not take the link-stationary kernel"
+        fb = bq.bq_field_bytes(lat.h, prec, bq.BQ_EVEN)
+        one, tmp1 = lat.field(prec, bq.BQ_EVEN), lat.field(prec, bq.BQ_EVEN)
+        for k, got in enumerate(export_multi(bq, lat, out, nrhs, prec, bq.BQ_EVEN)):
+            ref = bqo.schur_apply(U, np.where(par, psis[k], 0), kappa, A=A, Ainv=Ainv)
+            assert relmax(got, ref) < 2 * TOL[prec], (prec, k)
+            bq.bq_schur_apply(lat.h, one, src[k * fb:(k + 1) * fb], tmp1, kappa, csw, prec)
+            assert torch.equal(one, out[k * fb:(k + 1) * fb]), (prec, k)
+        b = np.stack(psis)
+        b[1] = 0
+        x = np.zeros_like(b)
+        n0 = bq.bq_get_counters(lat.h)["ls"]
+        infos = bq.bq_solve_multi(lat.h, b, x, nrhs, kappa, 1e-10, bq.bq_solve_opts(inner_prec=prec, csw=csw, check_every=3))
+        assert bq.bq_get_counters(lat.h)["ls"] > n0
+    for k in range(nrhs):
+        assert infos[k].status == 0
+        if k != 1:
+            assert oracle_residual(U, x[k], b[k], kappa, A=A) <= 1e-10, k
