@@ -24,10 +24,11 @@ bq_status bq_schur_apply_dots(bq_lattice* lat, void* out, const void* in, void* 
 
 /* Launch accounting for benchmarks: out[0] = kernels launched through this handle since creation,
  * out[1..3] = hop applications (per right-hand side) with fp64 / fp32 / half storage (each is 1320 flop x Vh sites),
- * out[4] = launches of the link-stationary multi-rhs hop kernel (hop_ls.cuh) among them,
+ * out[4] = launches of the link-stationary multi-rhs hop kernels (hop_ls.cuh, hop_lsp.cuh) among them,
  * out[5..7] = of out[1..3], the applications that were no-ops: enqueued with a batch of solver iterations after their
- *            right-hand side had converged, they return at entry (the solver's device-side `done` flag); useful = out[1..3] - out[5..7]. */
-bq_status bq_get_counters(const bq_lattice* lat, unsigned long long* out /*[8]*/);
+ *            right-hand side had converged, they return at entry (the solver's device-side `done` flag); useful = out[1..3] - out[5..7],
+ * out[8] = of out[4], the launches of the direction-split kernel (hop_lsp.cuh) made outside CUDA-graph replays. */
+bq_status bq_get_counters(const bq_lattice* lat, unsigned long long* out /*[9]*/);
 
 /* Fused BLAS-1 on one-parity internal-layout fields, exposed for tests and benchmarks.
  * All complex scalars are (re, im) pairs of doubles on the HOST; results are written to HOST doubles after a

@@ -273,12 +273,12 @@ def bq_propagator(h, src_site, S, kappa, tol, opts: bq_solve_opts | None = None,
 
 def bq_get_counters(h):
     """{'launches': all kernels, 'hop_fp64' / 'hop_fp32' / 'hop_half': hop applications per right-hand side,
-    'ls': launches of the link-stationary multi-rhs kernel, 'idle_*': hop applications that returned at entry because
+    'ls': launches of the link-stationary multi-rhs kernels, 'lsp': of those, direct launches of the direction-split one, 'idle_*': hop applications that returned at entry because
     their right-hand side had already converged (useful = hop_* - idle_*)} since handle creation."""
-    out = (ctypes.c_ulonglong * 8)()
+    out = (ctypes.c_ulonglong * 9)()
     _check(h, lib().bq_get_counters(h, out))
     return {"launches": out[0], "hop_fp64": out[1], "hop_fp32": out[2], "hop_half": out[3], "ls": out[4],
-            "idle_fp64": out[5], "idle_fp32": out[6], "idle_half": out[7]}
+            "idle_fp64": out[5], "idle_fp32": out[6], "idle_half": out[7], "lsp": out[8]}
 
 
 BQ_K = {"hop": 0, "hop_xpay": 1, "hop_clovinv": 2, "hop_clov_xpay": 3, "schur": 4, "norm2": 5, "p_update": 6, "alpha": 7,

@@ -55,11 +55,14 @@ struct bq_lattice {
     int use_graphs;          // solver: replay the batches of inner iterations as CUDA graphs (default 1; env BQ_GRAPH=0 disables)
     int mrhs_patch;          // multi-rhs hop: 1 = patch mapping where the geometry allows (default), 0 = plain (env BQ_MRHS_PATCH)
     int hop_pdl;             // single-rhs hop: programmatic dependent launch when Vh <= this (default 262144; env BQ_PDL = 0 off, or a bound)
-    int mrhs_ls;             // multi-rhs hop: 1 = link-stationary kernel (hop_ls.cuh) where it applies (default), 0 = off (env BQ_MRHS_LS)
+    int mrhs_ls;             // multi-rhs hop: 2 = link-stationary kernels (default): hop_ls.cuh for fp32 / half storage, the direction-split
+                             // hop_lsp.cuh for fp64 with >= 8 right-hand sides; 1 = hop_ls.cuh only; 3 = hop_lsp.cuh wherever it applies;
+                             // 0 = off (env BQ_MRHS_LS)
     const SolverScalars* hop_done;   // set by the solver around its inner iterations: hop launches test these `done` flags (HopArgs::done)
     unsigned long long n_launch;      // kernels launched through this handle
     unsigned long long n_hop[3];      // hop applications (per right-hand side) per storage precision
-    unsigned long long n_ls;          // launches of the link-stationary multi-rhs hop kernel (hop_ls.cuh)
+    unsigned long long n_ls;          // launches of the link-stationary multi-rhs hop kernels (hop_ls.cuh, hop_lsp.cuh)
+    unsigned long long n_lsp;         // of n_ls: direct (not graph-replayed) launches of the direction-split kernel (hop_lsp.cuh)
     unsigned long long n_hop_idle[3]; // of n_hop: applications enqueued in a batch of solver iterations after their right-hand side had
                                       // stopped — the kernel returned at entry (HopArgs::done), no flop was executed
     char err[512];

@@ -35,6 +35,7 @@ extern "C" bq_status bq_get_counters(const bq_lattice* lat, unsigned long long* 
     out[0] = lat->n_launch;
     for (int p = 0; p < 3; p++) out[1 + p] = lat->n_hop[p];
     out[4] = lat->n_ls;
+    out[8] = lat->n_lsp;
     for (int p = 0; p < 3; p++) out[5 + p] = lat->n_hop_idle[p];
     return BQ_OK;
 }

@@ -376,6 +376,7 @@ hop_kernel_mrhs(const HopArgs<typename Prec<PREC>::comp> a) {
 }
 
 #include "hop_ls.cuh"
+#include "hop_lsp.cuh"
 
 // <<<grid, block, 0, stream>>> with the programmatic-stream-serialization attribute when `pdl` (see hop_kernel)
 template <class K, class A> static void hop_launch_pdl(K kern, int grid, int block, cudaStream_t stream, const A& a, bool pdl) {
@@ -435,8 +436,10 @@ bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const void* z, 
     const bool pdl = !multi && lat->hop_pdl && g.Vh <= lat->hop_pdl;     // programmatic dependent launch on small lattices
     a.done = lat->hop_done;
     // link-stationary kernel (hop_ls.cuh) where the geometry, the operand strides and the epilogue allow
-    const bool use_ls = multi && !(dag && rmode) && ls_eligible<PREC>(lat, m, in, z, rmode == 1 ? red->w : nullptr, cl_mode);
-    if (use_ls) nslots = (g.Lxh / 8) * (g.L[1] / LS_BY) * (g.L[2] / LS_BZ) * (g.L[3] / LS_BT);
+    // direction-split pipelined form of it (hop_lsp.cuh; Wilson epilogues, all precisions) first, then the one-thread-per-site form
+    const bool use_lp = multi && !(dag && rmode) && lp_eligible<PREC>(lat, m, in, z, rmode == 1 ? red->w : nullptr, cl_mode);
+    const bool use_ls = !use_lp && multi && !(dag && rmode) && ls_eligible<PREC>(lat, m, in, z, rmode == 1 ? red->w : nullptr, cl_mode);
+    if (use_ls || use_lp) nslots = (g.Lxh / 8) * (g.L[1] / LS_BY) * (g.L[2] / LS_BZ) * (g.L[3] / LS_BT);
     a.w = nullptr; a.partials = nullptr;
     if (rmode) {
         if ((rmode != 1 && rmode != 2) || !red->sc || (rmode == 1 && !red->w) || !z)
@@ -458,9 +461,17 @@ bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const void* z, 
     else return bq_set_error(lat, BQ_EINVAL, "bq_hop: unsupported epilogue (cl_mode=%d, z=%p)", cl_mode, z);
     // the dagger hop exists without fused reductions (the CG of the normal equations reduces on the plain hop)
     if (dag && rmode) return bq_set_error(lat, BQ_EINVAL, "bq_hop: the dagger hop has no fused reduction");
-    if (use_ls) {
-        if constexpr (PREC != BQ_FP64) {
+    if (use_ls || use_lp) {
+        bool launched = false;
+        if (use_lp) {
+            BQ_TRY((lp_launch<PREC, RECON>(lat, a, cplx, rmode, dag, m, lat->hop_done, stream)));
+            lat->n_lsp++;
+            launched = true;
+        } else if constexpr (PREC != BQ_FP64) {
             BQ_TRY((ls_launch<PREC, RECON>(lat, a, cplx, rmode, dag, m, lat->hop_done, stream, cl_mode)));
+            launched = true;
+        }
+        if (launched) {
             BQ_CHECK_LAUNCH(lat);
             lat->n_hop[PREC] += nrhs;
             lat->n_ls++;

@@ -28,6 +28,9 @@
 
 #include <cuda.h>
 
+#include <cstdio>
+#include <cstdlib>
+
 #include <type_traits>
 
 #ifndef LS_BY
@@ -82,6 +85,7 @@ template <typename C> struct LsParams {
     HopArgs<C> a;
     LsMaps m;
     int nxt, nyb, nzb;           // x tiles per row; blocks in y, z
+    int gy, gz, gt;              // launch order of the blocks: bricks of nxt x gy x gz x gt blocks (ls_block_coords)
     int tk_in, tk_z, tk_w;       // t'-extent between consecutive right-hand sides of in / z / w (their byte strides in t slices)
     const SolverScalars* done;   // solver: per-rhs states whose `done` flag switches a right-hand side off (nullptr: all run)
 };
@@ -119,6 +123,41 @@ template <int BYTES> __device__ __forceinline__ void ls_cp_async(unsigned int ds
 // arrive on `bar` once all cp.async of this thread issued so far have landed (the arrival is part of the barrier's count)
 __device__ __forceinline__ void ls_cp_async_arrive(unsigned int bar) {
     asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
+}
+
+// Launch order of the blocks.  The CTAs in flight at one time (one or two per SM) work on consecutive block indices, and what
+// one block reads as halo is the interior of its neighbours: whatever two neighbours do not read within the same wave must
+// survive in L2 from one wave to the next, against a working set of ~200 MB per wave (12 right-hand sides x 148-296 blocks).
+// With the blocks in lexicographic order (x, y, z, t) a wave is a slab of 1-2 t slices and every t halo — the largest,
+// since the blocks are one site thick in t — is re-read from HBM (fp64, 12 rhs: 5.7 GB of DRAM reads where 3.6 GB are
+// compulsory).  So the index runs over compact bricks of nxt x gy x gz x gt blocks (4 x 4 x 4 where the extents divide:
+// 128 blocks ~ one wave), bricks following one another in t first.
+__host__ __device__ inline int ls_brick_dim(int n) { return n % 4 == 0 ? 4 : (n % 2 == 0 ? 2 : 1); }
+inline void ls_brick(int nyb, int nzb, int ntb, int& gy, int& gz, int& gt) {
+    gy = ls_brick_dim(nyb); gz = ls_brick_dim(nzb); gt = ls_brick_dim(ntb);
+    static int cap[3] = {0, 0, 0};     // A/B switch: BQ_LS_BRICK="y,z,t" caps the brick (1,1,1 = lexicographic order)
+    if (!cap[0]) {
+        cap[0] = cap[1] = cap[2] = 4;
+        if (const char* e = getenv("BQ_LS_BRICK")) sscanf(e, "%d,%d,%d", &cap[0], &cap[1], &cap[2]);
+        for (int i = 0; i < 3; i++) if (cap[i] < 1) cap[i] = 1;
+    }
+    while (gy > cap[0]) gy /= 2;
+    while (gz > cap[1]) gz /= 2;
+    while (gt > cap[2]) gt /= 2;
+}
+__device__ __forceinline__ void ls_block_coords(int b, int nxt, int nyb, int nzb, int gy, int gz, int gt, int& xt, int& yb, int& zb, int& tb) {
+    xt = b % nxt; b /= nxt;
+    const int iy = b % gy; b /= gy;
+    const int iz = b % gz; b /= gz;
+    const int it = b % gt; b /= gt;
+    // bricks: t fastest, then y, then z
+    const int by = nyb / gy;
+    // number of bricks in t is implied by the grid size: b = bt + nbt * (byi + by * bzi) with nbt = gridDim.x / (nxt * nyb * nzb * gt)
+    const int nbt = (int)(gridDim.x / (unsigned)(nxt * nyb * nzb * gt));
+    const int bt = b % nbt; b /= nbt;
+    const int byi = b % by;
+    const int bzi = b / by;
+    yb = byi * gy + iy; zb = bzi * gz + iz; tb = bt * gt + it;
 }
 
 // ---- one of the 8 hops with the neighbour spinor in shared memory and the link in registers (arithmetic = hop_dir) ----
@@ -256,11 +295,8 @@ __global__ void __launch_bounds__(LS_THREADS, LS_MINB) hop_ls_kernel(const __gri
 
     const int tid = threadIdx.x, s8 = tid & 7, tl = tid >> 3;
     const int ty = tl % LS_BY, tz = (tl / LS_BY) % LS_BZ, tt = tl / (LS_BY * LS_BZ);
-    int b = blockIdx.x;
-    const int xt = b % P.nxt; b /= P.nxt;
-    const int yb = b % P.nyb; b /= P.nyb;
-    const int zb = b % P.nzb;
-    const int tb = b / P.nzb;
+    int xt, yb, zb, tb;
+    ls_block_coords(blockIdx.x, P.nxt, P.nyb, P.nzb, P.gy, P.gz, P.gt, xt, yb, zb, tb);
     const int y0 = yb * LS_BY, z0 = zb * LS_BZ, t0 = tb * LS_BT;
     const int xh = 8 * xt + s8, y = y0 + ty, z = z0 + tz, t = t0 + tt;
     const int Vh = a.Vh;
@@ -591,6 +627,7 @@ static bq_status ls_launch(bq_lattice* lat, const HopArgs<typename Prec<PREC>::c
     const size_t slice = (size_t)P.nxt * g.L[1] * g.L[2] * G::TS;
     P.tk_in = (int)(m->s_in / slice); P.tk_z = a.z ? (int)(m->s_z / slice) : 0; P.tk_w = a.w ? (int)(m->s_w / slice) : 0;
     P.done = done;
+    ls_brick(P.nyb, P.nzb, g.L[3] / LS_BT, P.gy, P.gz, P.gt);
     const int E = G::TS / (int)prec_real_bytes(PREC);
     bool ok = ls_make_map<PREC>(&P.m.in_c, a.in, g, m->nrhs, P.tk_in, E, LS_BY, LS_BZ, LS_BT) &&
               ls_make_map<PREC>(&P.m.in_y, a.in, g, m->nrhs, P.tk_in, E, 1, LS_BZ, LS_BT) &&

@@ -77,7 +77,7 @@ extern "C" bq_status bq_lattice_create(int Lx, int Ly, int Lz, int Lt, const dou
         const char* pdl = getenv("BQ_PDL");           // A/B switch: programmatic dependent launch of the single-rhs hop (hop_kernels.cuh)
         lat->hop_pdl = pdl ? atoi(pdl) : 262144;
         const char* ls = getenv("BQ_MRHS_LS");        // A/B switch: link-stationary multi-rhs hop (hop_ls.cuh)
-        lat->mrhs_ls = ls ? atoi(ls) : 1;
+        lat->mrhs_ls = ls ? atoi(ls) : 2;
         const char* gph = getenv("BQ_GRAPH");         // A/B switch: CUDA-graph replay of the solver's iteration batches (solve.cu)
         lat->use_graphs = gph ? atoi(gph) : 1;
     }

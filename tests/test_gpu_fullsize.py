@@ -85,9 +85,9 @@ def test_config3_32x32x32x64_hop_every_site(bq):
 
 
 def test_config3_multirhs_x12_every_site(bq):
-    """32^3 x 64 fp32 and half storage, 12 right-hand sides in one launch (the link-stationary kernel, as kbench and
-    bench.py time it): every output site of every right-hand side against the oracle, and every right-hand side bit
-    for bit against the single-rhs kernel."""
+    """32^3 x 64 fp32, half and fp64 storage, 12 right-hand sides in one launch (the link-stationary kernels, as kbench and
+    bench.py time them: hop_ls.cuh for fp32 / half, the direction-split hop_lsp.cuh for fp64): every output site of every
+    right-hand side against the oracle, and every right-hand side bit for bit against the single-rhs kernel."""
     import torch
     L, kappa, nrhs = (32, 32, 32, 64), 0.125, 12
     seed = inputs.BASE_SEED + 3
@@ -97,15 +97,16 @@ def test_config3_multirhs_x12_every_site(bq):
     refs = [oracle_even_hop(U, p, kappa, L) for p in psis]
     with bq.Lattice(L) as lat:
         bq.bq_gauge_load(lat.h, U)
-        for prec, tol in ((bq.BQ_FP32, 1e-5), (bq.BQ_HALF, 5e-3)):
+        for prec, tol in ((bq.BQ_FP32, 1e-5), (bq.BQ_HALF, 5e-3), (bq.BQ_FP64, 1e-12)):
             fb = bq.bq_field_bytes(lat.h, prec, bq.BQ_EVEN)
             src = torch.cat([lat.import_field(p, prec, bq.BQ_ODD) for p in psis])
             out = torch.zeros(nrhs * fb, dtype=torch.uint8, device="cuda")
             one = lat.field(prec, bq.BQ_EVEN)
             for recon in (bq.BQ_RECON18, bq.BQ_RECON12):
-                n0 = bq.bq_get_counters(lat.h)["ls"]
+                c0 = bq.bq_get_counters(lat.h)
                 bq.bq_wilson_apply_multi(lat.h, out, src, nrhs, kappa, bq.BQ_EVEN, prec, recon)
-                assert bq.bq_get_counters(lat.h)["ls"] == n0 + 1
+                c1 = bq.bq_get_counters(lat.h)
+                assert c1["ls"] == c0["ls"] + 1 and c1["lsp"] == c0["lsp"] + (1 if prec == bq.BQ_FP64 else 0)
                 for k in range(nrhs):
                     bq.bq_wilson_apply(lat.h, one, src[k * fb:(k + 1) * fb], kappa, bq.BQ_EVEN, prec, recon)
                     assert torch.equal(one, out[k * fb:(k + 1) * fb]), (prec, recon, k)

@@ -368,3 +368,112 @@ def test_ls_clover_schur_and_solve(bq, prec):
         assert infos[k].status == 0
         if k != 1:
             assert oracle_residual(U, x[k], b[k], kappa, A=A) <= 1e-10, k
+
+
+# ---------------------------------------------------------------------------------------------------
+# Direction-split pipelined link-stationary kernel (hop_lsp.cuh): two threads per site, four directions each, the
+# accumulator handed over through shared memory in the order of the single-rhs kernel — so the results must again be bit
+# for bit those of hop_kernel.  By default it serves fp64 with >= 8 right-hand sides; BQ_MRHS_LS=3 (read when the handle
+# is created) sends every eligible launch through it.
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("L", LS_LATTICES)
+@pytest.mark.parametrize("prec", [0, 1, 2])
+@pytest.mark.parametrize("nrhs", [2, 3, 12])
+def test_hop_lsp_parity(bq, L, prec, nrhs, monkeypatch):
+    import torch
+    monkeypatch.setenv("BQ_MRHS_LS", "3")
+    kappa = 0.125
+    U = inputs.gauge(L, 91, 0.5)
+    psis = rhs_set(L, nrhs, 92)
+    recon = nrhs % 2
+    for bc in (None, GENERAL_BC):
+        with bq.Lattice(L, bc) as lat:
+            bq.bq_gauge_load(lat.h, U)
+            for p in (0, 1):
+                src = import_multi(bq, lat, psis, prec, 1 - p)
+                fb = bq.bq_field_bytes(lat.h, prec, p)
+                out = torch.zeros(nrhs * fb, dtype=torch.uint8, device="cuda")
+                n0 = bq.bq_get_counters(lat.h)["lsp"]
+                bq.bq_wilson_apply_multi(lat.h, out, src, nrhs, kappa, p, prec, recon)
+                assert bq.bq_get_counters(lat.h)["lsp"] == n0 + 1, "the direction-split kernel did not take this launch"
+                got = export_multi(bq, lat, out, nrhs, prec, p)
+                one = lat.field(prec, p)
+                for k in range(nrhs):
+                    ref = bqo.hop_restricted(U, psis[k], kappa, p, bc=bc)
+                    assert relmax(got[k], ref) < TOL[prec], (L, prec, nrhs, k, p)
+                    bq.bq_wilson_apply(lat.h, one, src[k * fb:(k + 1) * fb], kappa, p, prec, recon)
+                    assert torch.equal(one, out[k * fb:(k + 1) * fb]), (L, prec, nrhs, k, p)
+
+
+@pytest.mark.parametrize("prec", [0, 1, 2])
+def test_lsp_full_apply_schur_and_dagger(bq, prec, monkeypatch):
+    """[even | odd] buffers (operand stride = two fields), the xpay epilogue, the Schur operator and the dagger modes through
+    the direction-split kernel, every right-hand side against the oracle."""
+    import torch
+    monkeypatch.setenv("BQ_MRHS_LS", "3")
+    L, kappa, nrhs = (16, 4, 8, 4), 0.12, 5
+    U = inputs.gauge(L, 93, 0.4)
+    psis = rhs_set(L, nrhs, 94)
+    par = (inputs.site_parity(L) == 0)[..., None, None]
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        src = import_multi(bq, lat, psis, prec, bq.BQ_FULL)
+        out = torch.zeros_like(src)
+        n0 = bq.bq_get_counters(lat.h)["lsp"]
+        bq.bq_wilson_apply_multi(lat.h, out, src, nrhs, kappa, bq.BQ_FULL, prec, bq.BQ_RECON18)
+        assert bq.bq_get_counters(lat.h)["lsp"] == n0 + 2
+        for k, got in enumerate(export_multi(bq, lat, out, nrhs, prec, bq.BQ_FULL)):
+            assert relmax(got, bqo.dirac_apply(U, psis[k], kappa)) < TOL[prec], k
+        src_e = import_multi(bq, lat, psis, prec, bq.BQ_EVEN)
+        out_e, tmp = torch.zeros_like(src_e), torch.zeros_like(src_e)
+        bq.bq_schur_apply_multi(lat.h, out_e, src_e, tmp, nrhs, kappa, 0.0, prec)
+        assert bq.bq_get_counters(lat.h)["lsp"] == n0 + 4
+        for k, got in enumerate(export_multi(bq, lat, out_e, nrhs, prec, bq.BQ_EVEN)):
+            ref = bqo.schur_apply(U, np.where(par, psis[k], 0), kappa)
+            assert relmax(got, ref) < 2 * TOL[prec], (prec, k)
+
+
+@pytest.mark.parametrize("inner,method", [(1, 0), (2, 0), (1, 1), (0, 0)])
+def test_solve_multi_lsp(bq, inner, method, monkeypatch):
+    """Batched Wilson solve whose hops all run through the direction-split kernel (fused inner products in role B, per-rhs done
+    flags, dagger hops for CGNR, fp64 outer residuals); one zero and one tiny right-hand side stop early."""
+    monkeypatch.setenv("BQ_MRHS_LS", "3")
+    L, kappa, nrhs = (16, 4, 4, 8), 0.1215, 6
+    U = inputs.gauge(L, 95, 0.5)
+    b = np.stack(rhs_set(L, nrhs, 96))
+    b[1] = 0
+    b[2] *= 1e-6
+    x = np.zeros_like(b)
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        infos = bq.bq_solve_multi(lat.h, b, x, nrhs, kappa, 1e-10, bq.bq_solve_opts(inner_prec=inner, method=method, check_every=3))
+        assert bq.bq_get_counters(lat.h)["lsp"] > 0
+        x1 = np.zeros_like(b[0])
+        info1 = bq.bq_solve(lat.h, b[0], x1, kappa, 1e-10, bq.bq_solve_opts(inner_prec=inner, method=method, check_every=3))
+    for k in range(nrhs):
+        assert infos[k].status == 0
+        if k == 1:
+            assert not x[k].any()
+        else:
+            assert oracle_residual(U, x[k], b[k], kappa) <= 1e-10, k
+    assert np.linalg.norm(x[0] - x1) / np.linalg.norm(x1) < 1e-9
+    assert abs(infos[0].inner_iters - info1.inner_iters) <= 1      # the fused inner products are summed in another order
+
+
+def test_lsp_is_the_default_for_fp64_batches(bq):
+    """Without the switch: fp64 with >= 8 right-hand sides takes the direction-split kernel, fp32 the one-thread-per-site one."""
+    import torch
+    L, kappa, nrhs = (16, 4, 4, 4), 0.125, 8
+    U = inputs.gauge(L, 97, 0.5)
+    psis = rhs_set(L, nrhs, 98)
+    with bq.Lattice(L) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        for prec, want in ((0, 1), (1, 0)):
+            src = import_multi(bq, lat, psis, prec, 1)
+            out = torch.zeros_like(src)
+            c0 = bq.bq_get_counters(lat.h)
+            bq.bq_wilson_apply_multi(lat.h, out, src, nrhs, kappa, 0, prec, bq.BQ_RECON18)
+            c1 = bq.bq_get_counters(lat.h)
+            assert c1["ls"] == c0["ls"] + 1 and c1["lsp"] == c0["lsp"] + want, (prec, c0, c1)
+            for k, got in enumerate(export_multi(bq, lat, out, nrhs, prec, 0)):
+                assert relmax(got, bqo.hop_restricted(U, psis[k], kappa, 0)) < TOL[prec], (prec, k)
