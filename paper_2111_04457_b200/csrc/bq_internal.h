@@ -58,6 +58,7 @@ struct bq_lattice {
     int mrhs_ls;             // multi-rhs hop: 2 = link-stationary kernels (default): hop_ls.cuh for fp32 / half storage, the direction-split
                              // hop_lsp.cuh for fp64 with >= 8 right-hand sides; 1 = hop_ls.cuh only; 3 = hop_lsp.cuh wherever it applies;
                              // 0 = off (env BQ_MRHS_LS)
+    int hop_small;           // single-rhs hop, fp32: the uncapped-register build of the kernel when Vh <= this (default 2 x SMs x 128 = 37888: every CTA resident at once; env BQ_HOP_SMALL)
     const SolverScalars* hop_done;   // set by the solver around its inner iterations: hop launches test these `done` flags (HopArgs::done)
     unsigned long long n_launch;      // kernels launched through this handle
     unsigned long long n_hop[3];      // hop applications (per right-hand side) per storage precision

@@ -253,8 +253,15 @@ __device__ __forceinline__ void hop_site(const HopArgs<typename Prec<PREC>::comp
     store_spinor<PREC, true>(out, Vh, h, acc);
 }
 
-template <int PREC, int RECON, int EPI, bool CPLX, int RED, bool DAG = false>
-__global__ void __launch_bounds__(HOP_BLOCK, PREC == BQ_FP64 ? HOP_MINB_64 : (PREC == BQ_FP32 ? HOP_MINB_LO : HOP_MINB_HALF))
+// SMALL: the same kernel compiled without a register cap, for lattices that do not fill the chip (16^4: 256 CTAs, 7 warps per SM):
+// there the hop is a chain of L2 round trips, not a bandwidth matter, and with 255 registers ptxas keeps the loads of more
+// directions in flight at once.  fp32 storage, real boundary phases, no dagger.  Measured (profiles/r2_small_lattice_ab.txt, A/B in one
+// call, BQ_HOP_SMALL=0 vs on): 16^4: hop 7.0 -> 4.7 us (18-real), 6.2 -> 5.6 us (12-real), Schur operator 13.2 -> 9.2 us, BiCGStab
+// iteration 55.2 -> 51.0 us; 16^3 x 32 (512 CTAs: two waves at the 2 CTAs per SM the uncapped build allows): 8.6 -> 9.0 us, worse — hence the
+// bound Vh <= 2 x SMs x 128.  Half storage gained on the bare hop (5.4 -> 4.7 us) but lost on the whole iteration (45.1 -> 47.3 us) and keeps
+// the capped build.
+template <int PREC, int RECON, int EPI, bool CPLX, int RED, bool DAG = false, bool SMALL = false>
+__global__ void __launch_bounds__(HOP_BLOCK, SMALL ? 1 : (PREC == BQ_FP64 ? HOP_MINB_64 : (PREC == BQ_FP32 ? HOP_MINB_LO : HOP_MINB_HALF)))
 hop_kernel(const HopArgs<typename Prec<PREC>::comp> a) {
     using C = typename Prec<PREC>::comp;
     // Programmatic dependent launch (small lattices, where a hop lasts a few microseconds and the launch latency between two
@@ -434,6 +441,7 @@ bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const void* z, 
     }
     const int rmode = red ? red->mode : 0;
     const bool pdl = !multi && lat->hop_pdl && g.Vh <= lat->hop_pdl;     // programmatic dependent launch on small lattices
+    const bool small = !multi && PREC == BQ_FP32 && g.Vh <= lat->hop_small;
     a.done = lat->hop_done;
     // link-stationary kernel (hop_ls.cuh) where the geometry, the operand strides and the epilogue allow
     // direction-split pipelined form of it (hop_lsp.cuh; Wilson epilogues, all precisions) first, then the one-thread-per-site form
@@ -500,6 +508,7 @@ bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const void* z, 
             else hop_kernel_mrhs<PREC, RECON, E, false, R><<<grid, block, 0, stream>>>(a);           \
         } else {                                                                                    \
             if (cplx) hop_launch_pdl(hop_kernel<PREC, RECON, E, true, R>, grid, HOP_BLOCK, stream, a, pdl);        \
+            else if (small) hop_launch_pdl(hop_kernel<PREC, RECON, E, false, R, false, PREC == BQ_FP32>, grid, HOP_BLOCK, stream, a, pdl); \
             else hop_launch_pdl(hop_kernel<PREC, RECON, E, false, R>, grid, HOP_BLOCK, stream, a, pdl);            \
         }                                                                                           \
     } while (0)

@@ -78,6 +78,13 @@ extern "C" bq_status bq_lattice_create(int Lx, int Ly, int Lz, int Lt, const dou
         lat->hop_pdl = pdl ? atoi(pdl) : 262144;
         const char* ls = getenv("BQ_MRHS_LS");        // A/B switch: link-stationary multi-rhs hop (hop_ls.cuh)
         lat->mrhs_ls = ls ? atoi(ls) : 2;
+        const char* sm = getenv("BQ_HOP_SMALL");      // A/B switch: uncapped-register hop kernel on small lattices (hop_kernels.cuh)
+        int nsm = 148, cur = 0;                       // default: lattices whose CTAs (128 sites each) are all resident at once at 2 CTAs per SM
+        if (cudaGetDevice(&cur) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, cur) != cudaSuccess) {
+            cudaGetLastError();
+            nsm = 148;
+        }
+        lat->hop_small = sm ? atoi(sm) : 2 * nsm * 128;
         const char* gph = getenv("BQ_GRAPH");         // A/B switch: CUDA-graph replay of the solver's iteration batches (solve.cu)
         lat->use_graphs = gph ? atoi(gph) : 1;
     }
