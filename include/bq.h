@@ -172,10 +172,10 @@ typedef struct {
     int inner_prec;    /* bq_prec: BQ_FP64 = plain fp64 BiCGStab, no outer loop; BQ_FP32 / BQ_HALF = defect correction */
     int recon;         /* bq_recon used by the inner operator (the fp64 outer operator always uses 18 reals)          */
     double csw;        /* 0 = Wilson; otherwise the clover term is built for (csw, kappa)                              */
-    double inner_tol;  /* relative residual reduction asked of one inner solve; <= 0 = default (1e-5 fp32, 5e-2 half)    */
+    double inner_tol;  /* relative residual reduction asked of one inner solve; <= 0 = default (1e-5 fp32, 2e-3 half)    */
     int max_inner;     /* cap on inner iterations per outer cycle; <= 0 = default (1000 fp32/fp64, 100 half)          */
     int max_outer;     /* cap on outer cycles; <= 0 = default (50)                                                    */
-    int check_every;   /* inner iterations between host polls of the device-side convergence flag; <= 0 = default (8) */
+    int check_every;   /* inner iterations between host polls of the device-side convergence flag; <= 0 = default (8; half: 4) */
     int method;        /* bq_method: BQ_BICGSTAB (0, default) or BQ_CGNR = CG on the normal equations M^^dag M^ e = M^^dag r   */
     int lexical;       /* 0 (default): even-odd preconditioned Schur system; 1: BiCGStab on the full matrix D itself
                           (the paper's `lex` operator); bq_solve only, BQ_BICGSTAB only       */
