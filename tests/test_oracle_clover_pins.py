@@ -143,3 +143,64 @@ def test_p9_clover_schur(rough):
     x, info = bqo.bicgstab(U, b, kappa, tol=1e-12, A=A)
     assert info["status"] == 0
     assert np.linalg.norm(x.reshape(-1) - np.linalg.solve(D, b.reshape(-1))) / np.linalg.norm(x) < 1e-11
+
+
+# ---------------------------------------------------------------------------------------------------
+# P6 in every plane.  test_p6_abelian_flux_field_strength fixes F only in the x-y plane; a mistake in the leaf construction of
+# another plane (a transposed pair of directions, a wrong shift, a sign) or in which sigma_mu_nu meets which F_mu_nu would pass
+# it.  The same closed form holds in each of the six planes: constant abelian flux B in the (mu, nu) plane.
+# ---------------------------------------------------------------------------------------------------
+def flux_background_plane(L, mu, nu, k=1):
+    """U_mu(x) = exp(-i B x_nu T), U_nu(x) = exp(+i B L_nu x_mu T) on x_nu = L_nu - 1, else 1; B = 2 pi k / (L_mu L_nu), T = diag(1, 1, -2):
+    every (mu, nu) plaquette equals exp(i B T), every other plaquette is 1.  Array axes: U[t, z, y, x, direction]."""
+    B = 2 * np.pi * k / (L[mu] * L[nu])
+    U = inputs.unit_gauge(L)
+    d = np.diag(T8).real
+    ax = {0: 3, 1: 2, 2: 1, 3: 0}                    # lattice direction -> array axis
+    for c in range(L[nu]):
+        idx = [slice(None)] * 4
+        idx[ax[nu]] = c
+        U[tuple(idx) + (mu,)] = np.diag(np.exp(-1j * B * c * d))
+    for c in range(L[mu]):
+        idx = [slice(None)] * 4
+        idx[ax[nu]] = L[nu] - 1
+        idx[ax[mu]] = c
+        U[tuple(idx) + (nu,)] = np.diag(np.exp(1j * B * L[nu] * c * d))
+    return U, B
+
+
+PLANES = [(0, 1), (0, 2), (0, 3), (1, 2), (1, 3), (2, 3)]
+
+
+@pytest.mark.parametrize("mu,nu", PLANES)
+def test_p6_abelian_flux_in_every_plane(mu, nu):
+    L = [2, 2, 2, 2]
+    L[mu], L[nu] = 6, 4                               # different extents: a transposed pair of directions changes B
+    L = tuple(L)
+    U, B = flux_background_plane(L, mu, nu)
+    expect = np.diag([np.sin(B), np.sin(B), -np.sin(2 * B)]).astype(complex)
+    for a, b in PLANES:
+        F = bqo.field_strength(U, a, b)
+        if (a, b) == (mu, nu):
+            assert np.abs(F - expect).max() < 1e-15, (mu, nu)
+            assert np.abs(bqo.field_strength(U, b, a) + expect).max() < 1e-15
+        else:
+            assert np.abs(F).max() < 1e-15, (mu, nu, a, b)
+
+
+@pytest.mark.parametrize("mu,nu", PLANES)
+def test_clover_matrix_pairs_sigma_with_the_right_plane(mu, nu):
+    """On the flux background of plane (mu, nu) the site matrix is exactly 1 - csw kappa sigma_mu_nu (x) diag(sin B, sin B, -sin 2B), with
+    sigma_mu_nu = (i/2)[gamma_mu, gamma_nu] built here from the gamma matrices that P1 pins: which sigma multiplies which F, and with
+    which sign, in every plane."""
+    L = [2, 2, 2, 2]
+    L[mu], L[nu] = 6, 4
+    L = tuple(L)
+    csw, kappa = 1.3, 0.11
+    U, B = flux_background_plane(L, mu, nu)
+    g = [bqo.gamma(m) for m in range(4)]
+    sig = 0.5j * (g[mu] @ g[nu] - g[nu] @ g[mu])
+    F = np.diag([np.sin(B), np.sin(B), -np.sin(2 * B)]).astype(complex)
+    expect = np.eye(12) - csw * kappa * np.kron(sig, F)          # index = 3 * spin + colour
+    A = bqo.clover_build(U, csw, kappa)
+    assert np.abs(A - expect).max() < 1e-14, (mu, nu)
