@@ -94,6 +94,37 @@ def test_hop_parity(bq, L, prec, recon):
                 assert np.all(got[~np.broadcast_to(mask, got.shape)] == 0)
 
 
+@pytest.mark.parametrize("L", [(8, 8, 8, 8), (6, 6, 4, 10)])
+@pytest.mark.parametrize("recon", RECONS)
+def test_small_lattice_build_of_the_fp32_hop(bq, L, recon, monkeypatch):
+    """On lattices whose CTAs are all resident at once the fp32 hop runs an uncapped-register build of the same kernel
+    (hop_kernel<..., SMALL>; BQ_HOP_SMALL is read when the handle is made).  Both builds against the oracle, and bit for bit against each
+    other: plain hop, xpay / clover epilogues through the Schur operator with its fused inner products."""
+    import torch
+    kappa, csw = 0.125, 1.0
+    U, psi = make_case(L, 23, 0.5)
+    ref = bqo.hop_restricted(U, psi, kappa, 0)
+    outs = {}
+    for small in ("0", "1000000"):
+        monkeypatch.setenv("BQ_HOP_SMALL", small)
+        with bq.Lattice(L) as lat:
+            bq.bq_gauge_load(lat.h, U)
+            src = lat.import_field(psi, bq.BQ_FP32, bq.BQ_ODD)
+            out = lat.field(bq.BQ_FP32, bq.BQ_EVEN)
+            bq.bq_wilson_apply(lat.h, out, src, kappa, bq.BQ_EVEN, bq.BQ_FP32, recon)
+            assert relmax(lat.export_field(out, bq.BQ_FP32, bq.BQ_EVEN), ref) < TOL[bq.BQ_FP32], (L, recon, small)
+            src_e = lat.import_field(psi, bq.BQ_FP32, bq.BQ_EVEN)
+            res = [out.clone()]
+            for c in (0.0, csw):
+                o, tmp = lat.field(bq.BQ_FP32, bq.BQ_EVEN), lat.field(bq.BQ_FP32, bq.BQ_EVEN)
+                d1 = bq.bq_schur_apply_dots(lat.h, o, src_e, tmp, kappa, c, bq.BQ_FP32, recon, src_e)        # <w, out>
+                d2, d3 = bq.bq_schur_apply_dots(lat.h, o, src_e, tmp, kappa, c, bq.BQ_FP32, recon)           # <out, in>, <out, out>
+                res += [o.clone(), torch.tensor([d1.real, d1.imag, d2.real, d2.imag, d3], dtype=torch.float64)]
+            outs[small] = res
+    for x, y in zip(outs["0"], outs["1000000"]):
+        assert torch.equal(x, y)
+
+
 @pytest.mark.parametrize("prec", PRECS)
 @pytest.mark.parametrize("recon", RECONS)
 def test_full_wilson_apply(bq, prec, recon):
