@@ -43,6 +43,9 @@
 #define LS_BT 1
 #endif
 
+#ifndef LS_LINK_NOALLOC
+#define LS_LINK_NOALLOC 1     // fp32 links of the prologue: ld.global.nc.L1::no_allocate (A/B switch; x12 hop 637.4 -> 630.4 us, x2 193.7 -> 188.5 us)
+#endif
 constexpr int LS_NT = LS_BY * LS_BZ * LS_BT;      // tiles (rows of 8 sites) per block
 constexpr int LS_THREADS = 8 * LS_NT;             // one thread per output site
 constexpr int LS_MAX_RHS = 32;                    // right-hand sides per launch (active list = one ballot)
@@ -178,6 +181,23 @@ __device__ __forceinline__ void ls_load_link(LsLink<PREC, RECON>& L, const void*
             L.l1 = make_uint4(d.x, d.y, 0u, 0u);
             L.lt = 0u;
         }
+    } else if constexpr (PREC == BQ_FP32 && LS_LINK_NOALLOC) {
+        // read-only streaming loads that do not allocate in L1 (ld.global.nc.L1::no_allocate): same values as load_link
+        using A = LinkAddr<PREC, RECON>;
+        const char* bp = static_cast<const char*>(ublock);
+        constexpr int NR = (RECON == BQ_RECON12) ? 12 : 18;
+#pragma unroll
+        for (int k = 0; k < NR / 4; k++) {
+            float4 d;
+            asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(d.x), "=f"(d.y), "=f"(d.z), "=f"(d.w) : "l"(bp + A::word(Vh, idx, k)));
+            L.u[4 * k] = d.x; L.u[4 * k + 1] = d.y; L.u[4 * k + 2] = d.z; L.u[4 * k + 3] = d.w;
+        }
+        if constexpr (NR == 18) {
+            float2 d;
+            asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(d.x), "=f"(d.y) : "l"(bp + A::tail(Vh, idx)));
+            L.u[16] = d.x; L.u[17] = d.y;
+        }
+        if constexpr (NR == 12) reconstruct_row2(L.u);
     } else {
         load_link<PREC, RECON, true>(ublock, Vh, idx, L.u);    // 12-real: row 2 rebuilt here, once for all right-hand sides
     }
