@@ -361,7 +361,7 @@ __global__ void __launch_bounds__(LP_THREADS, PREC == BQ_FP64 ? 1 : 2) hop_lsp_k
 
     // ---- the pipeline: step i = A on right-hand side i, B on right-hand side i - 1 ----
     for (int i = 0; i <= nact; i++) {
-        if (lp_tid() < LP_SITES) {
+        if (!roleB) {       // (a bool that ptxas keeps in a predicate register: no S2R on the critical path of the step)
             if (i < nact) {
                 const char* cb = reinterpret_cast<const char*>(lp_smem) + Q::R_C + (i % Q::NC) * Q::CS;
                 const char* hb = reinterpret_cast<const char*>(lp_smem) + Q::R_A + (i % Q::NA) * Q::AHS;
@@ -471,7 +471,7 @@ __global__ void __launch_bounds__(LP_THREADS, PREC == BQ_FP64 ? 1 : 2) hop_lsp_k
             }
         }
         __syncthreads();     // A is done with C(i), AH(i) and has handed right-hand side i over; B is done with C(i-1), BH(i-1)
-        if (RED && i >= 1 && lp_tid() >= LP_SITES && lp_tid() < LP_SITES + NRED) {
+        if (RED && i >= 1 && roleB && lp_tid() < LP_SITES + NRED) {
             const int j = i - 1, q0 = lp_tid() - LP_SITES;
             const double* sw = s_red + (j & 1) * NRED * (LP_SITES / 32) + q0 * (LP_SITES / 32);
             double v = 0;
