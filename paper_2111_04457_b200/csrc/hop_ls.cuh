@@ -22,8 +22,9 @@
 // Per (site, rhs) the arithmetic is hop.cuh's, direction by direction in the same order, so results are bit for bit
 // those of hop_kernel / hop_kernel_mrhs.  fp32 and half storage; all four epilogues (Wilson and clover) with the fused reductions:
 // for the clover ones the block's clover tiles sit in shared memory for all right-hand sides (one more TMA copy per block).
-// Needs Lx % 16 == 0 (tiles are pieces of x-rows) and extents divisible by the block; anything else (and fp64, clover
-// epilogues) takes hop_kernel_mrhs.
+// Needs Lx % 16 == 0 (tiles are pieces of x-rows) and extents divisible by the block; anything else takes hop_kernel_mrhs.  fp64 (288
+// link registers do not exist) takes the direction-split form of this kernel, hop_lsp.cuh, from 8 right-hand sides on.  Blocks are
+// launched in 4 x 4 x 4 bricks (ls_block_coords) so that the CTAs in flight share their halos in L2.
 #pragma once
 
 #include <cuda.h>
