@@ -477,3 +477,28 @@ def test_lsp_is_the_default_for_fp64_batches(bq):
             assert c1["ls"] == c0["ls"] + 1 and c1["lsp"] == c0["lsp"] + want, (prec, c0, c1)
             for k, got in enumerate(export_multi(bq, lat, out, nrhs, prec, 0)):
                 assert relmax(got, bqo.hop_restricted(U, psis[k], kappa, 0)) < TOL[prec], (prec, k)
+
+
+@pytest.mark.parametrize("nrhs", [16, 19])
+def test_lsp_fp64_full_and_chunked_batches(bq, nrhs):
+    """fp64, default kernel choice: 16 right-hand sides (the most one launch holds) and 19 (two chunks of 10 + 9, both >= 8) go through the
+    direction-split kernel; every right-hand side against the oracle and bit for bit against the single-rhs kernel."""
+    import torch
+    L, kappa = (16, 4, 8, 2), 0.125
+    U = inputs.gauge(L, 101, 0.5)
+    psis = rhs_set(L, nrhs, 102)
+    with bq.Lattice(L, GENERAL_BC) as lat:
+        bq.bq_gauge_load(lat.h, U)
+        src = import_multi(bq, lat, psis, 0, 1)
+        fb = bq.bq_field_bytes(lat.h, 0, 0)
+        out = torch.zeros(nrhs * fb, dtype=torch.uint8, device="cuda")
+        c0 = bq.bq_get_counters(lat.h)
+        bq.bq_wilson_apply_multi(lat.h, out, src, nrhs, kappa, 0, 0, bq.BQ_RECON18)
+        c1 = bq.bq_get_counters(lat.h)
+        nlaunch = (nrhs + 15) // 16
+        assert c1["lsp"] == c0["lsp"] + nlaunch and c1["ls"] == c0["ls"] + nlaunch
+        one = lat.field(0, 0)
+        for k, got in enumerate(export_multi(bq, lat, out, nrhs, 0, 0)):
+            assert relmax(got, bqo.hop_restricted(U, psis[k], kappa, 0, bc=GENERAL_BC)) < TOL[0], k
+            bq.bq_wilson_apply(lat.h, one, src[k * fb:(k + 1) * fb], kappa, 0, 0, bq.BQ_RECON18)
+            assert torch.equal(one, out[k * fb:(k + 1) * fb]), k
