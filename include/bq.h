@@ -263,6 +263,51 @@ bq_status bq_dd_wilson_apply(bq_lattice* const* ranks, int nranks, void* const* 
 bq_status bq_dd_solve(bq_lattice* const* ranks, int nranks, const double* const* b, double* const* x, double kappa, double tol,
                       int max_iter, bq_solve_info* info);
 
+/* ---------------------------------------------------------------------------------------------
+ * A reduction for callers that cannot allocate device memory.
+ *
+ * Every other call of this library that sums over a field (the solver's |r|^2 and inner products) keeps its
+ * per-block partial sums in a workspace the handle obtains with cudaMalloc on first use.  That is a problem for a host
+ * program which has given the whole GPU to an allocator of its own (a deep-learning framework's caching allocator, a
+ * serving process with a fixed arena: a foreign cudaMalloc fails or eats into the arena), for code that runs while
+ * another thread captures a stream in the global capture mode (cudaMalloc is forbidden there and breaks that capture),
+ * and for monitoring loops that must not stall the device on an allocation.  This one entry point serves them:
+ *
+ *   *result = |a|^2 = sum over the nsites sites of a, and the 24 reals of each, of v^2
+ *
+ * (the squared norm the solver's stopping test of invert(), is built on).  It creates no handle, calls no
+ * cudaMalloc / cudaFree / allocating library routine, and uses a fixed scratch array compiled into libbq.so:
+ * BQ_NOALLOC_SCRATCH_BYTES of device memory that EVERY GPU on which the library is loaded holds until the process
+ * exits, whether or not this call is ever made.
+ *
+ *   a       DEVICE pointer, 16-byte aligned: an internal-layout field of precision prec as bq_field_import makes it —
+ *           one parity (nsites = V/2) or [even | odd] (nsites = V); the caller owns it, it is only read.
+ *   nsites  sites in a; a multiple of 8, at most BQ_NOALLOC_MAX_SITES (one scratch slot per 1024 sites) — a larger field
+ *           is refused with BQ_EINVAL and a message that says so; sum it in pieces.  nsites = 0 gives 0.
+ *   result  DEVICE pointer to one double, 8-byte aligned, the caller's; written by the kernel (no host synchronisation:
+ *           read it after the stream has reached this point).
+ *   stream  cudaStream_t of the CURRENT device (NULL = legacy default stream): one small memset node + one kernel.
+ *   err     optional HOST buffer of errlen bytes that receives the reason when the call does not return BQ_OK.
+ *
+ * Arithmetic: as bq_blas_norm2 / the solver — fp64 throughout for BQ_FP64; for BQ_FP32 and BQ_HALF (mantissa x site
+ * norm) squares are summed in fp32 per thread and in fp64 across threads.  The order of the additions is fixed, so the
+ * result is bitwise reproducible, but it is not the order of the handle-based path: the two agree to rounding
+ * (1e-13 relative in fp64, 1e-6 in fp32 / half), not bit for bit.
+ *
+ * First call on a device: looks up that device's copy of the scratch array (cudaGetSymbolAddress, with the device
+ * current; this may also make the CUDA runtime load the library's kernels).  Make that first call at start-up — in
+ * particular before any stream capture begins — so that later calls are a memset and a launch and nothing else.
+ * Sharing: all calls on one device use the same scratch array, which keeps what the previous call left in it.  The
+ * arrival counter is cleared on `stream` before every launch; the partial sums are overwritten before they are read.
+ * Consequently two calls that may overlap on the GPU (different streams without an ordering between them, or two host
+ * threads) race on the array and give garbage: order them on one stream or with events.
+ * Errors: BQ_EINVAL (NULL / misaligned pointer, bad prec, nsites not a multiple of 8 or beyond the maximum), BQ_ECUDA.
+ * --------------------------------------------------------------------------------------------- */
+#define BQ_NOALLOC_MAX_SITES 16777216             /* 16384 scratch slots x 1024 sites (48^3 x 96 is 10.6 M sites) */
+#define BQ_NOALLOC_SCRATCH_BYTES (131072 + 256)   /* 16384 partial sums of 8 bytes + a 256-byte slot for the arrival counter */
+bq_status bq_field_norm2_noalloc(const void* a, long long nsites, bq_prec prec, double* result, void* stream, char* err,
+                                 size_t errlen);
+
 #ifdef __cplusplus
 }
 #endif

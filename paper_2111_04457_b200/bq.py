@@ -31,6 +31,7 @@ EXPORTS = [
     "bq_blas_bicg_update", "bq_get_counters", "bq_bench_kernel", "bq_schur_apply_dots",
     "bq_wilson_apply_multi", "bq_schur_apply_multi", "bq_bench_kernel_multi", "bq_solve_multi", "bq_dirac_apply_mode", "bq_schur_apply_mode", "bq_propagator",
     "bq_lattice_create_sub", "bq_dd_face_bytes", "bq_dd_pack", "bq_dd_unpack", "bq_dd_wilson_apply", "bq_dd_solve",
+    "bq_field_norm2_noalloc",
 ]
 
 
@@ -100,6 +101,7 @@ def lib():
         L.bq_dd_unpack.argtypes = [_vp, _vp, _pp, _d, _i, _i, _i, _vp]
         L.bq_dd_wilson_apply.argtypes = [_pp, _i, _pp, _pp, _d, _i, _i, _i, _vp]
         L.bq_dd_solve.argtypes = [_pp, _i, _pp, _pp, _d, _d, _i, ctypes.POINTER(bq_solve_info)]
+        L.bq_field_norm2_noalloc.argtypes = [_vp, ctypes.c_longlong, _i, _vp, _vp, ctypes.c_char_p, ctypes.c_size_t]
         for name in EXPORTS:
             if name not in ("bq_status_string", "bq_last_error"):
                 getattr(L, name).restype = _i
@@ -306,6 +308,16 @@ def bq_blas_norm2(h, a, prec):
     r = ctypes.c_double(0)
     _check(h, lib().bq_blas_norm2(h, _ptr(a), prec, ctypes.byref(r)))
     return r.value
+
+
+def bq_field_norm2_noalloc(a, nsites, prec, result, stream=None):
+    """|a|^2 of an internal-layout field of nsites sites into `result` (one float64 on the device) — the entry point for
+    callers that must not allocate device memory (include/bq.h): no handle, no workspace; its scratch is a fixed array
+    inside libbq.so.  Nothing is synchronised: read `result` once the stream has got there."""
+    err = ctypes.create_string_buffer(512)
+    st = lib().bq_field_norm2_noalloc(_ptr(a), int(nsites), prec, _ptr(result), _stream_ptr(stream), err, len(err))
+    if st != BQ_OK:
+        raise BqError(st, f"{lib().bq_status_string(st).decode()}: {err.value.decode()}")
 
 
 def bq_blas_cdot(h, a, b, prec):
