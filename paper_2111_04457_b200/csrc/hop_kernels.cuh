@@ -386,14 +386,14 @@ hop_kernel_mrhs(const HopArgs<typename Prec<PREC>::comp> a) {
 #include "hop_lsp.cuh"
 
 // <<<grid, block, 0, stream>>> with the programmatic-stream-serialization attribute when `pdl` (see hop_kernel)
-template <class K, class A> static void hop_launch_pdl(K kern, int grid, int block, cudaStream_t stream, const A& a, bool pdl) {
+template <class K, class A> static cudaError_t hop_launch_pdl(K kern, int grid, int block, cudaStream_t stream, const A& a, bool pdl) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = 0; cfg.stream = stream;
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
-    cudaLaunchKernelEx(&cfg, kern, a);
+    return cudaLaunchKernelEx(&cfg, kern, a);
 }
 
 template <int PREC, int RECON>
@@ -497,8 +497,8 @@ bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const void* z, 
             if (cplx) hop_kernel_mrhs<PREC, RECON, E, true, 0, true><<<grid, block, 0, stream>>>(a);  \
             else hop_kernel_mrhs<PREC, RECON, E, false, 0, true><<<grid, block, 0, stream>>>(a);      \
         } else {                                                                                    \
-            if (cplx) hop_launch_pdl(hop_kernel<PREC, RECON, E, true, 0, true>, grid, HOP_BLOCK, stream, a, pdl);   \
-            else hop_launch_pdl(hop_kernel<PREC, RECON, E, false, 0, true>, grid, HOP_BLOCK, stream, a, pdl);       \
+            if (cplx) lerr = hop_launch_pdl(hop_kernel<PREC, RECON, E, true, 0, true>, grid, HOP_BLOCK, stream, a, pdl);   \
+            else lerr = hop_launch_pdl(hop_kernel<PREC, RECON, E, false, 0, true>, grid, HOP_BLOCK, stream, a, pdl);       \
         }                                                                                           \
     } while (0)
 #define BQ_HOP_LAUNCH(E, R)                                                                         \
@@ -507,11 +507,12 @@ bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const void* z, 
             if (cplx) hop_kernel_mrhs<PREC, RECON, E, true, R><<<grid, block, 0, stream>>>(a);       \
             else hop_kernel_mrhs<PREC, RECON, E, false, R><<<grid, block, 0, stream>>>(a);           \
         } else {                                                                                    \
-            if (cplx) hop_launch_pdl(hop_kernel<PREC, RECON, E, true, R>, grid, HOP_BLOCK, stream, a, pdl);        \
-            else if (small) hop_launch_pdl(hop_kernel<PREC, RECON, E, false, R, false, PREC == BQ_FP32>, grid, HOP_BLOCK, stream, a, pdl); \
-            else hop_launch_pdl(hop_kernel<PREC, RECON, E, false, R>, grid, HOP_BLOCK, stream, a, pdl);            \
+            if (cplx) lerr = hop_launch_pdl(hop_kernel<PREC, RECON, E, true, R>, grid, HOP_BLOCK, stream, a, pdl);        \
+            else if (small) lerr = hop_launch_pdl(hop_kernel<PREC, RECON, E, false, R, false, PREC == BQ_FP32>, grid, HOP_BLOCK, stream, a, pdl); \
+            else lerr = hop_launch_pdl(hop_kernel<PREC, RECON, E, false, R>, grid, HOP_BLOCK, stream, a, pdl);            \
         }                                                                                           \
     } while (0)
+    cudaError_t lerr = cudaSuccess;   // status of cudaLaunchKernelEx (the <<<>>> launches report through cudaGetLastError below)
     // fused reductions exist for the xpay epilogues only (the second hop of M^, which produces v and t)
     if (dag) {
         switch (epi) {
@@ -534,6 +535,7 @@ bq_status launch_hop(bq_lattice* lat, void* out, const void* in, const void* z, 
     }
 #undef BQ_HOP_LAUNCH
 #undef BQ_HOP_LAUNCH_DAG
+    BQ_CUDA(lat, lerr);
     BQ_CHECK_LAUNCH(lat);
     lat->n_hop[PREC] += nrhs;     // counted per right-hand side: each is 1320 flop x Vh sites
     if (rmode) {

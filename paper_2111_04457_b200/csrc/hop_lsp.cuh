@@ -508,11 +508,15 @@ template <int PREC> static bool lp_eligible(const bq_lattice* lat, const HopMult
 template <int PREC, int RECON, int EPI, bool CPLX, int RED, bool DAG>
 static bq_status lp_launch_one(bq_lattice* lat, const LpParams<typename Prec<PREC>::comp>& P, int grid, cudaStream_t stream) {
     constexpr size_t smem = LpGeom<PREC>::TOTAL;
-    static bool attr_set = false;
+    // the shared-memory limit is a property of the (kernel, device) pair: remember it per device ordinal, not per process
+    static bool attr_set[64] = {};
+    int dev = 0;
+    BQ_CUDA(lat, cudaGetDevice(&dev));
+    const bool known = dev >= 0 && dev < 64;
     auto kern = hop_lsp_kernel<PREC, RECON, EPI, CPLX, RED, DAG>;
-    if (!attr_set) {
+    if (!known || !attr_set[dev]) {
         BQ_CUDA(lat, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
+        if (known) attr_set[dev] = true;
     }
     kern<<<grid, LP_THREADS, smem, stream>>>(P);
     return BQ_OK;
