@@ -463,6 +463,7 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
         }
         if (e == cudaSuccess) e = cudaEventRecord(w->evp[0], s);
         if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        if (e != cudaSuccess || st != BQ_OK) w->blas.nrhs = 1;
         if (e != cudaSuccess) return bq_set_error(lat, BQ_ECUDA, "%s: import failed: %s", fn, cudaGetErrorString(e));
         BQ_TRY(st);
     }
@@ -484,15 +485,26 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
     // |b_k|^2 over the full lattice (two parities)
     double* bnorm = static_cast<double*>(calloc(5 * (size_t)n, sizeof(double)));
     int* ik = static_cast<int*>(calloc(7 * (size_t)n, sizeof(int)));
-    if (!bnorm || !ik) { free(bnorm); free(ik); return bq_set_error(lat, BQ_ENOMEM, "%s: host allocation failed", fn); }
+    if (!bnorm || !ik) { free(bnorm); free(ik); w->blas.nrhs = 1; return bq_set_error(lat, BQ_ENOMEM, "%s: host allocation failed", fn); }
     double *target = bnorm + n, *prev_rnorm = bnorm + 2 * n, *rnorm = bnorm + 3 * n, *true_rel = bnorm + 4 * n;
     int *stalled = ik, *inner_total = ik + n, *restarts = ik + 2 * n, *cycles = ik + 3 * n, *fin = ik + 4 * n, *stat = ik + 5 * n, *dead = ik + 6 * n;
     bq_status result = BQ_OK;
-    // every early exit below goes through `fail` so that the host scratch is released
+    // every early exit below goes through `bail`: once the export of x has been enqueued on the side stream the library may
+    // still be writing the caller's x, so a failure waits for both streams before it returns (errors of the waits themselves are
+    // ignored: the status being returned is the one that matters), puts the context back to one right-hand side and
+    // releases the host scratch
+    auto bail = [&](bq_status st) {
+        cudaStreamSynchronize(w->side);
+        cudaStreamSynchronize(s);
+        w->blas.nrhs = 1;
+        free(bnorm);
+        free(ik);
+        return st;
+    };
 #define SOLVE_TRY(expr)                         \
     do {                                        \
         bq_status _s = (expr);                  \
-        if (_s != BQ_OK) { free(bnorm); free(ik); return _s; } \
+        if (_s != BQ_OK) return bail(_s);       \
     } while (0)
     {
         BlasCtx cb = c;
@@ -506,9 +518,7 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
     bool any_nonzero = false;
     for (int k = 0; k < n; k++)
         if (!isfinite(bnorm[k])) {
-            free(bnorm); free(ik);
-            w->blas.nrhs = 1;
-            return bq_set_error(lat, BQ_EINVAL, "%s: right-hand side %d contains NaN or Inf", fn, k);
+            return bail(bq_set_error(lat, BQ_EINVAL, "%s: right-hand side %d contains NaN or Inf", fn, k));
         }
     for (int k = 0; k < n; k++) {
         bnorm[k] = sqrt(bnorm[k]);
@@ -521,7 +531,7 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
     for (int k = 0; k < n; k++)
         if (bnorm[k] == 0.0) {
             cudaError_t e = cudaMemsetAsync(xx + (size_t)k * 2 * fb64, 0, 2 * fb64, s);
-            if (e != cudaSuccess) { free(bnorm); free(ik); return bq_set_error(lat, BQ_ECUDA, "%s: memset failed", fn); }
+            if (e != cudaSuccess) return bail(bq_set_error(lat, BQ_ECUDA, "%s: memset failed", fn));
         }
     cudaEventRecord(w->evp[1], s);
     cudaEventRecord(w->evp[2], s);
@@ -545,7 +555,7 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
             // r = b^_e - M^ x_e in fp64  (declared zero guess, first cycle: M^ x_e = 0 without applying the operator)
             if (o.x0_zero && outer == 0) {
                 cudaError_t e = cudaMemsetAsync(w->t, 0, fb64 * n, s);
-                if (e != cudaSuccess) { free(bnorm); free(ik); return bq_set_error(lat, BQ_ECUDA, "%s: memset failed", fn); }
+                if (e != cudaSuccess) return bail(bq_set_error(lat, BQ_ECUDA, "%s: memset failed", fn));
             } else {
                 // x_e of rhs k lives at xx + k*2*fb64: Schur with input stride 2*fb64 = two hops by hand
                 const HopMulti m1 = hm(2 * fb64, fb64, 0), m2 = hm(fb64, fb64, 2 * fb64);
@@ -621,7 +631,7 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
         {
             cudaError_t e = cudaEventRecord(w->ev_side, s);
             if (e == cudaSuccess) e = cudaStreamWaitEvent(w->side, w->ev_side, 0);
-            if (e != cudaSuccess) { free(bnorm); free(ik); return bq_set_error(lat, BQ_ECUDA, "%s: %s", fn, cudaGetErrorString(e)); }
+            if (e != cudaSuccess) return bail(bq_set_error(lat, BQ_ECUDA, "%s: %s", fn, cudaGetErrorString(e)));
         }
         // ---- ... while the true residual |b - D x| / |b| is computed on the full lattice in fp64 ----
         for (int p = 0; p < 2; p++) {
@@ -645,7 +655,7 @@ static bq_status solve_impl(bq_lattice* lat, const double* b, double* x, int nrh
             if (e == cudaSuccess) e = cudaStreamWaitEvent(s, w->ev_side, 0);
             if (e == cudaSuccess) e = cudaEventRecord(w->ev1, s);
             if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-            if (e != cudaSuccess) { free(bnorm); free(ik); return bq_set_error(lat, BQ_ECUDA, "%s: export failed: %s", fn, cudaGetErrorString(e)); }
+            if (e != cudaSuccess) return bail(bq_set_error(lat, BQ_ECUDA, "%s: export failed: %s", fn, cudaGetErrorString(e)));
         }
     } else {
         // nothing to solve (all right-hand sides zero): x = 0
@@ -892,6 +902,7 @@ extern "C" bq_status bq_schur_apply_dots(bq_lattice* lat, void* out, const void*
     SolverWork* w = nullptr;
     BQ_TRY(blas_entry(lat, prec, &w));
     if (!dots) return bq_set_error(lat, BQ_EINVAL, "bq_schur_apply_dots: dots is NULL");
+    if (lat->sub) return bq_set_error(lat, BQ_EINVAL, "bq_schur_apply_dots: not on a sub-lattice handle");
     const HopRed red{w_vec ? 1 : 2, w_vec, w->blas.sc};
     k_set_bicg_scalars<<<1, 1, 0, w->blas.stream>>>(w->blas.sc, 1, 0, 1, 0);   // rho = 1: alpha = 1 / <w, out>
     BQ_CHECK_LAUNCH(lat);
