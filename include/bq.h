@@ -235,7 +235,8 @@ bq_status bq_propagator(bq_lattice* lat, const int* src_site /*[4]*/, double* S,
  * coords[4] = this rank's position (rank number = coords[0] + grid[0]*(coords[1] + ...)); bc_phase = the GLOBAL boundary
  * phases.  bq_gauge_load takes the rank's LOCAL block of the link field (no ghost links are needed).  On such a handle
  * bq_wilson_apply computes the INTERIOR part of the hop (hops that leave the rank in a partitioned direction contribute
- * nothing); the rest arrives through the faces:
+ * nothing); the rest arrives through the faces.  Every other operator call (bq_dirac_apply, bq_schur_apply, the *_mode and
+ * *_multi forms) and the solvers return BQ_EINVAL on a handle with a partitioned direction instead of an interior-only result:
  *   bq_dd_pack    send[2*mu + side], partitioned directions only: 12 reals per boundary site of the input parity, in the
  *                 storage type (bq_dd_face_bytes): side 0 = slice x_mu = 0, spin-projected with (1 - g_mu), for the rank
  *                 BELOW; side 1 = slice x_mu = l_mu - 1, projected with (1 + g_mu) and multiplied by U_mu^dag, for the rank ABOVE.

@@ -74,6 +74,21 @@ bq_status bq_hop(bq_lattice* lat, void* out, const void* in, const void* z, doub
 static bool valid_prec(int p) { return p == BQ_FP64 || p == BQ_FP32 || p == BQ_HALF; }
 static bool valid_recon(int r) { return r == BQ_RECON18 || r == BQ_RECON12; }
 
+// On a sub-lattice handle with a partitioned direction the hop kernels compute the INTERIOR part only (off-rank hops get
+// weight zero; the rest arrives through bq_dd_unpack).  bq_wilson_apply documents that; every other operator call would
+// return a silently incomplete result, so it refuses such a handle.
+static bool partitioned(const bq_lattice* lat) {
+    return lat->sub && (lat->grid[0] > 1 || lat->grid[1] > 1 || lat->grid[2] > 1 || lat->grid[3] > 1);
+}
+#define BQ_REJECT_PARTITIONED(lat, fn)                                                                                              \
+    do {                                                                                                                            \
+        if (partitioned(lat))                                                                                                       \
+            return bq_set_error(lat, BQ_EINVAL, fn ": a sub-lattice handle computes interior hops only; use bq_wilson_apply + bq_dd_pack / bq_dd_unpack, or bq_dd_wilson_apply"); \
+    } while (0)
+
+static bq_status dirac_apply_impl(bq_lattice* lat, void* out, const void* in, double kappa, double csw, bq_prec prec, bq_recon recon,
+                                  void* stream);
+
 extern "C" bq_status bq_wilson_apply(bq_lattice* lat, void* out, const void* in, double kappa, bq_parity parity, bq_prec prec,
                                      bq_recon recon, void* stream) {
     if (!lat) return BQ_EINVAL;
@@ -84,11 +99,18 @@ extern "C" bq_status bq_wilson_apply(bq_lattice* lat, void* out, const void* in,
     if (parity == BQ_EVEN || parity == BQ_ODD)
         return bq_hop(lat, out, in, nullptr, -kappa, (int)parity, prec, recon, nullptr, 0, s);
     if (parity != BQ_FULL) return bq_set_error(lat, BQ_EINVAL, "bq_wilson_apply: bad parity %d", (int)parity);
-    return bq_dirac_apply(lat, out, in, kappa, 0.0, prec, recon, stream);
+    return dirac_apply_impl(lat, out, in, kappa, 0.0, prec, recon, stream);   // on a sub-lattice: the interior part of D, as documented
 }
 
 extern "C" bq_status bq_dirac_apply(bq_lattice* lat, void* out, const void* in, double kappa, double csw, bq_prec prec,
                                     bq_recon recon, void* stream) {
+    if (!lat) return BQ_EINVAL;
+    BQ_REJECT_PARTITIONED(lat, "bq_dirac_apply");
+    return dirac_apply_impl(lat, out, in, kappa, csw, prec, recon, stream);
+}
+
+static bq_status dirac_apply_impl(bq_lattice* lat, void* out, const void* in, double kappa, double csw, bq_prec prec, bq_recon recon,
+                                  void* stream) {
     if (!lat) return BQ_EINVAL;
     if (!out || !in || out == in) return bq_set_error(lat, BQ_EINVAL, "bq_dirac_apply: out/in NULL or aliased");
     if (!valid_prec(prec) || !valid_recon(recon)) return bq_set_error(lat, BQ_EINVAL, "bq_dirac_apply: bad prec/recon");
@@ -112,6 +134,8 @@ extern "C" bq_status bq_dirac_apply(bq_lattice* lat, void* out, const void* in, 
 
 extern "C" bq_status bq_schur_apply(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw,
                                     bq_prec prec, bq_recon recon, void* stream) {
+    if (!lat) return BQ_EINVAL;
+    BQ_REJECT_PARTITIONED(lat, "bq_schur_apply");
     return bq_schur_red(lat, out, in, tmp, kappa, csw, prec, recon, static_cast<cudaStream_t>(stream), nullptr, 0);
 }
 
@@ -166,6 +190,7 @@ bq_status bq_dirac_full(bq_lattice* lat, void* out, const void* in, double kappa
 extern "C" bq_status bq_dirac_apply_mode(bq_lattice* lat, void* out, const void* in, void* tmp, double kappa, double csw,
                                          bq_mode mode, bq_prec prec, bq_recon recon, void* stream) {
     if (!lat) return BQ_EINVAL;
+    BQ_REJECT_PARTITIONED(lat, "bq_dirac_apply_mode");
     if (!out || !in || out == in) return bq_set_error(lat, BQ_EINVAL, "bq_dirac_apply_mode: out/in NULL or aliased");
     if (!valid_prec(prec) || !valid_recon(recon)) return bq_set_error(lat, BQ_EINVAL, "bq_dirac_apply_mode: bad prec/recon");
     if (!lat->have_gauge) return bq_set_error(lat, BQ_ENOGAUGE, "bq_dirac_apply_mode: no gauge field loaded");
@@ -184,6 +209,7 @@ extern "C" bq_status bq_dirac_apply_mode(bq_lattice* lat, void* out, const void*
 extern "C" bq_status bq_schur_apply_mode(bq_lattice* lat, void* out, const void* in, void* tmp, void* tmp2, double kappa, double csw,
                                          bq_mode mode, bq_prec prec, bq_recon recon, void* stream) {
     if (!lat) return BQ_EINVAL;
+    BQ_REJECT_PARTITIONED(lat, "bq_schur_apply_mode");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     switch (mode) {
         case BQ_MODE_D: return bq_schur_red(lat, out, in, tmp, kappa, csw, prec, recon, s, nullptr, 0, false);
@@ -203,6 +229,7 @@ extern "C" bq_status bq_schur_apply_mode(bq_lattice* lat, void* out, const void*
 extern "C" bq_status bq_wilson_apply_multi(bq_lattice* lat, void* out, const void* in, int nrhs, double kappa, bq_parity parity,
                                            bq_prec prec, bq_recon recon, void* stream) {
     if (!lat) return BQ_EINVAL;
+    BQ_REJECT_PARTITIONED(lat, "bq_wilson_apply_multi");
     if (!out || !in || out == in) return bq_set_error(lat, BQ_EINVAL, "bq_wilson_apply_multi: out/in NULL or aliased");
     if (nrhs < 1) return bq_set_error(lat, BQ_EINVAL, "bq_wilson_apply_multi: nrhs must be >= 1");
     if (!valid_prec(prec) || !valid_recon(recon)) return bq_set_error(lat, BQ_EINVAL, "bq_wilson_apply_multi: bad prec/recon");
@@ -225,6 +252,7 @@ extern "C" bq_status bq_wilson_apply_multi(bq_lattice* lat, void* out, const voi
 extern "C" bq_status bq_schur_apply_multi(bq_lattice* lat, void* out, const void* in, void* tmp, int nrhs, double kappa, double csw,
                                           bq_prec prec, bq_recon recon, void* stream) {
     if (!lat) return BQ_EINVAL;
+    BQ_REJECT_PARTITIONED(lat, "bq_schur_apply_multi");
     if (nrhs < 1) return bq_set_error(lat, BQ_EINVAL, "bq_schur_apply_multi: nrhs must be >= 1");
     return bq_schur_red(lat, out, in, tmp, kappa, csw, prec, recon, static_cast<cudaStream_t>(stream), nullptr, nrhs);
 }

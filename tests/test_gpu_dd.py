@@ -166,8 +166,51 @@ def test_dd_errors(bq):
             bq.bq_solve(R.lats[0].h, b, np.zeros_like(b), 0.12, 1e-10)
         with pytest.raises(bq.BqError):                                          # clover is not built on sub-lattices
             bq.bq_clover_apply(R.lats[0].h, 1.0, 0.12, None, None, bq.BQ_FULL, 0, bq.BQ_FP64)
+        # on a handle with a partitioned direction only bq_wilson_apply (the documented interior hop) runs; the composite
+        # operators would return an interior-only result and refuse instead
+        lat0 = R.lats[0]
+        fo, fe, ft = lat0.field(bq.BQ_FP32, bq.BQ_ODD), lat0.field(bq.BQ_FP32, bq.BQ_EVEN), lat0.field(bq.BQ_FP32, bq.BQ_EVEN)
+        full_in, full_out = lat0.field(bq.BQ_FP32, bq.BQ_FULL), lat0.field(bq.BQ_FP32, bq.BQ_FULL)
+        bq.bq_wilson_apply(lat0.h, fe, fo, 0.12, bq.BQ_EVEN, bq.BQ_FP32)
+        bq.bq_wilson_apply(lat0.h, full_out, full_in, 0.12, bq.BQ_FULL, bq.BQ_FP32)
+        for call in (lambda: bq.bq_dirac_apply(lat0.h, full_out, full_in, 0.12, 0.0, bq.BQ_FP32),
+                     lambda: bq.bq_schur_apply(lat0.h, fe, ft, fo, 0.12, 0.0, bq.BQ_FP32),
+                     lambda: bq.bq_dirac_apply_mode(lat0.h, full_out, full_in, None, 0.12, 0.0, bq.BQ_MODE_DDAG, bq.BQ_FP32),
+                     lambda: bq.bq_schur_apply_mode(lat0.h, fe, ft, fo, None, 0.12, 0.0, bq.BQ_MODE_D, bq.BQ_FP32),
+                     lambda: bq.bq_wilson_apply_multi(lat0.h, fe, fo, 1, 0.12, bq.BQ_EVEN, bq.BQ_FP32),
+                     lambda: bq.bq_schur_apply_multi(lat0.h, fe, ft, fo, 1, 0.12, 0.0, bq.BQ_FP32)):
+            with pytest.raises(bq.BqError) as e:
+                call()
+            assert e.value.status == bq.BQ_EINVAL and "interior" in str(e.value)
         with pytest.raises(bq.BqError):                                          # one handle for a two-rank grid
             src = R.lats[0].field(bq.BQ_FP32, bq.BQ_ODD)
             bq.bq_dd_wilson_apply([R.lats[0].h], [R.lats[0].field(bq.BQ_FP32)], [src], 0.12, 0, bq.BQ_FP32)
+    finally:
+        R.close()
+
+
+@pytest.mark.parametrize("prec", [0, 1])
+def test_distributed_hop_single_rank(bq, prec):
+    """dd.DistributedHop.apply — the call a process per GPU makes — executed on the one GPU with a 1 x 1 x 1 x 1 grid: no face
+    leaves the rank, so no process group is needed, but the whole sequence runs: pack on the side stream, the interior hop on
+    the current (non-default) stream, the wait, unpack.  The result is the oracle's hop on the global lattice."""
+    import torch
+    L, grid, kappa = (8, 4, 4, 8), (1, 1, 1, 1), 0.125
+    U = inputs.gauge(L, 1211, 0.5)
+    psi = inputs.spinor(L, 1212)
+    R = Ranks(bq, L, grid, U, GENERAL_BC)
+    try:
+        hop = dd.DistributedHop(bq, R.lats[0], 0, grid, prec)
+        assert all(b is None for b in hop.send + hop.recv)
+        work = torch.cuda.Stream()
+        for p in (0, 1):
+            src = R.import_field(psi, prec, 1 - p)[0]
+            out = R.lats[0].field(prec, p)
+            torch.cuda.synchronize()
+            with torch.cuda.stream(work):
+                hop.apply(out, src, kappa, p)
+            work.synchronize()
+            ref = bqo.hop_restricted(U, psi, kappa, p, bc=GENERAL_BC)
+            assert relmax(R.export_field([out], prec, p), ref) < TOL[prec]
     finally:
         R.close()
