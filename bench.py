@@ -349,6 +349,16 @@ def main():
     outs = [lat.field(prec, bq.BQ_EVEN) for _ in range(NSETS)]
     for i in range(max(3, args.warmup)):
         bq.bq_wilson_apply(lat.h, outs[i % NSETS], srcs[i % NSETS], kappa, bq.BQ_EVEN, prec, recon)
+    # A/B for the clock sampler (its polling thread shares the GIL with the launch loop below and adds NVML driver calls while
+    # the measurement is in flight): the same K launches timed once with no sampler running, reported beside the headline
+    torch.cuda.synchronize()
+    ab0, ab1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ab0.record()
+    for i in range(args.steps):
+        bq.bq_wilson_apply(lat.h, outs[i % NSETS], srcs[i % NSETS], kappa, bq.BQ_EVEN, prec, recon)
+    ab1.record()
+    torch.cuda.synchronize()
+    sampler_off_us = ab0.elapsed_time(ab1) * 1e3 / args.steps
     c0 = bq.bq_get_counters(lat.h)
     sampler = ClockSampler(local_rank)
     sampler.start()
@@ -376,6 +386,8 @@ def main():
                "median_us_per_launch": float(np.median(rep_us)),
                "protocol": "the K timed launches cut into consecutive repeats by CUDA events; median over repeats (rank 0)"}
     ms_per_step = ms / args.steps
+    repeats["sampler_ab"] = {"sampler_off_us_per_launch": sampler_off_us, "sampler_on_us_per_launch": ms_per_step * 1e3,
+                             "what": "the same K launches timed without the NVML polling thread, right before the headline region (rank 0)"}
     gflops = world * FLOP_PER_SITE * Vh / (ms_per_step * 1e-3) / 1e9
     bps = BYTES_PER_SITE[(args.prec, args.recon)]
     peak, peak_src = peaks()
@@ -420,7 +432,8 @@ def main():
                "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
                "what": "bq_solve host->host, BASELINE config 4 (32^3x64 Wilson-clover csw=1 kappa=0.1215, fp32 inner / fp64 outer "
                        "BiCGStab to 1e-10, zero initial guess declared with opts.x0_zero): flops of the USEFUL hops (4 per accepted inner iteration + "
-                       "the fixed ones of the outer loop; hops enqueued after convergence return at entry and are not counted) / wall time "
+                       "the fixed ones of the outer loop; hops enqueued after convergence return at entry and are not counted — the idle count is inferred on the host, "
+                       "exact for convergence, up to 2 hops too high per breakdown restart, see include/bq_test.h) / wall time "
                        "incl. H2D of b, layout conversion, solve, D2H of x; median of the timed solves",
                "time_to_solution_s": dt, "times_s": times, "device_seconds": infos[-1].seconds,
                "phase_seconds": dict(zip(("h2d+import", "prepare", "iterate", "reconstruct+residual", "export+d2h"), list(infos[-1].phase_seconds))), "inner_iters": infos[-1].inner_iters,

@@ -26,7 +26,12 @@ bq_status bq_schur_apply_dots(bq_lattice* lat, void* out, const void* in, void* 
  * out[1..3] = hop applications (per right-hand side) with fp64 / fp32 / half storage (each is 1320 flop x Vh sites),
  * out[4] = launches of the link-stationary multi-rhs hop kernels (hop_ls.cuh, hop_lsp.cuh) among them,
  * out[5..7] = of out[1..3], the applications that were no-ops: enqueued with a batch of solver iterations after their
- *            right-hand side had converged, they return at entry (the solver's device-side `done` flag); useful = out[1..3] - out[5..7],
+ *            right-hand side had converged, they return at entry (the solver's device-side `done` flag); useful = out[1..3] - out[5..7].
+ *            The count is INFERRED ON THE HOST, 4 x (iterations enqueued - iterations the device reports done), and so
+ *            assumes an iteration that was not accepted ran no hop.  That is exact for convergence (the flag is set by the
+ *            last kernel of an iteration) but not for a breakdown, whose flag is set in the middle of an iteration after its
+ *            first two hops have run: there out[5..7] is too high by up to 2 per broken-down right-hand side and cycle, and
+ *            "useful" correspondingly too low — a bias against the library's own flop rate, never in its favour,
  * out[8] = of out[4], the launches of the direction-split kernel (hop_lsp.cuh) made outside CUDA-graph replays. */
 bq_status bq_get_counters(const bq_lattice* lat, unsigned long long* out /*[9]*/);
 
