@@ -1,6 +1,7 @@
 """Domain decomposition helpers (opt-in; include/bq.h "Domain decomposition").
 
-No arithmetic of the method lives here: rank <-> coordinates, cutting a global canonical array into the ranks' local
+No field arithmetic lives here (every operation on a vector is a kernel of libbq.so; DistributedSolver advances only the
+four complex scalars of the BiCGStab recurrence from all-reduced sums): rank <-> coordinates, cutting a global canonical array into the ranks' local
 blocks (array slicing), the schedule of the halo exchange (who sends which face to whom), and — for one process per
 GPU — the transport of the face buffers between bq_dd_pack and bq_dd_unpack through torch.distributed point-to-point
 calls (NCCL over NVLink on GPUs; the same schedule runs on the gloo backend with CPU tensors, which is how it is tested
@@ -87,23 +88,42 @@ def exchange_faces(send, recv, rank, grid, group=None):
         req.wait()
 
 
+def sum_over_ranks(values, group=None, on_host=True):
+    """The all-reduce of one reduction point of the distributed solver: the packed list of this rank's partial sums -> their
+    sums over all ranks, as floats (a CPU tensor for gloo, a device tensor for NCCL).  One collective per call."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(v) for v in values], dtype=torch.float64, device="cpu" if on_host else "cuda")
+    if dist.is_initialized() and dist.get_world_size(group) > 1:
+        dist.all_reduce(t, group=group)
+    return t.tolist()
+
+
 class DistributedHop:
     """One process per GPU: out = -kappa H_{p,1-p} in on this rank's sub-lattice, halo exchange through torch.distributed.
-    pack and the transfers run on a side stream while the interior hop runs on the current stream (the
-    communication is overlapped with the bulk); unpack follows both.  UNMEASURED on hardware."""
+    pack runs on a side stream and the interior hop on the current stream, enqueued BEFORE the host waits for any
+    transfer (the communication is overlapped with the bulk); unpack follows both.
+    host_staging=False: the face buffers travel as device tensors (NCCL over NVLink).  host_staging=True: they are copied
+    to pinned host tensors on the side stream, exchanged there (the gloo backend moves CPU tensors only) and copied back —
+    the form the GPU test runs with two processes sharing the one GPU.  UNMEASURED on multi-GPU hardware."""
 
-    def __init__(self, bq, lat, rank, grid, prec, group=None):
+    def __init__(self, bq, lat, rank, grid, prec, group=None, host_staging=False):
         import torch
         self.bq, self.lat, self.rank, self.grid, self.prec, self.group = bq, lat, rank, tuple(grid), prec, group
+        self.host = bool(host_staging)
         self.side = torch.cuda.Stream()
         dt = torch.float64 if prec == bq.BQ_FP64 else torch.float32
         self.send, self.recv = [None] * 8, [None] * 8
+        self.h_send, self.h_recv = [None] * 8, [None] * 8
         for mu in range(4):
             if self.grid[mu] > 1:
                 n = bq.bq_dd_face_bytes(lat.h, mu, prec) // (8 if prec == bq.BQ_FP64 else 4)
                 for s in range(2):
                     self.send[2 * mu + s] = torch.empty(n, dtype=dt, device="cuda")
                     self.recv[2 * mu + s] = torch.empty(n, dtype=dt, device="cuda")
+                    if self.host:
+                        self.h_send[2 * mu + s] = torch.empty(n, dtype=dt).pin_memory()
+                        self.h_recv[2 * mu + s] = torch.empty(n, dtype=dt).pin_memory()
 
     def apply(self, out, inp, kappa, parity, recon=0):
         import torch
@@ -111,7 +131,112 @@ class DistributedHop:
         self.side.wait_stream(cur)
         with torch.cuda.stream(self.side):
             bq.bq_dd_pack(self.lat.h, self.send, inp, parity, self.prec, recon, self.side)
-            exchange_faces(self.send, self.recv, self.rank, self.grid, self.group)
+            if self.host:
+                for d, h in zip(self.send, self.h_send):
+                    if d is not None:
+                        h.copy_(d, non_blocking=True)
         bq.bq_wilson_apply(self.lat.h, out, inp, kappa, parity, self.prec, recon, cur)      # interior
+        with torch.cuda.stream(self.side):
+            if self.host:
+                self.side.synchronize()                       # the packed faces are on the host
+                exchange_faces(self.h_send, self.h_recv, self.rank, self.grid, self.group)
+                for d, h in zip(self.recv, self.h_recv):
+                    if d is not None:
+                        d.copy_(h, non_blocking=True)
+            else:
+                exchange_faces(self.send, self.recv, self.rank, self.grid, self.group)
         cur.wait_stream(self.side)
         bq.bq_dd_unpack(self.lat.h, out, self.recv, -kappa, parity, self.prec, recon, cur)
+
+
+class DistributedSolver:
+    """One process per GPU: D x = b for the Wilson matrix (csw = 0) on the GLOBAL lattice, each rank holding its local block —
+    the even-odd Schur system M^ x_e = b^_e, M^ = 1 - kappa^2 H_eo H_oe, solved by fp64 BiCGStab (reading O4, the recurrences
+    of bq_dd_solve / solve.cu), then x_o = b_o + kappa H_oe x_e.  Every operator application is two DistributedHop.apply
+    calls (halo exchange per hop); every vector operation is one of the library's fused BLAS-1 kernels on the rank's fields;
+    every inner product is the rank's device reduction followed by ONE torch.distributed.all_reduce of the packed scalars of
+    that reduction point (2, 3 and 3 doubles per iteration) — the only places where the ranks meet besides the faces.  The
+    handful of complex scalars (rho, alpha, omega, beta) are advanced here on the host, identically on every rank, from the
+    all-reduced sums.  UNMEASURED on multi-GPU hardware; tested with two processes sharing one GPU over gloo."""
+
+    def __init__(self, bq, lat, rank, grid, group=None, host_staging=False):
+        self.bq, self.lat, self.group, self.host = bq, lat, group, bool(host_staging)
+        self.hop = DistributedHop(bq, lat, rank, grid, bq.BQ_FP64, group, host_staging)
+
+    def _sum_over_ranks(self, values):
+        return sum_over_ranks(values, self.group, on_host=self.host)
+
+    def _schur(self, out, inp, tmp_o, tmp_e, kappa):
+        """out = M^ inp = inp - (-kappa H_eo)(-kappa H_oe) inp."""
+        bq = self.bq
+        self.hop.apply(tmp_o, inp, kappa, bq.BQ_ODD)
+        self.hop.apply(tmp_e, tmp_o, kappa, bq.BQ_EVEN)
+        out.copy_(inp)
+        bq.bq_blas_caxpy(self.lat.h, -1.0, tmp_e, out, bq.BQ_FP64)
+
+    def solve(self, b_local, x_local, kappa, tol, max_iter=1000):
+        """b_local: this rank's canonical complex128 block [lt, lz, ly, lx, 4, 3]; x_local: same shape, receives the solution
+        (zero initial guess).  Returns {"iters", "schur_rel_residual", "converged"}."""
+        import torch
+        bq, lat = self.bq, self.lat
+        P64, h = bq.BQ_FP64, lat.h
+        fb = bq.bq_field_bytes(h, P64, bq.BQ_EVEN)
+        bfull = lat.import_field(b_local, P64, bq.BQ_FULL)
+        be, bo = bfull[:fb], bfull[fb:]
+        new = lambda: lat.field(P64, bq.BQ_EVEN)
+        bnorm2, = self._sum_over_ranks([bq.bq_blas_norm2(h, be, P64) + bq.bq_blas_norm2(h, bo, P64)])
+        x, tmp_o, tmp_e, v, s, t, ptmp = new(), new(), new(), new(), new(), new(), new()
+        # b^_e = b_e + kappa H_eo b_o
+        self.hop.apply(tmp_e, bo, kappa, bq.BQ_EVEN)
+        bhat = be.clone()
+        bq.bq_blas_caxpy(h, -1.0, tmp_e, bhat, P64)
+        r = bhat.clone()
+        rhat, p = r.clone(), r.clone()
+        r2, = self._sum_over_ranks([bq.bq_blas_norm2(h, r, P64)])
+        rho = complex(r2, 0.0)
+        target2 = tol * tol * bnorm2
+        iters, converged = 0, r2 <= target2
+        while not converged and iters < max_iter:
+            self._schur(v, p, tmp_o, tmp_e, kappa)
+            d = bq.bq_blas_cdot(h, rhat, v, P64)
+            re, im = self._sum_over_ranks([d.real, d.imag])
+            rv = complex(re, im)
+            if rv == 0 or rho == 0:
+                break                                               # breakdown
+            alpha = rho / rv
+            s.copy_(r)
+            bq.bq_blas_caxpy(h, -alpha, v, s, P64)
+            self._schur(t, s, tmp_o, tmp_e, kappa)
+            d = bq.bq_blas_cdot(h, t, s, P64)
+            re, im, tt = self._sum_over_ranks([d.real, d.imag, bq.bq_blas_norm2(h, t, P64)])
+            if tt == 0:
+                break
+            omega = complex(re, im) / tt
+            lr2, lrr = bq.bq_blas_bicg_update(h, alpha, omega, p, s, t, rhat, x, r, P64)     # x += alpha p + omega s; r = s - omega t
+            r2, re, im = self._sum_over_ranks([lr2, lrr.real, lrr.imag])
+            iters += 1
+            if r2 <= target2:
+                converged = True
+                break
+            rho_new = complex(re, im)
+            if omega == 0:
+                break
+            beta = (rho_new / rho) * (alpha / omega)
+            rho = rho_new
+            bq.bq_blas_caxpy(h, -omega, v, p, P64)                   # p = r + beta (p - omega v)
+            ptmp.copy_(r)
+            bq.bq_blas_caxpy(h, beta, p, ptmp, P64)
+            p, ptmp = ptmp, p
+        # the residual of the Schur system, recomputed with the operator
+        self._schur(t, x, tmp_o, tmp_e, kappa)
+        bq.bq_blas_caxpy(h, -1.0, t, bhat, P64)
+        res2, = self._sum_over_ranks([bq.bq_blas_norm2(h, bhat, P64)])
+        # x_o = b_o + kappa H_oe x_e
+        self.hop.apply(tmp_o, x, kappa, bq.BQ_ODD)
+        xo = bo.clone()
+        bq.bq_blas_caxpy(h, -1.0, tmp_o, xo, P64)
+        torch.cuda.synchronize()
+        xfull = torch.cat([x, xo])
+        x_local[...] = lat.export_field(xfull, P64, bq.BQ_FULL)
+        rel = (res2 / bnorm2) ** 0.5 if bnorm2 > 0 else 0.0
+        return {"iters": iters, "schur_rel_residual": rel, "converged": bool(rel <= tol)}

@@ -63,6 +63,9 @@ for it in range(3):                                           # the same buffers
     for mu, sside, dest, rside, src in dd.face_schedule(rank, grid):
         want = float(1000 * src + 10 * mu + sside)
         assert torch.all(recv[2 * mu + rside] == want), (rank, mu, rside, recv[2 * mu + rside][0].item(), want)
+# the packed scalars of one reduction point of dd.DistributedSolver: one all-reduce, identical sums on every rank
+got = dd.sum_over_ranks([1.5 + rank, -2.0 * rank, 0.25], on_host=True)
+assert got == [1.5 + 2.5, -2.0, 0.5], got
 dist.barrier()
 dist.destroy_process_group()
 print("ok", rank)
