@@ -44,6 +44,17 @@
  * the test / benchmark hooks of bq_test.h) run on a stream the handle owns — a blocking stream, i.e. ordered with the legacy
  * default stream exactly as the legacy stream is with itself — because batches of solver iterations are replayed as
  * CUDA graphs and the legacy stream cannot be captured.
+ *
+ * Environment switches.  Six variables are read (bq_lattice_create; BQ_LS_BRICK at the first multi-rhs launch) — measurement
+ * A/B switches of the kernels' launch strategy kept for the tables in DESIGN.md; none changes a result (every variant
+ * computes the same bits), the defaults are the measured best, and a production build needs none of them:
+ *   BQ_GRAPH=0        solver: launch the batches of inner iterations eagerly instead of replaying CUDA graphs
+ *   BQ_PDL=0|<Vh>     single-rhs hop: programmatic dependent launch off, or only when Vh <= the bound (default 262144)
+ *   BQ_HOP_SMALL=<Vh> single-rhs fp32 hop: uncapped-register build when Vh <= the bound (default 2 x SMs x 128)
+ *   BQ_MRHS_LS=0..3   multi-rhs hop: 0 = per-(site, rhs) kernel only, 1 = link-stationary kernel for fp32 / half only,
+ *                     2 (default) = that + the direction-split fp64 kernel from 8 right-hand sides on, 3 = direction-split wherever it applies
+ *   BQ_MRHS_PATCH=0   multi-rhs per-(site, rhs) kernel: plain instead of patch thread mapping
+ *   BQ_LS_BRICK=y,z,t link-stationary kernels: cap of the launch-order brick (default 4,4,4; 1,1,1 = lexicographic)
  * ---------------------------------------------------------------------------------------------
  */
 #ifndef BQ_H

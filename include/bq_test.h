@@ -1,7 +1,7 @@
 /* bq_test.h — test and benchmark hooks of libbq.so.  NOT part of the product boundary (that is include/bq.h, the
  * calls SURVEY.md §8(b) lists): these entry points expose internal kernels of the hot path one by one so that the tests
  * can check them against the oracle (fused BLAS-1; fused inner products of the hop epilogue) and so that
- * bench.py / kbench.py can time them with CUDA events on the library's own stream and count launches.
+ * bench.py (the contract line and its --kernels table) can time them with CUDA events on the library's own stream and count launches.
  * Same conventions as bq.h: extern "C", plain pointers, bq_status returns, internal-layout DEVICE fields.
  */
 #ifndef BQ_TEST_H

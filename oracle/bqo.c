@@ -26,6 +26,9 @@
  * free-field eigenvalue conj(lambda), point-source stencil, numpy.linalg.solve.
  * Unpinned readings: S5 (trace part of F_mu_nu is NOT subtracted; `traceless` flag, default 0)
  * and S9 (meaning of nconv/diff) — "parity unpinned" for those two choices, see DESIGN.md §3.
+ * (The arithmetic of the optional traceless branch is pinned against the pinned default by
+ * tests/test_oracle_clover_pins.py::test_traceless_option_removes_exactly_the_trace; which of the two the paper
+ * means stays the unpinned reading S5.)
  */
 #include <complex.h>
 #include <math.h>

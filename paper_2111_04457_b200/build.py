@@ -23,7 +23,7 @@ STAMP = LIB + ".stamp"
 OBJDIR = os.path.join(HERE, "build")
 
 UNITS = ["lattice.cu", "hop.cu", "hop_inst_fp64_18.cu", "hop_inst_fp64_12.cu", "hop_inst_fp32_18.cu", "hop_inst_fp32_12.cu",
-         "hop_inst_half_18.cu", "hop_inst_half_12.cu", "clover.cu", "blas.cu", "solve.cu", "dd.cu", "noalloc.cu"]
+         "hop_inst_half_18.cu", "hop_inst_half_12.cu", "clover.cu", "blas.cu", "solve.cu", "bench_hooks.cu", "dd.cu", "noalloc.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "--extended-lambda", "-Xcompiler", "-fPIC", "-I", INCLUDE, "-I", CSRC,

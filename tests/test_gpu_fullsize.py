@@ -85,7 +85,7 @@ def test_config3_32x32x32x64_hop_every_site(bq):
 
 
 def test_config3_multirhs_x12_every_site(bq):
-    """32^3 x 64 fp32, half and fp64 storage, 12 right-hand sides in one launch (the link-stationary kernels, as kbench and
+    """32^3 x 64 fp32, half and fp64 storage, 12 right-hand sides in one launch (the link-stationary kernels, as bench.py --kernels and
     bench.py time them: hop_ls.cuh for fp32 / half, the direction-split hop_lsp.cuh for fp64): every output site of every
     right-hand side against the oracle, and every right-hand side bit for bit against the single-rhs kernel."""
     import torch

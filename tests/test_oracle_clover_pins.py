@@ -204,3 +204,31 @@ def test_clover_matrix_pairs_sigma_with_the_right_plane(mu, nu):
     expect = np.eye(12) - csw * kappa * np.kron(sig, F)          # index = 3 * spin + colour
     A = bqo.clover_build(U, csw, kappa)
     assert np.abs(A - expect).max() < 1e-14, (mu, nu)
+
+
+def test_traceless_option_removes_exactly_the_trace():
+    """Reading S5 keeps the trace of F_mu_nu (the default everywhere in this repository).  The oracle's optional `traceless`
+    branch is pinned to the pinned default: F' = F - (tr F / 3) 1 in every plane on every site, tr F' = 0, and — since
+    sigma_mu_nu is traceless — the site trace of the clover matrix A is 12 either way, while A itself differs where tr F != 0.
+    An abelian U(1)^3 field (phases not summing to zero per link) has tr F != 0, so the branch is exercised, not vacuous."""
+    L = (4, 4, 2, 2)
+    rng = np.random.default_rng(77)
+    Lx, Ly, Lz, Lt = L
+    ph = rng.uniform(-0.6, 0.6, size=(Lt, Lz, Ly, Lx, 4, 3))
+    U = np.zeros((Lt, Lz, Ly, Lx, 4, 3, 3), dtype=np.complex128)
+    for c in range(3):
+        U[..., c, c] = np.exp(1j * ph[..., c])
+    eye = np.eye(3)
+    saw_trace = False
+    for mu in range(4):
+        for nu in range(mu + 1, 4):
+            F = bqo.field_strength(U, mu, nu)
+            Ft = bqo.field_strength(U, mu, nu, traceless=True)
+            tr = np.trace(F, axis1=-2, axis2=-1)
+            saw_trace = saw_trace or np.abs(tr).max() > 1e-3
+            assert np.abs(Ft - (F - tr[..., None, None] / 3.0 * eye)).max() < 1e-14
+            assert np.abs(np.trace(Ft, axis1=-2, axis2=-1)).max() < 1e-14
+    assert saw_trace
+    A, At = bqo.clover_build(U, 1.3, 0.12), bqo.clover_build(U, 1.3, 0.12, traceless=True)
+    assert np.abs(np.trace(A, axis1=-2, axis2=-1) - 12).max() < 1e-12 and np.abs(np.trace(At, axis1=-2, axis2=-1) - 12).max() < 1e-12
+    assert np.abs(A - At).max() > 1e-4
