@@ -256,7 +256,9 @@ bq_status bq_propagator(bq_lattice* lat, const int* src_site /*[4]*/, double* S,
  *                 x_mu = 0).  out += scale * (...), scale = the factor the interior call used (-kappa for bq_wilson_apply);
  *                 the global boundary phase is applied here on the ranks at the edge of the grid.
  * A process per GPU moves send -> recv with peer copies or NCCL send/recv between pack and unpack while the interior
- * call runs (paper_2111_04457_b200/dd.py).  UNMEASURED on hardware: no multi-GPU node was available to this build.
+ * call runs (paper_2111_04457_b200/dd.py: DistributedHop, and DistributedSolver = the BiCGStab of bq_dd_solve with one
+ * all-reduce of the packed partial sums per reduction point; both executed by two processes sharing one GPU in
+ * tests/test_gpu_dd_multiprocess.py).  UNMEASURED on multi-GPU hardware: no such node was available to this build.
  *
  * bq_dd_wilson_apply / bq_dd_solve: the same with VIRTUAL RANKS — all nranks = prod(grid) handles in this process on one
  * device (ranks[r] at rank number r), faces moved by device copies: what the tests compare with the oracle on the global

@@ -57,8 +57,17 @@ static_assert(LS_NT % 8 == 0 && LS_THREADS % 32 == 0 && LS_THREADS <= 1024, "blo
 static_assert((LS_BY * LS_BZ) % 4 == 0 && (LS_BZ * LS_BT) % 4 == 0 && (LS_BY * LS_BT) % 4 == 0,
               "every halo region must be a multiple of 4 tiles (128-byte alignment of the TMA destinations in half storage)");
 
-// shared-memory geometry of one stage (one right-hand side): byte offsets of the regions
-template <int PREC> struct LsGeom {
+#ifndef LS_WIDEX
+#define LS_WIDEX 0            // conflict-free placement of the x-halo sites in shared memory: A/B switch, OFF — measured slower on B200
+#endif                        // (fp32 x12 hop 660 vs 631 us, x4 308 vs 279, x2 215 vs 189; profiles/r3_ls_widex_ab.txt)
+// shared-memory geometry of one stage (one right-hand side): byte offsets of the regions.
+// WIDEX: the x-halo site of a row sits in 16-byte slot 0 (rows that read it as their forward neighbour) or slot 7 (backward) of a
+// 128-byte line of its own per (row pair, word).  The 7 other threads of the row read slots 1..7 (resp. 0..6) of the centre tile
+// with the same LDS.128, so the halo slot is the one bank group they leave free; in the compact form (8 rows share a pseudo tile,
+// slot = row & 7) 7 of 8 rows replay every x-direction load once (profiles/r2_hop_ls.md: 17 % of the shared wavefronts).
+// Removing those replays this way did NOT pay: the stage grows by 4.5 KB and the 96 cp.async of the x halo scatter over 48 lines
+// instead of 12; the kernel got 5-14 % slower, so the compact form stays the default.
+template <int PREC, bool WIDEX = false> struct LsGeom {
     static constexpr int S = PREC == BQ_FP64 ? 192 : (PREC == BQ_FP32 ? 96 : 52);   // bytes per site
     static constexpr int TS = 8 * S;                                               // bytes per tile
     static constexpr bool SPLIT_T = PREC != BQ_HALF;      // spin pairs in separate planes: t halos are half tiles
@@ -69,7 +78,8 @@ template <int PREC> struct LsGeom {
     static constexpr int ZM = YP + LS_BZ * LS_BT * TS, ZP = ZM + LS_BY * LS_BT * TS;
     static constexpr int TM = ZP + LS_BY * LS_BT * TS, TP = TM + LS_BY * LS_BZ * HT;
     static constexpr int X = TP + LS_BY * LS_BZ * HT;     // x halo sites, 8 to a pseudo tile
-    static constexpr int STAGE = (X + (LS_NT / 8) * TS + 127) / 128 * 128;
+    static constexpr int XBYTES = WIDEX ? (LS_NT / 2) * NW * 128 : (LS_NT / 8) * TS;
+    static constexpr int STAGE = (X + XBYTES + 127) / 128 * 128;
     static constexpr int TX = X;                          // bytes a stage receives through TMA (everything but the x halo)
     static constexpr int OPER = LS_NT * TS;               // one interior-only operand buffer (z or w)
     static constexpr int CLS = 72 * (PREC == BQ_FP64 ? 8 : (PREC == BQ_FP32 ? 4 : 2));   // clover blocks: bytes per site = 3 spinor-fp-tiles' worth per 8 sites
@@ -291,16 +301,19 @@ template <int PREC> __device__ __forceinline__ void ls_load_site(const char* til
     }
 }
 
+// wide x-halo placement: fp32, Wilson epilogues (with the clover tiles resident the 9 KB it costs would end two CTAs per SM)
+template <int PREC, int EPI> __host__ __device__ constexpr bool ls_widex() { return LS_WIDEX && PREC == BQ_FP32 && EPI < 2 && LS_NT % 2 == 0 && LS_BY % 2 == 0; }
 template <int EPI, int RED> __host__ __device__ constexpr int ls_stages() { return (EPI == 0 && LS_MINB == 1) ? 3 : 2; }
 template <int PREC, int EPI, int RED> __host__ __device__ constexpr size_t ls_smem_bytes() {
-    return (size_t)ls_stages<EPI, RED>() * LsGeom<PREC>::STAGE + (EPI == 1 ? LsGeom<PREC>::OPER : 0) + (EPI == 1 && RED == 1 ? LsGeom<PREC>::OPER : 0) +
+    return (size_t)ls_stages<EPI, RED>() * LsGeom<PREC, ls_widex<PREC, EPI>()>::STAGE + (EPI == 1 ? LsGeom<PREC>::OPER : 0) + (EPI == 1 && RED == 1 ? LsGeom<PREC>::OPER : 0) +
            (EPI >= 2 ? LsGeom<PREC>::CLOV : 0) + 256 /* mbarriers, active list */ + (RED ? 2 * 3 * (LS_THREADS / 32) * sizeof(double) : 0);
 }
 
 template <int PREC, int RECON, int EPI, bool CPLX, int RED, bool DAG>
 __global__ void __launch_bounds__(LS_THREADS, LS_MINB) hop_ls_kernel(const __grid_constant__ LsParams<typename Prec<PREC>::comp> P) {
     using C = typename Prec<PREC>::comp;
-    using G = LsGeom<PREC>;
+    constexpr bool WX = ls_widex<PREC, EPI>();
+    using G = LsGeom<PREC, WX>;
     constexpr int NS = ls_stages<EPI, RED>();
     constexpr int NRED = RED == 1 ? 2 : 3;
     extern __shared__ __align__(128) unsigned char ls_smem[];
@@ -365,7 +378,7 @@ __global__ void __launch_bounds__(LS_THREADS, LS_MINB) hop_ls_kernel(const __gri
             xdst = dtile + 384 + (jr & 7) * 4;
         } else {
             xsrc = tile * G::TS + jk * 128 + site * 16;
-            xdst = dtile + jk * 128 + (jr & 7) * 16;
+            xdst = WX ? G::X + ((jr >> 1) * G::NW + jk) * 128 + (jrr ? 0 : 7 * 16) : dtile + jk * 128 + (jr & 7) * 16;
         }
     }
     const size_t slice_bytes = (size_t)P.nxt * a.Ly * a.Lz * G::TS;
@@ -431,7 +444,8 @@ __global__ void __launch_bounds__(LS_THREADS, LS_MINB) hop_ls_kernel(const __gri
     const bool wyf = (y == a.Ly - 1), wyb = (y == 0), wzf = (z == a.Lz - 1), wzb = (z == 0), wtf = (t == a.Lt - 1), wtb = (t == 0);
     int off[8];
     {
-        const int ctile = G::C + tl * G::TS, xslot = G::X + (tl >> 3) * G::TS + (tl & 7) * 16;
+        const int ctile = G::C + tl * G::TS;
+        const int xslot = WX ? G::X + (tl >> 1) * G::NW * 128 + (r ? 0 : 7 * 16) : G::X + (tl >> 3) * G::TS + (tl & 7) * 16;
         const int pf = r ? s8 + 1 : s8, pb = r ? s8 : s8 - 1;
         off[0] = pf < 8 ? ctile + pf * 16 : xslot;
         off[1] = pb >= 0 ? ctile + pb * 16 : xslot;
